@@ -1,0 +1,103 @@
+"""TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+ctypes access to the plain-C oracle (``ttc_oracle.c``: Eq. 1 of PAPER.md:39 as one odometer
+loop) and to the paper's OpenMP reference loop (``ttc_ref_omp.c``).  Only
+``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` / ``--impl
+reference`` legs may import this package.  It imports nothing from the product package.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libttc_oracle.so")
+_SOURCES = [os.path.join(_HERE, "ttc_oracle.c"), os.path.join(_HERE, "ttc_ref_omp.c")]
+# -ffp-contract=off: one rounding per operation (reading A7); never -ffast-math.
+# No -march=native: the oracle is "as it stands, never tuned".
+_CFLAGS = ["-O2", "-std=c11", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-fPIC", "-shared"]
+
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (building the checker is not using it)."""
+    newest = max(os.path.getmtime(s) for s in _SOURCES)
+    if force or not os.path.exists(_LIB_PATH) or os.path.getmtime(_LIB_PATH) < newest:
+        tmp = _LIB_PATH + ".tmp.%d" % os.getpid()
+        subprocess.check_call(["gcc", *_CFLAGS, "-o", tmp, *_SOURCES])
+        os.replace(tmp, _LIB_PATH)
+    return _LIB_PATH
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        i64p = ctypes.POINTER(ctypes.c_int64)
+        i32p = ctypes.POINTER(ctypes.c_int)
+        for name in ("ttc_oracle_transpose", "ttc_ref_omp_transpose"):
+            fn = getattr(lib, name)
+            fn.restype = ctypes.c_int
+            fn.argtypes = [ctypes.c_int, ctypes.c_int, i64p, i32p, i64p, i64p,
+                           ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+        lib.ttc_oracle_offsets.restype = ctypes.c_int
+        lib.ttc_oracle_offsets.argtypes = [ctypes.c_int, i64p, i32p, i64p, i64p, i64p, i64p, i64p]
+        lib.ttc_ref_omp_threads.restype = ctypes.c_int
+        _lib = lib
+    return _lib
+
+
+_NP = {0: np.float32, 1: np.float64, 2: np.complex64, 3: np.complex128}
+
+
+def _i64(seq: Optional[Sequence[int]]):
+    if seq is None:
+        return None
+    return (ctypes.c_int64 * len(seq))(*[int(x) for x in seq])
+
+
+def _call(fn, dtype: int, sizes, perm, lda, ldb, alpha, A: np.ndarray, beta, B: np.ndarray) -> None:
+    npdt = _NP[dtype]
+    if A.dtype != npdt or B.dtype != npdt:
+        raise TypeError("A/B dtype does not match dtype code %d" % dtype)
+    if not (A.flags.c_contiguous and B.flags.c_contiguous and B.flags.writeable):
+        raise ValueError("A and B must be flat contiguous buffers, B writeable")
+    n = len(sizes)
+    a = np.array([alpha], dtype=npdt)
+    b = np.array([beta], dtype=npdt)
+    rc = fn(dtype, n, _i64(sizes), (ctypes.c_int * n)(*[int(p) for p in perm]), _i64(lda), _i64(ldb),
+            a.ctypes.data_as(ctypes.c_void_p), A.ctypes.data_as(ctypes.c_void_p),
+            b.ctypes.data_as(ctypes.c_void_p), B.ctypes.data_as(ctypes.c_void_p))
+    if rc != 0:
+        raise ValueError("oracle rejected its arguments (code %d)" % rc)
+
+
+def transpose(dtype: int, sizes, perm, lda, ldb, alpha, A: np.ndarray, beta, B: np.ndarray) -> None:
+    """In-place update of the flat buffer ``B`` by Eq. 1.  Single thread."""
+    _call(_load().ttc_oracle_transpose, dtype, sizes, perm, lda, ldb, alpha, A, beta, B)
+
+
+def ref_omp_transpose(dtype: int, sizes, perm, lda, ldb, alpha, A: np.ndarray, beta, B: np.ndarray) -> None:
+    """The paper's OpenMP reference loop nest, all host cores."""
+    _call(_load().ttc_ref_omp_transpose, dtype, sizes, perm, lda, ldb, alpha, A, beta, B)
+
+
+def ref_omp_threads() -> int:
+    return int(_load().ttc_ref_omp_threads())
+
+
+def offsets(sizes, perm, lda, ldb, index):
+    """(offA, offB) in elements of the logical element with A multi-index ``index``."""
+    n = len(sizes)
+    oa = ctypes.c_int64()
+    ob = ctypes.c_int64()
+    rc = _load().ttc_oracle_offsets(n, _i64(sizes), (ctypes.c_int * n)(*[int(p) for p in perm]),
+                                    _i64(lda), _i64(ldb), _i64(index), ctypes.byref(oa), ctypes.byref(ob))
+    if rc != 0:
+        raise ValueError("oracle rejected its arguments (code %d)" % rc)
+    return int(oa.value), int(ob.value)
