@@ -1,0 +1,183 @@
+/*
+ * ttc.h -- C ABI of libttc.so: out-of-place N-dimensional tensor transposition-and-update
+ *
+ *         B_{Pi(i_0,...,i_{N-1})}  <-  alpha * A_{i_0,...,i_{N-1}}  +  beta * B_{Pi(i_0,...,i_{N-1})}
+ *
+ * (arXiv 1607.01249 "TTC", Eq. 1) on column-major tensors (index 0 is
+ * stride-1, PAPER.md:49 fn 2) with one optional leading dimension per index (sub-tensors,
+ * BLAS-style packing; Fig. 2 and Fig. 3), for the data types
+ * s, d, c, z of PAPER.md:75.  Every step of the operation runs in hand-written sm_100a
+ * CUDA kernels; there is no CPU fallback.
+ *
+ * Notation used by every call (DESIGN.md "Readings" A1-A4):
+ *   sizes[k]  extent of A's index i_k
+ *   perm[k]   the A-index that sits at position k of B, i.e. B's k-th extent is
+ *             sizes[perm[k]]          (merge example PAPER.md:63; Fig. 2)
+ *   lda[k]    leading dimension of A's index k  (>= sizes[k]);  NULL = contiguous
+ *   ldb[k]    leading dimension of B's POSITION k (>= sizes[perm[k]]); NULL = contiguous
+ *   element strides: sA[0]=1, sA[k]=sA[k-1]*lda[k-1];  tB[0]=1, tB[k]=tB[k-1]*ldb[k-1]
+ *   lda[N-1] / ldb[N-1] are validated but never used for addressing.
+ *
+ * Ownership: the caller owns A, B and the stream.  A plan owns only its own small host
+ * state (and, for ttc_execute_host, a private pair of device staging buffers).  While
+ * ttc_plan auto-tunes it allocates scratch device buffers of the real spans of A and B
+ * and frees them before it returns; the caller's tensors are never touched by tuning.
+ *
+ * Thread safety: distinct plans may be used from distinct threads.  One plan must not be
+ * executed, re-tuned or destroyed concurrently from two threads.
+ */
+#ifndef TTC_H_
+#define TTC_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TTC_MAX_RANK 16
+
+/* s, d, c, z of PAPER.md:75.  Complex = interleaved (re, im). */
+typedef enum { TTC_F32 = 0, TTC_F64 = 1, TTC_C64 = 2, TTC_C128 = 3 } ttc_dtype;
+
+typedef enum {
+    TTC_OK = 0,
+    TTC_ERR_INVALID_ARG = 1,      /* NULL pointer, N < 1, N > TTC_MAX_RANK, negative size, bad dtype */
+    TTC_ERR_NOT_PERMUTATION = 2,  /* perm is not a permutation of 0..N-1                             */
+    TTC_ERR_BAD_LD = 3,           /* lda[k] < sizes[k] or ldb[k] < sizes[perm[k]]                    */
+    TTC_ERR_UNSUPPORTED = 4,      /* spans overflow int64 / more than 2^62 elements                  */
+    TTC_ERR_ALLOC = 5,            /* host or device allocation failed                                */
+    TTC_ERR_CUDA = 6,             /* a CUDA call failed (no device, launch error, ...)               */
+    TTC_ERR_MISALIGNED = 7        /* A or B is not aligned to its own element size                   */
+} ttc_status;
+
+/* Kernel classes. */
+typedef enum {
+    TTC_KERNEL_NONE = 0,    /* empty tensor: ttc_execute is a no-op                                   */
+    TTC_KERNEL_COPY = 1,    /* K1: direct global->global, 128-bit rows when stride-1 index is shared  */
+    TTC_KERNEL_TILE = 2,    /* K2: shared-memory tiled transpose in the plane (stride-1 of A, of B)   */
+    TTC_KERNEL_GATHER = 3,  /* K3: K2 whose tile sides are coarsened over several leading indices     */
+    TTC_KERNEL_WIDE = 4,    /* K2 on "wide elements": a >=16-byte run that leads both A and B         */
+    TTC_KERNEL_TMA = 5      /* K2/K3 whose A-side tile is fetched by one TMA tensor-map box load      */
+} ttc_kernel_class;
+
+typedef struct ttc_plan_s* ttc_plan_t;
+
+/* What the plan decided.  All arrays are in canonical order (ascending stride in A). */
+typedef struct {
+    int      dtype;                       /* ttc_dtype                                             */
+    int      rank;                        /* rank N as given                                       */
+    int      canon_rank;                  /* rank after dropping extent-1 indices and merging      */
+    int64_t  canon_extent[TTC_MAX_RANK];  /* (e, sA, sB) triples of the canonical form */
+    int64_t  canon_stride_a[TTC_MAX_RANK];
+    int64_t  canon_stride_b[TTC_MAX_RANK];
+    int64_t  numel;                       /* logical elements |A|                                  */
+    int64_t  span_a, span_b;              /* 1 + largest element offset touched in A / in B        */
+    int      tuned;                       /* 1 if the winners were timed on the device             */
+    int      n_candidates[2];             /* [0]: beta == 0 variants, [1]: beta != 0               */
+    int      chosen[2];                   /* index of the winner in each list                      */
+    float    chosen_us[2];                /* its tuned time in microseconds (0 if not tuned)       */
+} ttc_info;
+
+/* One candidate implementation (loop order x blocking; here also kernel class). */
+typedef struct {
+    int      kernel;          /* ttc_kernel_class                                              */
+    int      vec_a, vec_b;    /* elements per global access on the A side / B side             */
+    int      tile_u, tile_w;  /* tile extent along A's leading side / B's leading side (elements; 0 for K1) */
+    int      n_u, n_w;        /* number of canonical indices coarsened into each side          */
+    int      threads;         /* CTA size                                                      */
+    int      smem_bytes;      /* dynamic shared memory per CTA                                 */
+    int      loop_order;      /* 0: macro-tiles walk A linearly, 1: walk B linearly            */
+    int      grid;            /* CTAs launched (persistent grid), 0 if not yet fixed           */
+    float    est_cost;        /* heuristic cost used for ranking (lower is better)             */
+    float    tuned_us;        /* measured time, 0 if this candidate was not timed              */
+    int64_t  n_tiles;         /* macro-tiles (K2/K3) or vector items (K1)                      */
+    int      tile_ext[TTC_MAX_RANK];  /* tile extent per canonical index (1 = outside the tile) */
+} ttc_candidate_info;
+
+/*
+ * ttc_plan -- validate, canonicalise (drop extent-1 indices, merge indices that Pi keeps
+ * adjacent and that are contiguous in both tensors: PAPER.md:63, 95 fn 5), enumerate and
+ * rank candidate kernels and, if a CUDA device is present and the
+ * environment does not say TTC_TUNE=0, time the best TTC_TUNE_TOPK (default 16) of them on
+ * the device for beta == 0 and for beta != 0 and keep the fastest of each.
+ * All pointers are HOST pointers, read before the call returns.
+ * Returns NULL on error; ttc_last_error() then says why.  Sizes of 0 give a valid plan
+ * whose execution does nothing.  Without a CUDA device the plan is still built (heuristic
+ * choice, tuned = 0) so that it can be inspected; executing it returns TTC_ERR_CUDA.
+ */
+ttc_plan_t ttc_plan(ttc_dtype dtype, int N, const int64_t* sizes, const int* perm,
+                    const int64_t* lda, const int64_t* ldb);
+
+/*
+ * ttc_execute -- Eq. 1 as ONE kernel launch on `cuda_stream` (a cudaStream_t;
+ * NULL = the legacy default stream).  Asynchronous; never synchronises.
+ *   alpha, beta  HOST pointers to one scalar of the plan's dtype (complex: re, im); read
+ *                before the call returns.  beta == 0 (both parts) => B is never read.
+ *   A            DEVICE pointer, span_a elements; never written; padding never read.
+ *   B            DEVICE pointer, span_b elements; only the elements Pi maps onto are
+ *                written; padding never touched.  A and B must not overlap.
+ * Pointers only have to be aligned to the element size; when they are not 16-byte aligned
+ * a narrower-vector candidate of the same plan is launched instead of the tuned one.
+ * Errors: TTC_ERR_INVALID_ARG (NULL plan/alpha/beta, NULL A or B for a non-empty tensor),
+ * TTC_ERR_MISALIGNED, TTC_ERR_CUDA (launch failed; the CUDA error state is left as is).
+ */
+ttc_status ttc_execute(ttc_plan_t plan, const void* alpha, const void* A,
+                       const void* beta, void* B, void* cuda_stream);
+
+/*
+ * ttc_execute_host -- the same operation for HOST buffers A (span_a elements) and B
+ * (span_b elements): copies A (and B when beta != 0, or when B has padding that has to
+ * survive) to the plan's private device staging buffers, runs ttc_execute, copies B back
+ * and waits for it.  Synchronous.  Pinned host memory makes the copies faster but is not
+ * required.
+ */
+ttc_status ttc_execute_host(ttc_plan_t plan, const void* alpha, const void* A_host,
+                            const void* beta, void* B_host, void* cuda_stream);
+
+/* ttc_destroy -- frees the plan (and its staging buffers).  NULL is allowed. */
+ttc_status ttc_destroy(ttc_plan_t plan);
+
+/* Thread-local status of the last ttc_plan / ttc_canonicalize call on this thread. */
+ttc_status ttc_last_error(void);
+const char* ttc_status_string(ttc_status status);
+
+/* ttc_plan_info -- fills *out.  TTC_ERR_INVALID_ARG on NULL. */
+ttc_status ttc_plan_info(ttc_plan_t plan, ttc_info* out);
+
+/* Candidate lists of a plan: which = 0 for the beta == 0 list, 1 for beta != 0. */
+int        ttc_plan_num_candidates(ttc_plan_t plan, int which);
+ttc_status ttc_plan_candidate(ttc_plan_t plan, int which, int index, ttc_candidate_info* out);
+/* Force a candidate (tests, search-quality experiments).  index = -1 restores the winner. */
+ttc_status ttc_plan_select(ttc_plan_t plan, int which, int index);
+/*
+ * ttc_plan_tune -- (re-)time the `top_k` best-ranked candidates (<= 0: all) of both lists,
+ * `reps` timed launches each (minimum kept), and select the fastest.
+ * Needs a CUDA device.  Uses scratch buffers, never the caller's tensors.
+ */
+ttc_status ttc_plan_tune(ttc_plan_t plan, int top_k, int reps);
+
+/*
+ * ttc_canonicalize -- stage 1 alone, host only, no device needed: writes the
+ * canonical (extent, stride in A, stride in B) triples, ascending in A-stride, into the
+ * three output arrays (room for TTC_MAX_RANK each) and returns the canonical rank
+ * (0 for an empty tensor, -1 on error with ttc_last_error() set).
+ */
+int ttc_canonicalize(int N, const int64_t* sizes, const int* perm,
+                     const int64_t* lda, const int64_t* ldb,
+                     int64_t* extent_out, int64_t* stride_a_out, int64_t* stride_b_out);
+
+/* Kernels launched by this library in this process so far (bench.py's gpu_launches). */
+int64_t ttc_launch_count(void);
+
+/* Host-only self-check hook for the fast-divmod constants the kernels use:
+ * returns n / d computed with the (multiplier, shift) pair the plan generator would build
+ * for divisor d.  Valid for 0 <= n < 2^31, 1 <= d < 2^31. */
+uint32_t ttc_debug_fastdiv(uint32_t n, uint32_t d);
+
+const char* ttc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TTC_H_ */

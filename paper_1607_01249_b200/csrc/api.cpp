@@ -1,0 +1,343 @@
+// api.cpp -- the C ABI of include/ttc.h: plan construction (stages 1-3), the on-device
+// autotuner (stages 4-6 of PAPER.md:69 without the compiler: candidates are pre-instantiated
+// kernels with run-time parameters), the in-process solution cache (the paper's SQL lookup,
+// PAPER.md:63), execution and host staging.
+#include <cuda_runtime.h>
+
+#include <atomic>
+#include <cstdlib>
+#include <cstring>
+#include <map>
+#include <mutex>
+#include <string>
+#include <vector>
+
+#include "ttc_internal.h"
+
+using namespace ttc;
+
+struct ttc_plan_s {
+    ttc_dtype dtype;
+    int rank;
+    Canon canon;
+    std::vector<Candidate> cands[2];   // [0]: beta == 0, [1]: beta != 0, ranked by est_cost
+    int winner[2] = {-1, -1};          // tuned (or heuristic) choice
+    int forced[2] = {-1, -1};          // ttc_plan_select override
+    int scalar[2] = {-1, -1};          // best candidate that needs only element alignment
+    bool tuned = false;
+    bool have_device = false;
+    int sm_count = 148;
+    int max_smem = 227 * 1024;
+    void* stage_a = nullptr;
+    void* stage_b = nullptr;
+};
+
+namespace {
+
+thread_local ttc_status g_last_error = TTC_OK;
+std::atomic<int64_t> g_launches{0};
+
+struct CacheEntry { int winner[2]; float us[2]; };
+std::mutex g_cache_mu;
+std::map<std::string, CacheEntry> g_cache;
+
+std::string cache_key(const ttc_plan_s* p) {
+    std::string k;
+    k.append((const char*)&p->dtype, sizeof(p->dtype));
+    k.append((const char*)&p->canon.rank, sizeof(int));
+    k.append((const char*)p->canon.d, sizeof(CanonDim) * p->canon.rank);
+    k.append((const char*)&p->sm_count, sizeof(int));
+    return k;
+}
+
+int env_int(const char* name, int dflt) {
+    const char* v = std::getenv(name);
+    if (!v || !*v) return dflt;
+    return std::atoi(v);
+}
+
+bool is_zero(ttc_dtype dt, const void* s) {
+    switch (dt) {
+        case TTC_F32: return *(const float*)s == 0.0f;
+        case TTC_F64: return *(const double*)s == 0.0;
+        case TTC_C64: return ((const float*)s)[0] == 0.0f && ((const float*)s)[1] == 0.0f;
+        default: return ((const double*)s)[0] == 0.0 && ((const double*)s)[1] == 0.0;
+    }
+}
+
+Scalar to_scalar(ttc_dtype dt, const void* s) {
+    switch (dt) {
+        case TTC_F32: return Scalar{(double)*(const float*)s, 0.0};
+        case TTC_F64: return Scalar{*(const double*)s, 0.0};
+        case TTC_C64: return Scalar{(double)((const float*)s)[0], (double)((const float*)s)[1]};
+        default: return Scalar{((const double*)s)[0], ((const double*)s)[1]};
+    }
+}
+
+// Make candidate `idx` launchable (shared-memory opt-in, occupancy-derived persistent grid).
+bool ensure_prepared(ttc_plan_s* p, int which, int idx) {
+    Candidate& c = p->cands[which][idx];
+    if (c.info.grid > 0) return true;
+    return prepare_candidate(&c, p->dtype, p->sm_count) == 0 && c.info.grid > 0;
+}
+
+ttc_status tune(ttc_plan_s* p, int top_k, int reps) {
+    if (!p->have_device) return TTC_ERR_CUDA;
+    if (p->canon.empty) return TTC_OK;
+    const size_t es = (size_t)elem_size(p->dtype);
+    void *a = nullptr, *b = nullptr;
+    if (cudaMalloc(&a, (size_t)p->canon.spanA * es) != cudaSuccess) { cudaGetLastError(); return TTC_ERR_ALLOC; }
+    if (cudaMalloc(&b, (size_t)p->canon.spanB * es) != cudaSuccess) { cudaGetLastError(); cudaFree(a); return TTC_ERR_ALLOC; }
+    cudaStream_t st;
+    cudaEvent_t e0, e1;
+    cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    cudaMemsetAsync(a, 0, (size_t)p->canon.spanA * es, st);
+    cudaMemsetAsync(b, 0, (size_t)p->canon.spanB * es, st);
+    const Scalar alpha{1.0, 0.0};
+    ttc_status rc = TTC_OK;
+    if (reps < 1) reps = 3;
+    for (int which = 0; which < 2; ++which) {
+        const Scalar beta{which ? 1.0 : 0.0, 0.0};
+        std::vector<Candidate>& cs = p->cands[which];
+        const int n = top_k <= 0 ? (int)cs.size() : std::min<int>(top_k, (int)cs.size());
+        int best = -1;
+        float best_us = 0.f;
+        for (int i = 0; i < (int)cs.size(); ++i) {
+            // the scalar fallback is always timed so that it is known to work
+            if (i >= n && i != p->scalar[which]) continue;
+            if (!ensure_prepared(p, which, i)) continue;
+            if (launch_candidate(cs[i], p->dtype, alpha, beta, a, b, st) != 0) { cudaGetLastError(); continue; }
+            float us = 1e30f;
+            bool ok = true;
+            for (int g = 0; g < 3 && ok; ++g) {   // minimum over groups (min of 3 runs)
+                cudaEventRecord(e0, st);
+                for (int r = 0; r < reps; ++r) ok &= launch_candidate(cs[i], p->dtype, alpha, beta, a, b, st) == 0;
+                cudaEventRecord(e1, st);
+                if (cudaEventSynchronize(e1) != cudaSuccess) { ok = false; break; }
+                float ms = 0.f;
+                cudaEventElapsedTime(&ms, e0, e1);
+                us = std::min(us, ms * 1000.f / reps);
+            }
+            g_launches += 1 + 3 * reps;
+            if (!ok) { cudaGetLastError(); continue; }
+            cs[i].info.tuned_us = us;
+            if (best < 0 || us < best_us) { best = i; best_us = us; }
+        }
+        if (best >= 0) p->winner[which] = best;
+    }
+    if (cudaStreamSynchronize(st) != cudaSuccess) rc = TTC_ERR_CUDA;
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaStreamDestroy(st);
+    cudaFree(a);
+    cudaFree(b);
+    if (rc == TTC_OK) p->tuned = true;
+    return rc;
+}
+
+}  // namespace
+
+extern "C" {
+
+ttc_plan_t ttc_plan(ttc_dtype dtype, int N, const int64_t* sizes, const int* perm,
+                    const int64_t* lda, const int64_t* ldb) {
+    if ((int)dtype < 0 || (int)dtype > 3) { g_last_error = TTC_ERR_INVALID_ARG; return nullptr; }
+    ttc_plan_s* p = new (std::nothrow) ttc_plan_s();
+    if (!p) { g_last_error = TTC_ERR_ALLOC; return nullptr; }
+    p->dtype = dtype;
+    p->rank = N;
+    ttc_status st = canonicalize(N, sizes, perm, lda, ldb, &p->canon);
+    if (st != TTC_OK) { delete p; g_last_error = st; return nullptr; }
+
+    int dev = 0, count = 0;
+    if (cudaGetDeviceCount(&count) == cudaSuccess && count > 0 && cudaGetDevice(&dev) == cudaSuccess) {
+        int v = 0;
+        p->have_device = true;
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) p->sm_count = v;
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) == cudaSuccess && v > 0) p->max_smem = v;
+    } else {
+        cudaGetLastError();
+    }
+
+    for (int which = 0; which < 2; ++which) {
+        generate_candidates(p->canon, dtype, which == 1, p->sm_count, p->max_smem, &p->cands[which]);
+        std::vector<Candidate>& cs = p->cands[which];
+        const int es = elem_size(dtype);
+        for (int i = 0; i < (int)cs.size(); ++i) {
+            if (cs[i].align_a == es && cs[i].align_b == es && p->scalar[which] < 0) p->scalar[which] = i;
+        }
+        p->winner[which] = cs.empty() ? -1 : 0;
+    }
+
+    if (p->have_device && !p->canon.empty && env_int("TTC_TUNE", 1) != 0) {
+        const std::string key = cache_key(p);
+        bool hit = false;
+        {
+            std::lock_guard<std::mutex> lk(g_cache_mu);
+            auto it = g_cache.find(key);
+            if (it != g_cache.end()) {
+                hit = true;
+                for (int w = 0; w < 2; ++w) {
+                    p->winner[w] = it->second.winner[w];
+                    p->cands[w][p->winner[w]].info.tuned_us = it->second.us[w];
+                }
+                p->tuned = true;
+            }
+        }
+        if (!hit && tune(p, env_int("TTC_TUNE_TOPK", 24), 3) == TTC_OK) {
+            std::lock_guard<std::mutex> lk(g_cache_mu);
+            CacheEntry e;
+            for (int w = 0; w < 2; ++w) {
+                e.winner[w] = p->winner[w];
+                e.us[w] = p->cands[w][p->winner[w]].info.tuned_us;
+            }
+            g_cache[key] = e;
+        }
+    }
+    g_last_error = TTC_OK;
+    return p;
+}
+
+ttc_status ttc_execute(ttc_plan_t p, const void* alpha, const void* A, const void* beta, void* B,
+                       void* cuda_stream) {
+    if (!p || !alpha || !beta) return TTC_ERR_INVALID_ARG;
+    if (p->canon.empty) return TTC_OK;
+    if (!A || !B) return TTC_ERR_INVALID_ARG;
+    const int es = elem_size(p->dtype);
+    const int esa = es > 8 ? 8 : es;   // complex128 only needs the alignment of its parts
+    if (((uintptr_t)A % esa) != 0 || ((uintptr_t)B % esa) != 0) return TTC_ERR_MISALIGNED;
+    if (!p->have_device) return TTC_ERR_CUDA;
+    const int which = is_zero(p->dtype, beta) ? 0 : 1;
+    int idx = p->forced[which] >= 0 ? p->forced[which] : p->winner[which];
+    if (idx < 0) return TTC_ERR_UNSUPPORTED;
+    const Candidate* c = &p->cands[which][idx];
+    if (((uintptr_t)A % c->align_a) != 0 || ((uintptr_t)B % c->align_b) != 0) {
+        idx = p->scalar[which];
+        if (idx < 0) return TTC_ERR_MISALIGNED;
+        c = &p->cands[which][idx];
+        if (((uintptr_t)A % c->align_a) != 0 || ((uintptr_t)B % c->align_b) != 0) return TTC_ERR_MISALIGNED;
+    }
+    if (!ensure_prepared(p, which, idx)) return TTC_ERR_CUDA;
+    const int rc = launch_candidate(*c, p->dtype, to_scalar(p->dtype, alpha), to_scalar(p->dtype, beta), A, B, cuda_stream);
+    g_launches += 1;
+    return rc == 0 ? TTC_OK : TTC_ERR_CUDA;
+}
+
+ttc_status ttc_execute_host(ttc_plan_t p, const void* alpha, const void* A_host, const void* beta,
+                            void* B_host, void* cuda_stream) {
+    if (!p || !alpha || !beta) return TTC_ERR_INVALID_ARG;
+    if (p->canon.empty) return TTC_OK;
+    if (!A_host || !B_host) return TTC_ERR_INVALID_ARG;
+    if (!p->have_device) return TTC_ERR_CUDA;
+    const size_t es = (size_t)elem_size(p->dtype);
+    const size_t bytes_a = (size_t)p->canon.spanA * es, bytes_b = (size_t)p->canon.spanB * es;
+    if (!p->stage_a && cudaMalloc(&p->stage_a, bytes_a) != cudaSuccess) { cudaGetLastError(); return TTC_ERR_ALLOC; }
+    if (!p->stage_b && cudaMalloc(&p->stage_b, bytes_b) != cudaSuccess) { cudaGetLastError(); return TTC_ERR_ALLOC; }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    if (cudaMemcpyAsync(p->stage_a, A_host, bytes_a, cudaMemcpyHostToDevice, st) != cudaSuccess) return TTC_ERR_CUDA;
+    // B travels to the device when it is read (beta != 0) or has padding that must survive
+    const bool b_in = !is_zero(p->dtype, beta) || p->canon.spanB != p->canon.numel;
+    if (b_in && cudaMemcpyAsync(p->stage_b, B_host, bytes_b, cudaMemcpyHostToDevice, st) != cudaSuccess) return TTC_ERR_CUDA;
+    ttc_status rc = ttc_execute(p, alpha, p->stage_a, beta, p->stage_b, cuda_stream);
+    if (rc != TTC_OK) return rc;
+    if (cudaMemcpyAsync(B_host, p->stage_b, bytes_b, cudaMemcpyDeviceToHost, st) != cudaSuccess) return TTC_ERR_CUDA;
+    if (cudaStreamSynchronize(st) != cudaSuccess) return TTC_ERR_CUDA;
+    return TTC_OK;
+}
+
+ttc_status ttc_destroy(ttc_plan_t p) {
+    if (!p) return TTC_OK;
+    if (p->stage_a) cudaFree(p->stage_a);
+    if (p->stage_b) cudaFree(p->stage_b);
+    delete p;
+    return TTC_OK;
+}
+
+ttc_status ttc_last_error(void) { return g_last_error; }
+
+const char* ttc_status_string(ttc_status s) {
+    switch (s) {
+        case TTC_OK: return "TTC_OK";
+        case TTC_ERR_INVALID_ARG: return "TTC_ERR_INVALID_ARG";
+        case TTC_ERR_NOT_PERMUTATION: return "TTC_ERR_NOT_PERMUTATION";
+        case TTC_ERR_BAD_LD: return "TTC_ERR_BAD_LD";
+        case TTC_ERR_UNSUPPORTED: return "TTC_ERR_UNSUPPORTED";
+        case TTC_ERR_ALLOC: return "TTC_ERR_ALLOC";
+        case TTC_ERR_CUDA: return "TTC_ERR_CUDA";
+        case TTC_ERR_MISALIGNED: return "TTC_ERR_MISALIGNED";
+    }
+    return "TTC_ERR_UNKNOWN";
+}
+
+ttc_status ttc_plan_info(ttc_plan_t p, ttc_info* out) {
+    if (!p || !out) return TTC_ERR_INVALID_ARG;
+    std::memset(out, 0, sizeof(*out));
+    out->dtype = (int)p->dtype;
+    out->rank = p->rank;
+    out->canon_rank = p->canon.rank;
+    for (int i = 0; i < p->canon.rank; ++i) {
+        out->canon_extent[i] = p->canon.d[i].e;
+        out->canon_stride_a[i] = p->canon.d[i].sA;
+        out->canon_stride_b[i] = p->canon.d[i].sB;
+    }
+    out->numel = p->canon.numel;
+    out->span_a = p->canon.spanA;
+    out->span_b = p->canon.spanB;
+    out->tuned = p->tuned ? 1 : 0;
+    for (int w = 0; w < 2; ++w) {
+        out->n_candidates[w] = (int)p->cands[w].size();
+        const int idx = p->forced[w] >= 0 ? p->forced[w] : p->winner[w];
+        out->chosen[w] = idx;
+        out->chosen_us[w] = idx >= 0 ? p->cands[w][idx].info.tuned_us : 0.f;
+    }
+    return TTC_OK;
+}
+
+int ttc_plan_num_candidates(ttc_plan_t p, int which) {
+    if (!p || which < 0 || which > 1) return -1;
+    return (int)p->cands[which].size();
+}
+
+ttc_status ttc_plan_candidate(ttc_plan_t p, int which, int index, ttc_candidate_info* out) {
+    if (!p || !out || which < 0 || which > 1) return TTC_ERR_INVALID_ARG;
+    if (index < 0 || index >= (int)p->cands[which].size()) return TTC_ERR_INVALID_ARG;
+    *out = p->cands[which][index].info;
+    return TTC_OK;
+}
+
+ttc_status ttc_plan_select(ttc_plan_t p, int which, int index) {
+    if (!p || which < 0 || which > 1) return TTC_ERR_INVALID_ARG;
+    if (index < -1 || index >= (int)p->cands[which].size()) return TTC_ERR_INVALID_ARG;
+    p->forced[which] = index;
+    return TTC_OK;
+}
+
+ttc_status ttc_plan_tune(ttc_plan_t p, int top_k, int reps) {
+    if (!p) return TTC_ERR_INVALID_ARG;
+    return tune(p, top_k, reps);
+}
+
+int ttc_canonicalize(int N, const int64_t* sizes, const int* perm, const int64_t* lda,
+                     const int64_t* ldb, int64_t* extent_out, int64_t* stride_a_out, int64_t* stride_b_out) {
+    Canon c;
+    if (!extent_out || !stride_a_out || !stride_b_out) { g_last_error = TTC_ERR_INVALID_ARG; return -1; }
+    ttc_status st = canonicalize(N, sizes, perm, lda, ldb, &c);
+    g_last_error = st;
+    if (st != TTC_OK) return -1;
+    for (int i = 0; i < c.rank; ++i) {
+        extent_out[i] = c.d[i].e;
+        stride_a_out[i] = c.d[i].sA;
+        stride_b_out[i] = c.d[i].sB;
+    }
+    return c.rank;
+}
+
+int64_t ttc_launch_count(void) { return g_launches.load(); }
+
+uint32_t ttc_debug_fastdiv(uint32_t n, uint32_t d) { return fd_div(n, make_fastdiv(d)); }
+
+const char* ttc_version(void) { return "ttc-b200 0.1 (sm_100a)"; }
+
+}  // extern "C"

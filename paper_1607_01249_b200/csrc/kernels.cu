@@ -1,0 +1,416 @@
+// kernels.cu -- the sm_100a kernels of libttc.so and their launchers.
+//
+//   direct_kernel  K1 of SURVEY.md 8(a): global -> global, one 4..16-byte vector per item along
+//                  the index that is stride-1 in A and in B ("copy a whole column
+//                  at a time"); also the always-valid scalar fallback for any strides.
+//   tile_kernel    K2/K3: one macro-tile per CTA iteration, staged through
+//                  shared memory (the micro-tile transpose is done in shared memory
+//                  on CUDA).  The tile is an N-D box, so several small leading indices can be
+//                  coarsened into each side; 16-byte global accesses on both sides; the read of
+//                  B for beta != 0 is fused into the store phase; persistent grid-stride loop
+//                  over macro-tiles in the candidate's loop order.
+//
+// Arithmetic (Eq. 1): every product and sum is rounded separately
+// (__fmul_rn/__fadd_rn, never contracted into FMA) so the result is bit-identical to the
+// definition evaluated in the tensor's own precision (reading A7).
+#include <cuda_runtime.h>
+
+#include <cstdio>
+
+#include "ttc_internal.h"
+
+namespace ttc {
+
+// ------------------------------------------------------------------------------------------
+// Element types and axpby
+// ------------------------------------------------------------------------------------------
+template <int DT> struct ElemT;
+template <> struct ElemT<TTC_F32>  { using T = float;   static constexpr int ES = 4; };
+template <> struct ElemT<TTC_F64>  { using T = double;  static constexpr int ES = 8; };
+template <> struct ElemT<TTC_C64>  { using T = float2;  static constexpr int ES = 8; };
+template <> struct ElemT<TTC_C128> { using T = double2; static constexpr int ES = 16; };
+
+__device__ __forceinline__ float scale(const Scalar& s, float a) { return __fmul_rn((float)s.re, a); }
+__device__ __forceinline__ double scale(const Scalar& s, double a) { return __dmul_rn(s.re, a); }
+__device__ __forceinline__ float2 scale(const Scalar& s, float2 a) {
+    const float sr = (float)s.re, si = (float)s.im;
+    return make_float2(__fsub_rn(__fmul_rn(sr, a.x), __fmul_rn(si, a.y)),
+                       __fadd_rn(__fmul_rn(sr, a.y), __fmul_rn(si, a.x)));
+}
+__device__ __forceinline__ double2 scale(const Scalar& s, double2 a) {
+    return make_double2(__dsub_rn(__dmul_rn(s.re, a.x), __dmul_rn(s.im, a.y)),
+                        __dadd_rn(__dmul_rn(s.re, a.y), __dmul_rn(s.im, a.x)));
+}
+__device__ __forceinline__ float add(float a, float b) { return __fadd_rn(a, b); }
+__device__ __forceinline__ double add(double a, double b) { return __dadd_rn(a, b); }
+__device__ __forceinline__ float2 add(float2 a, float2 b) { return make_float2(__fadd_rn(a.x, b.x), __fadd_rn(a.y, b.y)); }
+__device__ __forceinline__ double2 add(double2 a, double2 b) { return make_double2(__dadd_rn(a.x, b.x), __dadd_rn(a.y, b.y)); }
+
+// A vector of V elements moved as one 4/8/16-byte access.
+template <int BYTES> struct RawT;
+template <> struct RawT<4>  { using T = uint32_t; };
+template <> struct RawT<8>  { using T = uint2; };
+template <> struct RawT<16> { using T = uint4; };
+
+template <typename T, int V>
+union Pack {
+    typename RawT<sizeof(T) * V>::T raw;
+    T e[V];
+    __device__ Pack() {}
+};
+
+template <typename R> __device__ __forceinline__ R ld_stream(const void* p) {
+    return __ldcs(reinterpret_cast<const R*>(p));    // read once: evict-first
+}
+template <typename R> __device__ __forceinline__ R ld_plain(const void* p) {
+    return *reinterpret_cast<const R*>(p);
+}
+template <typename R> __device__ __forceinline__ void st_global(void* p, const R& v) {
+    *reinterpret_cast<R*>(p) = v;
+}
+
+// ------------------------------------------------------------------------------------------
+// K1: direct kernel
+// ------------------------------------------------------------------------------------------
+constexpr int kDirectThreads = 256;
+constexpr int kDirectUnroll = 4;
+
+template <int DT, int V, bool BETA, bool IDX64>
+__global__ void __launch_bounds__(kDirectThreads)
+direct_kernel(const __grid_constant__ DirectParams P, const void* __restrict__ Ain, void* __restrict__ Bout,
+              const Scalar alpha, const Scalar beta) {
+    using T = typename ElemT<DT>::T;
+    using PackT = Pack<T, V>;
+    using Raw = typename RawT<sizeof(T) * V>::T;
+    using idx_t = typename std::conditional<IDX64, uint64_t, uint32_t>::type;
+    const char* A = static_cast<const char*>(Ain);
+    char* B = static_cast<char*>(Bout);
+    const idx_t n = (idx_t)P.n_items;
+    const idx_t stride = (idx_t)gridDim.x * blockDim.x;
+    const idx_t first = (idx_t)blockIdx.x * blockDim.x + threadIdx.x;
+    // chunks of kDirectUnroll * stride items; inside a chunk thread handles first + k*stride
+    for (idx_t base = 0; base < n; base += stride * kDirectUnroll) {
+        PackT a[kDirectUnroll], b[kDirectUnroll];
+        int64_t ob[kDirectUnroll];
+        bool ok[kDirectUnroll];
+#pragma unroll
+        for (int k = 0; k < kDirectUnroll; ++k) {
+            const idx_t q = base + first + (idx_t)k * stride;
+            ok[k] = q < n && q >= base;   // q >= base guards 32-bit wrap-around
+            if (ok[k]) {
+                int64_t oa = 0;
+                ob[k] = 0;
+                idx_t r = q;
+#pragma unroll 1
+                for (int d = 0; d < P.nd; ++d) {
+                    idx_t c;
+                    if (IDX64) {
+                        const idx_t nn = (idx_t)P.dims[d].n;
+                        const idx_t qq = r / nn;
+                        c = r - qq * nn;
+                        r = qq;
+                    } else {
+                        const uint32_t qq = fd_div((uint32_t)r, P.dims[d].div);
+                        c = (uint32_t)r - qq * P.dims[d].div.d;
+                        r = qq;
+                    }
+                    oa += (int64_t)c * P.dims[d].sA;
+                    ob[k] += (int64_t)c * P.dims[d].sB;
+                }
+                a[k].raw = ld_stream<Raw>(A + oa * (int64_t)sizeof(T));
+                if (BETA) b[k].raw = ld_plain<Raw>(B + ob[k] * (int64_t)sizeof(T));
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < kDirectUnroll; ++k) {
+            if (ok[k]) {
+                PackT o;
+#pragma unroll
+                for (int j = 0; j < V; ++j) {
+                    T x = scale(alpha, a[k].e[j]);
+                    if (BETA) x = add(x, scale(beta, b[k].e[j]));
+                    o.e[j] = x;
+                }
+                st_global<Raw>(B + ob[k] * (int64_t)sizeof(T), o.raw);
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// K2/K3: tile kernel
+// ------------------------------------------------------------------------------------------
+constexpr int kTileUnroll = 4;
+
+template <int DT, int VA, int VB, bool SAME, bool BETA>
+__global__ void __launch_bounds__(kTileThreads)
+tile_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, void* __restrict__ Bout,
+            const Scalar alpha, const Scalar beta) {
+    using T = typename ElemT<DT>::T;
+    constexpr int ES = (int)sizeof(T);
+    using RawA = typename RawT<ES * VA>::T;
+    using RawB = typename RawT<ES * VB>::T;
+    extern __shared__ __align__(16) unsigned char smem[];
+    const TileSmemLayout L = tile_smem_layout(P, ES);
+    int2* tabs[4];
+    uint8_t* vals[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        tabs[i] = reinterpret_cast<int2*>(smem + L.tab[i]);
+        vals[i] = smem + L.val[i];
+    }
+    int32_t* vext = reinterpret_cast<int32_t*>(smem + L.vext);
+    unsigned char* tile = smem + L.tile;
+    const int tid = threadIdx.x;
+    const int NT = blockDim.x;
+    const char* A = static_cast<const char*>(Ain);
+    char* B = static_cast<char*>(Bout);
+
+    // Offset tables: entry -> (global element offset, tile element offset), once per CTA.
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const Table& tb = P.tab[i];
+        for (int idx = tid; idx < tb.n; idx += NT) {
+            uint32_t r = (uint32_t)idx;
+            int32_t g = 0, s = 0;
+#pragma unroll 1
+            for (int k = 0; k < tb.nd; ++k) {
+                const uint32_t qq = fd_div(r, tb.d[k].div);
+                const uint32_t c = r - qq * tb.d[k].div.d;
+                r = qq;
+                g += (int32_t)c * (int32_t)tb.d[k].sG;
+                s += (int32_t)c * tb.d[k].sS;
+            }
+            tabs[i][idx] = make_int2(g, s);
+        }
+    }
+    __syncthreads();
+
+    for (uint32_t tile_id = blockIdx.x; tile_id < P.n_tiles; tile_id += gridDim.x) {
+        // macro-tile id -> tile coordinates in the candidate's loop order
+        int64_t baseA = 0, baseB = 0;
+        bool edge = false;
+        {
+            uint32_t r = tile_id;
+#pragma unroll 1
+            for (int g = 0; g < P.nG; ++g) {
+                const uint32_t qq = fd_div(r, P.g[g].div);
+                const uint32_t c = r - qq * P.g[g].div.d;
+                r = qq;
+                const int32_t start = (int32_t)c * P.g[g].t;
+                baseA += (int64_t)start * P.g[g].sA;
+                baseB += (int64_t)start * P.g[g].sB;
+                const int32_t left = P.g[g].e - start;
+                edge |= left < P.g[g].t;
+                if (tid == 0) vext[g] = left < P.g[g].t ? left : P.g[g].t;
+            }
+        }
+        if (edge) {  // remainder tile: mark which table entries are inside the tensor
+            __syncthreads();
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const Table& tb = P.tab[i];
+                for (int idx = tid; idx < tb.n; idx += NT) {
+                    uint32_t r = (uint32_t)idx;
+                    bool ok = true;
+#pragma unroll 1
+                    for (int k = 0; k < tb.nd; ++k) {
+                        const uint32_t qq = fd_div(r, tb.d[k].div);
+                        const uint32_t c = r - qq * tb.d[k].div.d;
+                        r = qq;
+                        ok &= (int32_t)c * tb.d[k].step < vext[tb.d[k].gslot];
+                    }
+                    vals[i][idx] = ok ? 1 : 0;
+                }
+            }
+            __syncthreads();
+        }
+
+        // ---- load phase: A -> tile, enumerated in ascending A-stride --------------------
+        const char* Ab = A + baseA * ES;
+        for (uint32_t q0 = tid; q0 < P.itemsA; q0 += NT * kTileUnroll) {
+            RawA v[kTileUnroll];
+            int32_t so[kTileUnroll];
+            bool ok[kTileUnroll];
+#pragma unroll
+            for (int k = 0; k < kTileUnroll; ++k) {
+                const uint32_t q = q0 + k * NT;
+                ok[k] = q < P.itemsA;
+                if (ok[k]) {
+                    const uint32_t hi = fd_div(q, P.divAlo);
+                    const uint32_t lo = q - hi * P.divAlo.d;
+                    const int2 el = tabs[0][lo], eh = tabs[1][hi];
+                    if (edge) ok[k] = vals[0][lo] & vals[1][hi];
+                    so[k] = el.y + eh.y;
+                    if (ok[k]) v[k] = ld_stream<RawA>(Ab + (int64_t)(el.x + eh.x) * ES);
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < kTileUnroll; ++k)
+                if (ok[k]) *reinterpret_cast<RawA*>(tile + so[k] * ES) = v[k];
+        }
+        __syncthreads();
+
+        // ---- store phase: tile -> B, enumerated in ascending B-stride -------------------
+        char* Bb = B + baseB * ES;
+        for (uint32_t p0 = tid; p0 < P.itemsB; p0 += NT * kTileUnroll) {
+            Pack<T, VB> bv[kTileUnroll];
+            int32_t so[kTileUnroll], go[kTileUnroll];
+            bool ok[kTileUnroll];
+#pragma unroll
+            for (int k = 0; k < kTileUnroll; ++k) {
+                const uint32_t p = p0 + k * NT;
+                ok[k] = p < P.itemsB;
+                if (ok[k]) {
+                    const uint32_t hi = fd_div(p, P.divBlo);
+                    const uint32_t lo = p - hi * P.divBlo.d;
+                    const int2 el = tabs[2][lo], eh = tabs[3][hi];
+                    if (edge) ok[k] = vals[2][lo] & vals[3][hi];
+                    so[k] = el.y + eh.y;
+                    go[k] = el.x + eh.x;
+                    if (BETA && ok[k]) bv[k].raw = ld_plain<RawB>(Bb + (int64_t)go[k] * ES);
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < kTileUnroll; ++k) {
+                if (ok[k]) {
+                    Pack<T, VB> a, o;
+                    if (SAME || VB == 1) {
+                        a.raw = *reinterpret_cast<const RawB*>(tile + so[k] * ES);
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < VB; ++j)
+                            a.e[j] = *reinterpret_cast<const T*>(tile + (so[k] + j * P.sstepB) * ES);
+                    }
+#pragma unroll
+                    for (int j = 0; j < VB; ++j) {
+                        T x = scale(alpha, a.e[j]);
+                        if (BETA) x = add(x, scale(beta, bv[k].e[j]));
+                        o.e[j] = x;
+                    }
+                    st_global<RawB>(Bb + (int64_t)go[k] * ES, o.raw);
+                }
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Dispatch: (dtype, vector widths, beta != 0) -> kernel instance
+// ------------------------------------------------------------------------------------------
+using TileFn = void (*)(const TileParams, const void*, void*, const Scalar, const Scalar);
+using DirectFn = void (*)(const DirectParams, const void*, void*, const Scalar, const Scalar);
+
+template <int DT, int VA, int VB, bool SAME>
+static TileFn tile_fn_beta(bool beta) {
+    return beta ? (TileFn)tile_kernel<DT, VA, VB, SAME, true> : (TileFn)tile_kernel<DT, VA, VB, SAME, false>;
+}
+
+template <int DT>
+static TileFn tile_fn(int va, int vb, bool same, bool beta) {
+    constexpr int MV = 16 / ElemT<DT>::ES;   // elements per 16-byte access
+    if constexpr (MV > 1) {
+        if (same && va == MV && vb == MV) return tile_fn_beta<DT, MV, MV, true>(beta);
+        if (same) return nullptr;
+        if (va == MV && vb == MV) return tile_fn_beta<DT, MV, MV, false>(beta);
+        if (va == MV && vb == 1) return tile_fn_beta<DT, MV, 1, false>(beta);
+        if (va == 1 && vb == MV) return tile_fn_beta<DT, 1, MV, false>(beta);
+    }
+    if (va == 1 && vb == 1) return tile_fn_beta<DT, 1, 1, false>(beta);
+    return nullptr;
+}
+
+template <int DT, int V>
+static DirectFn direct_fn_v(bool beta, bool idx64) {
+    if (beta) return idx64 ? (DirectFn)direct_kernel<DT, V, true, true> : (DirectFn)direct_kernel<DT, V, true, false>;
+    return idx64 ? (DirectFn)direct_kernel<DT, V, false, true> : (DirectFn)direct_kernel<DT, V, false, false>;
+}
+
+template <int DT>
+static DirectFn direct_fn(int vec, bool beta, bool idx64) {
+    constexpr int MV = 16 / ElemT<DT>::ES;
+    if constexpr (MV > 1) {
+        if (vec == MV) return direct_fn_v<DT, MV>(beta, idx64);
+    }
+    if (vec == 1) return direct_fn_v<DT, 1>(beta, idx64);
+    return nullptr;
+}
+
+static TileFn get_tile_fn(ttc_dtype dt, const Candidate& c) {
+    const TileParams& p = c.tp;
+    switch (dt) {
+        case TTC_F32: return tile_fn<TTC_F32>(p.vecA, p.vecB, p.same != 0, c.beta_nz);
+        case TTC_F64: return tile_fn<TTC_F64>(p.vecA, p.vecB, p.same != 0, c.beta_nz);
+        case TTC_C64: return tile_fn<TTC_C64>(p.vecA, p.vecB, p.same != 0, c.beta_nz);
+        case TTC_C128: return tile_fn<TTC_C128>(p.vecA, p.vecB, p.same != 0, c.beta_nz);
+    }
+    return nullptr;
+}
+
+static DirectFn get_direct_fn(ttc_dtype dt, const Candidate& c) {
+    switch (dt) {
+        case TTC_F32: return direct_fn<TTC_F32>(c.dp.vec, c.beta_nz, c.idx64);
+        case TTC_F64: return direct_fn<TTC_F64>(c.dp.vec, c.beta_nz, c.idx64);
+        case TTC_C64: return direct_fn<TTC_C64>(c.dp.vec, c.beta_nz, c.idx64);
+        case TTC_C128: return direct_fn<TTC_C128>(c.dp.vec, c.beta_nz, c.idx64);
+    }
+    return nullptr;
+}
+
+int prepare_candidate(Candidate* cand, ttc_dtype dtype, int sm_count) {
+    if (cand->info.kernel == TTC_KERNEL_COPY) {
+        DirectFn fn = get_direct_fn(dtype, *cand);
+        if (!fn) return (int)cudaErrorInvalidValue;
+        int occ = 0;
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kDirectThreads, 0);
+        if (e != cudaSuccess) return (int)e;
+        if (occ < 1) occ = 1;
+        const uint64_t per_cta = (uint64_t)kDirectThreads * kDirectUnroll;
+        uint64_t need = (cand->dp.n_items + per_cta - 1) / per_cta;
+        uint64_t cap = (uint64_t)sm_count * (uint64_t)occ;
+        cand->info.threads = kDirectThreads;
+        cand->info.smem_bytes = 0;
+        cand->info.grid = (int)(need < cap ? (need ? need : 1) : cap);
+        return 0;
+    }
+    TileFn fn = get_tile_fn(dtype, *cand);
+    if (!fn) return (int)cudaErrorInvalidValue;
+    const int smem = (int)tile_smem_layout(cand->tp, elem_size(dtype)).total;
+    // The attribute belongs to the kernel function, which many candidates share: raise it once
+    // to the device's opt-in maximum instead of per candidate.
+    int dev = 0, optin = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    if (e != cudaSuccess) return (int)e;
+    if (smem > optin) return (int)cudaErrorInvalidConfiguration;
+    e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+    if (e != cudaSuccess) return (int)e;
+    int occ = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, cand->tp.threads, smem);
+    if (e != cudaSuccess) return (int)e;
+    if (occ < 1) return (int)cudaErrorInvalidConfiguration;
+    const uint64_t cap = (uint64_t)sm_count * (uint64_t)occ;
+    cand->info.threads = cand->tp.threads;
+    cand->info.smem_bytes = smem;
+    cand->info.grid = (int)(cand->tp.n_tiles < cap ? cand->tp.n_tiles : cap);
+    return 0;
+}
+
+int launch_candidate(const Candidate& cand, ttc_dtype dtype, const Scalar& alpha, const Scalar& beta,
+                     const void* A, void* B, void* stream) {
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (cand.info.grid <= 0) return (int)cudaErrorInvalidConfiguration;
+    if (cand.info.kernel == TTC_KERNEL_COPY) {
+        DirectFn fn = get_direct_fn(dtype, cand);
+        if (!fn) return (int)cudaErrorInvalidValue;
+        fn<<<cand.info.grid, kDirectThreads, 0, st>>>(cand.dp, A, B, alpha, beta);
+    } else {
+        TileFn fn = get_tile_fn(dtype, cand);
+        if (!fn) return (int)cudaErrorInvalidValue;
+        fn<<<cand.info.grid, cand.tp.threads, cand.info.smem_bytes, st>>>(cand.tp, A, B, alpha, beta);
+    }
+    return (int)cudaGetLastError();   // launch-configuration errors only; clears them
+}
+
+}  // namespace ttc

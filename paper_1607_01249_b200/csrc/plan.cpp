@@ -1,0 +1,524 @@
+// plan.cpp -- stages 2-3 of the paper's pipeline: enumerate candidate
+// implementations (kernel class x blocking x loop order x vector width), estimate their cost
+// with heuristics and keep a bounded, ranked list.  Host only; timing happens in api.cpp.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <set>
+#include <string>
+
+#include "ttc_internal.h"
+
+namespace ttc {
+
+namespace {
+
+constexpr int kMaxImplementations = 200;   // the paper's default bound
+constexpr int64_t kInt31 = (int64_t)1 << 31;
+
+struct TileSpec {
+    int32_t t[kMaxRank];   // tile extent per canonical index (1 = outside the tile)
+};
+
+// ----------------------------------------------------------------------------------------
+// Shared-memory bank model: wavefronts needed by one warp-wide access of `sz` bytes per lane
+// at byte addresses addr[0..n) (32 banks x 4 bytes; 8-byte accesses are served per half-warp,
+// 16-byte accesses per quarter-warp; lanes reading the same word are broadcast).
+// ----------------------------------------------------------------------------------------
+int smem_wavefronts(const int64_t* addr, int n, int sz) {
+    const int lanes_per_group = sz <= 4 ? 32 : (sz == 8 ? 16 : 8);
+    int total = 0;
+    for (int g0 = 0; g0 < n; g0 += lanes_per_group) {
+        int64_t words[32 * 4];
+        int nw = 0;
+        for (int l = g0; l < std::min(n, g0 + lanes_per_group); ++l)
+            for (int w = 0; w < std::max(1, sz / 4); ++w) words[nw++] = addr[l] / 4 + w;
+        std::sort(words, words + nw);
+        nw = (int)(std::unique(words, words + nw) - words);
+        int per_bank[32] = {0};
+        int worst = 0;
+        for (int i = 0; i < nw; ++i) worst = std::max(worst, ++per_bank[words[i] & 31]);
+        total += worst;
+    }
+    return total;
+}
+
+struct PhaseDim { int dim; int32_t n, step; };
+
+// Enumerate entry `idx` of a phase (dims fastest first) and return its tile offset in elements.
+int64_t phase_smem_offset(const std::vector<PhaseDim>& ph, const int32_t* ss, int64_t idx) {
+    int64_t s = 0;
+    for (const PhaseDim& p : ph) {
+        const int64_t c = idx % p.n;
+        idx /= p.n;
+        s += c * p.step * ss[p.dim];
+    }
+    return s;
+}
+
+// Relative smem cost (>= 1) of both phases for the given tile strides.
+double smem_conflict_cost(const std::vector<PhaseDim>& phA, const std::vector<PhaseDim>& phB,
+                          const int32_t* ss, int es, int vecA, int vecB, bool same, int sstepB,
+                          int64_t itemsA, int64_t itemsB) {
+    double got = 0, ideal = 0;
+    const int warps = 8;
+    int64_t addr[32];
+    for (int w = 0; w < warps; ++w) {
+        // spread the sampled warps over the tile
+        const int64_t startA = (itemsA / 32) * w / warps * 32;
+        int n = 0;
+        for (int l = 0; l < 32 && startA + l < itemsA; ++l) addr[n++] = phase_smem_offset(phA, ss, startA + l) * es;
+        if (n) {
+            got += smem_wavefronts(addr, n, es * vecA);
+            ideal += std::max(1.0, n * es * vecA / 128.0);
+        }
+        const int64_t startB = (itemsB / 32) * w / warps * 32;
+        n = 0;
+        for (int l = 0; l < 32 && startB + l < itemsB; ++l) addr[n++] = phase_smem_offset(phB, ss, startB + l) * es;
+        if (n) {
+            if (same || vecB == 1) {
+                got += smem_wavefronts(addr, n, es * vecB);
+                ideal += std::max(1.0, n * es * vecB / 128.0);
+            } else {
+                for (int j = 0; j < vecB; ++j) {
+                    int64_t a2[32];
+                    for (int l = 0; l < n; ++l) a2[l] = addr[l] + (int64_t)j * sstepB * es;
+                    got += smem_wavefronts(a2, n, es);
+                    ideal += std::max(1.0, n * es / 128.0);
+                }
+            }
+        }
+    }
+    return ideal > 0 ? got / ideal : 1.0;
+}
+
+// Efficiency model of a contiguous run of `bytes` in global memory (sector / DRAM-page use).
+double run_eff(double bytes) {
+    if (bytes >= 4096) return 1.0;
+    return bytes / (bytes + 48.0) / (4096.0 / (4096.0 + 48.0));
+}
+
+bool split_tables(const std::vector<PhaseDim>& ph, int* split_out) {
+    // lo = ph[0..k), hi = ph[k..): both <= kMaxTabEntries entries and <= kMaxTab dims;
+    // choose k that minimises lo.n + hi.n.
+    const int n = (int)ph.size();
+    int best = -1;
+    int64_t best_sum = 0;
+    for (int k = 1; k <= n; ++k) {
+        int64_t lo = 1, hi = 1;
+        for (int i = 0; i < k; ++i) lo *= ph[i].n;
+        for (int i = k; i < n; ++i) hi *= ph[i].n;
+        if (k > kMaxTab || n - k > kMaxTab) continue;
+        if (lo > kMaxTabEntries || hi > kMaxTabEntries) continue;
+        if (best < 0 || lo + hi < best_sum) { best = k; best_sum = lo + hi; }
+    }
+    *split_out = best;
+    return best >= 0;
+}
+
+}  // namespace
+
+namespace {
+
+// Largest vector (in elements) legal for global accesses along canonical index `lead` of
+// tensor X (strideOf gives that tensor's strides): the index is stride-1, its extent and
+// tile extent are multiples of the vector, and every other stride keeps 16-byte alignment.
+int legal_vec(const Canon& c, int lead, bool sideA, int32_t t_lead, int mv) {
+    if (mv <= 1) return 1;
+    const int64_t s = sideA ? c.d[lead].sA : c.d[lead].sB;
+    if (s != 1) return 1;
+    if (c.d[lead].e % mv != 0 || t_lead % mv != 0) return 1;
+    for (int i = 0; i < c.rank; ++i) {
+        if (i == lead) continue;
+        const int64_t si = sideA ? c.d[i].sA : c.d[i].sB;
+        if (si % mv != 0) return 1;
+    }
+    return mv;
+}
+
+// Build one tile-kernel candidate.  Returns false if the combination is not legal.
+bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const TileSpec& spec,
+                          int loop_order, int want_va, int want_vb, int max_smem, Candidate* out) {
+    const int es = elem_size(dtype);
+    const int mv = 16 / es;
+    Candidate cand;
+    cand.beta_nz = beta_nz;
+    TileParams& P = cand.tp;
+    std::memset(&P, 0, sizeof(P));
+
+    std::vector<int> ta, tb;   // tile indices by ascending A-stride / B-stride
+    for (int i = 0; i < c.rank; ++i)
+        if (spec.t[i] > 1) ta.push_back(i);
+    for (int k = 0; k < c.rank; ++k)
+        if (spec.t[c.orderB[k]] > 1) tb.push_back(c.orderB[k]);
+    if (ta.empty()) return false;
+    const int A0 = ta[0], B0 = tb[0];
+    const int va = legal_vec(c, A0, true, spec.t[A0], mv);
+    const int vb = legal_vec(c, B0, false, spec.t[B0], mv);
+    if (want_va > va || want_vb > vb) return false;
+    const bool same = (A0 == B0) && want_va == mv && want_vb == mv && mv > 1;
+    if (A0 == B0 && want_va != want_vb) return false;   // nothing gained by mixing widths on one index
+    P.vecA = want_va;
+    P.vecB = want_vb;
+    P.same = same ? 1 : 0;
+    P.threads = kTileThreads;
+
+    // Phase enumerations (entries along the vectorised leading index count vectors).
+    std::vector<PhaseDim> phA, phB;
+    for (int i : ta) phA.push_back(PhaseDim{i, spec.t[i] / (i == A0 ? want_va : 1), i == A0 ? want_va : 1});
+    for (int i : tb) phB.push_back(PhaseDim{i, spec.t[i] / (i == B0 ? want_vb : 1), i == B0 ? want_vb : 1});
+    int64_t itemsA = 1, itemsB = 1;
+    for (auto& p : phA) itemsA *= p.n;
+    for (auto& p : phB) itemsB *= p.n;
+    int splitA, splitB;
+    if (!split_tables(phA, &splitA) || !split_tables(phB, &splitB)) return false;
+
+    // Shared-memory strides: dense in A order, padded (in units that keep vector alignment)
+    // where the bank model says the store phase would conflict.
+    const int unit = std::max(want_va, same ? mv : 1);
+    int32_t ss[kMaxRank];
+    int32_t best_ss[kMaxRank];
+    double best_cost = 1e30;
+    int64_t best_elems = 0;
+    const int levels = (int)ta.size() - 1;
+    const int search_levels = std::min(levels, 3);
+    static const int pad_opts[] = {0, 1, 2, 3, 4};
+    const int n_opts = 5;
+    int combos = 1;
+    for (int i = 0; i < search_levels; ++i) combos *= n_opts;
+    for (int combo = 0; combo < combos; ++combo) {
+        int cc = combo;
+        int64_t stride = 1;
+        bool ok = true;
+        for (int i = 0; i < c.rank; ++i) ss[i] = 0;
+        for (size_t k = 0; k < ta.size(); ++k) {
+            if (k > 0) {
+                int pad = 0;
+                if ((int)k <= search_levels) { pad = pad_opts[cc % n_opts] * unit; cc /= n_opts; }
+                stride = stride * spec.t[ta[k - 1]];
+                stride = (stride + unit - 1) / unit * unit + pad;
+            }
+            if (stride >= kInt31) { ok = false; break; }
+            ss[ta[k]] = (int32_t)stride;
+        }
+        if (!ok) continue;
+        const int64_t elems = (int64_t)ss[ta.back()] * spec.t[ta.back()];
+        if (elems * es > max_smem) continue;
+        const double conf = smem_conflict_cost(phA, phB, ss, es, want_va, want_vb, same, ss[B0], itemsA, itemsB);
+        const double cost = conf + 1e-3 * (double)elems * es / 1024.0;
+        if (cost < best_cost) {
+            best_cost = cost;
+            best_elems = elems;
+            std::memcpy(best_ss, ss, sizeof(ss));
+        }
+    }
+    if (best_cost >= 1e30) return false;
+    std::memcpy(ss, best_ss, sizeof(ss));
+    P.tile_elems = (uint32_t)best_elems;
+    P.sstepB = ss[B0];
+    P.itemsA = (uint32_t)itemsA;
+    P.itemsB = (uint32_t)itemsB;
+
+    // Macro-tile grid in loop order: 0 = ascending A-stride, 1 = ascending B-stride.
+    int gslot_of[kMaxRank];
+    int64_t n_tiles = 1;
+    P.nG = c.rank;
+    for (int k = 0; k < c.rank; ++k) {
+        const int i = loop_order == 0 ? k : c.orderB[k];
+        if (c.d[i].e >= kInt31) return false;
+        const int64_t nt = (c.d[i].e + spec.t[i] - 1) / spec.t[i];
+        GridDim& g = P.g[k];
+        g.div = make_fastdiv((uint32_t)nt);
+        g.sA = c.d[i].sA;
+        g.sB = c.d[i].sB;
+        g.e = (int32_t)c.d[i].e;
+        g.t = spec.t[i];
+        gslot_of[i] = k;
+        n_tiles *= nt;
+        if (n_tiles >= kInt31) return false;
+    }
+    P.n_tiles = (uint32_t)n_tiles;
+
+    // Offset tables.
+    auto fill = [&](Table& tb_, const std::vector<PhaseDim>& ph, int lo, int hi, bool sideA) -> bool {
+        tb_.nd = hi - lo;
+        int64_t n = 1, span = 0;
+        for (int k = lo; k < hi; ++k) {
+            const PhaseDim& p = ph[k];
+            TabDim& d = tb_.d[k - lo];
+            d.div = make_fastdiv((uint32_t)p.n);
+            d.n = p.n;
+            d.step = p.step;
+            d.gslot = gslot_of[p.dim];
+            d.sS = ss[p.dim] * p.step;
+            d.sG = (sideA ? c.d[p.dim].sA : c.d[p.dim].sB) * p.step;
+            span += (int64_t)(p.n - 1) * d.sG;
+            n *= p.n;
+        }
+        tb_.n = (int32_t)n;
+        return span < kInt31 / 2;
+    };
+    if (!fill(P.tab[0], phA, 0, splitA, true) || !fill(P.tab[1], phA, splitA, (int)phA.size(), true) ||
+        !fill(P.tab[2], phB, 0, splitB, false) || !fill(P.tab[3], phB, splitB, (int)phB.size(), false))
+        return false;
+    P.divAlo = make_fastdiv((uint32_t)P.tab[0].n);
+    P.divBlo = make_fastdiv((uint32_t)P.tab[2].n);
+    if ((int)tile_smem_layout(P, es).total > max_smem) return false;
+
+    // Contiguous runs the tile touches in A and in B (elements): leading tile indices that are
+    // whole and contiguous extend the run.
+    auto run_len = [&](const std::vector<int>& order, bool sideA) {
+        int64_t run = 1, expect = 1;
+        for (int i : order) {
+            const int64_t s = sideA ? c.d[i].sA : c.d[i].sB;
+            if (s != expect) break;
+            run *= spec.t[i];
+            if (spec.t[i] != c.d[i].e) break;
+            expect = s * c.d[i].e;
+        }
+        return run;
+    };
+    const int64_t runA = run_len(ta, true), runB = run_len(tb, false);
+
+    ttc_candidate_info& I = cand.info;
+    I.kernel = same ? TTC_KERNEL_WIDE : (ta.size() > 2 ? TTC_KERNEL_GATHER : TTC_KERNEL_TILE);
+    I.vec_a = want_va;
+    I.vec_b = want_vb;
+    I.tile_u = (int)std::min<int64_t>(runA, INT32_MAX);
+    I.tile_w = (int)std::min<int64_t>(runB, INT32_MAX);
+    I.n_u = (int)ta.size();
+    I.n_w = (int)tb.size();
+    I.threads = P.threads;
+    I.smem_bytes = (int)tile_smem_layout(P, es).total;
+    I.loop_order = loop_order;
+    I.grid = 0;
+    I.n_tiles = n_tiles;
+    for (int i = 0; i < kMaxRank; ++i) I.tile_ext[i] = i < c.rank ? spec.t[i] : 0;
+    cand.align_a = want_va * es;
+    cand.align_b = want_vb * es;
+
+    // Cost heuristic: long contiguous runs on both sides, small remainders,
+    // few bank conflicts, enough bytes per tile to amortise its bookkeeping, enough tiles to
+    // fill the machine.
+    double waste = 1.0;
+    for (int i = 0; i < c.rank; ++i) {
+        const double nt = std::ceil((double)c.d[i].e / spec.t[i]);
+        waste *= nt * spec.t[i] / (double)c.d[i].e;
+    }
+    const double tile_bytes = (double)itemsA * want_va * es;
+    const double rd = 1.0 / run_eff((double)runA * es) * (want_va * es >= 16 ? 1.0 : 1.15);
+    const double wr = (beta_nz ? 2.0 : 1.0) / run_eff((double)runB * es) * (want_vb * es >= 16 ? 1.0 : 1.10);
+    double cost = (rd + wr) * waste;
+    cost *= 1.0 + 0.05 * (best_cost - 1.0);                   // smem conflicts are cheap but not free
+    cost *= 1.0 + 2048.0 / tile_bytes;                        // per-tile overhead
+    if (tile_bytes > 48 * 1024) cost *= 1.0 + (tile_bytes - 48 * 1024) / (256.0 * 1024);   // occupancy
+    if (n_tiles < 148 * 2) cost *= 1.0 + (148.0 * 2 - n_tiles) / (148.0 * 2);
+    I.est_cost = (float)cost;
+    *out = cand;
+    return true;
+}
+
+}  // namespace
+
+namespace {
+
+// One side of a tile: a prefix of the tensor's index order, all but the last taken whole.
+struct SideOpt {
+    std::vector<std::pair<int, int32_t>> dims;   // (canonical index, tile extent)
+    int64_t elems = 1;
+};
+
+// Tile extents of index extent `e` whose side (with `cum` elements already in it) comes close
+// to `target` elements: the largest divisor of e that fits, else a multiple of `mult`
+// (leaves a remainder tile).
+void partial_extents(int64_t e, int64_t cum, int64_t target, int mult, std::vector<int32_t>* out) {
+    const int64_t want = target / cum;
+    if (want < 2) return;
+    if (want >= e) { out->push_back((int32_t)e); return; }
+    int64_t best_div = 0;
+    for (int64_t d = want; d >= 2 && d * 2 > want; --d)
+        if (e % d == 0 && d % mult == 0) { best_div = d; break; }
+    if (best_div) out->push_back((int32_t)best_div);
+    const int64_t rounded = want / mult * mult;
+    if (rounded >= 2 && rounded != best_div) out->push_back((int32_t)rounded);
+}
+
+// Options for one side.  `order` = the tensor's index order; `taken` = tile extents already
+// fixed by the other side (0 = free).  Indices the other side holds whole are skipped (the run
+// continues through them); an index it holds partially ends the side.
+void side_options(const Canon& c, const std::vector<int>& order, const int32_t* taken, int mult,
+                  int es, std::vector<SideOpt>* out) {
+    static const int64_t targets_bytes[] = {32, 64, 128, 256, 512, 1024, 2048, 4096, 8192, 16384};
+    SideOpt base;
+    std::set<std::vector<std::pair<int, int32_t>>> seen;
+    for (size_t k = 0; k < order.size(); ++k) {
+        const int i = order[k];
+        if (taken[i]) {
+            if (taken[i] == c.d[i].e) continue;
+            break;
+        }
+        if ((int)base.dims.size() >= kMaxTab - 1) break;
+        const int m = (k == 0) ? mult : 1;
+        for (int64_t tb : targets_bytes) {
+            std::vector<int32_t> ext;
+            partial_extents(c.d[i].e, base.elems, std::max<int64_t>(1, tb / es), m, &ext);
+            for (int32_t t : ext) {
+                if (t >= c.d[i].e && t != c.d[i].e) continue;
+                SideOpt o = base;
+                o.dims.push_back({i, t});
+                o.elems = base.elems * t;
+                if (seen.insert(o.dims).second) out->push_back(o);
+            }
+        }
+        base.dims.push_back({i, (int32_t)std::min<int64_t>(c.d[i].e, INT32_MAX)});
+        base.elems *= c.d[i].e;
+        if (base.elems * es > 64 * 1024) break;
+    }
+}
+
+void add_direct(const Canon& c, ttc_dtype dtype, bool beta_nz, int loop_order, bool vector,
+                std::vector<Candidate>* out) {
+    const int es = elem_size(dtype);
+    const int mv = 16 / es;
+    Candidate cand;
+    cand.beta_nz = beta_nz;
+    DirectParams& P = cand.dp;
+    std::memset(&P, 0, sizeof(P));
+    // leading index: the one that is stride-1 in both tensors if there is one, else A's
+    int lead = 0;
+    for (int i = 0; i < c.rank; ++i)
+        if (c.d[i].sA == 1 && c.d[i].sB == 1) lead = i;
+    int vec = 1;
+    if (vector) {
+        const int va = legal_vec(c, lead, true, (int32_t)std::min<int64_t>(c.d[lead].e, 1 << 30) / mv * mv, mv);
+        const int vb = legal_vec(c, lead, false, (int32_t)std::min<int64_t>(c.d[lead].e, 1 << 30) / mv * mv, mv);
+        if (va != mv || vb != mv || mv == 1 || c.d[lead].e % mv != 0) return;
+        vec = mv;
+    }
+    std::vector<int> order;
+    order.push_back(lead);
+    for (int k = 0; k < c.rank; ++k) {
+        const int i = loop_order == 0 ? k : c.orderB[k];
+        if (i != lead) order.push_back(i);
+    }
+    P.nd = c.rank;
+    P.vec = vec;
+    uint64_t n_items = 1;
+    bool idx64 = false;
+    for (int k = 0; k < c.rank; ++k) {
+        const int i = order[k];
+        const int64_t n = c.d[i].e / (k == 0 ? vec : 1);
+        const int64_t step = (k == 0 ? vec : 1);
+        P.dims[k].n = (uint64_t)n;
+        P.dims[k].sA = c.d[i].sA * step;
+        P.dims[k].sB = c.d[i].sB * step;
+        if (n >= kInt31) idx64 = true; else P.dims[k].div = make_fastdiv((uint32_t)n);
+        n_items *= (uint64_t)n;
+    }
+    P.n_items = n_items;
+    if (n_items >= (uint64_t)kInt31 / 2) idx64 = true;
+    cand.idx64 = idx64;
+    cand.align_a = cand.align_b = vec * es;
+    ttc_candidate_info& I = cand.info;
+    I.kernel = TTC_KERNEL_COPY;
+    I.vec_a = I.vec_b = vec;
+    I.threads = 256;
+    I.loop_order = loop_order;
+    I.n_tiles = (int64_t)n_items;
+    for (int i = 0; i < kMaxRank; ++i) I.tile_ext[i] = i < c.rank ? 1 : 0;
+    // cost: contiguous runs seen by a warp on each side
+    auto run_of = [&](bool sideA) {
+        int64_t run = 1, expect = 1;
+        // the item order is `order`; a side's run extends while its strides follow the order
+        for (int k = 0; k < c.rank; ++k) {
+            const int i = order[k];
+            const int64_t s = sideA ? c.d[i].sA : c.d[i].sB;
+            if (s != expect) break;
+            run *= c.d[i].e;
+            expect = s * c.d[i].e;
+        }
+        return run;
+    };
+    const double ra = (double)run_of(true) * es, rb = (double)run_of(false) * es;
+    auto eff = [&](double r) { return r <= es ? es / 32.0 * 0.5 : run_eff(r); };
+    double cost = 1.0 / eff(ra) + (beta_nz ? 2.0 : 1.0) / eff(rb);
+    if (vec * es < 16) cost *= 1.25;
+    if (idx64) cost *= 1.5;
+    I.est_cost = (float)cost;
+    I.tile_u = (int)std::min<int64_t>(run_of(true), INT32_MAX);
+    I.tile_w = (int)std::min<int64_t>(run_of(false), INT32_MAX);
+    out->push_back(cand);
+}
+
+}  // namespace
+
+void generate_candidates(const Canon& c, ttc_dtype dtype, bool beta_nz, int sm_count,
+                         int max_smem_optin, std::vector<Candidate>* out) {
+    (void)sm_count;
+    out->clear();
+    if (c.empty || c.rank == 0) return;
+    const int es = elem_size(dtype);
+    const int mv = 16 / es;
+    const int max_smem = std::min(max_smem_optin > 0 ? max_smem_optin : 48 * 1024, 160 * 1024);
+
+    // K1 / fallback: direct kernels (always at least the scalar one, valid for any strides).
+    for (int lo = 0; lo < 2; ++lo) {
+        add_direct(c, dtype, beta_nz, lo, true, out);
+        add_direct(c, dtype, beta_nz, lo, false, out);
+    }
+
+    // K2 / K3: tiles.  A side = leading indices of A, B side = leading indices of B.
+    std::vector<int> orderA, orderB;
+    for (int i = 0; i < c.rank; ++i) { orderA.push_back(i); orderB.push_back(c.orderB[i]); }
+    bool fits32 = true;
+    for (int i = 0; i < c.rank; ++i) fits32 &= c.d[i].e < kInt31;
+    if (fits32 && c.rank >= 2) {
+        std::vector<SideOpt> optsA;
+        int32_t none[kMaxRank] = {0};
+        side_options(c, orderA, none, mv, es, &optsA);
+        std::set<std::string> seen;
+        for (const SideOpt& ua : optsA) {
+            int32_t taken[kMaxRank] = {0};
+            for (auto& d : ua.dims) taken[d.first] = d.second;
+            std::vector<SideOpt> optsB;
+            side_options(c, orderB, taken, mv, es, &optsB);
+            for (const SideOpt& wb : optsB) {
+                const int64_t bytes = ua.elems * wb.elems * es;
+                if (bytes < 2048 || bytes > max_smem) continue;
+                TileSpec spec;
+                for (int i = 0; i < kMaxRank; ++i) spec.t[i] = 1;
+                for (auto& d : ua.dims) spec.t[d.first] = d.second;
+                for (auto& d : wb.dims) spec.t[d.first] = d.second;
+                std::string key((const char*)spec.t, sizeof(int32_t) * c.rank);
+                if (!seen.insert(key).second) continue;
+                static const int vopts[4][2] = {{16, 16}, {16, 1}, {1, 16}, {1, 1}};
+                for (int lo = 0; lo < 2; ++lo) {
+                    for (auto& vo : vopts) {
+                        const int va = vo[0] == 16 ? mv : 1, vb = vo[1] == 16 ? mv : 1;
+                        if (mv == 1 && (vo[0] == 16 || vo[1] == 16)) continue;
+                        Candidate cand;
+                        if (build_tile_candidate(c, dtype, beta_nz, spec, lo, va, vb, max_smem, &cand))
+                            out->push_back(cand);
+                    }
+                }
+            }
+        }
+    }
+
+    // Bounded list ordered by estimated cost.
+    std::stable_sort(out->begin(), out->end(),
+                     [](const Candidate& a, const Candidate& b) { return a.info.est_cost < b.info.est_cost; });
+    if ((int)out->size() > kMaxImplementations) {
+        // keep the scalar direct fallback whatever its rank
+        Candidate fallback;
+        bool have = false;
+        for (auto& cd : *out)
+            if (cd.info.kernel == TTC_KERNEL_COPY && cd.info.vec_a == 1) { fallback = cd; have = true; break; }
+        out->resize(kMaxImplementations);
+        bool kept = false;
+        for (auto& cd : *out) kept |= (cd.info.kernel == TTC_KERNEL_COPY && cd.info.vec_a == 1);
+        if (have && !kept) out->back() = fallback;
+    }
+}
+
+}  // namespace ttc

@@ -1,0 +1,186 @@
+// ttc_internal.h -- structures shared by the host planner and the CUDA kernels of libttc.so.
+// Nothing here is visible through the C ABI (include/ttc.h).  Not shared with oracle/.
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "ttc.h"
+
+#if defined(__CUDACC__)
+#define TTC_HD __host__ __device__ __forceinline__
+#else
+#define TTC_HD inline
+#endif
+
+namespace ttc {
+
+constexpr int kMaxRank = TTC_MAX_RANK;
+constexpr int kMaxTab = 6;           // canonical indices enumerated by one offset table
+constexpr int kMaxTabEntries = 2048; // entries of one offset table
+constexpr int kTileThreads = 256;    // default CTA size of the tile kernel
+
+// ---------------------------------------------------------------------------------------
+// Fast division of a 31-bit numerator by a plan-time constant (Granlund-Montgomery):
+//   s = ceil(log2 d), m = floor(2^32 (2^s - d) / d) + 1, n / d = (mulhi(m, n) + n) >> s
+// exact for 0 <= n < 2^31 (the sum cannot overflow 32 bits).  SURVEY.md 8(a) row H6.
+// ---------------------------------------------------------------------------------------
+struct FastDiv {
+    uint32_t d, m, s, pad;
+};
+
+inline FastDiv make_fastdiv(uint32_t d) {
+    FastDiv f{d, 1u, 0u, 0u};
+    if (d <= 1) { f.d = 1; return f; }
+    uint32_t s = 0;
+    while ((1ull << s) < d) ++s;
+    f.s = s;
+    f.m = (uint32_t)((((1ull << s) - d) << 32) / d + 1);
+    return f;
+}
+
+TTC_HD uint32_t fd_div(uint32_t n, const FastDiv& f) {
+#if defined(__CUDA_ARCH__)
+    return (__umulhi(f.m, n) + n) >> f.s;
+#else
+    return (uint32_t)(((((uint64_t)f.m * n) >> 32) + n) >> f.s);
+#endif
+}
+
+TTC_HD void fd_divmod(uint32_t n, const FastDiv& f, uint32_t& q, uint32_t& r) {
+    q = fd_div(n, f);
+    r = n - q * f.d;
+}
+
+// ---------------------------------------------------------------------------------------
+// Canonical transposition (stage 1): (extent, stride in A, stride in B) per
+// index, ascending stride in A, no extent-1 index, nothing left to merge.
+// ---------------------------------------------------------------------------------------
+struct CanonDim {
+    int64_t e, sA, sB;
+};
+
+struct Canon {
+    int rank = 0;
+    CanonDim d[kMaxRank];
+    int64_t numel = 0;
+    int64_t spanA = 0, spanB = 0;  // 1 + max offset (elements); 0 if empty
+    bool empty = false;
+    int orderB[kMaxRank];          // canonical indices by ascending stride in B
+};
+
+ttc_status canonicalize(int N, const int64_t* sizes, const int* perm, const int64_t* lda,
+                        const int64_t* ldb, Canon* out);
+
+// ---------------------------------------------------------------------------------------
+// Kernel parameter blocks (passed by value as __grid_constant__).
+// ---------------------------------------------------------------------------------------
+
+// K1 (and the always-valid fallback): direct global->global.  Item q (one vector of `vec`
+// elements along dims[0], or one element) is split by successive fast-divmods over
+// dims[0..nd) (dims[0] fastest; the order of the others is the candidate's loop order).
+struct DirectDim {
+    FastDiv div;        // by the number of items along this dim
+    int64_t sA, sB;     // element stride per item step (already multiplied by vec for dim 0)
+    uint64_t n;         // items along this dim (64-bit path)
+};
+struct DirectParams {
+    int nd;
+    int vec;            // elements per item
+    uint64_t n_items;
+    DirectDim dims[kMaxRank];
+};
+
+// K2/K3: macro-tile = box of tile extents t_i over the canonical indices (t_i = 1 outside the
+// tile).  Two enumerations of the box: phase A (ascending stride in A, used by the load) and
+// phase B (ascending stride in B, used by the store).  Each enumeration is factorised into a
+// fast ("lo") and a slow ("hi") group of indices; the kernel builds one table per group that
+// gives (offset in the global tensor, offset in the shared-memory tile) of every group entry.
+struct TabDim {
+    FastDiv div;        // by `n`
+    int32_t n;          // entries along this index = t / step
+    int32_t step;       // elements per entry step (vec for the vectorised leading index, else 1)
+    int32_t gslot;      // position of this index in TileParams::g (for edge-tile validity)
+    int32_t sS;         // shared-memory stride per entry step (elements)
+    int64_t sG;         // global stride per entry step (elements)
+};
+struct Table {
+    int32_t nd;
+    int32_t n;          // product of TabDim::n
+    TabDim d[kMaxTab];
+};
+struct GridDim {        // one coordinate of the macro-tile grid, in loop order (first = fastest)
+    FastDiv div;        // by the number of tiles along this index
+    int64_t sA, sB;     // element strides of the index
+    int32_t e;          // full extent of the index
+    int32_t t;          // tile extent (1 if the index is outside the tile)
+};
+struct TileParams {
+    int nG;
+    int vecA, vecB;     // elements per global access in the load / store phase
+    int same;           // 1: the vectorised index leads A and B (chunks move unchanged)
+    int sstepB;         // smem stride between the vecB elements one store gathers (!same)
+    int threads;
+    uint32_t n_tiles;
+    uint32_t itemsA, itemsB;      // table entries per tile: Alo.n*Ahi.n, Blo.n*Bhi.n
+    uint32_t tile_elems;          // shared-memory tile size in elements (with padding)
+    FastDiv divAlo, divBlo;       // item -> (lo, hi)
+    Table tab[4];                 // 0: A lo, 1: A hi, 2: B lo, 3: B hi
+    GridDim g[kMaxRank];
+};
+
+// Shared-memory carve-up (bytes), identical on host and device.
+struct TileSmemLayout {
+    uint32_t tab[4];     // int2 tables
+    uint32_t val[4];     // uint8 validity of each table entry (edge tiles only)
+    uint32_t vext;       // int32 valid extent per grid index
+    uint32_t tile;       // tile data (16-byte aligned)
+    uint32_t total;
+};
+TTC_HD TileSmemLayout tile_smem_layout(const TileParams& P, int es) {
+    TileSmemLayout L;
+    uint32_t o = 0;
+    for (int i = 0; i < 4; ++i) { L.tab[i] = o; o += 8u * (uint32_t)P.tab[i].n; }
+    for (int i = 0; i < 4; ++i) { L.val[i] = o; o += ((uint32_t)P.tab[i].n + 3u) & ~3u; }
+    L.vext = o; o += 4u * kMaxRank;
+    o = (o + 15u) & ~15u;
+    L.tile = o; o += P.tile_elems * (uint32_t)es;
+    L.total = o;
+    return L;
+}
+
+// ---------------------------------------------------------------------------------------
+// A candidate = kernel class + blocking + loop order + launch shape.
+// ---------------------------------------------------------------------------------------
+struct Candidate {
+    ttc_candidate_info info{};
+    bool beta_nz = false;
+    bool idx64 = false;          // K1: item count / offsets need 64-bit arithmetic
+    int  align_a = 1, align_b = 1;  // required pointer alignment in bytes
+    DirectParams dp{};
+    TileParams tp{};
+};
+
+struct Scalar {         // alpha or beta, as doubles (re, im); narrowed in the launcher
+    double re, im;
+};
+
+void generate_candidates(const Canon& c, ttc_dtype dtype, bool beta_nz, int sm_count,
+                         int max_smem_optin, std::vector<Candidate>* out);
+
+// Launch one candidate.  Returns the CUDA error code (0 = success) as int.
+int launch_candidate(const Candidate& cand, ttc_dtype dtype, const Scalar& alpha, const Scalar& beta,
+                     const void* A, void* B, void* stream);
+// Configure dynamic shared memory / occupancy-derived grid for a candidate (needs a device).
+int prepare_candidate(Candidate* cand, ttc_dtype dtype, int sm_count);
+
+inline int elem_size(ttc_dtype t) {
+    switch (t) {
+        case TTC_F32: return 4;
+        case TTC_F64: return 8;
+        case TTC_C64: return 8;
+        default: return 16;
+    }
+}
+
+}  // namespace ttc
