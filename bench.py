@@ -1,0 +1,354 @@
+#!/usr/bin/env python
+"""bench.py -- effective transpose bandwidth of libttc.so on B200 (BASELINE.json `metric`).
+
+Workload at N=1 (and per rank at N>1, "replicas only"): BASELINE.json configs[1],
+fp64 4-D tensor 96x72x64x56 (198 MB), all 23 non-identity permutations, alpha=1, beta=0.
+One STEP = the whole hot path over that batch: 23 ttc_execute launches, one per permutation
+(plans are built and autotuned once, before the timed region, as the paper generates code
+once per transposition).  value = (2 * |A| * 8 bytes * 23 * ranks) / step time.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--detail PATH]
+
+stdout carries exactly ONE JSON line.  --detail additionally writes per-config results of all
+five BASELINE.json configs (cold L2, min of 3 and median) to PATH as JSON.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "effective transpose GB/s ((2|3)\u00b7|A| bytes / device time) and % of B200 HBM peak"
+UNIT = "GB/s"
+WORKLOAD = "configs[1]: fp64 96x72x64x56 (198 MB), all 23 non-identity permutations, alpha=1, beta=0"
+NOMINAL_HBM_GBS = 8000.0      # north_star's "~8 TB/s"
+FALLBACK_HBM_GBS = 6650.0     # B200_PROFILING.md fallback
+
+
+def measured_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (measured)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "B200_PROFILING.md fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (profiling recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+    NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except Exception:
+                continue
+            for name, v in zip(self.NAMES, r[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None,
+                "sm_max_mhz": max(mx) if mx else None, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------ CPU legs
+REF_SAMPLE_PERMS = [(2, 3, 0, 1), (3, 1, 2, 0), (1, 3, 0, 2)]   # canonical rank 2, 3, 4
+
+
+def time_oracle(perms, A, B) -> float:
+    """Seconds the oracle (as it stands, 1 thread) needs for the given c2 permutations."""
+    import oracle
+    from paper_1607_01249_b200 import workloads as wl
+    t0 = time.perf_counter()
+    for perm in perms:
+        w = wl.config2(perm)
+        oracle.transpose(w.dtype, w.sizes, w.perm, None, None, 1.0, A, 0.0, B)
+    return time.perf_counter() - t0
+
+
+def run_reference(args) -> None:
+    """--impl reference: the oracle on the host cores, same metric/config; a step is a bounded
+    sample (3 of the 23 permutations: canonical rank 2, 3 and 4)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_1607_01249_b200 import workloads as wl
+    steps = args.steps if args.steps is not None else 3
+    warmup = args.warmup if args.warmup is not None else 1
+    w0 = wl.config2(REF_SAMPLE_PERMS[0])
+    A, B = w0.make_a(), w0.make_b()
+    for _ in range(warmup):
+        time_oracle(REF_SAMPLE_PERMS, A, B)
+    t = 0.0
+    for _ in range(steps):
+        t += time_oracle(REF_SAMPLE_PERMS, A, B)
+    bytes_per_step = sum(wl.config2(p).algorithmic_bytes for p in REF_SAMPLE_PERMS)
+    value = bytes_per_step * steps / t / 1e9
+    sample = "%d of the 23 permutations per step: %s, whole 198 MB tensor each" % (
+        len(REF_SAMPLE_PERMS), REF_SAMPLE_PERMS)
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": steps, "warmup": warmup, "ms_per_step": t / steps * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic (seeded SplitMix64)",
+        "config": {"workload": WORKLOAD, "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+# ------------------------------------------------------------------------------ GPU arm
+def cold_times(torch, ttc, plan, w, a_dev, b_dev, flush, reps: int):
+    """Per-launch device times (us) with L2 flushed before every run."""
+    out = []
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for _ in range(reps):
+        flush.zero_()
+        e0.record()
+        ttc.ttc_execute(plan, w.alpha, a_dev, w.beta, b_dev)
+        e1.record()
+        e1.synchronize()
+        out.append(e0.elapsed_time(e1) * 1e3)
+    return out
+
+
+def detail_all_configs(torch, ttc, wl, path: str, peak: float) -> None:
+    """Per-config report of all five BASELINE.json configs (north_star: 'reported per config')."""
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    rows = []
+    for w in wl.baseline_configs():
+        plan = ttc.ttc_plan(w.dtype, w.n, w.sizes, w.perm, w.lda, w.ldb)
+        info = ttc.ttc_plan_info(plan)
+        a_dev = torch.from_numpy(w.make_a()).cuda()
+        b_dev = torch.from_numpy(w.make_b()).cuda()
+        for _ in range(3):
+            ttc.ttc_execute(plan, w.alpha, a_dev, w.beta, b_dev)
+        ts = cold_times(torch, ttc, plan, w, a_dev, b_dev, flush, 21)
+        which = 1 if w.beta_nonzero else 0
+        cand = ttc.ttc_plan_candidate(plan, which, info.chosen[which])
+        t3, tm = min(ts[:3]), statistics.median(ts)
+        gbs = w.algorithmic_bytes / (min(ts) * 1e-6) / 1e9
+        rows.append({"config": w.name, "perm": list(w.perm), "bytes": w.algorithmic_bytes,
+                     "us_min_of_3": t3, "us_median_21": tm, "us_min_21": min(ts),
+                     "gbs_min_of_3": w.algorithmic_bytes / t3 / 1e3,
+                     "gbs_median": w.algorithmic_bytes / tm / 1e3, "gbs_best": gbs,
+                     "gibs_median": w.algorithmic_bytes / tm / 1e3 * 1e9 / 2 ** 30,
+                     "frac_of_8TBs": w.algorithmic_bytes / tm / 1e3 / NOMINAL_HBM_GBS,
+                     "frac_of_measured_copy": w.algorithmic_bytes / tm / 1e3 / peak,
+                     "chosen": ttc.describe_candidate(cand, info.canon_rank),
+                     "n_candidates": info.n_candidates[which]})
+        ttc.ttc_destroy(plan)
+        del a_dev, b_dev
+    with open(path, "w") as fh:
+        json.dump(rows, fh, indent=1)
+
+
+def run_ours(args) -> None:
+    import torch
+    from paper_1607_01249_b200 import ttc            # raises if libttc.so cannot be built/loaded
+    from paper_1607_01249_b200 import workloads as wl
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU path")
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    steps = args.steps if args.steps is not None else 200
+    warmup = max(3, args.warmup if args.warmup is not None else 5)
+    peak, peak_src = measured_peak()
+
+    works = list(wl.config2_all())
+    plans = [ttc.ttc_plan(w.dtype, w.n, w.sizes, w.perm) for w in works]      # tuned here, untimed
+    A_host = works[0].make_a()
+    a_dev = torch.from_numpy(A_host).cuda()
+    b_dev = torch.zeros_like(a_dev)
+    step_bytes = sum(w.algorithmic_bytes for w in works)
+    stream = torch.cuda.current_stream()
+
+    def one_step(events=None):
+        for i, (p, w) in enumerate(zip(plans, works)):
+            if events is not None:
+                events[i][0].record(stream)
+            ttc.ttc_execute(p, 1.0, a_dev, 0.0, b_dev, stream)
+            if events is not None:
+                events[i][1].record(stream)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(warmup):
+        one_step()
+    # per-launch events for the roofline of the dominant kernel, live in the timed region
+    ev = [[(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+           for _ in works] for _ in range(steps)] if not args.no_launch_events else None
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.25)
+    barrier()
+    launches0 = ttc.ttc_launch_count()
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0.record(stream)
+    for s in range(steps):
+        one_step(ev[s] if ev else None)
+    t1.record(stream)
+    barrier()
+    launches = ttc.ttc_launch_count() - launches0
+    clocks = sampler.stop()
+    ms = torch.tensor([t0.elapsed_time(t1)], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+    ms_total = float(ms.item())
+    value = step_bytes * steps * world / (ms_total * 1e-3) / 1e9
+
+    # per-permutation launch durations (median over steps) and the roofline of the tile kernel
+    per_perm, infos = [], []
+    for i, (p, w) in enumerate(zip(plans, works)):
+        info = ttc.ttc_plan_info(p)
+        cand = ttc.ttc_plan_candidate(p, 0, info.chosen[0])
+        us = statistics.median(ev[s][i][0].elapsed_time(ev[s][i][1]) for s in range(steps)) * 1e3 if ev else None
+        infos.append((w, cand, info))
+        per_perm.append({"perm": "".join(map(str, w.perm)), "kernel": ttc.KERNEL_NAMES[cand.kernel],
+                         "us": us, "gbs": (w.algorithmic_bytes / us / 1e3) if us else None,
+                         "chosen": ttc.describe_candidate(cand, info.canon_rank)})
+    roofline = None
+    if ev:
+        dom = [r for r in per_perm if r["kernel"] != "copy"]
+        dom_us = sum(r["us"] for r in dom)
+        achieved = works[0].algorithmic_bytes * len(dom) / dom_us / 1e3
+        roofline = {"bound": "hbm", "kernel": "tile_kernel (K2/K3), %d of 23 launches per step" % len(dom),
+                    "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                    "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
+                    "avg_launch_us": dom_us / len(dom), "algorithmic_bytes_per_launch": works[0].algorithmic_bytes,
+                    "share_of_step": dom_us / sum(r["us"] for r in per_perm), "traffic": None}
+        tr = os.path.join(ROOT, "profiles", "traffic_r01.json")
+        if os.path.exists(tr):
+            roofline["traffic"] = json.load(open(tr)).get("tile_kernel_dram_bytes_per_launch")
+
+    # ---- end to end through the public host-buffer call: pinned host A -> device, kernel,
+    # device -> pinned host B, every permutation, inside the timed region
+    e2e_steps = max(1, min(steps, args.e2e_steps))
+    a_pin = torch.from_numpy(A_host).pin_memory()
+    b_pin = torch.zeros_like(a_pin).pin_memory()
+    a_np, b_np = a_pin.numpy(), b_pin.numpy()
+
+    def e2e_step():
+        for p in plans:
+            ttc.ttc_execute_host(p, 1.0, a_np, 0.0, b_np, stream)
+
+    e2e_step()
+    barrier()
+    w0 = time.perf_counter()
+    t0.record(stream)
+    for _ in range(e2e_steps):
+        e2e_step()
+    t1.record(stream)
+    barrier()
+    wall = time.perf_counter() - w0
+    ms = torch.tensor([max(t0.elapsed_time(t1), wall * 1e3)], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+    e2e_value = step_bytes * e2e_steps * world / (float(ms.item()) * 1e-3) / 1e9
+    nbytes = a_pin.numel() * a_pin.element_size()
+    e2e = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes * len(plans),
+           "d2h_bytes_per_step": nbytes * len(plans), "steps": e2e_steps,
+           "api": "ttc_execute_host (pinned host A and B)"}
+    # last e2e result doubles as a live parity spot check of the timed configuration
+    last = works[-1]
+    idx = np.random.default_rng(0).integers(0, last.numel, 4096)
+
+    if args.detail and rank == 0:
+        detail_all_configs(torch, ttc, wl, args.detail, peak)
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        B_or = np.zeros_like(A_host)
+        perms = [w.perm for w in works]
+        secs = time_oracle(perms, A_host, B_or)
+        # the oracle's last permutation is the e2e leg's last permutation: compare samples
+        if not np.array_equal(B_or[idx], b_np[idx]):
+            raise SystemExit("bench.py: GPU result differs from the oracle on sampled outputs")
+        cpu = {"value": step_bytes / secs / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "seconds": secs, "sample": "one whole step: all 23 permutations once, single thread"}
+
+    for p in plans:
+        ttc.ttc_destroy(p)
+    if rank == 0:
+        gbs = [r["gbs"] for r in per_perm if r["gbs"]]
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps,
+                "warmup": warmup, "ms_per_step": ms_total / steps, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+                "data": "synthetic (seeded SplitMix64 uniform [-1,1))",
+                "config": {"workload": WORKLOAD, "parallelism": "replicas only (no collective)",
+                           "l2": "inputs larger than L2: A and B are 198 MB each, L2 is 126 MB; "
+                                 "no explicit flush between launches",
+                           "launches_per_step": len(plans)},
+                "frac_of_measured_copy": value / world / peak, "frac_of_nominal_8TBs": value / world / NOMINAL_HBM_GBS,
+                "per_perm_gbs": {"min": min(gbs), "median": statistics.median(gbs), "max": max(gbs)} if gbs else None,
+                "per_perm": per_perm, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
+                "gpu_launches": launches, "clocks": clocks}
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main() -> None:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=None)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--detail", default=None, help="write per-config results of all 5 configs here")
+    ap.add_argument("--no-launch-events", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

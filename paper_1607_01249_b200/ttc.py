@@ -138,9 +138,18 @@ def ttc_plan(dtype: int, N: int, sizes, perm, lda=None, ldb=None) -> int:
     return h
 
 
+_plan_dtype = {}     # plan handle -> numpy dtype of its scalars (marshalling cache)
+
+
+def _scalar_dtype(plan: int):
+    dt = _plan_dtype.get(plan)
+    if dt is None:
+        dt = _plan_dtype[plan] = NP_DTYPE[ttc_plan_info(plan).dtype]
+    return dt
+
+
 def ttc_execute(plan: int, alpha, A, beta, B, stream=None) -> None:
-    info = ttc_plan_info(plan)
-    npdt = NP_DTYPE[info.dtype]
+    npdt = _scalar_dtype(plan)
     a = np.array([alpha], dtype=npdt)
     b = np.array([beta], dtype=npdt)
     rc = lib.ttc_execute(plan, a.ctypes.data, _ptr(A), b.ctypes.data, _ptr(B), _stream(stream))
@@ -149,8 +158,7 @@ def ttc_execute(plan: int, alpha, A, beta, B, stream=None) -> None:
 
 
 def ttc_execute_host(plan: int, alpha, A_host, beta, B_host, stream=None) -> None:
-    info = ttc_plan_info(plan)
-    npdt = NP_DTYPE[info.dtype]
+    npdt = _scalar_dtype(plan)
     a = np.array([alpha], dtype=npdt)
     b = np.array([beta], dtype=npdt)
     rc = lib.ttc_execute_host(plan, a.ctypes.data, _ptr(A_host), b.ctypes.data, _ptr(B_host), _stream(stream))
@@ -159,6 +167,7 @@ def ttc_execute_host(plan: int, alpha, A_host, beta, B_host, stream=None) -> Non
 
 
 def ttc_destroy(plan: int) -> None:
+    _plan_dtype.pop(plan, None)
     lib.ttc_destroy(plan)
 
 

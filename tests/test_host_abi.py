@@ -1,0 +1,169 @@
+"""CPU-only tests of the host side of libttc.so: the library loads and exports every symbol
+include/ttc.h declares, argument validation, the canonicaliser (stage 1),
+the fast-divmod constants and the candidate generator (stages 2-3).
+No kernel is launched here."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_1607_01249_b200 import ttc
+from paper_1607_01249_b200 import workloads as wl
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def header_symbols():
+    text = open(os.path.join(ROOT, "include", "ttc.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(ttc_[a-z_0-9]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol():
+    syms = header_symbols()
+    assert "ttc_plan" in syms and "ttc_execute" in syms and "ttc_destroy" in syms
+    for s in syms:
+        assert hasattr(ttc.lib, s), "libttc.so does not export %s" % s
+    assert sorted(ttc.EXPORTS) == syms
+    assert "sm_100a" in ttc.ttc_version()
+
+
+def test_struct_layouts_match_header():
+    """The ctypes mirrors must have the C sizes (int64 alignment included)."""
+    assert ctypes.sizeof(ttc.ttc_info) == 4 * 4 + 3 * 16 * 8 + 3 * 8 + 4 + 2 * 4 + 2 * 4 + 2 * 4 + 4
+    assert ctypes.sizeof(ttc.ttc_candidate_info) % 8 == 0
+
+
+@pytest.mark.parametrize("args,status", [
+    (dict(dtype=9, sizes=(2, 2), perm=(0, 1)), "INVALID_ARG"),
+    (dict(dtype=0, sizes=(2, 2), perm=(0, 0)), "NOT_PERMUTATION"),
+    (dict(dtype=0, sizes=(2, 2), perm=(0, 2)), "NOT_PERMUTATION"),
+    (dict(dtype=0, sizes=(2, -1), perm=(0, 1)), "INVALID_ARG"),
+    (dict(dtype=0, sizes=(4, 3), perm=(1, 0), lda=(3, 3)), "BAD_LD"),
+    (dict(dtype=0, sizes=(4, 3), perm=(1, 0), ldb=(4, 4)), "BAD_LD"),      # ldb[0] pairs with sizes[perm[0]]=3? no: 4>=3 ok, ldb[1]=4>=4
+    (dict(dtype=0, sizes=(2 ** 40, 2 ** 40), perm=(1, 0)), "UNSUPPORTED"),
+])
+def test_plan_argument_errors(args, status):
+    if args.get("ldb") == (4, 4):
+        args = dict(args, ldb=(2, 4))     # ldb[0] = 2 < sizes[perm[0]] = 3
+    with pytest.raises(ttc.TTCError) as ei:
+        ttc.ttc_plan(args["dtype"], len(args["sizes"]), args["sizes"], args["perm"],
+                     args.get("lda"), args.get("ldb"))
+    assert ttc.STATUS_NAMES[ei.value.status] == "TTC_ERR_" + status
+
+
+def test_rank_limits():
+    with pytest.raises(ttc.TTCError):
+        ttc.ttc_plan(0, 17, (1,) * 17, tuple(range(17)))
+    p = ttc.ttc_plan(0, 16, (2,) * 16, tuple(reversed(range(16))))
+    assert ttc.ttc_plan_info(p).canon_rank == 16
+    ttc.ttc_destroy(p)
+
+
+# --------------------------------------------------------------------- canonicaliser
+def test_merge_example_of_the_paper():
+    """Pi(i0,i1,i2) = (i1,i2,i0) is the 2-D transposition with size(i1)*size(i2)."""
+    assert ttc.ttc_canonicalize((5, 3, 4), (1, 2, 0)) == [(5, 1, 12), (12, 5, 1)]
+    # config 1: (2,0,1) fuses (i0,i1): 2-D transpose of (23040, 128)
+    assert ttc.ttc_canonicalize((160, 144, 128), (2, 0, 1)) == [(23040, 1, 128), (128, 23040, 1)]
+
+
+def test_identity_collapses_to_one_index():
+    assert ttc.ttc_canonicalize((4, 5, 6), (0, 1, 2)) == [(120, 1, 1)]
+
+
+def test_padding_blocks_merging():
+    """fn 5: merging needs ld(i_m) = size(i_m), in A and in B (reading A11)."""
+    assert len(ttc.ttc_canonicalize((4, 5, 6), (0, 1, 2), lda=(4, 7, 6))) == 2
+    assert len(ttc.ttc_canonicalize((4, 5, 6), (0, 1, 2), ldb=(5, 5, 6))) == 3 - 1
+    assert ttc.ttc_canonicalize((4, 5, 6), (0, 1, 2), lda=(4, 7, 6)) == [(20, 1, 1), (6, 28, 20)]
+
+
+def test_extent_one_indices_are_dropped_but_keep_their_stride_effect():
+    """Reading A12: an extent-1 index with ld > 1 still multiplies later strides."""
+    got = ttc.ttc_canonicalize((3, 1, 5), (2, 1, 0), lda=(4, 2, 5), ldb=(5, 3, 3))
+    assert got == [(3, 1, 15), (5, 8, 1)]
+    assert ttc.ttc_canonicalize((1, 1, 1), (2, 0, 1)) == [(1, 1, 1)]
+    assert ttc.ttc_canonicalize((3, 0, 2), (2, 0, 1)) == []
+
+
+def test_config_canonical_forms_match_survey_table():
+    """c4 and c5 canonical (e, sA, sB) triples; c2 rank histogram 3/9/11."""
+    w = wl.config4()
+    assert ttc.ttc_canonicalize(w.sizes, w.perm, w.lda) == [(8, 1, 1), (768, 8, 32768), (4096, 6208, 8)]
+    w = wl.config5()
+    assert ttc.ttc_canonicalize(w.sizes, w.perm) == [
+        (7, 1, 320), (96, 7, 179200), (5, 672, 64), (80, 3360, 2240), (64, 268800, 1)]
+    ranks = [len(ttc.ttc_canonicalize(c.sizes, c.perm)) for c in wl.config2_all()]
+    assert (ranks.count(2), ranks.count(3), ranks.count(4)) == (3, 9, 11)
+    assert len(ttc.ttc_canonicalize(wl.config3().sizes, wl.config3().perm)) == 6
+
+
+def test_canonical_form_preserves_the_offset_map():
+    """The canonical triples enumerate exactly the same (offA, offB) pairs as the definition
+    (checked against numpy index arithmetic, not against the oracle)."""
+    rng = np.random.default_rng(7)
+    for _ in range(40):
+        n = int(rng.integers(1, 6))
+        sizes = tuple(int(x) for x in rng.choice([1, 2, 3, 4, 5], size=n))
+        perm = tuple(int(x) for x in rng.permutation(n))
+        szb = tuple(sizes[p] for p in perm)
+        lda = tuple(int(s + rng.integers(0, 2)) for s in sizes)
+        ldb = tuple(int(s + rng.integers(0, 2)) for s in szb)
+        sA = np.cumprod((1,) + lda[:-1])
+        tB = np.cumprod((1,) + ldb[:-1])
+        idx = np.indices(sizes).reshape(n, -1)
+        offA = (idx * sA[:, None]).sum(0)
+        offB = sum(idx[perm[k]] * tB[k] for k in range(n))
+        want = set(zip(offA.tolist(), offB.tolist()))
+        can = ttc.ttc_canonicalize(sizes, perm, lda, ldb)
+        cidx = np.indices([c[0] for c in can]).reshape(len(can), -1)
+        ca = sum(cidx[i] * can[i][1] for i in range(len(can)))
+        cb = sum(cidx[i] * can[i][2] for i in range(len(can)))
+        assert set(zip(ca.tolist(), cb.tolist())) == want
+        assert all(c[0] > 1 for c in can) or len(can) == 1
+
+
+# --------------------------------------------------------------------- fast divmod
+def test_fastdiv_is_exact():
+    rng = np.random.default_rng(5)
+    ds = [1, 2, 3, 5, 7, 24, 56, 96, 672, 4608, 65535, 65537, 2 ** 30 - 1, 2 ** 31 - 1] + \
+        [int(x) for x in rng.integers(1, 2 ** 31, 40)]
+    for d in ds:
+        ns = [0, 1, d - 1, d, d + 1, 2 * d - 1, 2 ** 31 - 1] + [int(x) for x in rng.integers(0, 2 ** 31, 50)]
+        for n in ns:
+            if 0 <= n < 2 ** 31:
+                assert ttc.lib.ttc_debug_fastdiv(n, d) == n // d, (n, d)
+
+
+# --------------------------------------------------------------------- candidate generator
+def test_candidates_exist_for_every_config_and_are_ranked():
+    for w in wl.baseline_configs():
+        p = ttc.ttc_plan(w.dtype, w.n, w.sizes, w.perm, w.lda, w.ldb)
+        try:
+            info = ttc.ttc_plan_info(p)
+            assert info.numel == w.numel
+            for which in (0, 1):
+                n = ttc.ttc_plan_num_candidates(p, which)
+                assert 1 <= n <= 200                     # PAPER.md:65 default bound
+                cs = [ttc.ttc_plan_candidate(p, which, i) for i in range(n)]
+                costs = [c.est_cost for c in cs]
+                assert costs == sorted(costs)
+                # an always-valid scalar fallback exists
+                assert any(c.kernel == 1 and c.vec_a == 1 for c in cs)
+                for c in cs:
+                    assert c.smem_bytes <= 227 * 1024
+        finally:
+            ttc.ttc_destroy(p)
+
+
+def test_copy_class_configs_rank_a_vector_copy_first():
+    """stride-1-unchanged cases are whole-column copies."""
+    for perm in [(0, 1, 3, 2), (0, 2, 1, 3), (0, 3, 2, 1)]:
+        w = wl.config2(perm)
+        p = ttc.ttc_plan(w.dtype, w.n, w.sizes, w.perm)
+        c = ttc.ttc_plan_candidate(p, 0, 0)
+        assert c.vec_a * 8 == 16 and c.vec_b * 8 == 16
+        ttc.ttc_destroy(p)
