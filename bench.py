@@ -197,6 +197,9 @@ def run_ours(args) -> None:
     peak, peak_src = measured_peak()
 
     works = list(wl.config2_all())
+    if args.perms:     # profiling aid (ncu captures of single permutations); not the headline workload
+        keep = {tuple(int(ch) for ch in x) for x in args.perms.split(",")}
+        works = [w for w in works if w.perm in keep]
     plans = [ttc.ttc_plan(w.dtype, w.n, w.sizes, w.perm) for w in works]      # tuned here, untimed
     A_host = works[0].make_a()
     a_dev = torch.from_numpy(A_host).cuda()
@@ -320,7 +323,8 @@ def run_ours(args) -> None:
                 "warmup": warmup, "ms_per_step": ms_total / steps, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f64",
                 "data": "synthetic (seeded SplitMix64 uniform [-1,1))",
-                "config": {"workload": WORKLOAD, "parallelism": "replicas only (no collective)",
+                "config": {"workload": WORKLOAD if not args.perms else WORKLOAD + " -- SUBSET " + args.perms,
+                           "parallelism": "replicas only (no collective)",
                            "l2": "inputs larger than L2: A and B are 198 MB each, L2 is 126 MB; "
                                  "no explicit flush between launches",
                            "launches_per_step": len(plans)},
@@ -341,6 +345,8 @@ def main() -> None:
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--detail", default=None, help="write per-config results of all 5 configs here")
+    ap.add_argument("--perms", default=None, help="comma-separated subset of the 23 permutations, e.g. 1023,3021 "
+                    "(profiling aid; the step is then NOT the headline workload)")
     ap.add_argument("--no-launch-events", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -88,7 +88,9 @@ typedef struct {
     int      threads;         /* CTA size                                                      */
     int      smem_bytes;      /* dynamic shared memory per CTA                                 */
     int      loop_order;      /* 0: macro-tiles walk A linearly, 1: walk B linearly            */
-    int      grid;            /* CTAs launched (persistent grid), 0 if not yet fixed           */
+    int      sched;           /* 0: static persistent grid-stride, 1: dynamic (cluster launch control) */
+    int      grid;            /* CTAs launched, 0 if not yet fixed (dynamic: one per work item, most of
+                                 which are cancelled and taken over by the resident CTAs)      */
     float    est_cost;        /* heuristic cost used for ranking (lower is better)             */
     float    tuned_us;        /* measured time, 0 if this candidate was not timed              */
     int64_t  n_tiles;         /* macro-tiles (K2/K3) or vector items (K1)                      */
@@ -99,8 +101,10 @@ typedef struct {
  * ttc_plan -- validate, canonicalise (drop extent-1 indices, merge indices that Pi keeps
  * adjacent and that are contiguous in both tensors: PAPER.md:63, 95 fn 5), enumerate and
  * rank candidate kernels and, if a CUDA device is present and the
- * environment does not say TTC_TUNE=0, time the best TTC_TUNE_TOPK (default 16) of them on
- * the device for beta == 0 and for beta != 0 and keep the fastest of each.
+ * environment does not say TTC_TUNE=0, time them in rank order on the device, for beta == 0
+ * and for beta != 0, and keep the fastest of each.  The search of one list ends
+ * after TTC_TUNE_TOPK candidates (default 0 = all, the paper's exhaustive mode) or, once 16
+ * have been timed, when TTC_TUNE_BUDGET_MS (default 400) milliseconds have passed.
  * All pointers are HOST pointers, read before the call returns.
  * Returns NULL on error; ttc_last_error() then says why.  Sizes of 0 give a valid plan
  * whose execution does nothing.  Without a CUDA device the plan is still built (heuristic

@@ -5,6 +5,7 @@
 #include <cuda_runtime.h>
 
 #include <atomic>
+#include <chrono>
 #include <cstdlib>
 #include <cstring>
 #include <map>
@@ -81,7 +82,7 @@ bool ensure_prepared(ttc_plan_s* p, int which, int idx) {
     return prepare_candidate(&c, p->dtype, p->sm_count) == 0 && c.info.grid > 0;
 }
 
-ttc_status tune(ttc_plan_s* p, int top_k, int reps) {
+ttc_status tune(ttc_plan_s* p, int top_k, int reps, int budget_ms) {
     if (!p->have_device) return TTC_ERR_CUDA;
     if (p->canon.empty) return TTC_OK;
     const size_t es = (size_t)elem_size(p->dtype);
@@ -104,9 +105,16 @@ ttc_status tune(ttc_plan_s* p, int top_k, int reps) {
         const int n = top_k <= 0 ? (int)cs.size() : std::min<int>(top_k, (int)cs.size());
         int best = -1;
         float best_us = 0.f;
+        const auto t_start = std::chrono::steady_clock::now();
+        bool over_budget = false;
         for (int i = 0; i < (int)cs.size(); ++i) {
+            // rank order; after the first 16 the list's time budget can end the search
+            if (i >= 16 && !over_budget) {
+                const double ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_start).count();
+                over_budget = budget_ms > 0 && ms > budget_ms;
+            }
             // the scalar fallback is always timed so that it is known to work
-            if (i >= n && i != p->scalar[which]) continue;
+            if ((i >= n || over_budget) && i != p->scalar[which]) continue;
             if (!ensure_prepared(p, which, i)) continue;
             if (launch_candidate(cs[i], p->dtype, alpha, beta, a, b, st) != 0) { cudaGetLastError(); continue; }
             float us = 1e30f;
@@ -186,7 +194,7 @@ ttc_plan_t ttc_plan(ttc_dtype dtype, int N, const int64_t* sizes, const int* per
                 p->tuned = true;
             }
         }
-        if (!hit && tune(p, env_int("TTC_TUNE_TOPK", 24), 3) == TTC_OK) {
+        if (!hit && tune(p, env_int("TTC_TUNE_TOPK", 0), 3, env_int("TTC_TUNE_BUDGET_MS", 400)) == TTC_OK) {
             std::lock_guard<std::mutex> lk(g_cache_mu);
             CacheEntry e;
             for (int w = 0; w < 2; ++w) {
@@ -316,7 +324,7 @@ ttc_status ttc_plan_select(ttc_plan_t p, int which, int index) {
 
 ttc_status ttc_plan_tune(ttc_plan_t p, int top_k, int reps) {
     if (!p) return TTC_ERR_INVALID_ARG;
-    return tune(p, top_k, reps);
+    return tune(p, top_k, reps, 0);
 }
 
 int ttc_canonicalize(int N, const int64_t* sizes, const int* perm, const int64_t* lda,

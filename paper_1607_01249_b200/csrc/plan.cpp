@@ -3,6 +3,7 @@
 // with heuristics and keep a bounded, ranked list.  Host only; timing happens in api.cpp.
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <set>
 #include <string>
@@ -138,7 +139,7 @@ int legal_vec(const Canon& c, int lead, bool sideA, int32_t t_lead, int mv) {
 
 // Build one tile-kernel candidate.  Returns false if the combination is not legal.
 bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const TileSpec& spec,
-                          int loop_order, int want_va, int want_vb, int max_smem, Candidate* out) {
+                          int loop_order, int want_va, int want_vb, int max_smem, int sched, Candidate* out) {
     const int es = elem_size(dtype);
     const int mv = 16 / es;
     Candidate cand;
@@ -162,6 +163,7 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
     P.vecB = want_vb;
     P.same = same ? 1 : 0;
     P.threads = kTileThreads;
+    P.dyn = sched;
 
     // Phase enumerations (entries along the vectorised leading index count vectors).
     std::vector<PhaseDim> phA, phB;
@@ -291,6 +293,7 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
     I.threads = P.threads;
     I.smem_bytes = (int)tile_smem_layout(P, es).total;
     I.loop_order = loop_order;
+    I.sched = sched;
     I.grid = 0;
     I.n_tiles = n_tiles;
     for (int i = 0; i < kMaxRank; ++i) I.tile_ext[i] = i < c.rank ? spec.t[i] : 0;
@@ -376,7 +379,7 @@ void side_options(const Canon& c, const std::vector<int>& order, const int32_t* 
     }
 }
 
-void add_direct(const Canon& c, ttc_dtype dtype, bool beta_nz, int loop_order, bool vector,
+void add_direct(const Canon& c, ttc_dtype dtype, bool beta_nz, int loop_order, bool vector, int sched,
                 std::vector<Candidate>* out) {
     const int es = elem_size(dtype);
     const int mv = 16 / es;
@@ -416,7 +419,13 @@ void add_direct(const Canon& c, ttc_dtype dtype, bool beta_nz, int loop_order, b
         n_items *= (uint64_t)n;
     }
     P.n_items = n_items;
+    const uint64_t per_chunk = (uint64_t)kDirectThreads * kDirectUnroll;
+    const uint64_t n_chunks = (n_items + per_chunk - 1) / per_chunk;
+    if (n_chunks >= (uint64_t)kInt31) return;    // > 2^41 vectors: cannot be resident in HBM
+    P.n_chunks = (uint32_t)n_chunks;
+    P.dyn = sched;
     if (n_items >= (uint64_t)kInt31 / 2) idx64 = true;
+    if (c.spanA >= kInt31 || c.spanB >= kInt31) idx64 = true;   // 32-bit element offsets otherwise
     cand.idx64 = idx64;
     cand.align_a = cand.align_b = vec * es;
     ttc_candidate_info& I = cand.info;
@@ -424,6 +433,7 @@ void add_direct(const Canon& c, ttc_dtype dtype, bool beta_nz, int loop_order, b
     I.vec_a = I.vec_b = vec;
     I.threads = 256;
     I.loop_order = loop_order;
+    I.sched = sched;
     I.n_tiles = (int64_t)n_items;
     for (int i = 0; i < kMaxRank; ++i) I.tile_ext[i] = i < c.rank ? 1 : 0;
     // cost: contiguous runs seen by a warp on each side
@@ -461,11 +471,20 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, bool beta_nz, int sm_c
     const int mv = 16 / es;
     const int max_smem = std::min(max_smem_optin > 0 ? max_smem_optin : 48 * 1024, 160 * 1024);
 
-    // K1 / fallback: direct kernels (always at least the scalar one, valid for any strides).
-    for (int lo = 0; lo < 2; ++lo) {
-        add_direct(c, dtype, beta_nz, lo, true, out);
-        add_direct(c, dtype, beta_nz, lo, false, out);
+    // Work distribution (row H6): dynamic (cluster launch control) unless TTC_SCHED says
+    // "static" (persistent grid-stride) or "both" (both variants compete in the tuner).
+    std::vector<int> scheds = {1};
+    if (const char* e = std::getenv("TTC_SCHED")) {
+        if (!std::strcmp(e, "static")) scheds = {0};
+        else if (!std::strcmp(e, "both")) scheds = {1, 0};
     }
+
+    // K1 / fallback: direct kernels (always at least the scalar one, valid for any strides).
+    for (int sched : scheds)
+        for (int lo = 0; lo < 2; ++lo) {
+            add_direct(c, dtype, beta_nz, lo, true, sched, out);
+            add_direct(c, dtype, beta_nz, lo, false, sched, out);
+        }
 
     // K2 / K3: tiles.  A side = leading indices of A, B side = leading indices of B.
     std::vector<int> orderA, orderB;
@@ -496,9 +515,11 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, bool beta_nz, int sm_c
                     for (auto& vo : vopts) {
                         const int va = vo[0] == 16 ? mv : 1, vb = vo[1] == 16 ? mv : 1;
                         if (mv == 1 && (vo[0] == 16 || vo[1] == 16)) continue;
-                        Candidate cand;
-                        if (build_tile_candidate(c, dtype, beta_nz, spec, lo, va, vb, max_smem, &cand))
-                            out->push_back(cand);
+                        for (int sched : scheds) {
+                            Candidate cand;
+                            if (build_tile_candidate(c, dtype, beta_nz, spec, lo, va, vb, max_smem, sched, &cand))
+                                out->push_back(cand);
+                        }
                     }
                 }
             }

@@ -19,6 +19,8 @@ constexpr int kMaxRank = TTC_MAX_RANK;
 constexpr int kMaxTab = 6;           // canonical indices enumerated by one offset table
 constexpr int kMaxTabEntries = 2048; // entries of one offset table
 constexpr int kTileThreads = 256;    // default CTA size of the tile kernel
+constexpr int kDirectThreads = 256;  // CTA size of the direct kernel
+constexpr int kDirectUnroll = 4;     // vectors per thread and work item of the direct kernel
 
 // ---------------------------------------------------------------------------------------
 // Fast division of a 31-bit numerator by a plan-time constant (Granlund-Montgomery):
@@ -87,6 +89,8 @@ struct DirectDim {
 struct DirectParams {
     int nd;
     int vec;            // elements per item
+    int dyn;            // 1: work items handed out by cluster launch control, 0: static grid-stride
+    uint32_t n_chunks;  // work items: chunks of kDirectThreads * kDirectUnroll vectors
     uint64_t n_items;
     DirectDim dims[kMaxRank];
 };
@@ -121,6 +125,7 @@ struct TileParams {
     int same;           // 1: the vectorised index leads A and B (chunks move unchanged)
     int sstepB;         // smem stride between the vecB elements one store gathers (!same)
     int threads;
+    int dyn;            // 1: macro-tiles handed out by cluster launch control, 0: static grid-stride
     uint32_t n_tiles;
     uint32_t itemsA, itemsB;      // table entries per tile: Alo.n*Ahi.n, Blo.n*Bhi.n
     uint32_t tile_elems;          // shared-memory tile size in elements (with padding)
