@@ -60,7 +60,7 @@ int64_t phase_smem_offset(const std::vector<PhaseDim>& ph, const int32_t* ss, in
 // Relative smem cost (>= 1) of both phases for the given tile strides.
 double smem_conflict_cost(const std::vector<PhaseDim>& phA, const std::vector<PhaseDim>& phB,
                           const int32_t* ss, int es, int vecA, int vecB, bool same, int sstepB,
-                          int64_t itemsA, int64_t itemsB) {
+                          int64_t itemsA, int64_t itemsB, bool splitA) {
     double got = 0, ideal = 0;
     const int warps = 8;
     int64_t addr[32];
@@ -70,7 +70,15 @@ double smem_conflict_cost(const std::vector<PhaseDim>& phA, const std::vector<Ph
         int n = 0;
         for (int l = 0; l < 32 && startA + l < itemsA; ++l) addr[n++] = phase_smem_offset(phA, ss, startA + l) * es;
         if (n) {
-            got += smem_wavefronts(addr, n, es * vecA);
+            if (!splitA) {
+                got += smem_wavefronts(addr, n, es * vecA);
+            } else {   // the vecA elements of a global vector are stored one by one
+                for (int j = 0; j < vecA; ++j) {
+                    int64_t a2[32];
+                    for (int l = 0; l < n; ++l) a2[l] = addr[l] + (int64_t)j * es;
+                    got += smem_wavefronts(a2, n, es);
+                }
+            }
             ideal += std::max(1.0, n * es * vecA / 128.0);
         }
         const int64_t startB = (itemsB / 32) * w / warps * 32;
@@ -177,17 +185,23 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
 
     // Shared-memory strides: dense in A order, padded (in units that keep vector alignment)
     // where the bank model says the store phase would conflict.
-    const int unit = std::max(want_va, same ? mv : 1);
+    // Two ways to land a global vector of want_va elements in the tile: one vector store (rows
+    // of the tile must then stay vector-aligned, so paddings are multiples of the vector) or
+    // want_va element stores (any padding; this is what makes a transposing read of 8-byte
+    // elements conflict-free, which needs an odd row pitch).
     int32_t ss[kMaxRank];
     int32_t best_ss[kMaxRank];
     double best_cost = 1e30;
     int64_t best_elems = 0;
+    int best_split = 0;
     const int levels = (int)ta.size() - 1;
     const int search_levels = std::min(levels, 3);
     static const int pad_opts[] = {0, 1, 2, 3, 4};
     const int n_opts = 5;
     int combos = 1;
     for (int i = 0; i < search_levels; ++i) combos *= n_opts;
+    for (int split = 0; split < ((want_va > 1 && !same) ? 2 : 1); ++split) {
+    const int unit = split ? 1 : std::max(want_va, same ? mv : 1);
     for (int combo = 0; combo < combos; ++combo) {
         int cc = combo;
         int64_t stride = 1;
@@ -206,20 +220,36 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
         if (!ok) continue;
         const int64_t elems = (int64_t)ss[ta.back()] * spec.t[ta.back()];
         if (elems * es > max_smem) continue;
-        const double conf = smem_conflict_cost(phA, phB, ss, es, want_va, want_vb, same, ss[B0], itemsA, itemsB);
-        const double cost = conf + 1e-3 * (double)elems * es / 1024.0;
+        const double conf = smem_conflict_cost(phA, phB, ss, es, want_va, want_vb, same, ss[B0], itemsA, itemsB, split != 0);
+        // a split store costs want_va - 1 extra instructions per item: worth it only for a real gain
+        const double cost = conf + 1e-3 * (double)elems * es / 1024.0 + (split ? 0.08 : 0.0);
         if (cost < best_cost) {
             best_cost = cost;
             best_elems = elems;
+            best_split = split;
             std::memcpy(best_ss, ss, sizeof(ss));
         }
+    }
     }
     if (best_cost >= 1e30) return false;
     std::memcpy(ss, best_ss, sizeof(ss));
     P.tile_elems = (uint32_t)best_elems;
     P.sstepB = ss[B0];
+    P.splitA = best_split;
     P.itemsA = (uint32_t)itemsA;
     P.itemsB = (uint32_t)itemsB;
+    {   // fast path: few items per thread, and byte offsets inside the tile fit 31 bits
+        int64_t spA = 0, spB = 0;
+        for (int i = 0; i < c.rank; ++i) {
+            spA += (int64_t)(spec.t[i] - 1) * c.d[i].sA;
+            spB += (int64_t)(spec.t[i] - 1) * c.d[i].sB;
+        }
+        static const bool fast_ok = std::getenv("TTC_FAST") && std::atoi(std::getenv("TTC_FAST")) != 0;
+        const int64_t most = std::max(itemsA, itemsB);
+        P.fast = (fast_ok && most <= (int64_t)kTileSlots * kTileThreadsFast &&
+                  (spA + 1) * es < kInt31 && (spB + 1) * es < kInt31) ? 1 : 0;
+        if (P.fast) P.threads = most <= (int64_t)kTileSlots * 128 ? 128 : (most <= (int64_t)kTileSlots * 256 ? 256 : 512);
+    }
 
     // Macro-tile grid in loop order: 0 = ascending A-stride, 1 = ascending B-stride.
     int gslot_of[kMaxRank];
