@@ -267,9 +267,11 @@ def run_ours(args) -> None:
                     "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
                     "avg_launch_us": dom_us / len(dom), "algorithmic_bytes_per_launch": works[0].algorithmic_bytes,
                     "share_of_step": dom_us / sum(r["us"] for r in per_perm), "traffic": None}
-        tr = os.path.join(ROOT, "profiles", "traffic_r01.json")
+        tr = os.path.join(ROOT, "profiles", "traffic_r01.csv")     # from the ncu --set full capture
         if os.path.exists(tr):
-            roofline["traffic"] = json.load(open(tr)).get("tile_kernel_dram_bytes_per_launch")
+            for ln in open(tr):
+                if ln.startswith("tile_kernel_dram_bytes_per_launch,"):
+                    roofline["traffic"] = int(ln.split(",")[1])
 
     # ---- end to end through the public host-buffer call: pinned host A -> device, kernel,
     # device -> pinned host B, every permutation, inside the timed region

@@ -229,8 +229,8 @@ direct_kernel(const __grid_constant__ DirectParams P, const void* __restrict__ A
 // ------------------------------------------------------------------------------------------
 constexpr int kTileUnroll = 4;
 
-template <int DT, int VA, int VB, bool SAME, bool BETA, bool FAST>
-__global__ void __launch_bounds__(FAST ? kTileThreadsFast : kTileThreads)
+template <int DT, int VA, int VB, bool SAME, bool BETA>
+__global__ void __launch_bounds__(kTileThreads)
 tile_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, void* __restrict__ Bout,
             const Scalar alpha, const Scalar beta) {
     using T = typename ElemT<DT>::T;
@@ -278,30 +278,6 @@ tile_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
     }
     __syncthreads();
 
-    // Fast path (tile has at most kTileSlots items per thread and phase): the item -> offset map
-    // does not depend on the macro-tile, so each thread keeps the offsets of its own items in
-    // registers for the whole life of the CTA; an interior tile then costs no index arithmetic.
-    int32_t gA[FAST ? kTileSlots : 1], sA[FAST ? kTileSlots : 1], gB[FAST ? kTileSlots : 1], sB[FAST ? kTileSlots : 1];   // s* < 0: no item
-    if constexpr (FAST) {
-#pragma unroll
-        for (int k = 0; k < kTileSlots; ++k) {
-            const uint32_t q = tid + k * NT;
-            gA[k] = 0; sA[k] = -1; gB[k] = 0; sB[k] = -1;
-            if (q < P.itemsA) {
-                const uint32_t hi = fd_div(q, P.divAlo);
-                const int2 el = tabs[0][q - hi * P.divAlo.d], eh = tabs[1][hi];
-                gA[k] = (el.x + eh.x) * ES;
-                sA[k] = (el.y + eh.y) * ES;
-            }
-            if (q < P.itemsB) {
-                const uint32_t hi = fd_div(q, P.divBlo);
-                const int2 el = tabs[2][q - hi * P.divBlo.d], eh = tabs[3][hi];
-                gB[k] = (el.x + eh.x) * ES;
-                sB[k] = (el.y + eh.y) * ES;
-            }
-        }
-    }
-
     uint32_t tile_id = blockIdx.x;
     for (;;) {
         sched.prefetch();
@@ -346,46 +322,6 @@ tile_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
 
         const char* Ab = A + baseA * ES;
         char* Bb = B + baseB * ES;
-        if (FAST && !edge) {
-          if constexpr (FAST) {
-            {
-                RawA v[kTileSlots];
-#pragma unroll
-                for (int k = 0; k < kTileSlots; ++k)
-                    if (sA[k] >= 0) v[k] = ld_stream<RawA>(Ab + gA[k]);
-#pragma unroll
-                for (int k = 0; k < kTileSlots; ++k)
-                    if (sA[k] >= 0) st_tile<T, VA, RawA>(tile + sA[k], v[k], P.splitA != 0);
-            }
-            __syncthreads();
-            Pack<T, VB> bv[kTileSlots];
-            if (BETA) {
-#pragma unroll
-                for (int k = 0; k < kTileSlots; ++k)
-                    if (sB[k] >= 0) bv[k].raw = ld_plain<RawB>(Bb + gB[k]);
-            }
-#pragma unroll
-            for (int k = 0; k < kTileSlots; ++k) {
-                if (sB[k] >= 0) {
-                    Pack<T, VB> a, o;
-                    if (SAME || VB == 1) {
-                        a.raw = *reinterpret_cast<const RawB*>(tile + sB[k]);
-                    } else {
-#pragma unroll
-                        for (int j = 0; j < VB; ++j)
-                            a.e[j] = *reinterpret_cast<const T*>(tile + sB[k] + j * P.sstepB * ES);
-                    }
-#pragma unroll
-                    for (int j = 0; j < VB; ++j) {
-                        T x = scale(alpha, a.e[j]);
-                        if (BETA) x = add(x, scale(beta, bv[k].e[j]));
-                        o.e[j] = x;
-                    }
-                    st_global<RawB>(Bb + gB[k], o.raw);
-                }
-            }
-          }
-        } else {
         // ---- load phase: A -> tile, enumerated in ascending A-stride --------------------
         for (uint32_t q0 = tid; q0 < P.itemsA; q0 += NT * kTileUnroll) {
             RawA v[kTileUnroll];
@@ -450,7 +386,6 @@ tile_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
                 }
             }
         }
-        }   // generic path
         const bool more = sched.next(tile_id, P.n_tiles);
         if (!more) break;
         __syncthreads();   // tile and scheduler response are free again
@@ -464,22 +399,21 @@ using TileFn = void (*)(const TileParams, const void*, void*, const Scalar, cons
 using DirectFn = void (*)(const DirectParams, const void*, void*, const Scalar, const Scalar);
 
 template <int DT, int VA, int VB, bool SAME>
-static TileFn tile_fn_beta(bool beta, bool fast) {
-    if (fast) return beta ? (TileFn)tile_kernel<DT, VA, VB, SAME, true, true> : (TileFn)tile_kernel<DT, VA, VB, SAME, false, true>;
-    return beta ? (TileFn)tile_kernel<DT, VA, VB, SAME, true, false> : (TileFn)tile_kernel<DT, VA, VB, SAME, false, false>;
+static TileFn tile_fn_beta(bool beta) {
+    return beta ? (TileFn)tile_kernel<DT, VA, VB, SAME, true> : (TileFn)tile_kernel<DT, VA, VB, SAME, false>;
 }
 
 template <int DT>
-static TileFn tile_fn(int va, int vb, bool same, bool beta, bool fast) {
+static TileFn tile_fn(int va, int vb, bool same, bool beta) {
     constexpr int MV = 16 / ElemT<DT>::ES;   // elements per 16-byte access
     if constexpr (MV > 1) {
-        if (same && va == MV && vb == MV) return tile_fn_beta<DT, MV, MV, true>(beta, fast);
+        if (same && va == MV && vb == MV) return tile_fn_beta<DT, MV, MV, true>(beta);
         if (same) return nullptr;
-        if (va == MV && vb == MV) return tile_fn_beta<DT, MV, MV, false>(beta, fast);
-        if (va == MV && vb == 1) return tile_fn_beta<DT, MV, 1, false>(beta, fast);
-        if (va == 1 && vb == MV) return tile_fn_beta<DT, 1, MV, false>(beta, fast);
+        if (va == MV && vb == MV) return tile_fn_beta<DT, MV, MV, false>(beta);
+        if (va == MV && vb == 1) return tile_fn_beta<DT, MV, 1, false>(beta);
+        if (va == 1 && vb == MV) return tile_fn_beta<DT, 1, MV, false>(beta);
     }
-    if (va == 1 && vb == 1) return tile_fn_beta<DT, 1, 1, false>(beta, fast);
+    if (va == 1 && vb == 1) return tile_fn_beta<DT, 1, 1, false>(beta);
     return nullptr;
 }
 
@@ -502,10 +436,10 @@ static DirectFn direct_fn(int vec, bool beta, bool idx64) {
 static TileFn get_tile_fn(ttc_dtype dt, const Candidate& c) {
     const TileParams& p = c.tp;
     switch (dt) {
-        case TTC_F32: return tile_fn<TTC_F32>(p.vecA, p.vecB, p.same != 0, c.beta_nz, p.fast != 0);
-        case TTC_F64: return tile_fn<TTC_F64>(p.vecA, p.vecB, p.same != 0, c.beta_nz, p.fast != 0);
-        case TTC_C64: return tile_fn<TTC_C64>(p.vecA, p.vecB, p.same != 0, c.beta_nz, p.fast != 0);
-        case TTC_C128: return tile_fn<TTC_C128>(p.vecA, p.vecB, p.same != 0, c.beta_nz, p.fast != 0);
+        case TTC_F32: return tile_fn<TTC_F32>(p.vecA, p.vecB, p.same != 0, c.beta_nz);
+        case TTC_F64: return tile_fn<TTC_F64>(p.vecA, p.vecB, p.same != 0, c.beta_nz);
+        case TTC_C64: return tile_fn<TTC_C64>(p.vecA, p.vecB, p.same != 0, c.beta_nz);
+        case TTC_C128: return tile_fn<TTC_C128>(p.vecA, p.vecB, p.same != 0, c.beta_nz);
     }
     return nullptr;
 }

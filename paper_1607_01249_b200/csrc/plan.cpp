@@ -238,18 +238,6 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
     P.splitA = best_split;
     P.itemsA = (uint32_t)itemsA;
     P.itemsB = (uint32_t)itemsB;
-    {   // fast path: few items per thread, and byte offsets inside the tile fit 31 bits
-        int64_t spA = 0, spB = 0;
-        for (int i = 0; i < c.rank; ++i) {
-            spA += (int64_t)(spec.t[i] - 1) * c.d[i].sA;
-            spB += (int64_t)(spec.t[i] - 1) * c.d[i].sB;
-        }
-        static const bool fast_ok = std::getenv("TTC_FAST") && std::atoi(std::getenv("TTC_FAST")) != 0;
-        const int64_t most = std::max(itemsA, itemsB);
-        P.fast = (fast_ok && most <= (int64_t)kTileSlots * kTileThreadsFast &&
-                  (spA + 1) * es < kInt31 && (spB + 1) * es < kInt31) ? 1 : 0;
-        if (P.fast) P.threads = most <= (int64_t)kTileSlots * 128 ? 128 : (most <= (int64_t)kTileSlots * 256 ? 256 : 512);
-    }
 
     // Macro-tile grid in loop order: 0 = ascending A-stride, 1 = ascending B-stride.
     int gslot_of[kMaxRank];

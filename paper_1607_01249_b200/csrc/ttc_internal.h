@@ -19,8 +19,6 @@ constexpr int kMaxRank = TTC_MAX_RANK;
 constexpr int kMaxTab = 6;           // canonical indices enumerated by one offset table
 constexpr int kMaxTabEntries = 2048; // entries of one offset table
 constexpr int kTileThreads = 256;    // default CTA size of the tile kernel
-constexpr int kTileThreadsFast = 512;  // largest CTA of its fast path
-constexpr int kTileSlots = 4;        // fast path of the tile kernel: items per thread and phase
 constexpr int kDirectThreads = 256;  // CTA size of the direct kernel
 constexpr int kDirectUnroll = 4;     // vectors per thread and work item of the direct kernel
 
@@ -129,7 +127,6 @@ struct TileParams {
     int splitA;         // 1: a loaded vector is written to the tile as vecA element stores
     int threads;
     int dyn;            // 1: macro-tiles handed out by cluster launch control, 0: static grid-stride
-    int fast;           // 1: <= kTileSlots items per thread and phase: offsets live in registers
     uint32_t n_tiles;
     uint32_t itemsA, itemsB;      // table entries per tile: Alo.n*Ahi.n, Blo.n*Bhi.n
     uint32_t tile_elems;          // shared-memory tile size in elements (with padding)
