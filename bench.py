@@ -208,12 +208,13 @@ def run_ours(args) -> None:
     stream = torch.cuda.current_stream()
 
     def one_step(events=None):
+        # one event between consecutive launches: events[i] .. events[i + 1] brackets launch i
         for i, (p, w) in enumerate(zip(plans, works)):
             if events is not None:
-                events[i][0].record(stream)
+                events[i].record(stream)
             ttc.ttc_execute(p, 1.0, a_dev, 0.0, b_dev, stream)
-            if events is not None:
-                events[i][1].record(stream)
+        if events is not None:
+            events[len(plans)].record(stream)
 
     def barrier():
         torch.cuda.synchronize()
@@ -224,8 +225,8 @@ def run_ours(args) -> None:
     for _ in range(warmup):
         one_step()
     # per-launch events for the roofline of the dominant kernel, live in the timed region
-    ev = [[(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
-           for _ in works] for _ in range(steps)] if not args.no_launch_events else None
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(len(works) + 1)]
+          for _ in range(steps)] if not args.no_launch_events else None
     sampler = ClockSampler(local)
     sampler.start()
     time.sleep(0.25)
@@ -252,7 +253,7 @@ def run_ours(args) -> None:
     for i, (p, w) in enumerate(zip(plans, works)):
         info = ttc.ttc_plan_info(p)
         cand = ttc.ttc_plan_candidate(p, 0, info.chosen[0])
-        us = statistics.median(ev[s][i][0].elapsed_time(ev[s][i][1]) for s in range(steps)) * 1e3 if ev else None
+        us = statistics.median(ev[s][i].elapsed_time(ev[s][i + 1]) for s in range(steps)) * 1e3 if ev else None
         infos.append((w, cand, info))
         per_perm.append({"perm": "".join(map(str, w.perm)), "kernel": ttc.KERNEL_NAMES[cand.kernel],
                          "us": us, "gbs": (w.algorithmic_bytes / us / 1e3) if us else None,
