@@ -178,6 +178,16 @@ def detail_all_configs(torch, ttc, wl, path: str, peak: float) -> None:
         json.dump(rows, fh, indent=1)
 
 
+def whole_job_value(step_bytes: int, steps: int, world: int, ms_local: float, dist, device) -> tuple:
+    """(value in GB/s, ms) of the whole job: bytes of ALL ranks over the MAX of the ranks' device times."""
+    import torch
+    ms = torch.tensor([ms_local], dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+    ms_total = float(ms.item())
+    return step_bytes * steps * world / (ms_total * 1e-3) / 1e9, ms_total
+
+
 def run_ours(args) -> None:
     import torch
     from paper_1607_01249_b200 import ttc            # raises if libttc.so cannot be built/loaded
@@ -242,11 +252,7 @@ def run_ours(args) -> None:
     torch.cuda.cudart().cudaProfilerStop()
     launches = ttc.ttc_launch_count() - launches0
     clocks = sampler.stop()
-    ms = torch.tensor([t0.elapsed_time(t1)], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
-    ms_total = float(ms.item())
-    value = step_bytes * steps * world / (ms_total * 1e-3) / 1e9
+    value, ms_total = whole_job_value(step_bytes, steps, world, t0.elapsed_time(t1), dist, "cuda")
 
     # per-permutation launch durations (median over steps) and the roofline of the tile kernel
     per_perm, infos = [], []

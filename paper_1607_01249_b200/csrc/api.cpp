@@ -48,6 +48,11 @@ std::string cache_key(const ttc_plan_s* p) {
     k.append((const char*)&p->canon.rank, sizeof(int));
     k.append((const char*)p->canon.d, sizeof(CanonDim) * p->canon.rank);
     k.append((const char*)&p->sm_count, sizeof(int));
+    // the candidate lists (and so the winners' indices) depend on the generator's switches
+    const int n0 = (int)p->cands[0].size(), n1 = (int)p->cands[1].size();
+    k.append((const char*)&n0, sizeof(int));
+    k.append((const char*)&n1, sizeof(int));
+    if (const char* e = std::getenv("TTC_SCHED")) k.append(e);
     return k;
 }
 

@@ -132,3 +132,58 @@ def test_large_extent_2d_ragged_tail():
     """Several hundred tiles per side plus a ragged tail on both."""
     w = wl.Workload("rag", wl.F32, (1000 + 3, 777), (1, 0), 1.0, 0.0)
     all_candidates(w, stride=5)
+
+
+# ------------------------------------------------------------------ work distribution (row H6)
+@pytest.mark.parametrize("mode", ["static", "both"])
+def test_static_and_dynamic_distribution_agree(mode, monkeypatch):
+    """TTC_SCHED=static / both: the persistent grid-stride variants of every candidate are
+    bit-exact too (the default, cluster launch control, is what every other test runs)."""
+    monkeypatch.setenv("TTC_SCHED", mode)
+    for w in (wl.Workload("sched2d", wl.F64, (200 + 7, 150 + 3), (1, 0), 1.0, 0.0),
+              wl.Workload("sched4d", wl.F32, (24, 10, 9, 14), (3, 1, 0, 2), 1.5, 0.5),
+              wl.Workload("schedcp", wl.C64, (48, 20, 30), (0, 2, 1), 0.5 - 0.25j, 0.0)):
+        plan = ttc.ttc_plan(w.dtype, w.n, w.sizes, w.perm, w.lda, w.ldb)
+        try:
+            which = 1 if w.beta_nonzero else 0
+            n = ttc.ttc_plan_num_candidates(plan, which)
+            scheds = set()
+            for i in range(n):
+                if i >= 12 and i % 7:
+                    continue
+                scheds.add(ttc.ttc_plan_candidate(plan, which, i).sched)
+                check_bit_exact(w, plan=plan, candidate=i)
+            assert 0 in scheds
+            if mode == "both":
+                assert scheds == {0, 1}
+        finally:
+            ttc.ttc_destroy(plan)
+
+
+def test_many_tiles_per_cta_dynamic():
+    """Far more macro-tiles than resident CTAs, so the launch-control takeover path runs many
+    times per CTA (198 MB: ~7000 tiles on 148 x 6 CTAs), checked on sampled outputs by P1's
+    closed form: A holds its own logical index, B must hold the index its position maps to."""
+    w = wl.config2((2, 0, 3, 1))
+    n = w.numel
+    A = np.arange(n, dtype=np.float64)
+    a_dev = torch.from_numpy(A).cuda()
+    b_dev = torch.full((n,), -1.0, dtype=torch.float64, device="cuda")
+    plan = ttc.ttc_plan(w.dtype, w.n, w.sizes, w.perm)
+    ttc.ttc_execute(plan, 1.0, a_dev, 0.0, b_dev)
+    torch.cuda.synchronize()
+    ttc.ttc_destroy(plan)
+    got = b_dev.cpu().numpy()
+    rng = np.random.default_rng(7)
+    szb = w.sizes_b
+    for pos in rng.integers(0, n, 20000):
+        j, rem = [], int(pos)
+        for e in szb:                      # B position -> B multi-index (column-major)
+            j.append(rem % e)
+            rem //= e
+        i = [0] * 4
+        for k, pk in enumerate(w.perm):    # B position k holds A index perm[k]
+            i[pk] = j[k]
+        lin = i[0] + w.sizes[0] * (i[1] + w.sizes[1] * (i[2] + w.sizes[2] * i[3]))
+        assert got[pos] == float(lin)
+    assert np.array_equal(np.sort(got), A)
