@@ -317,7 +317,7 @@ tile_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
                         const uint32_t qq = fd_div(r, tb.d[k].div);
                         const uint32_t c = r - qq * tb.d[k].div.d;
                         r = qq;
-                        ok &= (int32_t)c * tb.d[k].step < vext[tb.d[k].gslot];
+                        ok &= (int32_t)c * tb.d[k].step < vext[tb.d[k].gslot] * tb.d[k].vmul;
                     }
                     vals[i][idx] = ok ? 1 : 0;
                 }

@@ -44,7 +44,9 @@ int smem_wavefronts(const int64_t* addr, int n, int sz) {
     return total;
 }
 
-struct PhaseDim { int dim; int32_t n, step; };
+// One enumerated index of a phase.  `fused`: this entry stands for the tile's two leading A
+// indices taken as ONE contiguous run (smem and global stride 1), see build_tile_candidate.
+struct PhaseDim { int dim; int32_t n, step; bool fused = false; };
 
 // Enumerate entry `idx` of a phase (dims fastest first) and return its tile offset in elements.
 int64_t phase_smem_offset(const std::vector<PhaseDim>& ph, const int32_t* ss, int64_t idx) {
@@ -52,7 +54,7 @@ int64_t phase_smem_offset(const std::vector<PhaseDim>& ph, const int32_t* ss, in
     for (const PhaseDim& p : ph) {
         const int64_t c = idx % p.n;
         idx /= p.n;
-        s += c * p.step * ss[p.dim];
+        s += c * p.step * (p.fused ? 1 : ss[p.dim]);
     }
     return s;
 }
@@ -162,8 +164,24 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
         if (spec.t[c.orderB[k]] > 1) tb.push_back(c.orderB[k]);
     if (ta.empty()) return false;
     const int A0 = ta[0], B0 = tb[0];
-    const int va = legal_vec(c, A0, true, spec.t[A0], mv);
+    int va = legal_vec(c, A0, true, spec.t[A0], mv);
     const int vb = legal_vec(c, B0, false, spec.t[B0], mv);
+    // K3 for a tiny/odd stride-1 extent of A (c5: 7 complex64 = 56 bytes): when the tile takes the
+    // leading index whole and the next one continues it in memory, the two are ONE contiguous run
+    // for the load phase (7 x t1 elements), which can be vectorised although the leading extent
+    // alone cannot.  The tile keeps them dense (pitch of the second = extent of the first), so a
+    // loaded vector lands as one vector; the store phase still sees two indices.  Tiles never
+    // straddle the end of the second index (its extent is a multiple of its tile extent), so no
+    // vector is cut by a tile edge.
+    bool fuseA = false;
+    if (want_va > va && want_va == mv && ta.size() >= 2 && A0 != B0) {
+        const int A1 = ta[1];
+        bool ok = c.d[A0].sA == 1 && spec.t[A0] == c.d[A0].e && c.d[A1].sA == c.d[A0].e &&
+                  ((int64_t)spec.t[A0] * spec.t[A1]) % mv == 0 && c.d[A1].e % spec.t[A1] == 0 && A1 != B0;
+        for (int i = 0; i < c.rank && ok; ++i)
+            if (i != A0 && i != A1 && c.d[i].sA % mv != 0) ok = false;
+        if (ok) { fuseA = true; va = mv; }
+    }
     if (want_va > va || want_vb > vb) return false;
     const bool same = (A0 == B0) && want_va == mv && want_vb == mv && mv > 1;
     if (A0 == B0 && want_va != want_vb) return false;   // nothing gained by mixing widths on one index
@@ -175,7 +193,12 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
 
     // Phase enumerations (entries along the vectorised leading index count vectors).
     std::vector<PhaseDim> phA, phB;
-    for (int i : ta) phA.push_back(PhaseDim{i, spec.t[i] / (i == A0 ? want_va : 1), i == A0 ? want_va : 1});
+    if (fuseA) {
+        phA.push_back(PhaseDim{ta[1], (int32_t)((int64_t)spec.t[A0] * spec.t[ta[1]] / want_va), want_va, true});
+        for (size_t k = 2; k < ta.size(); ++k) phA.push_back(PhaseDim{ta[k], spec.t[ta[k]], 1});
+    } else {
+        for (int i : ta) phA.push_back(PhaseDim{i, spec.t[i] / (i == A0 ? want_va : 1), i == A0 ? want_va : 1});
+    }
     for (int i : tb) phB.push_back(PhaseDim{i, spec.t[i] / (i == B0 ? want_vb : 1), i == B0 ? want_vb : 1});
     int64_t itemsA = 1, itemsB = 1;
     for (auto& p : phA) itemsA *= p.n;
@@ -212,7 +235,9 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
                 int pad = 0;
                 if ((int)k <= search_levels) { pad = pad_opts[cc % n_opts] * unit; cc /= n_opts; }
                 stride = stride * spec.t[ta[k - 1]];
-                stride = (stride + unit - 1) / unit * unit + pad;
+                if (fuseA && k == 1) pad = 0;                       // the fused pair stays dense
+                else stride = (stride + unit - 1) / unit * unit;
+                stride += pad;
             }
             if (stride >= kInt31) { ok = false; break; }
             ss[ta[k]] = (int32_t)stride;
@@ -270,8 +295,14 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
             d.n = p.n;
             d.step = p.step;
             d.gslot = gslot_of[p.dim];
+            d.vmul = 1;
             d.sS = ss[p.dim] * p.step;
             d.sG = (sideA ? c.d[p.dim].sA : c.d[p.dim].sB) * p.step;
+            if (p.fused) {   // one run over (A0, A1): stride 1 in A and in the tile; valid up to e(A0) * vext(A1)
+                d.vmul = spec.t[A0];
+                d.sS = p.step;
+                d.sG = p.step;
+            }
             span += (int64_t)(p.n - 1) * d.sG;
             n *= p.n;
         }

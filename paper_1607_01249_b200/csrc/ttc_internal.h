@@ -105,6 +105,7 @@ struct TabDim {
     int32_t n;          // entries along this index = t / step
     int32_t step;       // elements per entry step (vec for the vectorised leading index, else 1)
     int32_t gslot;      // position of this index in TileParams::g (for edge-tile validity)
+    int32_t vmul;       // entry c is valid iff c * step < vext[gslot] * vmul (vmul > 1: fused leading pair)
     int32_t sS;         // shared-memory stride per entry step (elements)
     int64_t sG;         // global stride per entry step (elements)
 };
