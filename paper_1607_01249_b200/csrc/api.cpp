@@ -4,6 +4,7 @@
 // PAPER.md:63), execution and host staging.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <atomic>
 #include <chrono>
 #include <cstdlib>
@@ -138,7 +139,44 @@ ttc_status tune(ttc_plan_s* p, int top_k, int reps, int budget_ms) {
             cs[i].info.tuned_us = us;
             if (best < 0 || us < best_us) { best = i; best_us = us; }
         }
-        if (best >= 0) p->winner[which] = best;
+        // Final: the first pass ranks ~300 candidates whose best ones lie within the timer's
+        // noise of each other.  The 6 fastest are timed again, interleaved (each group of launches
+        // follows a DIFFERENT kernel, as it will in use), median of 5 rounds of 4 launches.
+        if (best >= 0) {
+            std::vector<int> fin;
+            for (int i = 0; i < (int)cs.size(); ++i)
+                if (cs[i].info.tuned_us > 0.f) fin.push_back(i);
+            std::sort(fin.begin(), fin.end(), [&](int x, int y) { return cs[x].info.tuned_us < cs[y].info.tuned_us; });
+            if (fin.size() > 6) fin.resize(6);
+            if (fin.size() > 1) {
+                const int rounds = 5, per = 4;
+                std::vector<std::vector<float>> t(fin.size());
+                bool ok = true;
+                for (int r = 0; r < rounds && ok; ++r)
+                    for (size_t f = 0; f < fin.size() && ok; ++f) {
+                        cudaEventRecord(e0, st);
+                        for (int k = 0; k < per; ++k) ok &= launch_candidate(cs[fin[f]], p->dtype, alpha, beta, a, b, st) == 0;
+                        cudaEventRecord(e1, st);
+                        if (cudaEventSynchronize(e1) != cudaSuccess) { ok = false; break; }
+                        float ms = 0.f;
+                        cudaEventElapsedTime(&ms, e0, e1);
+                        t[f].push_back(ms * 1000.f / per);
+                        g_launches += per;
+                    }
+                if (ok) {
+                    best = -1;
+                    for (size_t f = 0; f < fin.size(); ++f) {
+                        std::sort(t[f].begin(), t[f].end());
+                        const float med = t[f][t[f].size() / 2];
+                        cs[fin[f]].info.tuned_us = med;
+                        if (best < 0 || med < best_us) { best = fin[f]; best_us = med; }
+                    }
+                } else {
+                    cudaGetLastError();
+                }
+            }
+            p->winner[which] = best;
+        }
     }
     if (cudaStreamSynchronize(st) != cudaSuccess) rc = TTC_ERR_CUDA;
     cudaEventDestroy(e0);

@@ -203,6 +203,8 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
     int64_t itemsA = 1, itemsB = 1;
     for (auto& p : phA) itemsA *= p.n;
     for (auto& p : phB) itemsB *= p.n;
+    // small tiles run in 128-thread CTAs: the same threads per SM, shorter barrier waits
+    if (std::max(itemsA, itemsB) <= 4 * 256) P.threads = 128;
     int splitA, splitB;
     if (!split_tables(phA, &splitA) || !split_tables(phB, &splitB)) return false;
 
