@@ -187,3 +187,37 @@ def test_many_tiles_per_cta_dynamic():
         lin = i[0] + w.sizes[0] * (i[1] + w.sizes[1] * (i[2] + w.sizes[2] * i[3]))
         assert got[pos] == float(lin)
     assert np.array_equal(np.sort(got), A)
+
+
+def test_offsets_beyond_2_31_elements():
+    """64-bit addressing: a small logical tensor inside an A buffer of 2^31 + elements (8.6 GB of
+    fp32, leading dimension 2^11 x 1024 on index 1), so element offsets do not fit 31 bits: the
+    direct kernel's IDX64 instance and the tile kernel's 64-bit tile origins.  Every candidate
+    among the first 12 and every 9th after is checked against the oracle."""
+    free, _ = torch.cuda.mem_get_info()
+    if free < 12 * 2 ** 30:
+        pytest.skip("needs 12 GB of free device memory")
+    w = wl.Workload("big", wl.F32, (1024, 4, 1024), (2, 0, 1), 1.0, 0.0, lda=(1024, 2049, 1024))
+    A = w.make_a()                      # 1024 * 2049 * 1024 elements, NaN outside the sub-tensor
+    assert A.size > 2 ** 31
+    B0 = w.make_b()
+    want = oracle_transpose(w, A, B0)
+    a_dev = torch.from_numpy(A).cuda()
+    plan = ttc.ttc_plan(w.dtype, w.n, w.sizes, w.perm, w.lda, w.ldb)
+    try:
+        n = ttc.ttc_plan_num_candidates(plan, 0)
+        kinds = set()
+        for i in list(range(n)) + [-1]:
+            kernel = ttc.ttc_plan_candidate(plan, 0, i).kernel if i >= 0 else -1
+            if i >= 12 and i % 9 and kernel != 1:
+                continue
+            ttc.ttc_plan_select(plan, 0, i)
+            kinds.add(kernel)
+            b_dev = torch.from_numpy(B0).cuda()
+            ttc.ttc_execute(plan, w.alpha, a_dev, w.beta, b_dev)
+            torch.cuda.synchronize()
+            got = b_dev.cpu().numpy()
+            assert np.array_equal(bits(got), bits(want)), "candidate %d" % i
+        assert 1 in kinds            # the direct kernel (64-bit instance) was among them
+    finally:
+        ttc.ttc_destroy(plan)
