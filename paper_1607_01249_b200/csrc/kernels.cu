@@ -398,6 +398,195 @@ tile_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
 }
 
 // ------------------------------------------------------------------------------------------
+// K2/K3, warp-specialised: ring kernel (class TTC_KERNEL_TMA)
+//
+// Warp 0 is the producer: for each macro-tile it takes from WorkSched it issues one
+// cp.async.bulk (TMA bulk copy, global -> shared, completion on an mbarrier) per tile row into
+// the next free buffer of a ring of `P.ring` tile buffers.  The other warps are consumers: they
+// wait for a full buffer, run the store phase of tile_kernel on it (gather from the tile in
+// B order, alpha/beta, 16-byte stores) and hand the buffer back.  The load of the next tiles is
+// therefore in flight for the whole store phase of the current one, inside ONE CTA, instead of
+// relying on many resident CTAs to overlap the two streams.  Only for tilings without edge tiles
+// (every tile extent divides its index extent) and 16-byte rows.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    uint32_t done = 0;
+    while (!done) {
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                     : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    }
+}
+
+template <int DT, int VB, bool BETA>
+__global__ void __launch_bounds__(kRingThreads, BETA ? 3 : 5)
+ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, void* __restrict__ Bout,
+            const Scalar alpha, const Scalar beta) {
+    using T = typename ElemT<DT>::T;
+    constexpr int ES = (int)sizeof(T);
+    using RawB = typename RawT<ES * VB>::T;
+    extern __shared__ __align__(16) unsigned char smem[];
+    const TileSmemLayout L = tile_smem_layout(P, ES);
+    int2* tabs[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) tabs[i] = reinterpret_cast<int2*>(smem + L.tab[i]);
+    const int tid = threadIdx.x;
+    const int NT = blockDim.x;
+    const int S = P.ring;
+    const char* A = static_cast<const char*>(Ain);
+    char* B = static_cast<char*>(Bout);
+
+    __shared__ __align__(16) uint4 sched_resp;
+    __shared__ __align__(8) uint64_t sched_bar;
+    __shared__ __align__(8) uint64_t full_bar[kRingMaxStages], empty_bar[kRingMaxStages];
+    __shared__ uint32_t tile_of[kRingMaxStages];
+    WorkSched sched;
+    sched.init(P.dyn != 0, &sched_bar, &sched_resp);
+    const int n_cons_warps = (NT >> 5) - 1;
+    if (tid == 0) {
+        for (int s = 0; s < S; ++s) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"((uint32_t)__cvta_generic_to_shared(&full_bar[s])));
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(&empty_bar[s])), "r"(n_cons_warps));
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    // Offset tables (1: rows of the A side, 2/3: lo/hi of the B side), once per CTA.
+#pragma unroll
+    for (int i = 1; i < 4; ++i) {
+        const Table& tb = P.tab[i];
+        for (int idx = tid; idx < tb.n; idx += NT) {
+            uint32_t r = (uint32_t)idx;
+            int32_t g = 0, s = 0;
+#pragma unroll 1
+            for (int k = 0; k < tb.nd; ++k) {
+                const uint32_t qq = fd_div(r, tb.d[k].div);
+                const uint32_t c = r - qq * tb.d[k].div.d;
+                r = qq;
+                g += (int32_t)c * (int32_t)tb.d[k].sG;
+                s += (int32_t)c * tb.d[k].sS;
+            }
+            tabs[i][idx] = make_int2(g, s);
+        }
+    }
+    __syncthreads();
+
+    if (tid < 32) {
+        // ---------------- producer warp ----------------
+        const int lane = tid;
+        const int rows = P.tab[1].n;
+        uint32_t tile_id = blockIdx.x;
+        bool more = true;
+        for (uint32_t it = 0;; ++it) {
+            const int s = (int)(it % (uint32_t)S);
+            const uint32_t full_a = (uint32_t)__cvta_generic_to_shared(&full_bar[s]);
+            if (it >= (uint32_t)S)   // the consumers have handed this buffer back
+                mbar_wait((uint32_t)__cvta_generic_to_shared(&empty_bar[s]), ((it / (uint32_t)S) - 1u) & 1u);
+            if (!more) {             // end marker for the consumers
+                if (lane == 0) {
+                    tile_of[s] = 0xFFFFFFFFu;
+                    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(full_a) : "memory");
+                }
+                break;
+            }
+            sched.prefetch();
+            int64_t baseA = 0;
+            {
+                uint32_t r = tile_id;
+#pragma unroll 1
+                for (int g = 0; g < P.nG; ++g) {
+                    const uint32_t qq = fd_div(r, P.g[g].div);
+                    const uint32_t c = r - qq * P.g[g].div.d;
+                    r = qq;
+                    baseA += (int64_t)((int32_t)c * P.g[g].t) * P.g[g].sA;
+                }
+            }
+            const char* Ab = A + baseA * ES;
+            unsigned char* tile = smem + L.tile + (uint32_t)s * L.tile_stride;
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            if (lane == 0) {
+                tile_of[s] = tile_id;
+                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;"
+                             ::"r"(full_a), "r"(P.row_bytes * (uint32_t)rows) : "memory");
+            }
+            __syncwarp();
+            for (int row = lane; row < rows; row += 32) {
+                const int2 e = tabs[1][row];
+                const uint32_t dst = (uint32_t)__cvta_generic_to_shared(tile + e.y * ES);
+                asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                             ::"r"(dst), "l"(Ab + (int64_t)e.x * ES), "r"(P.row_bytes), "r"(full_a) : "memory");
+            }
+            more = sched.next(tile_id, P.n_tiles);
+            __syncwarp();
+        }
+        return;
+    }
+    // ---------------- consumer warps ----------------
+    const int ctid = tid - 32;
+    const int NC = NT - 32;
+    const int sstep = P.sstepB * ES;
+    const FastDiv dlo = P.divBlo;
+    for (uint32_t it = 0;; ++it) {
+        const int s = (int)(it % (uint32_t)S);
+        mbar_wait((uint32_t)__cvta_generic_to_shared(&full_bar[s]), (it / (uint32_t)S) & 1u);
+        const uint32_t tile_id = tile_of[s];
+        if (tile_id == 0xFFFFFFFFu) break;
+        int64_t baseB = 0;
+        {
+            uint32_t r = tile_id;
+#pragma unroll 1
+            for (int g = 0; g < P.nG; ++g) {
+                const uint32_t qq = fd_div(r, P.g[g].div);
+                const uint32_t c = r - qq * P.g[g].div.d;
+                r = qq;
+                baseB += (int64_t)((int32_t)c * P.g[g].t) * P.g[g].sB;
+            }
+        }
+        char* Bb = B + baseB * ES;
+        const unsigned char* tile = smem + L.tile + (uint32_t)s * L.tile_stride;
+        // store phase: tile -> B, enumerated in ascending B-stride (as in tile_kernel)
+        for (uint32_t p0 = ctid; p0 < P.itemsB; p0 += NC * kTileUnroll) {
+            Pack<T, VB> bv[kTileUnroll];
+            int32_t so[kTileUnroll], go[kTileUnroll];
+            bool ok[kTileUnroll];
+#pragma unroll
+            for (int k = 0; k < kTileUnroll; ++k) {
+                const uint32_t p = p0 + k * NC;
+                ok[k] = p < P.itemsB;
+                if (ok[k]) {
+                    const uint32_t hi = fd_div(p, dlo);
+                    const uint32_t lo = p - hi * dlo.d;
+                    const int2 el = tabs[2][lo], eh = tabs[3][hi];
+                    so[k] = (el.y + eh.y) * ES;
+                    go[k] = el.x + eh.x;
+                    if (BETA) bv[k].raw = ld_plain<RawB>(Bb + (int64_t)go[k] * ES);
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < kTileUnroll; ++k) {
+                if (ok[k]) {
+                    Pack<T, VB> a, o;
+                    if (VB == 1) {
+                        a.raw = *reinterpret_cast<const RawB*>(tile + so[k]);
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < VB; ++j) a.e[j] = *reinterpret_cast<const T*>(tile + so[k] + j * sstep);
+                    }
+#pragma unroll
+                    for (int j = 0; j < VB; ++j) {
+                        T x = scale(alpha, a.e[j]);
+                        if (BETA) x = add(x, scale(beta, bv[k].e[j]));
+                        o.e[j] = x;
+                    }
+                    st_global<RawB>(Bb + (int64_t)go[k] * ES, o.raw);
+                }
+            }
+        }
+        __syncwarp();
+        if ((tid & 31) == 0)   // this warp no longer reads the buffer
+            asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"((uint32_t)__cvta_generic_to_shared(&empty_bar[s])) : "memory");
+    }
+}
+
+// ------------------------------------------------------------------------------------------
 // Dispatch: (dtype, vector widths, beta != 0) -> kernel instance
 // ------------------------------------------------------------------------------------------
 using TileFn = void (*)(const TileParams, const void*, void*, const Scalar, const Scalar);
@@ -438,8 +627,27 @@ static DirectFn direct_fn(int vec, bool beta, bool idx64) {
     return nullptr;
 }
 
+template <int DT>
+static TileFn ring_fn(int vb, bool beta) {
+    constexpr int MV = 16 / ElemT<DT>::ES;
+    if constexpr (MV > 1) {
+        if (vb == MV) return beta ? (TileFn)ring_kernel<DT, MV, true> : (TileFn)ring_kernel<DT, MV, false>;
+    }
+    if (vb == 1) return beta ? (TileFn)ring_kernel<DT, 1, true> : (TileFn)ring_kernel<DT, 1, false>;
+    return nullptr;
+}
+
 static TileFn get_tile_fn(ttc_dtype dt, const Candidate& c) {
     const TileParams& p = c.tp;
+    if (p.ring > 0) {
+        switch (dt) {
+            case TTC_F32: return ring_fn<TTC_F32>(p.vecB, c.beta_nz);
+            case TTC_F64: return ring_fn<TTC_F64>(p.vecB, c.beta_nz);
+            case TTC_C64: return ring_fn<TTC_C64>(p.vecB, c.beta_nz);
+            case TTC_C128: return ring_fn<TTC_C128>(p.vecB, c.beta_nz);
+        }
+        return nullptr;
+    }
     switch (dt) {
         case TTC_F32: return tile_fn<TTC_F32>(p.vecA, p.vecB, p.same != 0, c.beta_nz);
         case TTC_F64: return tile_fn<TTC_F64>(p.vecA, p.vecB, p.same != 0, c.beta_nz);

@@ -14,7 +14,8 @@ namespace ttc {
 
 namespace {
 
-constexpr int kMaxImplementations = 200;   // the paper's default bound
+constexpr int kMaxImplementations = 300;   // the paper's default bound is 200; ours holds the
+                                           // ring-kernel twins as well, and a candidate costs ~1 ms to time
 constexpr int64_t kInt31 = (int64_t)1 << 31;
 
 struct TileSpec {
@@ -149,7 +150,7 @@ int legal_vec(const Canon& c, int lead, bool sideA, int32_t t_lead, int mv) {
 
 // Build one tile-kernel candidate.  Returns false if the combination is not legal.
 bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const TileSpec& spec,
-                          int loop_order, int want_va, int want_vb, int max_smem, int sched, Candidate* out) {
+                          int loop_order, int want_va, int want_vb, int max_smem, int sched, int ring, Candidate* out) {
     const int es = elem_size(dtype);
     const int mv = 16 / es;
     Candidate cand;
@@ -207,6 +208,22 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
     if (std::max(itemsA, itemsB) <= 4 * 256) P.threads = 128;
     int splitA, splitB;
     if (!split_tables(phA, &splitA) || !split_tables(phB, &splitB)) return false;
+    // Ring kernel (producer warp + consumer warps, `ring` tile buffers): every tile row along the
+    // (vectorised, possibly fused) leading A index is one cp.async.bulk, so rows and addresses must
+    // be 16-byte multiples, the tile layout 16-byte granular (no split stores), the rows the hi
+    // table of the A side, and no tile may be cut by the edge of the tensor.
+    if (ring) {
+        if (want_va * es != 16 || same) return false;
+        for (int i = 0; i < c.rank; ++i)
+            if (c.d[i].e % spec.t[i] != 0) return false;
+        int64_t hi = 1;
+        for (size_t k = 1; k < phA.size(); ++k) hi *= phA[k].n;
+        if (hi > kMaxTabEntries || (int)phA.size() - 1 > kMaxTab) return false;
+        splitA = 1;
+        P.ring = ring;
+        P.row_bytes = (uint32_t)((int64_t)phA[0].n * want_va * es);
+        P.threads = 32 + (itemsB <= 4 * 256 ? 128 : 256);
+    }
 
     // Shared-memory strides: dense in A order, padded (in units that keep vector alignment)
     // where the bank model says the store phase would conflict.
@@ -225,7 +242,7 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
     const int n_opts = 5;
     int combos = 1;
     for (int i = 0; i < search_levels; ++i) combos *= n_opts;
-    for (int split = 0; split < ((want_va > 1 && !same) ? 2 : 1); ++split) {
+    for (int split = 0; split < ((want_va > 1 && !same && !ring) ? 2 : 1); ++split) {
     const int unit = split ? 1 : std::max(want_va, same ? mv : 1);
     for (int combo = 0; combo < combos; ++combo) {
         int cc = combo;
@@ -246,7 +263,7 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
         }
         if (!ok) continue;
         const int64_t elems = (int64_t)ss[ta.back()] * spec.t[ta.back()];
-        if (elems * es > max_smem) continue;
+        if (elems * es * (ring ? ring : 1) > max_smem) continue;
         const double conf = smem_conflict_cost(phA, phB, ss, es, want_va, want_vb, same, ss[B0], itemsA, itemsB, split != 0);
         // a split store costs want_va - 1 extra instructions per item: worth it only for a real gain
         const double cost = conf + 1e-3 * (double)elems * es / 1024.0 + (split ? 0.08 : 0.0);
@@ -334,7 +351,7 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
     const int64_t runA = run_len(ta, true), runB = run_len(tb, false);
 
     ttc_candidate_info& I = cand.info;
-    I.kernel = same ? TTC_KERNEL_WIDE : (ta.size() > 2 ? TTC_KERNEL_GATHER : TTC_KERNEL_TILE);
+    I.kernel = ring ? TTC_KERNEL_TMA : same ? TTC_KERNEL_WIDE : (ta.size() > 2 ? TTC_KERNEL_GATHER : TTC_KERNEL_TILE);
     I.vec_a = want_va;
     I.vec_b = want_vb;
     I.tile_u = (int)std::min<int64_t>(runA, INT32_MAX);
@@ -530,6 +547,8 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, bool beta_nz, int sm_c
         else if (!std::strcmp(e, "both")) scheds = {1, 0};
     }
 
+    static const int ring_max = std::getenv("TTC_RING") ? std::atoi(std::getenv("TTC_RING")) : 2;
+
     // K1 / fallback: direct kernels (always at least the scalar one, valid for any strides).
     for (int sched : scheds)
         for (int lo = 0; lo < 2; ++lo) {
@@ -566,11 +585,13 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, bool beta_nz, int sm_c
                     for (auto& vo : vopts) {
                         const int va = vo[0] == 16 ? mv : 1, vb = vo[1] == 16 ? mv : 1;
                         if (mv == 1 && (vo[0] == 16 || vo[1] == 16)) continue;
-                        for (int sched : scheds) {
-                            Candidate cand;
-                            if (build_tile_candidate(c, dtype, beta_nz, spec, lo, va, vb, max_smem, sched, &cand))
-                                out->push_back(cand);
-                        }
+                        for (int sched : scheds)
+                            for (int ring = 0; ring <= ring_max; ring += 2) {
+                                if (ring && bytes > 32 * 1024) continue;
+                                Candidate cand;
+                                if (build_tile_candidate(c, dtype, beta_nz, spec, lo, va, vb, max_smem, sched, ring, &cand))
+                                    out->push_back(cand);
+                            }
                     }
                 }
             }

@@ -19,6 +19,8 @@ constexpr int kMaxRank = TTC_MAX_RANK;
 constexpr int kMaxTab = 6;           // canonical indices enumerated by one offset table
 constexpr int kMaxTabEntries = 2048; // entries of one offset table
 constexpr int kTileThreads = 256;    // default CTA size of the tile kernel
+constexpr int kRingMaxStages = 4;    // ring kernel: most tile buffers per CTA
+constexpr int kRingThreads = 32 + 256;  // ring kernel: producer warp + consumer warps (launch bound)
 constexpr int kDirectThreads = 256;  // CTA size of the direct kernel
 constexpr int kDirectUnroll = 4;     // vectors per thread and work item of the direct kernel
 
@@ -126,6 +128,8 @@ struct TileParams {
     int same;           // 1: the vectorised index leads A and B (chunks move unchanged)
     int sstepB;         // smem stride between the vecB elements one store gathers (!same)
     int splitA;         // 1: a loaded vector is written to the tile as vecA element stores
+    int ring;           // > 0: ring kernel with this many tile buffers (producer warp + consumer warps)
+    uint32_t row_bytes; // ring kernel: bytes of one tile row (one cp.async.bulk each); rows = tab[1].n
     int threads;
     int dyn;            // 1: macro-tiles handed out by cluster launch control, 0: static grid-stride
     uint32_t n_tiles;
@@ -141,7 +145,8 @@ struct TileSmemLayout {
     uint32_t tab[4];     // int2 tables
     uint32_t val[4];     // uint8 validity of each table entry (edge tiles only)
     uint32_t vext;       // int32 valid extent per grid index
-    uint32_t tile;       // tile data (16-byte aligned)
+    uint32_t tile;       // tile data (16-byte aligned); ring kernel: `ring` buffers of tile_stride bytes
+    uint32_t tile_stride;
     uint32_t total;
 };
 TTC_HD TileSmemLayout tile_smem_layout(const TileParams& P, int es) {
@@ -151,7 +156,9 @@ TTC_HD TileSmemLayout tile_smem_layout(const TileParams& P, int es) {
     for (int i = 0; i < 4; ++i) { L.val[i] = o; o += ((uint32_t)P.tab[i].n + 3u) & ~3u; }
     L.vext = o; o += 4u * kMaxRank;
     o = (o + 15u) & ~15u;
-    L.tile = o; o += P.tile_elems * (uint32_t)es;
+    L.tile = o;
+    L.tile_stride = (P.tile_elems * (uint32_t)es + 15u) & ~15u;
+    o += L.tile_stride * (uint32_t)(P.ring > 0 ? P.ring : 1);
     L.total = o;
     return L;
 }
