@@ -14,8 +14,8 @@ namespace ttc {
 
 namespace {
 
-constexpr int kMaxImplementations = 300;   // the paper's default bound is 200; ours holds the
-                                           // ring-kernel twins as well, and a candidate costs ~1 ms to time
+constexpr int kMaxImplementations = 400;   // the paper's default bound is 200; ours holds the
+                                           // ring-kernel variants as well, and a candidate costs ~1 ms to time
 constexpr int64_t kInt31 = (int64_t)1 << 31;
 
 struct TileSpec {
@@ -384,6 +384,7 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
     cost *= 1.0 + 2048.0 / tile_bytes;                        // per-tile overhead
     if (tile_bytes > 48 * 1024) cost *= 1.0 + (tile_bytes - 48 * 1024) / (256.0 * 1024);   // occupancy
     if (n_tiles < 148 * 2) cost *= 1.0 + (148.0 * 2 - n_tiles) / (148.0 * 2);
+    if (ring) cost *= 0.95;   // read and write streams overlap inside the CTA
     I.est_cost = (float)cost;
     *out = cand;
     return true;
@@ -547,7 +548,7 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, bool beta_nz, int sm_c
         else if (!std::strcmp(e, "both")) scheds = {1, 0};
     }
 
-    static const int ring_max = std::getenv("TTC_RING") ? std::atoi(std::getenv("TTC_RING")) : 2;
+    static const int ring_max = std::getenv("TTC_RING") ? std::atoi(std::getenv("TTC_RING")) : 4;
 
     // K1 / fallback: direct kernels (always at least the scalar one, valid for any strides).
     for (int sched : scheds)
@@ -587,7 +588,7 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, bool beta_nz, int sm_c
                         if (mv == 1 && (vo[0] == 16 || vo[1] == 16)) continue;
                         for (int sched : scheds)
                             for (int ring = 0; ring <= ring_max; ring += 2) {
-                                if (ring && bytes > 32 * 1024) continue;
+                                if (ring && bytes * ring > 64 * 1024) continue;   // 2 buffers <= 32 KB, 4 <= 16 KB
                                 Candidate cand;
                                 if (build_tile_candidate(c, dtype, beta_nz, spec, lo, va, vb, max_smem, sched, ring, &cand))
                                     out->push_back(cand);
