@@ -269,7 +269,10 @@ def run_ours(args) -> None:
         dom = [r for r in per_perm if r["kernel"] != "copy"]
         dom_us = sum(r["us"] for r in dom)
         achieved = works[0].algorithmic_bytes * len(dom) / dom_us / 1e3
-        roofline = {"bound": "hbm", "kernel": "tile_kernel (K2/K3), %d of 23 launches per step" % len(dom),
+        n_ring = sum(1 for r in dom if r["kernel"] == "tma")
+        roofline = {"bound": "hbm",
+                    "kernel": "K2/K3 transposing kernels (ring_kernel: %d, tile_kernel: %d) of %d launches per step" % (
+                        n_ring, len(dom) - n_ring, len(per_perm)),
                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                     "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
                     "avg_launch_us": dom_us / len(dom), "algorithmic_bytes_per_launch": works[0].algorithmic_bytes,
@@ -277,7 +280,7 @@ def run_ours(args) -> None:
         tr = os.path.join(ROOT, "profiles", "traffic_r01.csv")     # from the ncu --set full capture
         if os.path.exists(tr):
             for ln in open(tr):
-                if ln.startswith("tile_kernel_dram_bytes_per_launch,"):
+                if ln.startswith("transpose_kernel_dram_bytes_per_launch,"):
                     roofline["traffic"] = int(ln.split(",")[1])
 
     # ---- end to end through the public host-buffer call: pinned host A -> device, kernel,
