@@ -523,6 +523,7 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
     const int ctid = tid - 32;
     const int NC = NT - 32;
     const int sstep = P.sstepB * ES;
+    const bool same = P.same != 0;
     const FastDiv dlo = P.divBlo;
     for (uint32_t it = 0;; ++it) {
         const int s = (int)(it % (uint32_t)S);
@@ -564,7 +565,7 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
             for (int k = 0; k < kTileUnroll; ++k) {
                 if (ok[k]) {
                     Pack<T, VB> a, o;
-                    if (VB == 1) {
+                    if (VB == 1 || same) {   // same: the vector leads A and B, chunks move unchanged
                         a.raw = *reinterpret_cast<const RawB*>(tile + so[k]);
                     } else {
 #pragma unroll

@@ -213,7 +213,7 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
     // be 16-byte multiples, the tile layout 16-byte granular (no split stores), the rows the hi
     // table of the A side, and no tile may be cut by the edge of the tensor.
     if (ring) {
-        if (want_va * es != 16 || same) return false;
+        if (want_va * es != 16 || (same && want_vb * es != 16)) return false;
         for (int i = 0; i < c.rank; ++i)
             if (c.d[i].e % spec.t[i] != 0) return false;
         int64_t hi = 1;

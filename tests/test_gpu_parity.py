@@ -221,3 +221,75 @@ def test_offsets_beyond_2_31_elements():
         assert 1 in kinds            # the direct kernel (64-bit instance) was among them
     finally:
         ttc.ttc_destroy(plan)
+
+
+# ------------------------------------------------------------------ asynchrony of ttc_execute
+def test_cuda_graph_capture_and_replay():
+    """ttc_execute is one asynchronous kernel launch with no library-side state (the work
+    distribution needs no counters): it can be captured into a CUDA graph and replayed."""
+    w = wl.Workload("graph", wl.F64, (96, 36, 32, 14), (2, 0, 3, 1), 1.5, 0.5)
+    A, B0 = w.make_a(), w.make_b()
+    want = B0.copy()
+    for _ in range(3):                       # three updates of the same B (beta != 0 accumulates)
+        want = oracle_transpose(w, A, want)
+    plan = ttc.ttc_plan(w.dtype, w.n, w.sizes, w.perm)
+    try:
+        a_dev, b_dev = torch.from_numpy(A).cuda(), torch.from_numpy(B0).cuda()
+        side = torch.cuda.Stream()
+        g = torch.cuda.CUDAGraph()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            with torch.cuda.graph(g, stream=side):
+                ttc.ttc_execute(plan, w.alpha, a_dev, w.beta, b_dev, side)
+        for _ in range(3):
+            g.replay()
+        torch.cuda.synchronize()
+        assert np.array_equal(bits(b_dev.cpu().numpy()), bits(want))
+    finally:
+        ttc.ttc_destroy(plan)
+
+
+def test_concurrent_streams_do_not_interfere():
+    """Two plans running at the same time on two streams (each kernel hands out its own
+    macro-tiles through cluster launch control; nothing is shared between launches)."""
+    w1 = wl.config2((1, 0, 2, 3))
+    w2 = wl.Workload("conc", wl.F32, (160, 144, 128), (2, 0, 1), 1.0, 0.0)
+    A1, A2 = w1.make_a(), w2.make_a()
+    want1 = oracle_transpose(w1, A1, w1.make_b())
+    want2 = oracle_transpose(w2, A2, w2.make_b())
+    p1 = ttc.ttc_plan(w1.dtype, w1.n, w1.sizes, w1.perm)
+    p2 = ttc.ttc_plan(w2.dtype, w2.n, w2.sizes, w2.perm)
+    try:
+        a1, a2 = torch.from_numpy(A1).cuda(), torch.from_numpy(A2).cuda()
+        b1, b2 = torch.zeros_like(a1), torch.zeros_like(a2)
+        s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+        torch.cuda.synchronize()
+        for _ in range(4):
+            ttc.ttc_execute(p1, 1.0, a1, 0.0, b1, s1)
+            ttc.ttc_execute(p2, 1.0, a2, 0.0, b2, s2)
+            ttc.ttc_execute(p2, 1.0, a2, 0.0, b2, s2)
+        torch.cuda.synchronize()
+        assert np.array_equal(bits(b1.cpu().numpy()), bits(want1))
+        assert np.array_equal(bits(b2.cpu().numpy()), bits(want2))
+    finally:
+        ttc.ttc_destroy(p1)
+        ttc.ttc_destroy(p2)
+
+
+def test_ring_kernel_is_covered():
+    """The warp-specialised ring kernel (class tma) exists for a divisible tiling and is bit-exact
+    for every dtype, beta on and off, when forced."""
+    for dtype in ALL_DTYPES:
+        for beta_nz in (False, True):
+            alpha, beta = scalars(dtype, beta_nz)
+            w = wl.Workload("ring", dtype, (64, 24, 48), (2, 1, 0), alpha, beta)
+            plan = ttc.ttc_plan(w.dtype, w.n, w.sizes, w.perm)
+            try:
+                which = 1 if beta_nz else 0
+                ring = [i for i in range(ttc.ttc_plan_num_candidates(plan, which))
+                        if ttc.ttc_plan_candidate(plan, which, i).kernel == 5]
+                assert ring, "no ring candidate for dtype %d" % dtype
+                for i in ring[:10]:
+                    check_bit_exact(w, plan=plan, candidate=i)
+            finally:
+                ttc.ttc_destroy(plan)
