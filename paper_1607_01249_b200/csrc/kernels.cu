@@ -439,6 +439,7 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
     __shared__ __align__(8) uint64_t sched_bar;
     __shared__ __align__(8) uint64_t full_bar[kRingMaxStages], empty_bar[kRingMaxStages];
     __shared__ uint32_t tile_of[kRingMaxStages];
+    __shared__ uint32_t edge_of[kRingMaxStages];
     WorkSched sched;
     sched.init(P.dyn != 0, &sched_bar, &sched_resp);
     const int n_cons_warps = (NT >> 5) - 1;
@@ -489,6 +490,8 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
             }
             sched.prefetch();
             int64_t baseA = 0;
+            bool edge = false;
+            int32_t* vx = reinterpret_cast<int32_t*>(smem + L.rvext) + s * kMaxRank;
             {
                 uint32_t r = tile_id;
 #pragma unroll 1
@@ -496,23 +499,56 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
                     const uint32_t qq = fd_div(r, P.g[g].div);
                     const uint32_t c = r - qq * P.g[g].div.d;
                     r = qq;
-                    baseA += (int64_t)((int32_t)c * P.g[g].t) * P.g[g].sA;
+                    const int32_t start = (int32_t)c * P.g[g].t;
+                    baseA += (int64_t)start * P.g[g].sA;
+                    const int32_t left = P.g[g].e - start;
+                    edge |= left < P.g[g].t;
+                    if (lane == 0) vx[g] = left < P.g[g].t ? left : P.g[g].t;
                 }
             }
             const char* Ab = A + baseA * ES;
             unsigned char* tile = smem + L.tile + (uint32_t)s * L.tile_stride;
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            uint32_t row_bytes = P.row_bytes;
+            uint64_t row_ok = ~0ull;            // bit j: row lane + 32 j is inside the tensor
+            uint32_t n_rows = (uint32_t)rows;
+            if (edge) {   // remainder tile: shorter rows, fewer rows
+                __syncwarp();
+                const int valid = vx[P.lead_gslot] * P.lead_vmul * ES;
+                row_bytes = (uint32_t)valid < row_bytes ? (uint32_t)valid : row_bytes;
+                row_ok = 0;
+                const Table& tb = P.tab[1];
+                int j = 0;
+                for (int row = lane; row < rows; row += 32, ++j) {
+                    uint32_t r = (uint32_t)row;
+                    bool ok = true;
+#pragma unroll 1
+                    for (int k = 0; k < tb.nd; ++k) {
+                        const uint32_t qq = fd_div(r, tb.d[k].div);
+                        const uint32_t c = r - qq * tb.d[k].div.d;
+                        r = qq;
+                        ok &= (int32_t)c * tb.d[k].step < vx[tb.d[k].gslot] * tb.d[k].vmul;
+                    }
+                    if (ok) row_ok |= 1ull << j;
+                }
+                n_rows = __reduce_add_sync(0xFFFFFFFFu, (uint32_t)__popcll(row_ok));
+            }
             if (lane == 0) {
                 tile_of[s] = tile_id;
+                edge_of[s] = edge ? 1u : 0u;
                 asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;"
-                             ::"r"(full_a), "r"(P.row_bytes * (uint32_t)rows) : "memory");
+                             ::"r"(full_a), "r"(row_bytes * n_rows) : "memory");
             }
             __syncwarp();
-            for (int row = lane; row < rows; row += 32) {
-                const int2 e = tabs[1][row];
-                const uint32_t dst = (uint32_t)__cvta_generic_to_shared(tile + e.y * ES);
-                asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                             ::"r"(dst), "l"(Ab + (int64_t)e.x * ES), "r"(P.row_bytes), "r"(full_a) : "memory");
+            {
+                int j = 0;
+                for (int row = lane; row < rows; row += 32, ++j) {
+                    if (!((row_ok >> j) & 1ull)) continue;
+                    const int2 e = tabs[1][row];
+                    const uint32_t dst = (uint32_t)__cvta_generic_to_shared(tile + e.y * ES);
+                    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                                 ::"r"(dst), "l"(Ab + (int64_t)e.x * ES), "r"(row_bytes), "r"(full_a) : "memory");
+                }
             }
             more = sched.next(tile_id, P.n_tiles);
             __syncwarp();
@@ -543,6 +579,30 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
         }
         char* Bb = B + baseB * ES;
         const unsigned char* tile = smem + L.tile + (uint32_t)s * L.tile_stride;
+        const bool edge = edge_of[s] != 0;
+        uint8_t* v2 = smem + L.rval + (uint32_t)s * L.rval_stride;
+        uint8_t* v3 = v2 + (((uint32_t)P.tab[2].n + 3u) & ~3u);
+        if (edge) {   // mark which B-side table entries are inside the tensor (consumers only)
+            const int32_t* vx = reinterpret_cast<const int32_t*>(smem + L.rvext) + s * kMaxRank;
+#pragma unroll
+            for (int i = 2; i < 4; ++i) {
+                const Table& tb = P.tab[i];
+                uint8_t* val = i == 2 ? v2 : v3;
+                for (int idx = ctid; idx < tb.n; idx += NC) {
+                    uint32_t r = (uint32_t)idx;
+                    bool ok = true;
+#pragma unroll 1
+                    for (int k = 0; k < tb.nd; ++k) {
+                        const uint32_t qq = fd_div(r, tb.d[k].div);
+                        const uint32_t c = r - qq * tb.d[k].div.d;
+                        r = qq;
+                        ok &= (int32_t)c * tb.d[k].step < vx[tb.d[k].gslot] * tb.d[k].vmul;
+                    }
+                    val[idx] = ok ? 1 : 0;
+                }
+            }
+            asm volatile("bar.sync 1, %0;" ::"r"(NC) : "memory");
+        }
         // store phase: tile -> B, enumerated in ascending B-stride (as in tile_kernel)
         for (uint32_t p0 = ctid; p0 < P.itemsB; p0 += NC * kTileUnroll) {
             Pack<T, VB> bv[kTileUnroll];
@@ -556,9 +616,10 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
                     const uint32_t hi = fd_div(p, dlo);
                     const uint32_t lo = p - hi * dlo.d;
                     const int2 el = tabs[2][lo], eh = tabs[3][hi];
+                    if (edge) ok[k] = v2[lo] & v3[hi];
                     so[k] = (el.y + eh.y) * ES;
                     go[k] = el.x + eh.x;
-                    if (BETA) bv[k].raw = ld_plain<RawB>(Bb + (int64_t)go[k] * ES);
+                    if (BETA && ok[k]) bv[k].raw = ld_plain<RawB>(Bb + (int64_t)go[k] * ES);
                 }
             }
 #pragma unroll

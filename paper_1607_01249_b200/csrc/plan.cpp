@@ -210,12 +210,10 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
     if (!split_tables(phA, &splitA) || !split_tables(phB, &splitB)) return false;
     // Ring kernel (producer warp + consumer warps, `ring` tile buffers): every tile row along the
     // (vectorised, possibly fused) leading A index is one cp.async.bulk, so rows and addresses must
-    // be 16-byte multiples, the tile layout 16-byte granular (no split stores), the rows the hi
-    // table of the A side, and no tile may be cut by the edge of the tensor.
+    // be 16-byte multiples, the tile layout 16-byte granular (no split stores) and the rows the hi
+    // table of the A side.  Edge tiles get shorter and fewer rows.
     if (ring) {
         if (want_va * es != 16 || (same && want_vb * es != 16)) return false;
-        for (int i = 0; i < c.rank; ++i)
-            if (c.d[i].e % spec.t[i] != 0) return false;
         int64_t hi = 1;
         for (size_t k = 1; k < phA.size(); ++k) hi *= phA[k].n;
         if (hi > kMaxTabEntries || (int)phA.size() - 1 > kMaxTab) return false;
@@ -302,6 +300,10 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
         if (n_tiles >= kInt31) return false;
     }
     P.n_tiles = (uint32_t)n_tiles;
+    if (ring) {
+        P.lead_gslot = gslot_of[phA[0].dim];
+        P.lead_vmul = phA[0].fused ? spec.t[A0] : 1;
+    }
 
     // Offset tables.
     auto fill = [&](Table& tb_, const std::vector<PhaseDim>& ph, int lo, int hi, bool sideA) -> bool {

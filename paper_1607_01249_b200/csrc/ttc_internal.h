@@ -130,6 +130,7 @@ struct TileParams {
     int splitA;         // 1: a loaded vector is written to the tile as vecA element stores
     int ring;           // > 0: ring kernel with this many tile buffers (producer warp + consumer warps)
     uint32_t row_bytes; // ring kernel: bytes of one tile row (one cp.async.bulk each); rows = tab[1].n
+    int lead_gslot, lead_vmul;   // ring kernel: grid slot of the row's index and its validity multiplier
     int threads;
     int dyn;            // 1: macro-tiles handed out by cluster launch control, 0: static grid-stride
     uint32_t n_tiles;
@@ -147,6 +148,8 @@ struct TileSmemLayout {
     uint32_t vext;       // int32 valid extent per grid index
     uint32_t tile;       // tile data (16-byte aligned); ring kernel: `ring` buffers of tile_stride bytes
     uint32_t tile_stride;
+    uint32_t rval, rval_stride;   // ring kernel: per-buffer validity bytes of tables 2 and 3 (edge tiles)
+    uint32_t rvext;               // ring kernel: per-buffer valid extents (kMaxRank int32 each)
     uint32_t total;
 };
 TTC_HD TileSmemLayout tile_smem_layout(const TileParams& P, int es) {
@@ -155,6 +158,10 @@ TTC_HD TileSmemLayout tile_smem_layout(const TileParams& P, int es) {
     for (int i = 0; i < 4; ++i) { L.tab[i] = o; o += 8u * (uint32_t)P.tab[i].n; }
     for (int i = 0; i < 4; ++i) { L.val[i] = o; o += ((uint32_t)P.tab[i].n + 3u) & ~3u; }
     L.vext = o; o += 4u * kMaxRank;
+    L.rval = o;
+    L.rval_stride = (((uint32_t)P.tab[2].n + 3u) & ~3u) + (((uint32_t)P.tab[3].n + 3u) & ~3u);
+    L.rvext = L.rval + L.rval_stride * (uint32_t)(P.ring > 0 ? P.ring : 0);
+    o = L.rvext + 4u * kMaxRank * (uint32_t)(P.ring > 0 ? P.ring : 0);
     o = (o + 15u) & ~15u;
     L.tile = o;
     L.tile_stride = (P.tile_elems * (uint32_t)es + 15u) & ~15u;

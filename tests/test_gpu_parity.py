@@ -282,14 +282,18 @@ def test_ring_kernel_is_covered():
     for dtype in ALL_DTYPES:
         for beta_nz in (False, True):
             alpha, beta = scalars(dtype, beta_nz)
-            w = wl.Workload("ring", dtype, (64, 24, 48), (2, 1, 0), alpha, beta)
-            plan = ttc.ttc_plan(w.dtype, w.n, w.sizes, w.perm)
-            try:
-                which = 1 if beta_nz else 0
-                ring = [i for i in range(ttc.ttc_plan_num_candidates(plan, which))
-                        if ttc.ttc_plan_candidate(plan, which, i).kernel == 5]
-                assert ring, "no ring candidate for dtype %d" % dtype
-                for i in ring[:10]:
-                    check_bit_exact(w, plan=plan, candidate=i)
-            finally:
-                ttc.ttc_destroy(plan)
+            for w in (wl.Workload("ring", dtype, (64, 24, 48), (2, 1, 0), alpha, beta),
+                      # ragged: edge tiles with shorter and fewer rows, padded A and B
+                      wl.Workload("ringedge", dtype, (100, 37, 45), (1, 2, 0), alpha, beta,
+                                  lda=(104, 40, 45), ldb=(37, 47, 100)),
+                      wl.Workload("ringedge4", dtype, (36, 7, 11, 13), (3, 1, 0, 2), alpha, beta)):
+                plan = ttc.ttc_plan(w.dtype, w.n, w.sizes, w.perm, w.lda, w.ldb)
+                try:
+                    which = 1 if beta_nz else 0
+                    ring = [i for i in range(ttc.ttc_plan_num_candidates(plan, which))
+                            if ttc.ttc_plan_candidate(plan, which, i).kernel == 5]
+                    assert ring, "no ring candidate for %s dtype %d" % (w.name, dtype)
+                    for i in ring[:12] + ring[12::5]:
+                        check_bit_exact(w, plan=plan, candidate=i)
+                finally:
+                    ttc.ttc_destroy(plan)
