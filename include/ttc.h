@@ -105,6 +105,9 @@ typedef struct {
  * and for beta != 0, and keep the fastest of each.  The search of one list ends
  * after TTC_TUNE_TOPK candidates (default 0 = all, the paper's exhaustive mode) or, once 16
  * have been timed, when TTC_TUNE_BUDGET_MS (default 400) milliseconds have passed.
+ * Winners are remembered per process; if the environment names a file in TTC_CACHE_FILE they
+ * are also appended to it and loaded by later processes (the paper's database of known
+ * solutions), so that planning the same transposition again times nothing.
  * All pointers are HOST pointers, read before the call returns.
  * Returns NULL on error; ttc_last_error() then says why.  Sizes of 0 give a valid plan
  * whose execution does nothing.  Without a CUDA device the plan is still built (heuristic

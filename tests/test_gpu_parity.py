@@ -297,3 +297,28 @@ def test_ring_kernel_is_covered():
                         check_bit_exact(w, plan=plan, candidate=i)
                 finally:
                     ttc.ttc_destroy(plan)
+
+
+def test_solution_store_on_disk(tmp_path):
+    """TTC_CACHE_FILE: the first process tunes and appends its winners, the second plans the
+    same transposition from the file (tuned, same winners, nothing timed)."""
+    import json, os, subprocess, sys
+    cache = tmp_path / "ttc_solutions.txt"
+    code = (
+        "import json, sys; sys.path.insert(0, %r)\n"
+        "from paper_1607_01249_b200 import ttc\n"
+        "l0 = ttc.ttc_launch_count()\n"
+        "p = ttc.ttc_plan(ttc.TTC_F64, 3, (96, 40, 48), (2, 0, 1))\n"
+        "i = ttc.ttc_plan_info(p)\n"
+        "print(json.dumps({'tuned': i.tuned, 'chosen': list(i.chosen), 'launches': ttc.ttc_launch_count() - l0}))\n"
+    ) % os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, TTC_CACHE_FILE=str(cache))
+    runs = []
+    for _ in range(2):
+        out = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, env=env, timeout=300)
+        assert out.returncode == 0, out.stderr[-2000:]
+        runs.append(json.loads(out.stdout.strip().splitlines()[-1]))
+    assert cache.exists() and len(cache.read_text().splitlines()) == 1
+    assert runs[0]["tuned"] == 1 and runs[0]["launches"] > 0
+    assert runs[1]["tuned"] == 1 and runs[1]["launches"] == 0
+    assert runs[0]["chosen"] == runs[1]["chosen"]
