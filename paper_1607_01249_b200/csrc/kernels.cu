@@ -418,7 +418,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 }
 
 template <int DT, int VB, bool BETA>
-__global__ void __launch_bounds__(kRingThreads, BETA ? 3 : 5)
+__global__ void __launch_bounds__(kRingThreads, BETA ? 4 : 5)
 ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, void* __restrict__ Bout,
             const Scalar alpha, const Scalar beta) {
     using T = typename ElemT<DT>::T;

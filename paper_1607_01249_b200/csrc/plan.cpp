@@ -212,16 +212,29 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
     // (vectorised, possibly fused) leading A index is one cp.async.bulk, so rows and addresses must
     // be 16-byte multiples, the tile layout 16-byte granular (no split stores) and the rows the hi
     // table of the A side.  Edge tiles get shorter and fewer rows.
+    int row_dims = 1;
     if (ring) {
         if (want_va * es != 16 || (same && want_vb * es != 16)) return false;
-        int64_t hi = 1;
-        for (size_t k = 1; k < phA.size(); ++k) hi *= phA[k].n;
-        if (hi > kMaxTabEntries || (int)phA.size() - 1 > kMaxTab) return false;
-        splitA = 1;
+        // A row = the leading A indices of the tile that form ONE contiguous run in A: an index
+        // extends the row when the previous one is taken whole and continues in memory; the tile
+        // keeps those indices dense, so the run lands as one bulk copy (c4: 8 x t1 doubles instead
+        // of 64-byte rows; c3: 24 x t1 floats).  Only the last index of a row can be cut by an edge.
+        row_dims = 1;
+        while (row_dims < (int)phA.size()) {
+            const int pd = phA[row_dims - 1].dim, nd = phA[row_dims].dim;
+            if (spec.t[pd] != c.d[pd].e || c.d[nd].sA != c.d[pd].e * c.d[pd].sA) break;
+            ++row_dims;
+        }
+        int64_t row_items = 1, hi = 1;
+        for (int k = 0; k < row_dims; ++k) row_items *= phA[k].n;
+        for (size_t k = row_dims; k < phA.size(); ++k) hi *= phA[k].n;
+        if (hi > kMaxTabEntries || (int)phA.size() - row_dims > kMaxTab || row_items * want_va * es >= (1 << 20)) return false;
+        splitA = row_dims;
         P.ring = ring;
-        P.row_bytes = (uint32_t)((int64_t)phA[0].n * want_va * es);
+        P.row_bytes = (uint32_t)(row_items * want_va * es);
         P.threads = 32 + (itemsB <= 4 * 256 ? 128 : 256);
     }
+    const int dense_levels = ring ? row_dims + (fuseA ? 1 : 0) : (fuseA ? 2 : 1);   // ta[0..dense_levels) stay dense
 
     // Shared-memory strides: dense in A order, padded (in units that keep vector alignment)
     // where the bank model says the store phase would conflict.
@@ -252,7 +265,7 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
                 int pad = 0;
                 if ((int)k <= search_levels) { pad = pad_opts[cc % n_opts] * unit; cc /= n_opts; }
                 stride = stride * spec.t[ta[k - 1]];
-                if (fuseA && k == 1) pad = 0;                       // the fused pair stays dense
+                if ((int)k < dense_levels) pad = 0;                  // a fused pair / a bulk row stays dense
                 else stride = (stride + unit - 1) / unit * unit;
                 stride += pad;
             }
@@ -301,8 +314,10 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
     }
     P.n_tiles = (uint32_t)n_tiles;
     if (ring) {
-        P.lead_gslot = gslot_of[phA[0].dim];
-        P.lead_vmul = phA[0].fused ? spec.t[A0] : 1;
+        P.lead_gslot = gslot_of[phA[row_dims - 1].dim];          // the only index of a row an edge can cut
+        int64_t vm = phA[row_dims - 1].fused ? spec.t[A0] : 1;
+        for (int k = 0; k + 1 < row_dims; ++k) vm *= (int64_t)phA[k].n * phA[k].step;
+        P.lead_vmul = (int)vm;
     }
 
     // Offset tables.
@@ -330,10 +345,11 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
         tb_.n = (int32_t)n;
         return span < kInt31 / 2;
     };
-    if (!fill(P.tab[0], phA, 0, splitA, true) || !fill(P.tab[1], phA, splitA, (int)phA.size(), true) ||
+    if (!fill(P.tab[0], phA, 0, ring ? 0 : splitA, true) || !fill(P.tab[1], phA, splitA, (int)phA.size(), true) ||
         !fill(P.tab[2], phB, 0, splitB, false) || !fill(P.tab[3], phB, splitB, (int)phB.size(), false))
         return false;
-    P.divAlo = make_fastdiv((uint32_t)P.tab[0].n);
+    if (ring) P.tab[0].n = 0;   // the ring kernel has no lo table on the A side (rows are bulk copies)
+    P.divAlo = make_fastdiv((uint32_t)std::max(1, P.tab[0].n));
     P.divBlo = make_fastdiv((uint32_t)P.tab[2].n);
     if ((int)tile_smem_layout(P, es).total > max_smem) return false;
 
