@@ -322,3 +322,24 @@ def test_solution_store_on_disk(tmp_path):
     assert runs[0]["tuned"] == 1 and runs[0]["launches"] > 0
     assert runs[1]["tuned"] == 1 and runs[1]["launches"] == 0
     assert runs[0]["chosen"] == runs[1]["chosen"]
+
+
+@pytest.mark.parametrize("dtype", [wl.F32, wl.C64])
+def test_high_rank(dtype):
+    """Rank 10 and the library's maximum rank 16 (TTC_MAX_RANK) with extents 1..3: the N-D tile
+    tables (at most 6 indices per table), the merging of many indices and the grid decomposition."""
+    rng = np.random.default_rng(16)
+    for n in (10, 16):
+        for trial in range(3):
+            sizes = tuple(int(x) for x in rng.choice([1, 2, 2, 3], size=n))
+            perm = tuple(int(p) for p in rng.permutation(n))
+            alpha, beta = scalars(dtype, trial % 2 == 1)
+            w = wl.Workload("rank%d" % n, dtype, sizes, perm, alpha, beta)
+            plan = ttc.ttc_plan(w.dtype, w.n, w.sizes, w.perm)
+            try:
+                which = 1 if w.beta_nonzero else 0
+                ncand = ttc.ttc_plan_num_candidates(plan, which)
+                for i in list(range(0, ncand, max(1, ncand // 12))) + [-1]:
+                    check_bit_exact(w, plan=plan, candidate=i if i >= 0 else None)
+            finally:
+                ttc.ttc_destroy(plan)
