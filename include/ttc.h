@@ -58,7 +58,8 @@ typedef enum {
     TTC_KERNEL_TILE = 2,    /* K2: shared-memory tiled transpose in the plane (stride-1 of A, of B)   */
     TTC_KERNEL_GATHER = 3,  /* K3: K2 whose tile sides are coarsened over several leading indices     */
     TTC_KERNEL_WIDE = 4,    /* K2 on "wide elements": a >=16-byte run that leads both A and B         */
-    TTC_KERNEL_TMA = 5      /* K2/K3 whose A-side tile is fetched by one TMA tensor-map box load      */
+    TTC_KERNEL_TMA = 5      /* K2/K3 warp-specialised: a producer warp fetches the tile rows by TMA
+                               bulk copies (cp.async.bulk) into a ring of buffers, consumers store  */
 } ttc_kernel_class;
 
 typedef struct ttc_plan_s* ttc_plan_t;

@@ -138,7 +138,7 @@ Scalar to_scalar(ttc_dtype dt, const void* s) {
     }
 }
 
-// Make candidate `idx` launchable (shared-memory opt-in, occupancy-derived persistent grid).
+// Make candidate `idx` launchable (shared-memory opt-in, grid size).
 bool ensure_prepared(ttc_plan_s* p, int which, int idx) {
     Candidate& c = p->cands[which][idx];
     if (c.info.grid > 0) return true;

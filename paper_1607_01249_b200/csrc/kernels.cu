@@ -7,8 +7,10 @@
 //                  shared memory (the micro-tile transpose is done in shared memory
 //                  on CUDA).  The tile is an N-D box, so several small leading indices can be
 //                  coarsened into each side; 16-byte global accesses on both sides; the read of
-//                  B for beta != 0 is fused into the store phase; persistent grid-stride loop
-//                  over macro-tiles in the candidate's loop order.
+//                  B for beta != 0 is fused into the store phase; persistent CTAs take macro-tiles
+//                  in the candidate's loop order through WorkSched.
+//   ring_kernel    K2/K3, warp-specialised: a producer warp loads the tile rows with TMA bulk copies
+//                  into a ring of tile buffers, consumer warps run tile_kernel's store phase.
 //
 // Arithmetic (Eq. 1): every product and sum is rounded separately
 // (__fmul_rn/__fadd_rn, never contracted into FMA) so the result is bit-identical to the
