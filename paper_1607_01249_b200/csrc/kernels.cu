@@ -411,6 +411,18 @@ tile_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
 // relying on many resident CTAs to overlap the two streams.  Only for tilings without edge tiles
 // (every tile extent divides its index extent) and 16-byte rows.
 // ------------------------------------------------------------------------------------------
+// cp.async: global -> shared without a register stop (LDGSTS), BYTES = 4, 8 or 16.
+template <int BYTES>
+__device__ __forceinline__ void cp_async(unsigned char* smem_dst, const char* gsrc) {
+    const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+    if constexpr (BYTES == 16)
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
+    else if constexpr (BYTES == 8)
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
+    else
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(gsrc) : "memory");
+}
+
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     uint32_t done = 0;
     while (!done) {
@@ -447,7 +459,8 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
     const int n_cons_warps = (NT >> 5) - 1;
     if (tid == 0) {
         for (int s = 0; s < S; ++s) {
-            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"((uint32_t)__cvta_generic_to_shared(&full_bar[s])));
+            // full: one expect_tx arrival (bulk rows) or one arrival per producer lane (cp.async rows)
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(&full_bar[s])), "r"(P.row_async ? 32 : 1));
             asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(&empty_bar[s])), "r"(n_cons_warps));
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -484,10 +497,10 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
             if (it >= (uint32_t)S)   // the consumers have handed this buffer back
                 mbar_wait((uint32_t)__cvta_generic_to_shared(&empty_bar[s]), ((it / (uint32_t)S) - 1u) & 1u);
             if (!more) {             // end marker for the consumers
-                if (lane == 0) {
-                    tile_of[s] = 0xFFFFFFFFu;
+                if (lane == 0) tile_of[s] = 0xFFFFFFFFu;
+                __syncwarp();
+                if (lane == 0 || P.row_async)
                     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(full_a) : "memory");
-                }
                 break;
             }
             sched.prefetch();
@@ -535,6 +548,24 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
                 }
                 n_rows = __reduce_add_sync(0xFFFFFFFFu, (uint32_t)__popcll(row_ok));
             }
+            if (P.row_async) {
+                // Rows that are not 16-byte aligned (odd extents of 4/8-byte elements): the warp copies
+                // each row with element-sized cp.async (LDGSTS), 32 elements per instruction; each lane
+                // then lets the mbarrier track its copies (cp.async.mbarrier.arrive.noinc).
+                if (lane == 0) {
+                    tile_of[s] = tile_id;
+                    edge_of[s] = edge ? 1u : 0u;
+                }
+                const int len = (int)(row_bytes / ES);
+                for (int row = 0; row < rows; ++row) {
+                    if (edge && !((__shfl_sync(0xFFFFFFFFu, (unsigned)(row_ok >> (row >> 5)), row & 31)) & 1u)) continue;
+                    const int2 e = tabs[1][row];
+                    const char* src = Ab + (int64_t)e.x * ES;
+                    unsigned char* dst = tile + e.y * ES;
+                    for (int x = lane; x < len; x += 32) cp_async<ES < 16 ? ES : 16>(dst + x * ES, src + x * ES);
+                }
+                asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(full_a) : "memory");
+            } else {
             if (lane == 0) {
                 tile_of[s] = tile_id;
                 edge_of[s] = edge ? 1u : 0u;
@@ -551,6 +582,7 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
                     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                                  ::"r"(dst), "l"(Ab + (int64_t)e.x * ES), "r"(row_bytes), "r"(full_a) : "memory");
                 }
+            }
             }
             more = sched.next(tile_id, P.n_tiles);
             __syncwarp();

@@ -214,7 +214,14 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
     // table of the A side.  Edge tiles get shorter and fewer rows.
     int row_dims = 1;
     if (ring) {
-        if (want_va * es != 16 || (same && want_vb * es != 16)) return false;
+        if (same && want_vb * es != 16) return false;
+        if (want_va * es != 16) {
+            // rows that cannot be 16-byte bulk copies: element-sized cp.async rows, only where the
+            // vector form is not legal (otherwise the bulk twin of this candidate is the better one)
+            if (want_va != 1 || mv == 1 || legal_vec(c, A0, true, spec.t[A0] / mv * mv, mv) == mv || same ||
+                c.d[A0].sA != 1) return false;
+            P.row_async = 1;
+        }
         // A row = the leading A indices of the tile that form ONE contiguous run in A: an index
         // extends the row when the previous one is taken whole and continues in memory; the tile
         // keeps those indices dense, so the run lands as one bulk copy (c4: 8 x t1 doubles instead
