@@ -105,9 +105,9 @@ double smem_conflict_cost(const std::vector<PhaseDim>& phA, const std::vector<Ph
 }
 
 // Efficiency model of a contiguous run of `bytes` in global memory (sector / DRAM-page use).
-double run_eff(double bytes) {
+double run_eff(double bytes, double knee = 48.0) {
     if (bytes >= 4096) return 1.0;
-    return bytes / (bytes + 48.0) / (4096.0 / (4096.0 + 48.0));
+    return bytes / (bytes + knee) / (4096.0 / (4096.0 + knee));
 }
 
 bool split_tables(const std::vector<PhaseDim>& ph, int* split_out) {
@@ -403,13 +403,22 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
     }
     const double tile_bytes = (double)itemsA * want_va * es;
     const double rd = 1.0 / run_eff((double)runA * es) * (want_va * es >= 16 ? 1.0 : 1.15);
-    const double wr = (beta_nz ? 2.0 : 1.0) / run_eff((double)runB * es) * (want_vb * es >= 16 ? 1.0 : 1.10);
+    // short runs cost much less on the B side than on the A side: the 126 MB L2 merges the writes of
+    // neighbouring tiles before they reach DRAM (measured: 64-byte B runs win several c2 permutations)
+    const double wr = (beta_nz ? 2.0 : 1.0) / run_eff((double)runB * es, 12.0) * (want_vb * es >= 16 ? 1.0 : 1.10);
     double cost = (rd + wr) * waste;
     cost *= 1.0 + 0.05 * (best_cost - 1.0);                   // smem conflicts are cheap but not free
     cost *= 1.0 + 2048.0 / tile_bytes;                        // per-tile overhead
     if (tile_bytes > 48 * 1024) cost *= 1.0 + (tile_bytes - 48 * 1024) / (256.0 * 1024);   // occupancy
     if (n_tiles < 148 * 2) cost *= 1.0 + (148.0 * 2 - n_tiles) / (148.0 * 2);
     if (ring) cost *= 0.95;   // read and write streams overlap inside the CTA
+    if (P.row_async) {
+        // one producer warp copies the rows 32 elements per instruction plus ~6 instructions per
+        // row: short rows make the producer the bottleneck (measured: 32-element rows 2.7x, 64-element
+        // rows 1.6x the time of rows of 128 and more)
+        const double len = (double)P.row_bytes / es;
+        cost *= std::max(1.0, 0.4 * (std::ceil(len / 32.0) + 6.0) / (len / 32.0));
+    }
     I.est_cost = (float)cost;
     *out = cand;
     return true;
