@@ -147,7 +147,7 @@ def cold_times(torch, ttc, plan, w, a_dev, b_dev, flush, reps: int):
     return out
 
 
-def detail_all_configs(torch, ttc, wl, path: str, peak: float) -> None:
+def detail_all_configs(torch, ttc, wl, path: str, peak: float, profile: bool = False) -> None:
     """Per-config report of all five BASELINE.json configs (north_star: 'reported per config')."""
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     rows = []
@@ -159,6 +159,12 @@ def detail_all_configs(torch, ttc, wl, path: str, peak: float) -> None:
         for _ in range(3):
             ttc.ttc_execute(plan, w.alpha, a_dev, w.beta, b_dev)
         ts = cold_times(torch, ttc, plan, w, a_dev, b_dev, flush, 21)
+        if profile and not w.name.startswith("c2"):     # one launch per config for ncu --profile-from-start off
+            torch.cuda.synchronize()
+            torch.cuda.cudart().cudaProfilerStart()
+            ttc.ttc_execute(plan, w.alpha, a_dev, w.beta, b_dev)
+            torch.cuda.synchronize()
+            torch.cuda.cudart().cudaProfilerStop()
         which = 1 if w.beta_nonzero else 0
         cand = ttc.ttc_plan_candidate(plan, which, info.chosen[which])
         t3, tm = min(ts[:3]), statistics.median(ts)
@@ -266,7 +272,7 @@ def run_ours(args) -> None:
                          "chosen": ttc.describe_candidate(cand, info.canon_rank)})
     roofline = None
     if ev:
-        dom = [r for r in per_perm if r["kernel"] != "copy"]
+        dom = [r for r in per_perm if r["kernel"] != "copy"] or per_perm      # a copy-only --perms subset
         dom_us = sum(r["us"] for r in dom)
         achieved = works[0].algorithmic_bytes * len(dom) / dom_us / 1e3
         n_ring = sum(1 for r in dom if r["kernel"] == "tma")
@@ -316,7 +322,7 @@ def run_ours(args) -> None:
     idx = np.random.default_rng(0).integers(0, last.numel, 4096)
 
     if args.detail and rank == 0:
-        detail_all_configs(torch, ttc, wl, args.detail, peak)
+        detail_all_configs(torch, ttc, wl, args.detail, peak, args.profile_detail)
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -361,6 +367,8 @@ def main() -> None:
     ap.add_argument("--detail", default=None, help="write per-config results of all 5 configs here")
     ap.add_argument("--perms", default=None, help="comma-separated subset of the 23 permutations, e.g. 1023,3021 "
                     "(profiling aid; the step is then NOT the headline workload)")
+    ap.add_argument("--profile-detail", action="store_true", help="with --detail: one extra launch of c1, c3, c4, c5 "
+                    "inside a cudaProfilerStart/Stop range (for ncu --profile-from-start off)")
     ap.add_argument("--no-launch-events", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
