@@ -25,6 +25,15 @@
  *
  * Thread safety: distinct plans may be used from distinct threads.  One plan must not be
  * executed, re-tuned or destroyed concurrently from two threads.
+ *
+ * Environment (read when a plan is built):
+ *   TTC_TUNE=0            do not time anything: the heuristic's first choice is used
+ *   TTC_TUNE_TOPK=k       time only the k best-ranked candidates of each list (default 0 = all)
+ *   TTC_TUNE_BUDGET_MS=t  after the first 16 candidates, stop timing a list after t ms (default 400)
+ *   TTC_CACHE_FILE=path   solution store on disk (winners appended, reloaded by later processes)
+ *   TTC_SCHED=static|both work distribution: persistent grid-stride instead of / beside the default,
+ *                         dynamic distribution by cluster launch control
+ *   TTC_RING=0|2|4        largest ring of tile buffers of the warp-specialised kernel (0: none; default 4)
  */
 #ifndef TTC_H_
 #define TTC_H_
