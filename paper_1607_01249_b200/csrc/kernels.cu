@@ -431,8 +431,8 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     }
 }
 
-template <int DT, int VB, bool BETA>
-__global__ void __launch_bounds__(kRingThreads, BETA ? 4 : 5)
+template <int DT, int VB, bool BETA, bool PEEL>
+__global__ void __launch_bounds__(kRingThreads, PEEL ? 3 : BETA ? 4 : 5)
 ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, void* __restrict__ Bout,
             const Scalar alpha, const Scalar beta) {
     using T = typename ElemT<DT>::T;
@@ -560,9 +560,21 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
                 for (int row = 0; row < rows; ++row) {
                     if (edge && !((__shfl_sync(0xFFFFFFFFu, (unsigned)(row_ok >> (row >> 5)), row & 31)) & 1u)) continue;
                     const int2 e = tabs[1][row];
-                    const char* src = Ab + (int64_t)e.x * ES;
-                    unsigned char* dst = tile + e.y * ES;
-                    for (int x = lane; x < len; x += 32) cp_async<ES < 16 ? ES : 16>(dst + x * ES, src + x * ES);
+                    // one warp instruction copies 32 consecutive elements; pointers advance by constants
+                    const char* src = Ab + ((int64_t)e.x + lane) * ES;
+                    uint32_t dst = (uint32_t)__cvta_generic_to_shared(tile + (e.y + lane) * ES);
+                    const int n = (len - lane + 31) >> 5;
+#pragma unroll 4
+                    for (int i = 0; i < n; ++i) {
+                        if constexpr (ES == 4)
+                            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(src) : "memory");
+                        else if constexpr (ES == 8)
+                            asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
+                        else
+                            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+                        dst += 32 * ES;
+                        src += 32 * ES;
+                    }
                 }
                 asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(full_a) : "memory");
             } else {
@@ -637,6 +649,67 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
             }
             asm volatile("bar.sync 1, %0;" ::"r"(NC) : "memory");
         }
+        if constexpr (PEEL) {
+            // Peeled store phase for B rows that are not 16-byte aligned (odd extents): a row is cut
+            // into 16-byte ALIGNED windows of B; a window inside the row is one vector store, the
+            // windows over the row's two ends are element stores.  Item = (row, window).
+            const int len = edge ? reinterpret_cast<const int32_t*>(smem + L.rvext)[s * kMaxRank + P.peel_gslot] : P.peel_len;
+            const uint32_t nch = dlo.d;                                  // windows per row (divBlo is set to it)
+            const int bmis = (int)((reinterpret_cast<uintptr_t>(B) / ES) & (uintptr_t)(VB - 1));
+            for (uint32_t p0 = ctid; p0 < P.itemsB; p0 += NC * kTileUnroll) {
+                Pack<T, VB> bv[kTileUnroll];
+                int32_t so[kTileUnroll], go[kTileUnroll], s0[kTileUnroll];
+                bool ok[kTileUnroll];
+#pragma unroll
+                for (int k = 0; k < kTileUnroll; ++k) {
+                    const uint32_t p = p0 + k * NC;
+                    ok[k] = p < P.itemsB;
+                    if (ok[k]) {
+                        const uint32_t row = fd_div(p, dlo);
+                        const int2 eh = tabs[3][row];
+                        if (edge) ok[k] = v3[row] != 0;
+                        const int m = (bmis + (int)((baseB + eh.x) & (VB - 1))) & (VB - 1);
+                        s0[k] = (int)(p - row * nch) * VB - m;          // first element of the window, row-relative
+                        ok[k] = ok[k] && s0[k] + VB > 0 && s0[k] < len;
+                        so[k] = eh.y * ES;
+                        go[k] = eh.x;
+                        if (BETA && ok[k]) {
+                            const char* src = Bb + ((int64_t)go[k] + s0[k]) * ES;
+                            if (s0[k] >= 0 && s0[k] + VB <= len) {
+                                bv[k].raw = ld_plain<RawB>(src);
+                            } else {
+#pragma unroll
+                                for (int j = 0; j < VB; ++j)
+                                    if (s0[k] + j >= 0 && s0[k] + j < len) bv[k].e[j] = *reinterpret_cast<const T*>(src + j * ES);
+                            }
+                        }
+                    }
+                }
+#pragma unroll
+                for (int k = 0; k < kTileUnroll; ++k) {
+                    if (ok[k]) {
+                        Pack<T, VB> o;
+                        const bool full = s0[k] >= 0 && s0[k] + VB <= len;
+#pragma unroll
+                        for (int j = 0; j < VB; ++j) {
+                            if (full || (s0[k] + j >= 0 && s0[k] + j < len)) {
+                                T x = scale(alpha, *reinterpret_cast<const T*>(tile + so[k] + (s0[k] + j) * sstep));
+                                if (BETA) x = add(x, scale(beta, bv[k].e[j]));
+                                o.e[j] = x;
+                            }
+                        }
+                        char* dst = Bb + ((int64_t)go[k] + s0[k]) * ES;
+                        if (full) {
+                            st_global<RawB>(dst, o.raw);
+                        } else {
+#pragma unroll
+                            for (int j = 0; j < VB; ++j)
+                                if (s0[k] + j >= 0 && s0[k] + j < len) *reinterpret_cast<T*>(dst + j * ES) = o.e[j];
+                        }
+                    }
+                }
+            }
+        } else
         // store phase: tile -> B, enumerated in ascending B-stride (as in tile_kernel)
         for (uint32_t p0 = ctid; p0 < P.itemsB; p0 += NC * kTileUnroll) {
             Pack<T, VB> bv[kTileUnroll];
@@ -724,12 +797,13 @@ static DirectFn direct_fn(int vec, bool beta, bool idx64) {
 }
 
 template <int DT>
-static TileFn ring_fn(int vb, bool beta) {
+static TileFn ring_fn(int vb, bool beta, bool peel) {
     constexpr int MV = 16 / ElemT<DT>::ES;
     if constexpr (MV > 1) {
-        if (vb == MV) return beta ? (TileFn)ring_kernel<DT, MV, true> : (TileFn)ring_kernel<DT, MV, false>;
+        if (vb == MV && peel) return beta ? (TileFn)ring_kernel<DT, MV, true, true> : (TileFn)ring_kernel<DT, MV, false, true>;
+        if (vb == MV) return beta ? (TileFn)ring_kernel<DT, MV, true, false> : (TileFn)ring_kernel<DT, MV, false, false>;
     }
-    if (vb == 1) return beta ? (TileFn)ring_kernel<DT, 1, true> : (TileFn)ring_kernel<DT, 1, false>;
+    if (vb == 1 && !peel) return beta ? (TileFn)ring_kernel<DT, 1, true, false> : (TileFn)ring_kernel<DT, 1, false, false>;
     return nullptr;
 }
 
@@ -737,10 +811,10 @@ static TileFn get_tile_fn(ttc_dtype dt, const Candidate& c) {
     const TileParams& p = c.tp;
     if (p.ring > 0) {
         switch (dt) {
-            case TTC_F32: return ring_fn<TTC_F32>(p.vecB, c.beta_nz);
-            case TTC_F64: return ring_fn<TTC_F64>(p.vecB, c.beta_nz);
-            case TTC_C64: return ring_fn<TTC_C64>(p.vecB, c.beta_nz);
-            case TTC_C128: return ring_fn<TTC_C128>(p.vecB, c.beta_nz);
+            case TTC_F32: return ring_fn<TTC_F32>(p.vecB, c.beta_nz, p.peel != 0);
+            case TTC_F64: return ring_fn<TTC_F64>(p.vecB, c.beta_nz, p.peel != 0);
+            case TTC_C64: return ring_fn<TTC_C64>(p.vecB, c.beta_nz, p.peel != 0);
+            case TTC_C128: return ring_fn<TTC_C128>(p.vecB, c.beta_nz, p.peel != 0);
         }
         return nullptr;
     }

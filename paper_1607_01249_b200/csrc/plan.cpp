@@ -183,7 +183,10 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
             if (i != A0 && i != A1 && c.d[i].sA % mv != 0) ok = false;
         if (ok) { fuseA = true; va = mv; }
     }
-    if (want_va > va || want_vb > vb) return false;
+    // Ring kernel, peeled store phase: the B-leading index is stride-1 but its rows are not
+    // 16-byte aligned (odd extent or stride): rows are cut into aligned 16-byte windows of B.
+    const bool peelB = ring && mv > 1 && want_vb == mv && vb < mv && c.d[B0].sB == 1 && A0 != B0;
+    if (want_va > va || (want_vb > vb && !peelB)) return false;
     const bool same = (A0 == B0) && want_va == mv && want_vb == mv && mv > 1;
     if (A0 == B0 && want_va != want_vb) return false;   // nothing gained by mixing widths on one index
     P.vecA = want_va;
@@ -200,7 +203,8 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
     } else {
         for (int i : ta) phA.push_back(PhaseDim{i, spec.t[i] / (i == A0 ? want_va : 1), i == A0 ? want_va : 1});
     }
-    for (int i : tb) phB.push_back(PhaseDim{i, spec.t[i] / (i == B0 ? want_vb : 1), i == B0 ? want_vb : 1});
+    const int step_b = peelB ? 1 : want_vb;   // peeled: the tables enumerate single elements of the leading index
+    for (int i : tb) phB.push_back(PhaseDim{i, spec.t[i] / (i == B0 ? step_b : 1), i == B0 ? step_b : 1});
     int64_t itemsA = 1, itemsB = 1;
     for (auto& p : phA) itemsA *= p.n;
     for (auto& p : phB) itemsB *= p.n;
@@ -240,6 +244,15 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
         P.ring = ring;
         P.row_bytes = (uint32_t)(row_items * want_va * es);
         P.threads = 32 + (itemsB <= 4 * 256 ? 128 : 256);
+    }
+    if (peelB) {
+        int64_t rowsB = 1;
+        for (size_t k = 1; k < phB.size(); ++k) rowsB *= phB[k].n;
+        if (rowsB > kMaxTabEntries || (int)phB.size() - 1 > kMaxTab || phB[0].n > kMaxTabEntries) return false;
+        splitB = 1;
+        itemsB = rowsB * ((spec.t[B0] + mv - 1) / mv + 1);     // aligned windows that can touch a row
+        P.peel = 1;
+        P.peel_len = spec.t[B0];
     }
     const int dense_levels = ring ? row_dims + (fuseA ? 1 : 0) : (fuseA ? 2 : 1);   // ta[0..dense_levels) stay dense
 
@@ -358,6 +371,10 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
     if (ring) P.tab[0].n = 0;   // the ring kernel has no lo table on the A side (rows are bulk copies)
     P.divAlo = make_fastdiv((uint32_t)std::max(1, P.tab[0].n));
     P.divBlo = make_fastdiv((uint32_t)P.tab[2].n);
+    if (peelB) {
+        P.divBlo = make_fastdiv((uint32_t)((spec.t[B0] + mv - 1) / mv + 1));
+        P.peel_gslot = gslot_of[B0];
+    }
     if ((int)tile_smem_layout(P, es).total > max_smem) return false;
 
     // Contiguous runs the tile touches in A and in B (elements): leading tile indices that are
@@ -391,7 +408,7 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
     I.n_tiles = n_tiles;
     for (int i = 0; i < kMaxRank; ++i) I.tile_ext[i] = i < c.rank ? spec.t[i] : 0;
     cand.align_a = want_va * es;
-    cand.align_b = want_vb * es;
+    cand.align_b = peelB ? es : want_vb * es;
 
     // Cost heuristic: long contiguous runs on both sides, small remainders,
     // few bank conflicts, enough bytes per tile to amortise its bookkeeping, enough tiles to
