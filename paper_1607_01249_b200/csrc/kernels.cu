@@ -561,6 +561,18 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
                     if (edge && !((__shfl_sync(0xFFFFFFFFu, (unsigned)(row_ok >> (row >> 5)), row & 31)) & 1u)) continue;
                     const int2 e = tabs[1][row];
                     // one warp instruction copies 32 consecutive elements; pointers advance by constants
+                    if (ES == 4 && P.row_pairs) {   // 4-byte elements whose rows are all 8-byte aligned: pairs
+                        const char* src = Ab + ((int64_t)e.x + 2 * lane) * ES;
+                        uint32_t dst = (uint32_t)__cvta_generic_to_shared(tile + (e.y + 2 * lane) * ES);
+                        const int n = ((len >> 1) - lane + 31) >> 5;
+#pragma unroll 4
+                        for (int i = 0; i < n; ++i) {
+                            asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
+                            dst += 64 * ES;
+                            src += 64 * ES;
+                        }
+                        continue;
+                    }
                     const char* src = Ab + ((int64_t)e.x + lane) * ES;
                     uint32_t dst = (uint32_t)__cvta_generic_to_shared(tile + (e.y + lane) * ES);
                     const int n = (len - lane + 31) >> 5;

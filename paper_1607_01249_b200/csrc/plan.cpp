@@ -225,6 +225,15 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
             if (want_va != 1 || mv == 1 || legal_vec(c, A0, true, spec.t[A0] / mv * mv, mv) == mv || same ||
                 c.d[A0].sA != 1) return false;
             P.row_async = 1;
+            // 4-byte elements: rows can be copied as 8-byte pairs when every row start and length is
+            // even (all other A strides, the leading extent and tile extent) -- the tile rows then
+            // must start at even offsets too (pitches rounded to 2 below)
+            if (es == 4 && c.d[A0].e % 2 == 0 && spec.t[A0] % 2 == 0) {
+                bool even = true;
+                for (int i = 0; i < c.rank; ++i)
+                    if (i != A0 && c.d[i].sA % 2 != 0) even = false;
+                P.row_pairs = even ? 1 : 0;
+            }
         }
         // A row = the leading A indices of the tile that form ONE contiguous run in A: an index
         // extends the row when the previous one is taken whole and continues in memory; the tile
@@ -274,7 +283,7 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
     int combos = 1;
     for (int i = 0; i < search_levels; ++i) combos *= n_opts;
     for (int split = 0; split < ((want_va > 1 && !same && !ring) ? 2 : 1); ++split) {
-    const int unit = split ? 1 : std::max(want_va, same ? mv : 1);
+    const int unit = split ? 1 : std::max(std::max(want_va, same ? mv : 1), P.row_pairs ? 2 : 1);
     for (int combo = 0; combo < combos; ++combo) {
         int cc = combo;
         int64_t stride = 1;
@@ -407,7 +416,7 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
     I.grid = 0;
     I.n_tiles = n_tiles;
     for (int i = 0; i < kMaxRank; ++i) I.tile_ext[i] = i < c.rank ? spec.t[i] : 0;
-    cand.align_a = want_va * es;
+    cand.align_a = P.row_pairs ? 8 : want_va * es;
     cand.align_b = peelB ? es : want_vb * es;
 
     // Cost heuristic: long contiguous runs on both sides, small remainders,

@@ -130,6 +130,7 @@ struct TileParams {
     int splitA;         // 1: a loaded vector is written to the tile as vecA element stores
     int ring;           // > 0: ring kernel with this many tile buffers (producer warp + consumer warps)
     uint32_t row_bytes; // ring kernel: bytes of one tile row (one cp.async.bulk each); rows = tab[1].n
+    int row_pairs;      // ring kernel, cp.async rows of 4-byte elements: 1 = every row is 8-byte aligned (copy pairs)
     int row_async;      // ring kernel: 1 = rows are copied with element-sized cp.async (rows not 16-byte aligned)
     int peel, peel_len, peel_gslot;   // ring kernel, peeled store phase: B rows cut into aligned 16-byte windows
     int lead_gslot, lead_vmul;   // ring kernel: grid slot of the row's index and its validity multiplier
