@@ -286,7 +286,11 @@ def test_ring_kernel_is_covered():
                       # ragged: edge tiles with shorter and fewer rows, padded A and B
                       wl.Workload("ringedge", dtype, (100, 37, 45), (1, 2, 0), alpha, beta,
                                   lda=(104, 40, 45), ldb=(37, 47, 100)),
-                      wl.Workload("ringedge4", dtype, (36, 7, 11, 13), (3, 1, 0, 2), alpha, beta)):
+                      wl.Workload("ringedge4", dtype, (36, 7, 11, 13), (3, 1, 0, 2), alpha, beta),
+                      # rows that are not 16-byte aligned: cp.async rows (element-sized, or 8-byte pairs
+                      # of 4-byte elements when every row is 8-byte aligned) and the peeled store phase
+                      wl.Workload("ringodd", dtype, (131, 9, 67), (2, 0, 1), alpha, beta),
+                      wl.Workload("ringeven", dtype, (130, 22, 66), (2, 1, 0), alpha, beta, lda=(134, 22, 66))):
                 plan = ttc.ttc_plan(w.dtype, w.n, w.sizes, w.perm, w.lda, w.ldb)
                 try:
                     which = 1 if beta_nz else 0
@@ -295,6 +299,13 @@ def test_ring_kernel_is_covered():
                     assert ring, "no ring candidate for %s dtype %d" % (w.name, dtype)
                     for i in ring[:12] + ring[12::5]:
                         check_bit_exact(w, plan=plan, candidate=i)
+                    if w.name == "ringodd" and dtype != wl.C128:
+                        # cp.async rows (vec_a = 1) with the peeled, vector store phase (vec_b > 1)
+                        peeled = [i for i in ring if ttc.ttc_plan_candidate(plan, which, i).vec_a == 1
+                                  and ttc.ttc_plan_candidate(plan, which, i).vec_b > 1]
+                        assert peeled, "no peeled ring candidate for %s dtype %d" % (w.name, dtype)
+                        for i in peeled[:6]:
+                            check_bit_exact(w, plan=plan, candidate=i)
                 finally:
                     ttc.ttc_destroy(plan)
 
