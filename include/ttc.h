@@ -147,7 +147,9 @@ ttc_status ttc_execute(ttc_plan_t plan, const void* alpha, const void* A,
  * (span_b elements): copies A (and B when beta != 0, or when B has padding that has to
  * survive) to the plan's private device staging buffers, runs ttc_execute, copies B back
  * and waits for it.  Synchronous.  Pinned host memory makes the copies faster but is not
- * required.
+ * required.  Contiguous tensors of 16 MB and more are cut into up to 8 slabs along one index:
+ * slab c is copied in, transposed and copied out while slab c + 1 is on its way in (the link
+ * is full duplex), on two private copy streams and the caller's stream (TTC_HOST_PIPE=0: off).
  */
 ttc_status ttc_execute_host(ttc_plan_t plan, const void* alpha, const void* A_host,
                             const void* beta, void* B_host, void* cuda_stream);

@@ -33,6 +33,14 @@ struct ttc_plan_s {
     int max_smem = 227 * 1024;
     void* stage_a = nullptr;
     void* stage_b = nullptr;
+    // ttc_execute_host pipeline (contiguous tensors): the transposition is cut into `pipe_n` slabs
+    // along canonical index `pipe_d`; slab c is copied in, transposed by `pipe_sub` and copied out
+    // while slab c + 1 is on its way in (PCIe is full duplex).
+    int pipe_state = 0;                // 0: not looked at, 1: usable, -1: not usable
+    int pipe_d = -1, pipe_n = 0;
+    ttc_plan_s* pipe_sub = nullptr;
+    cudaStream_t pipe_in = nullptr, pipe_out = nullptr;
+    std::vector<cudaEvent_t> pipe_ev;  // 2 per slab: copied in, transposed
 };
 
 namespace {
@@ -247,6 +255,8 @@ ttc_status tune(ttc_plan_s* p, int top_k, int reps, int budget_ms) {
 
 }  // namespace
 
+static void finish_plan(ttc_plan_s* p);
+
 extern "C" {
 
 ttc_plan_t ttc_plan(ttc_dtype dtype, int N, const int64_t* sizes, const int* perm,
@@ -258,7 +268,16 @@ ttc_plan_t ttc_plan(ttc_dtype dtype, int N, const int64_t* sizes, const int* per
     p->rank = N;
     ttc_status st = canonicalize(N, sizes, perm, lda, ldb, &p->canon);
     if (st != TTC_OK) { delete p; g_last_error = st; return nullptr; }
+    finish_plan(p);
+    g_last_error = TTC_OK;
+    return p;
+}
 
+}  // extern "C"
+
+// Stages 2-6 for an already canonical transposition (also used for the slabs of ttc_execute_host).
+static void finish_plan(ttc_plan_s* p) {
+    const ttc_dtype dtype = p->dtype;
     int dev = 0, count = 0;
     if (cudaGetDeviceCount(&count) == cudaSuccess && count > 0 && cudaGetDevice(&dev) == cudaSuccess) {
         int v = 0;
@@ -307,9 +326,9 @@ ttc_plan_t ttc_plan(ttc_dtype dtype, int N, const int64_t* sizes, const int* per
             disk_store(key, e);
         }
     }
-    g_last_error = TTC_OK;
-    return p;
 }
+
+extern "C" {
 
 ttc_status ttc_execute(ttc_plan_t p, const void* alpha, const void* A, const void* beta, void* B,
                        void* cuda_stream) {
@@ -336,6 +355,59 @@ ttc_status ttc_execute(ttc_plan_t p, const void* alpha, const void* A, const voi
     return rc == 0 ? TTC_OK : TTC_ERR_CUDA;
 }
 
+}  // extern "C"
+
+// Set up the slab pipeline of ttc_execute_host once per plan.  Only for contiguous tensors (then
+// a slab of canonical index d is a 2-D block in A and in B: rows of e_d * s_d elements).
+static bool pipe_setup(ttc_plan_s* p) {
+    if (p->pipe_state != 0) return p->pipe_state > 0;
+    p->pipe_state = -1;
+    const Canon& c = p->canon;
+    const int64_t es = elem_size(p->dtype);
+    if (env_int("TTC_HOST_PIPE", 1) == 0 || c.rank < 2 || c.spanA != c.numel || c.spanB != c.numel ||
+        c.numel * es < (16 << 20)) return false;
+    int best_d = -1, best_n = 0;
+    int64_t best_w = 0;
+    for (int d = 0; d < c.rank; ++d) {
+        for (int n = 8; n >= 2; --n) {
+            if (c.d[d].e % n != 0) continue;
+            const int64_t range = c.d[d].e / n;
+            const int64_t wa = range * c.d[d].sA * es, wb = range * c.d[d].sB * es;
+            if (wa % 16 != 0 || wb % 16 != 0) continue;       // slab origins stay 16-byte aligned
+            const int64_t w = std::min(wa, wb);
+            if (w > best_w) { best_w = w; best_d = d; best_n = n; }
+            break;                                             // the largest n that divides is enough
+        }
+    }
+    if (best_d < 0 || best_w < (64 << 10)) return false;       // short rows make 2-D copies slow
+    ttc_plan_s* sub = new (std::nothrow) ttc_plan_s();
+    if (!sub) return false;
+    sub->dtype = p->dtype;
+    sub->rank = p->rank;
+    sub->canon = c;
+    sub->canon.d[best_d].e = c.d[best_d].e / best_n;
+    sub->canon.numel = c.numel / best_n;
+    sub->canon.spanA = sub->canon.spanB = 1;
+    for (int i = 0; i < c.rank; ++i) {
+        sub->canon.spanA += (sub->canon.d[i].e - 1) * sub->canon.d[i].sA;
+        sub->canon.spanB += (sub->canon.d[i].e - 1) * sub->canon.d[i].sB;
+    }
+    finish_plan(sub);
+    bool ok = sub->winner[0] >= 0 && sub->winner[1] >= 0 &&
+              cudaStreamCreateWithFlags(&p->pipe_in, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaStreamCreateWithFlags(&p->pipe_out, cudaStreamNonBlocking) == cudaSuccess;
+    p->pipe_ev.resize(2 * best_n + 1);
+    for (auto& e : p->pipe_ev) ok = ok && cudaEventCreateWithFlags(&e, cudaEventDisableTiming) == cudaSuccess;
+    if (!ok) { cudaGetLastError(); ttc_destroy(sub); return false; }
+    p->pipe_sub = sub;
+    p->pipe_d = best_d;
+    p->pipe_n = best_n;
+    p->pipe_state = 1;
+    return true;
+}
+
+extern "C" {
+
 ttc_status ttc_execute_host(ttc_plan_t p, const void* alpha, const void* A_host, const void* beta,
                             void* B_host, void* cuda_stream) {
     if (!p || !alpha || !beta) return TTC_ERR_INVALID_ARG;
@@ -347,9 +419,38 @@ ttc_status ttc_execute_host(ttc_plan_t p, const void* alpha, const void* A_host,
     if (!p->stage_a && cudaMalloc(&p->stage_a, bytes_a) != cudaSuccess) { cudaGetLastError(); return TTC_ERR_ALLOC; }
     if (!p->stage_b && cudaMalloc(&p->stage_b, bytes_b) != cudaSuccess) { cudaGetLastError(); return TTC_ERR_ALLOC; }
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    if (cudaMemcpyAsync(p->stage_a, A_host, bytes_a, cudaMemcpyHostToDevice, st) != cudaSuccess) return TTC_ERR_CUDA;
     // B travels to the device when it is read (beta != 0) or has padding that must survive
     const bool b_in = !is_zero(p->dtype, beta) || p->canon.spanB != p->canon.numel;
+    if (p->forced[0] < 0 && p->forced[1] < 0 && pipe_setup(p)) {
+        // Slab pipeline: copy-in stream, the caller's stream for the kernels, copy-out stream.
+        const CanonDim& D = p->canon.d[p->pipe_d];
+        const int n = p->pipe_n;
+        const size_t range = (size_t)(D.e / n);
+        const size_t wa = range * (size_t)D.sA * es, pa = (size_t)D.e * (size_t)D.sA * es, ha = bytes_a / pa;
+        const size_t wb = range * (size_t)D.sB * es, pb = (size_t)D.e * (size_t)D.sB * es, hb = bytes_b / pb;
+        bool ok = cudaEventRecord(p->pipe_ev[2 * n], st) == cudaSuccess &&
+                  cudaStreamWaitEvent(p->pipe_in, p->pipe_ev[2 * n], 0) == cudaSuccess &&
+                  cudaStreamWaitEvent(p->pipe_out, p->pipe_ev[2 * n], 0) == cudaSuccess;
+        for (int c = 0; c < n && ok; ++c) {
+            char* da = (char*)p->stage_a + c * wa;
+            char* db = (char*)p->stage_b + c * wb;
+            ok = cudaMemcpy2DAsync(da, pa, (const char*)A_host + c * wa, pa, wa, ha, cudaMemcpyHostToDevice, p->pipe_in) == cudaSuccess;
+            if (ok && b_in)
+                ok = cudaMemcpy2DAsync(db, pb, (const char*)B_host + c * wb, pb, wb, hb, cudaMemcpyHostToDevice, p->pipe_in) == cudaSuccess;
+            ok = ok && cudaEventRecord(p->pipe_ev[2 * c], p->pipe_in) == cudaSuccess &&
+                 cudaStreamWaitEvent(st, p->pipe_ev[2 * c], 0) == cudaSuccess;
+            if (!ok) break;
+            if (ttc_execute(p->pipe_sub, alpha, da, beta, db, cuda_stream) != TTC_OK) { ok = false; break; }
+            ok = cudaEventRecord(p->pipe_ev[2 * c + 1], st) == cudaSuccess &&
+                 cudaStreamWaitEvent(p->pipe_out, p->pipe_ev[2 * c + 1], 0) == cudaSuccess &&
+                 cudaMemcpy2DAsync((char*)B_host + c * wb, pb, db, pb, wb, hb, cudaMemcpyDeviceToHost, p->pipe_out) == cudaSuccess;
+        }
+        const bool s1 = cudaStreamSynchronize(p->pipe_in) == cudaSuccess;
+        const bool s2 = cudaStreamSynchronize(st) == cudaSuccess;
+        const bool s3 = cudaStreamSynchronize(p->pipe_out) == cudaSuccess;
+        return ok && s1 && s2 && s3 ? TTC_OK : TTC_ERR_CUDA;
+    }
+    if (cudaMemcpyAsync(p->stage_a, A_host, bytes_a, cudaMemcpyHostToDevice, st) != cudaSuccess) return TTC_ERR_CUDA;
     if (b_in && cudaMemcpyAsync(p->stage_b, B_host, bytes_b, cudaMemcpyHostToDevice, st) != cudaSuccess) return TTC_ERR_CUDA;
     ttc_status rc = ttc_execute(p, alpha, p->stage_a, beta, p->stage_b, cuda_stream);
     if (rc != TTC_OK) return rc;
@@ -362,6 +463,10 @@ ttc_status ttc_destroy(ttc_plan_t p) {
     if (!p) return TTC_OK;
     if (p->stage_a) cudaFree(p->stage_a);
     if (p->stage_b) cudaFree(p->stage_b);
+    if (p->pipe_sub) ttc_destroy(p->pipe_sub);
+    if (p->pipe_in) cudaStreamDestroy(p->pipe_in);
+    if (p->pipe_out) cudaStreamDestroy(p->pipe_out);
+    for (cudaEvent_t e : p->pipe_ev) if (e) cudaEventDestroy(e);
     delete p;
     return TTC_OK;
 }

@@ -354,3 +354,27 @@ def test_high_rank(dtype):
                     check_bit_exact(w, plan=plan, candidate=i if i >= 0 else None)
             finally:
                 ttc.ttc_destroy(plan)
+
+
+@pytest.mark.parametrize("beta_nz", [False, True])
+def test_execute_host_slab_pipeline(beta_nz):
+    """ttc_execute_host on contiguous tensors of >= 16 MB runs as a slab pipeline (copy in,
+    transpose, copy out overlapped); pinned and pageable host buffers, beta on and off."""
+    alpha, beta = (1.5, 0.5) if beta_nz else (1.0, 0.0)
+    for sizes, perm in (((256, 192, 128), (2, 0, 1)), ((96, 72, 64, 56), (1, 3, 0, 2))):
+        w = wl.Workload("hostpipe", wl.F32 if len(sizes) == 3 else wl.F64, sizes, perm, alpha, beta)
+        A, B0 = w.make_a(), w.make_b(init="uniform" if beta_nz else "nan")
+        want = oracle_transpose(w, A, B0)
+        plan = ttc.ttc_plan(w.dtype, w.n, w.sizes, w.perm)
+        try:
+            got = B0.copy()
+            ttc.ttc_execute_host(plan, w.alpha, A, w.beta, got)                 # pageable
+            assert np.array_equal(bits(got), bits(want))
+            a_pin = torch.from_numpy(A).pin_memory()
+            b_pin = torch.from_numpy(B0.copy()).pin_memory()
+            for _ in range(2):                                                  # pinned, twice (buffers reused)
+                b_pin.copy_(torch.from_numpy(B0))
+                ttc.ttc_execute_host(plan, w.alpha, a_pin.numpy(), w.beta, b_pin.numpy())
+                assert np.array_equal(bits(b_pin.numpy()), bits(want))
+        finally:
+            ttc.ttc_destroy(plan)
