@@ -379,7 +379,7 @@ static bool pipe_setup(ttc_plan_s* p) {
             break;                                             // the largest n that divides is enough
         }
     }
-    if (best_d < 0 || best_w < (64 << 10)) return false;       // short rows make 2-D copies slow
+    if (best_d < 0 || best_w < (2 << 10)) return false;        // very short rows make 2-D copies slow
     ttc_plan_s* sub = new (std::nothrow) ttc_plan_s();
     if (!sub) return false;
     sub->dtype = p->dtype;
