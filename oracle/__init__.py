@@ -45,6 +45,9 @@ def _load():
             fn.restype = ctypes.c_int
             fn.argtypes = [ctypes.c_int, ctypes.c_int, i64p, i32p, i64p, i64p,
                            ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+        lib.ttc_oracle_transpose_mixed.restype = ctypes.c_int
+        lib.ttc_oracle_transpose_mixed.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, i64p, i32p, i64p, i64p,
+                                                   ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
         lib.ttc_oracle_offsets.restype = ctypes.c_int
         lib.ttc_oracle_offsets.argtypes = [ctypes.c_int, i64p, i32p, i64p, i64p, i64p, i64p, i64p]
         lib.ttc_ref_omp_threads.restype = ctypes.c_int
@@ -80,6 +83,25 @@ def _call(fn, dtype: int, sizes, perm, lda, ldb, alpha, A: np.ndarray, beta, B: 
 def transpose(dtype: int, sizes, perm, lda, ldb, alpha, A: np.ndarray, beta, B: np.ndarray) -> None:
     """In-place update of the flat buffer ``B`` by Eq. 1.  Single thread."""
     _call(_load().ttc_oracle_transpose, dtype, sizes, perm, lda, ldb, alpha, A, beta, B)
+
+
+def transpose_mixed(dtype_a: int, dtype_b: int, sizes, perm, lda, ldb, alpha, A: np.ndarray, beta,
+                    B: np.ndarray) -> None:
+    """Mixed-precision Eq. 1 (reading M1): A of ``dtype_a`` is converted to B's
+    ``dtype_b`` and the update is evaluated in B's precision.  ``alpha``/``beta`` are of ``dtype_b``."""
+    if A.dtype != _NP[dtype_a] or B.dtype != _NP[dtype_b]:
+        raise TypeError("A/B dtype does not match the dtype codes")
+    if not (A.flags.c_contiguous and B.flags.c_contiguous and B.flags.writeable):
+        raise ValueError("A and B must be flat contiguous buffers, B writeable")
+    n = len(sizes)
+    a = np.array([alpha], dtype=_NP[dtype_b])
+    b = np.array([beta], dtype=_NP[dtype_b])
+    rc = _load().ttc_oracle_transpose_mixed(
+        dtype_a, dtype_b, n, _i64(sizes), (ctypes.c_int * n)(*[int(p) for p in perm]), _i64(lda), _i64(ldb),
+        a.ctypes.data_as(ctypes.c_void_p), A.ctypes.data_as(ctypes.c_void_p),
+        b.ctypes.data_as(ctypes.c_void_p), B.ctypes.data_as(ctypes.c_void_p))
+    if rc != 0:
+        raise ValueError("oracle rejected its arguments (code %d)" % rc)
 
 
 def ref_omp_transpose(dtype: int, sizes, perm, lda, ldb, alpha, A: np.ndarray, beta, B: np.ndarray) -> None:

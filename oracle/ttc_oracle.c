@@ -27,6 +27,12 @@
  *       precision, no FMA contraction (build with -ffp-contract=off, never -ffast-math).
  *   A9  complex multiply is the textbook (ar*br - ai*bi, ar*bi + ai*br), written by hand.
  *   A13 any zero extent => nothing to do.
+ *   M1  mixed precision ("different data types for the input tensor A and the
+ *       output tensor B", e.g. --dataType=sd: A single, B double; PAPER.md:75 lists sd, ds, cz,
+ *       zc): the paper does not say in which precision Eq. 1 is evaluated.  Reading: the element
+ *       of A is first converted to B's type (exact for s->d and c->z; ONE round-to-nearest-even
+ *       per real component for d->s and z->c, overflow to +-inf), then Eq. 1 is evaluated in B's
+ *       precision with alpha and beta scalars of B's type (ttc_oracle_transpose_mixed below).
  * Parity pins: every entry point here is pinned by tests/test_oracle_pins.py (P1-P13 of
  * SURVEY.md 8(c)); nothing is "parity unpinned".
  *
@@ -176,6 +182,107 @@ int ttc_oracle_transpose(int dtype, int N, const int64_t *sizes, const int *perm
                 double yr = pb[2 * offB], yi = pb[2 * offB + 1];
                 double q0 = br * yr, q1 = bi * yi, q2 = br * yi, q3 = bi * yr;
                 double ur = q0 - q1, ui = q2 + q3;
+                pb[2 * offB] = tr + ur;
+                pb[2 * offB + 1] = ti + ui;
+            }
+        } while (next_index(N, sizes, i));
+    }
+    return 0;
+}
+
+/* Mixed precision (reading M1 in the header): A has dtype_a, B has dtype_b,
+ * alpha and beta are scalars of dtype_b.  Allowed pairs: s->d, d->s, c->z, z->c; a pair of
+ * equal types is Eq. 1 itself (ttc_oracle_transpose).  Any other pair (real <-> complex) is
+ * rejected: the paper lists none.  The conversion is the C cast (float)x / (double)x, which
+ * is IEEE-754 convertFormat under the default rounding mode. */
+int ttc_oracle_transpose_mixed(int dtype_a, int dtype_b, int N, const int64_t *sizes, const int *perm,
+                               const int64_t *lda, const int64_t *ldb,
+                               const void *alpha, const void *A, const void *beta, void *B)
+{
+    int64_t sA[ORACLE_MAX_RANK], tB[ORACLE_MAX_RANK], i[ORACLE_MAX_RANK];
+    int k, rc;
+    if (dtype_a == dtype_b)
+        return ttc_oracle_transpose(dtype_b, N, sizes, perm, lda, ldb, alpha, A, beta, B);
+    if (!((dtype_a == ORACLE_F32 && dtype_b == ORACLE_F64) || (dtype_a == ORACLE_F64 && dtype_b == ORACLE_F32) ||
+          (dtype_a == ORACLE_C64 && dtype_b == ORACLE_C128) || (dtype_a == ORACLE_C128 && dtype_b == ORACLE_C64)))
+        return -11;
+    rc = check_args(dtype_b, N, sizes, perm, lda, ldb);
+    if (rc) return rc;
+    if (!alpha || !beta) return -8;
+    for (k = 0; k < N; ++k)
+        if (sizes[k] == 0) return 0;
+    if (!A || !B) return -9;
+    strides(N, sizes, perm, lda, ldb, sA, tB);
+    for (k = 0; k < N; ++k) i[k] = 0;
+
+    if (dtype_b == ORACLE_F64) {                     /* sd: A float, B double */
+        const double a = *(const double *)alpha, b = *(const double *)beta;
+        const float *pa = (const float *)A;
+        double *pb = (double *)B;
+        do {
+            OFFSETS();
+            double x = (double)pa[offA];             /* exact */
+            double t = a * x;
+            if (b == 0.0) {
+                pb[offB] = t;
+            } else {
+                double u = b * pb[offB];
+                pb[offB] = t + u;
+            }
+        } while (next_index(N, sizes, i));
+    } else if (dtype_b == ORACLE_F32) {              /* ds: A double, B float */
+        const float a = *(const float *)alpha, b = *(const float *)beta;
+        const double *pa = (const double *)A;
+        float *pb = (float *)B;
+        do {
+            OFFSETS();
+            float x = (float)pa[offA];               /* one rounding */
+            float t = a * x;
+            if (b == 0.0f) {
+                pb[offB] = t;
+            } else {
+                float u = b * pb[offB];
+                pb[offB] = t + u;
+            }
+        } while (next_index(N, sizes, i));
+    } else if (dtype_b == ORACLE_C128) {             /* cz: A complex float, B complex double */
+        const double ar = ((const double *)alpha)[0], ai = ((const double *)alpha)[1];
+        const double br = ((const double *)beta)[0], bi = ((const double *)beta)[1];
+        const float *pa = (const float *)A;
+        double *pb = (double *)B;
+        do {
+            OFFSETS();
+            double xr = (double)pa[2 * offA], xi = (double)pa[2 * offA + 1];
+            double p0 = ar * xr, p1 = ai * xi, p2 = ar * xi, p3 = ai * xr;   /* A9 */
+            double tr = p0 - p1, ti = p2 + p3;
+            if (br == 0.0 && bi == 0.0) {
+                pb[2 * offB] = tr;
+                pb[2 * offB + 1] = ti;
+            } else {
+                double yr = pb[2 * offB], yi = pb[2 * offB + 1];
+                double q0 = br * yr, q1 = bi * yi, q2 = br * yi, q3 = bi * yr;
+                double ur = q0 - q1, ui = q2 + q3;
+                pb[2 * offB] = tr + ur;
+                pb[2 * offB + 1] = ti + ui;
+            }
+        } while (next_index(N, sizes, i));
+    } else {                                         /* zc: A complex double, B complex float */
+        const float ar = ((const float *)alpha)[0], ai = ((const float *)alpha)[1];
+        const float br = ((const float *)beta)[0], bi = ((const float *)beta)[1];
+        const double *pa = (const double *)A;
+        float *pb = (float *)B;
+        do {
+            OFFSETS();
+            float xr = (float)pa[2 * offA], xi = (float)pa[2 * offA + 1];
+            float p0 = ar * xr, p1 = ai * xi, p2 = ar * xi, p3 = ai * xr;
+            float tr = p0 - p1, ti = p2 + p3;
+            if (br == 0.0f && bi == 0.0f) {
+                pb[2 * offB] = tr;
+                pb[2 * offB + 1] = ti;
+            } else {
+                float yr = pb[2 * offB], yi = pb[2 * offB + 1];
+                float q0 = br * yr, q1 = bi * yi, q2 = br * yi, q3 = bi * yr;
+                float ur = q0 - q1, ui = q2 + q3;
                 pb[2 * offB] = tr + ur;
                 pb[2 * offB + 1] = ti + ui;
             }
