@@ -127,6 +127,27 @@ ttc_plan_t ttc_plan(ttc_dtype dtype, int N, const int64_t* sizes, const int* per
                     const int64_t* lda, const int64_t* ldb);
 
 /*
+ * ttc_plan_mixed -- ttc_plan for a mixed-precision transposition ("dataType=
+ * s,d,c,z,sd,ds,cz,zc"; "different data types for the input tensor A and the output
+ * tensor B", e.g. sd: A single, B double).  `dtype_a` is the element type of A, `dtype_b` of B.
+ * Accepted pairs: equal types (then this IS ttc_plan(dtype_b, ...)), F32->F64 (sd), F64->F32 (ds),
+ * C64->C128 (cz), C128->C64 (zc); any other pair gives NULL / TTC_ERR_UNSUPPORTED.
+ * The paper does not say in which precision Eq. 1 is then evaluated; this library (DESIGN.md
+ * reading M1) converts each element of A to B's type as it is loaded -- exact for sd and cz, one
+ * IEEE-754 round-to-nearest-even per real component for ds and zc (overflow gives +-inf) -- and
+ * evaluates Eq. 1 in B's precision, products and sum rounded separately.  For ttc_execute and
+ * ttc_execute_host of such a plan, alpha and beta are scalars of B's type, A holds span_a
+ * elements of dtype_a and B span_b elements of dtype_b; ttc_info.dtype reports dtype_b and
+ * ttc_plan_dtype_a() reports dtype_a.  Everything else is as for ttc_plan.
+ */
+ttc_plan_t ttc_plan_mixed(ttc_dtype dtype_a, ttc_dtype dtype_b, int N, const int64_t* sizes,
+                          const int* perm, const int64_t* lda, const int64_t* ldb);
+
+/* Element type of A for this plan (equals ttc_info.dtype unless the plan came from
+ * ttc_plan_mixed); -1 for a NULL plan. */
+int ttc_plan_dtype_a(ttc_plan_t plan);
+
+/*
  * ttc_execute -- Eq. 1 as ONE kernel launch on `cuda_stream` (a cudaStream_t;
  * NULL = the legacy default stream).  Asynchronous; never synchronises.
  *   alpha, beta  HOST pointers to one scalar of the plan's dtype (complex: re, im); read

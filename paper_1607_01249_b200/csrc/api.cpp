@@ -20,7 +20,8 @@
 using namespace ttc;
 
 struct ttc_plan_s {
-    ttc_dtype dtype;
+    ttc_dtype dtype;                   // B's element type: Eq. 1 is evaluated in it
+    ttc_dtype dtype_a;                 // A's element type (differs for ttc_plan_mixed only)
     int rank;
     Canon canon;
     std::vector<Candidate> cands[2];   // [0]: beta == 0, [1]: beta != 0, ranked by est_cost
@@ -55,6 +56,7 @@ std::map<std::string, CacheEntry> g_cache;
 std::string cache_key(const ttc_plan_s* p) {
     std::string k;
     k.append((const char*)&p->dtype, sizeof(p->dtype));
+    if (p->dtype_a != p->dtype) { k.append("|a"); k.append((const char*)&p->dtype_a, sizeof(p->dtype_a)); }
     k.append((const char*)&p->canon.rank, sizeof(int));
     k.append((const char*)p->canon.d, sizeof(CanonDim) * p->canon.rank);
     k.append((const char*)&p->sm_count, sizeof(int));
@@ -150,22 +152,22 @@ Scalar to_scalar(ttc_dtype dt, const void* s) {
 bool ensure_prepared(ttc_plan_s* p, int which, int idx) {
     Candidate& c = p->cands[which][idx];
     if (c.info.grid > 0) return true;
-    return prepare_candidate(&c, p->dtype, p->sm_count) == 0 && c.info.grid > 0;
+    return prepare_candidate(&c, p->dtype, p->dtype_a, p->sm_count) == 0 && c.info.grid > 0;
 }
 
 ttc_status tune(ttc_plan_s* p, int top_k, int reps, int budget_ms) {
     if (!p->have_device) return TTC_ERR_CUDA;
     if (p->canon.empty) return TTC_OK;
-    const size_t es = (size_t)elem_size(p->dtype);
+    const size_t es = (size_t)elem_size(p->dtype), esA = (size_t)elem_size(p->dtype_a);
     void *a = nullptr, *b = nullptr;
-    if (cudaMalloc(&a, (size_t)p->canon.spanA * es) != cudaSuccess) { cudaGetLastError(); return TTC_ERR_ALLOC; }
+    if (cudaMalloc(&a, (size_t)p->canon.spanA * esA) != cudaSuccess) { cudaGetLastError(); return TTC_ERR_ALLOC; }
     if (cudaMalloc(&b, (size_t)p->canon.spanB * es) != cudaSuccess) { cudaGetLastError(); cudaFree(a); return TTC_ERR_ALLOC; }
     cudaStream_t st;
     cudaEvent_t e0, e1;
     cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
     cudaEventCreate(&e0);
     cudaEventCreate(&e1);
-    cudaMemsetAsync(a, 0, (size_t)p->canon.spanA * es, st);
+    cudaMemsetAsync(a, 0, (size_t)p->canon.spanA * esA, st);
     cudaMemsetAsync(b, 0, (size_t)p->canon.spanB * es, st);
     const Scalar alpha{1.0, 0.0};
     ttc_status rc = TTC_OK;
@@ -187,12 +189,12 @@ ttc_status tune(ttc_plan_s* p, int top_k, int reps, int budget_ms) {
             // the scalar fallback is always timed so that it is known to work
             if ((i >= n || over_budget) && i != p->scalar[which]) continue;
             if (!ensure_prepared(p, which, i)) continue;
-            if (launch_candidate(cs[i], p->dtype, alpha, beta, a, b, st) != 0) { cudaGetLastError(); continue; }
+            if (launch_candidate(cs[i], p->dtype, p->dtype_a, alpha, beta, a, b, st) != 0) { cudaGetLastError(); continue; }
             float us = 1e30f;
             bool ok = true;
             for (int g = 0; g < 3 && ok; ++g) {   // minimum over groups (min of 3 runs)
                 cudaEventRecord(e0, st);
-                for (int r = 0; r < reps; ++r) ok &= launch_candidate(cs[i], p->dtype, alpha, beta, a, b, st) == 0;
+                for (int r = 0; r < reps; ++r) ok &= launch_candidate(cs[i], p->dtype, p->dtype_a, alpha, beta, a, b, st) == 0;
                 cudaEventRecord(e1, st);
                 if (cudaEventSynchronize(e1) != cudaSuccess) { ok = false; break; }
                 float ms = 0.f;
@@ -220,7 +222,7 @@ ttc_status tune(ttc_plan_s* p, int top_k, int reps, int budget_ms) {
                 for (int r = 0; r < rounds && ok; ++r)
                     for (size_t f = 0; f < fin.size() && ok; ++f) {
                         cudaEventRecord(e0, st);
-                        for (int k = 0; k < per; ++k) ok &= launch_candidate(cs[fin[f]], p->dtype, alpha, beta, a, b, st) == 0;
+                        for (int k = 0; k < per; ++k) ok &= launch_candidate(cs[fin[f]], p->dtype, p->dtype_a, alpha, beta, a, b, st) == 0;
                         cudaEventRecord(e1, st);
                         if (cudaEventSynchronize(e1) != cudaSuccess) { ok = false; break; }
                         float ms = 0.f;
@@ -261,10 +263,17 @@ extern "C" {
 
 ttc_plan_t ttc_plan(ttc_dtype dtype, int N, const int64_t* sizes, const int* perm,
                     const int64_t* lda, const int64_t* ldb) {
-    if ((int)dtype < 0 || (int)dtype > 3) { g_last_error = TTC_ERR_INVALID_ARG; return nullptr; }
+    return ttc_plan_mixed(dtype, dtype, N, sizes, perm, lda, ldb);
+}
+
+ttc_plan_t ttc_plan_mixed(ttc_dtype dtype_a, ttc_dtype dtype, int N, const int64_t* sizes, const int* perm,
+                          const int64_t* lda, const int64_t* ldb) {
+    if ((int)dtype < 0 || (int)dtype > 3 || (int)dtype_a < 0 || (int)dtype_a > 3) { g_last_error = TTC_ERR_INVALID_ARG; return nullptr; }
+    if (!valid_pair(dtype_a, dtype)) { g_last_error = TTC_ERR_UNSUPPORTED; return nullptr; }
     ttc_plan_s* p = new (std::nothrow) ttc_plan_s();
     if (!p) { g_last_error = TTC_ERR_ALLOC; return nullptr; }
     p->dtype = dtype;
+    p->dtype_a = dtype_a;
     p->rank = N;
     ttc_status st = canonicalize(N, sizes, perm, lda, ldb, &p->canon);
     if (st != TTC_OK) { delete p; g_last_error = st; return nullptr; }
@@ -289,11 +298,11 @@ static void finish_plan(ttc_plan_s* p) {
     }
 
     for (int which = 0; which < 2; ++which) {
-        generate_candidates(p->canon, dtype, which == 1, p->sm_count, p->max_smem, &p->cands[which]);
+        generate_candidates(p->canon, dtype, p->dtype_a, which == 1, p->sm_count, p->max_smem, &p->cands[which]);
         std::vector<Candidate>& cs = p->cands[which];
-        const int es = elem_size(dtype);
+        const int es = elem_size(dtype), esA = elem_size(p->dtype_a);
         for (int i = 0; i < (int)cs.size(); ++i) {
-            if (cs[i].align_a == es && cs[i].align_b == es && p->scalar[which] < 0) p->scalar[which] = i;
+            if (cs[i].align_a == esA && cs[i].align_b == es && p->scalar[which] < 0) p->scalar[which] = i;
         }
         p->winner[which] = cs.empty() ? -1 : 0;
     }
@@ -335,9 +344,9 @@ ttc_status ttc_execute(ttc_plan_t p, const void* alpha, const void* A, const voi
     if (!p || !alpha || !beta) return TTC_ERR_INVALID_ARG;
     if (p->canon.empty) return TTC_OK;
     if (!A || !B) return TTC_ERR_INVALID_ARG;
-    const int es = elem_size(p->dtype);
-    const int esa = es > 8 ? 8 : es;   // complex128 only needs the alignment of its parts
-    if (((uintptr_t)A % esa) != 0 || ((uintptr_t)B % esa) != 0) return TTC_ERR_MISALIGNED;
+    const int es = elem_size(p->dtype), esA = elem_size(p->dtype_a);
+    const int al_b = es > 8 ? 8 : es, al_a = esA > 8 ? 8 : esA;   // complex128 only needs the alignment of its parts
+    if (((uintptr_t)A % al_a) != 0 || ((uintptr_t)B % al_b) != 0) return TTC_ERR_MISALIGNED;
     if (!p->have_device) return TTC_ERR_CUDA;
     const int which = is_zero(p->dtype, beta) ? 0 : 1;
     int idx = p->forced[which] >= 0 ? p->forced[which] : p->winner[which];
@@ -350,7 +359,7 @@ ttc_status ttc_execute(ttc_plan_t p, const void* alpha, const void* A, const voi
         if (((uintptr_t)A % c->align_a) != 0 || ((uintptr_t)B % c->align_b) != 0) return TTC_ERR_MISALIGNED;
     }
     if (!ensure_prepared(p, which, idx)) return TTC_ERR_CUDA;
-    const int rc = launch_candidate(*c, p->dtype, to_scalar(p->dtype, alpha), to_scalar(p->dtype, beta), A, B, cuda_stream);
+    const int rc = launch_candidate(*c, p->dtype, p->dtype_a, to_scalar(p->dtype, alpha), to_scalar(p->dtype, beta), A, B, cuda_stream);
     g_launches += 1;
     return rc == 0 ? TTC_OK : TTC_ERR_CUDA;
 }
@@ -363,7 +372,7 @@ static bool pipe_setup(ttc_plan_s* p) {
     if (p->pipe_state != 0) return p->pipe_state > 0;
     p->pipe_state = -1;
     const Canon& c = p->canon;
-    const int64_t es = elem_size(p->dtype);
+    const int64_t es = elem_size(p->dtype), esA = elem_size(p->dtype_a);
     if (env_int("TTC_HOST_PIPE", 1) == 0 || c.rank < 2 || c.spanA != c.numel || c.spanB != c.numel ||
         c.numel * es < (16 << 20)) return false;
     int best_d = -1, best_n = 0;
@@ -372,7 +381,7 @@ static bool pipe_setup(ttc_plan_s* p) {
         for (int n = 8; n >= 2; --n) {
             if (c.d[d].e % n != 0) continue;
             const int64_t range = c.d[d].e / n;
-            const int64_t wa = range * c.d[d].sA * es, wb = range * c.d[d].sB * es;
+            const int64_t wa = range * c.d[d].sA * esA, wb = range * c.d[d].sB * es;
             if (wa % 16 != 0 || wb % 16 != 0) continue;       // slab origins stay 16-byte aligned
             const int64_t w = std::min(wa, wb);
             if (w > best_w) { best_w = w; best_d = d; best_n = n; }
@@ -383,6 +392,7 @@ static bool pipe_setup(ttc_plan_s* p) {
     ttc_plan_s* sub = new (std::nothrow) ttc_plan_s();
     if (!sub) return false;
     sub->dtype = p->dtype;
+    sub->dtype_a = p->dtype_a;
     sub->rank = p->rank;
     sub->canon = c;
     sub->canon.d[best_d].e = c.d[best_d].e / best_n;
@@ -414,8 +424,8 @@ ttc_status ttc_execute_host(ttc_plan_t p, const void* alpha, const void* A_host,
     if (p->canon.empty) return TTC_OK;
     if (!A_host || !B_host) return TTC_ERR_INVALID_ARG;
     if (!p->have_device) return TTC_ERR_CUDA;
-    const size_t es = (size_t)elem_size(p->dtype);
-    const size_t bytes_a = (size_t)p->canon.spanA * es, bytes_b = (size_t)p->canon.spanB * es;
+    const size_t es = (size_t)elem_size(p->dtype), esA = (size_t)elem_size(p->dtype_a);
+    const size_t bytes_a = (size_t)p->canon.spanA * esA, bytes_b = (size_t)p->canon.spanB * es;
     if (!p->stage_a && cudaMalloc(&p->stage_a, bytes_a) != cudaSuccess) { cudaGetLastError(); return TTC_ERR_ALLOC; }
     if (!p->stage_b && cudaMalloc(&p->stage_b, bytes_b) != cudaSuccess) { cudaGetLastError(); return TTC_ERR_ALLOC; }
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
@@ -426,7 +436,7 @@ ttc_status ttc_execute_host(ttc_plan_t p, const void* alpha, const void* A_host,
         const CanonDim& D = p->canon.d[p->pipe_d];
         const int n = p->pipe_n;
         const size_t range = (size_t)(D.e / n);
-        const size_t wa = range * (size_t)D.sA * es, pa = (size_t)D.e * (size_t)D.sA * es, ha = bytes_a / pa;
+        const size_t wa = range * (size_t)D.sA * esA, pa = (size_t)D.e * (size_t)D.sA * esA, ha = bytes_a / pa;
         const size_t wb = range * (size_t)D.sB * es, pb = (size_t)D.e * (size_t)D.sB * es, hb = bytes_b / pb;
         bool ok = cudaEventRecord(p->pipe_ev[2 * n], st) == cudaSuccess &&
                   cudaStreamWaitEvent(p->pipe_in, p->pipe_ev[2 * n], 0) == cudaSuccess &&
@@ -549,6 +559,8 @@ int ttc_canonicalize(int N, const int64_t* sizes, const int* perm, const int64_t
     }
     return c.rank;
 }
+
+int ttc_plan_dtype_a(ttc_plan_t p) { return p ? (int)p->dtype_a : -1; }
 
 int64_t ttc_launch_count(void) { return g_launches.load(); }
 

@@ -18,6 +18,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdio>
+#include <type_traits>
 
 #include "ttc_internal.h"
 
@@ -26,11 +27,44 @@ namespace ttc {
 // ------------------------------------------------------------------------------------------
 // Element types and axpby
 // ------------------------------------------------------------------------------------------
+// DT is a "type pair": 0..3 = ttc_dtype with A and B of the same type; 4..7 = the mixed-precision
+// pairs of PAPER.md:75 (sd, ds, cz, zc).  T is B's type -- the type Eq. 1 is evaluated in and the
+// type of the shared-memory tile -- and TA is A's type, converted to T as it is loaded (reading M1).
+constexpr int kPairSD = 4, kPairDS = 5, kPairCZ = 6, kPairZC = 7;
 template <int DT> struct ElemT;
-template <> struct ElemT<TTC_F32>  { using T = float;   static constexpr int ES = 4; };
-template <> struct ElemT<TTC_F64>  { using T = double;  static constexpr int ES = 8; };
-template <> struct ElemT<TTC_C64>  { using T = float2;  static constexpr int ES = 8; };
-template <> struct ElemT<TTC_C128> { using T = double2; static constexpr int ES = 16; };
+template <> struct ElemT<TTC_F32>  { using T = float;   using TA = float;   static constexpr int ES = 4; };
+template <> struct ElemT<TTC_F64>  { using T = double;  using TA = double;  static constexpr int ES = 8; };
+template <> struct ElemT<TTC_C64>  { using T = float2;  using TA = float2;  static constexpr int ES = 8; };
+template <> struct ElemT<TTC_C128> { using T = double2; using TA = double2; static constexpr int ES = 16; };
+template <> struct ElemT<kPairSD>  { using T = double;  using TA = float;   static constexpr int ES = 8; };
+template <> struct ElemT<kPairDS>  { using T = float;   using TA = double;  static constexpr int ES = 4; };
+template <> struct ElemT<kPairCZ>  { using T = double2; using TA = float2;  static constexpr int ES = 16; };
+template <> struct ElemT<kPairZC>  { using T = float2;  using TA = double2; static constexpr int ES = 8; };
+// elements per vector: at most 16 bytes in A, in B and in the tile
+template <int DT> constexpr int max_vec_of() {
+    return 16 / (int)(sizeof(typename ElemT<DT>::T) > sizeof(typename ElemT<DT>::TA) ? sizeof(typename ElemT<DT>::T)
+                                                                                      : sizeof(typename ElemT<DT>::TA));
+}
+
+static int pair_id(ttc_dtype dtype, ttc_dtype dtype_a) {
+    if (dtype == dtype_a) return (int)dtype;
+    if (dtype_a == TTC_F32 && dtype == TTC_F64) return kPairSD;
+    if (dtype_a == TTC_F64 && dtype == TTC_F32) return kPairDS;
+    if (dtype_a == TTC_C64 && dtype == TTC_C128) return kPairCZ;
+    if (dtype_a == TTC_C128 && dtype == TTC_C64) return kPairZC;
+    return -1;
+}
+
+// Conversion of an element of A to B's type (reading M1): widening is exact, narrowing is one
+// round-to-nearest-even per real component (cvt.rn.f32.f64), as the C cast of the oracle.
+__device__ __forceinline__ float   cvt_to(float,   float a)   { return a; }
+__device__ __forceinline__ double  cvt_to(double,  double a)  { return a; }
+__device__ __forceinline__ float2  cvt_to(float2,  float2 a)  { return a; }
+__device__ __forceinline__ double2 cvt_to(double2, double2 a) { return a; }
+__device__ __forceinline__ double  cvt_to(double,  float a)   { return (double)a; }
+__device__ __forceinline__ float   cvt_to(float,   double a)  { return __double2float_rn(a); }
+__device__ __forceinline__ double2 cvt_to(double2, float2 a)  { return make_double2((double)a.x, (double)a.y); }
+__device__ __forceinline__ float2  cvt_to(float2,  double2 a) { return make_float2(__double2float_rn(a.x), __double2float_rn(a.y)); }
 
 __device__ __forceinline__ float scale(const Scalar& s, float a) { return __fmul_rn((float)s.re, a); }
 __device__ __forceinline__ double scale(const Scalar& s, double a) { return __dmul_rn(s.re, a); }
@@ -150,8 +184,11 @@ __global__ void __launch_bounds__(kDirectThreads)
 direct_kernel(const __grid_constant__ DirectParams P, const void* __restrict__ Ain, void* __restrict__ Bout,
               const Scalar alpha, const Scalar beta) {
     using T = typename ElemT<DT>::T;
+    using TA = typename ElemT<DT>::TA;
     using PackT = Pack<T, V>;
+    using PackA = Pack<TA, V>;
     using Raw = typename RawT<sizeof(T) * V>::T;
+    using RawA = typename RawT<sizeof(TA) * V>::T;
     using idx_t = typename std::conditional<IDX64, uint64_t, uint32_t>::type;
     using eoff_t = typename std::conditional<IDX64, int64_t, uint32_t>::type;   // element offsets
     const char* A = static_cast<const char*>(Ain);
@@ -168,7 +205,8 @@ direct_kernel(const __grid_constant__ DirectParams P, const void* __restrict__ A
     for (;;) {
         sched.prefetch();
         const idx_t first = (idx_t)chunk * (idx_t)(kDirectThreads * kDirectUnroll) + threadIdx.x;
-        PackT a[kDirectUnroll], b[kDirectUnroll];
+        PackA a[kDirectUnroll];
+        PackT b[kDirectUnroll];
         eoff_t oa[kDirectUnroll], ob[kDirectUnroll];
         idx_t r[kDirectUnroll];
         bool ok[kDirectUnroll];
@@ -203,7 +241,7 @@ direct_kernel(const __grid_constant__ DirectParams P, const void* __restrict__ A
 #pragma unroll
         for (int k = 0; k < kDirectUnroll; ++k) {
             if (ok[k]) {
-                a[k].raw = ld_stream<Raw>(A + (int64_t)oa[k] * (int64_t)sizeof(T));
+                a[k].raw = ld_stream<RawA>(A + (int64_t)oa[k] * (int64_t)sizeof(TA));
                 if (BETA) b[k].raw = ld_plain<Raw>(B + (int64_t)ob[k] * (int64_t)sizeof(T));
             }
         }
@@ -213,7 +251,7 @@ direct_kernel(const __grid_constant__ DirectParams P, const void* __restrict__ A
                 PackT o;
 #pragma unroll
                 for (int j = 0; j < V; ++j) {
-                    T x = scale(alpha, a[k].e[j]);
+                    T x = scale(alpha, cvt_to(T(), a[k].e[j]));
                     if (BETA) x = add(x, scale(beta, b[k].e[j]));
                     o.e[j] = x;
                 }
@@ -241,8 +279,11 @@ __global__ void __launch_bounds__(kTileThreads, BETA ? 4 : kTileMinCtas)
 tile_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, void* __restrict__ Bout,
             const Scalar alpha, const Scalar beta) {
     using T = typename ElemT<DT>::T;
-    constexpr int ES = (int)sizeof(T);
-    using RawA = typename RawT<ES * VA>::T;
+    using TA = typename ElemT<DT>::TA;
+    constexpr int ES = (int)sizeof(T);       // B and the tile
+    constexpr int ESA = (int)sizeof(TA);     // A
+    using RawA = typename RawT<ESA * VA>::T;
+    using RawS = typename RawT<ES * VA>::T;  // a loaded vector after conversion to T
     using RawB = typename RawT<ES * VB>::T;
     extern __shared__ __align__(16) unsigned char smem[];
     const TileSmemLayout L = tile_smem_layout(P, ES);
@@ -327,7 +368,7 @@ tile_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
             __syncthreads();
         }
 
-        const char* Ab = A + baseA * ES;
+        const char* Ab = A + baseA * ESA;
         char* Bb = B + baseB * ES;
         // ---- load phase: A -> tile, enumerated in ascending A-stride --------------------
         for (uint32_t q0 = tid; q0 < P.itemsA; q0 += NT * kTileUnroll) {
@@ -344,12 +385,23 @@ tile_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
                     const int2 el = tabs[0][lo], eh = tabs[1][hi];
                     if (edge) ok[k] = vals[0][lo] & vals[1][hi];
                     so[k] = el.y + eh.y;
-                    if (ok[k]) v[k] = ld_stream<RawA>(Ab + (int64_t)(el.x + eh.x) * ES);
+                    if (ok[k]) v[k] = ld_stream<RawA>(Ab + (int64_t)(el.x + eh.x) * ESA);
                 }
             }
 #pragma unroll
-            for (int k = 0; k < kTileUnroll; ++k)
-                if (ok[k]) st_tile<T, VA, RawA>(tile + so[k] * ES, v[k], P.splitA != 0);
+            for (int k = 0; k < kTileUnroll; ++k) {
+                if (!ok[k]) continue;
+                if constexpr (std::is_same<T, TA>::value) {
+                    st_tile<T, VA, RawA>(tile + so[k] * ES, v[k], P.splitA != 0);
+                } else {   // mixed precision: the tile holds B's type
+                    Pack<TA, VA> in;
+                    Pack<T, VA> cv;
+                    in.raw = v[k];
+#pragma unroll
+                    for (int j = 0; j < VA; ++j) cv.e[j] = cvt_to(T(), in.e[j]);
+                    st_tile<T, VA, RawS>(tile + so[k] * ES, cv.raw, P.splitA != 0);
+                }
+            }
         }
         __syncthreads();
 
@@ -780,7 +832,7 @@ static TileFn tile_fn_beta(bool beta) {
 
 template <int DT>
 static TileFn tile_fn(int va, int vb, bool same, bool beta) {
-    constexpr int MV = 16 / ElemT<DT>::ES;   // elements per 16-byte access
+    constexpr int MV = max_vec_of<DT>();   // elements per vector access
     if constexpr (MV > 1) {
         if (same && va == MV && vb == MV) return tile_fn_beta<DT, MV, MV, true>(beta);
         if (same) return nullptr;
@@ -800,7 +852,7 @@ static DirectFn direct_fn_v(bool beta, bool idx64) {
 
 template <int DT>
 static DirectFn direct_fn(int vec, bool beta, bool idx64) {
-    constexpr int MV = 16 / ElemT<DT>::ES;
+    constexpr int MV = max_vec_of<DT>();
     if constexpr (MV > 1) {
         if (vec == MV) return direct_fn_v<DT, MV>(beta, idx64);
     }
@@ -819,9 +871,9 @@ static TileFn ring_fn(int vb, bool beta, bool peel) {
     return nullptr;
 }
 
-static TileFn get_tile_fn(ttc_dtype dt, const Candidate& c) {
+static TileFn get_tile_fn(int dt, const Candidate& c) {
     const TileParams& p = c.tp;
-    if (p.ring > 0) {
+    if (p.ring > 0) {   // same-type pairs only: the bulk copies move A's bytes unconverted
         switch (dt) {
             case TTC_F32: return ring_fn<TTC_F32>(p.vecB, c.beta_nz, p.peel != 0);
             case TTC_F64: return ring_fn<TTC_F64>(p.vecB, c.beta_nz, p.peel != 0);
@@ -835,23 +887,33 @@ static TileFn get_tile_fn(ttc_dtype dt, const Candidate& c) {
         case TTC_F64: return tile_fn<TTC_F64>(p.vecA, p.vecB, p.same != 0, c.beta_nz);
         case TTC_C64: return tile_fn<TTC_C64>(p.vecA, p.vecB, p.same != 0, c.beta_nz);
         case TTC_C128: return tile_fn<TTC_C128>(p.vecA, p.vecB, p.same != 0, c.beta_nz);
+        case kPairSD: return tile_fn<kPairSD>(p.vecA, p.vecB, p.same != 0, c.beta_nz);
+        case kPairDS: return tile_fn<kPairDS>(p.vecA, p.vecB, p.same != 0, c.beta_nz);
+        case kPairCZ: return tile_fn<kPairCZ>(p.vecA, p.vecB, p.same != 0, c.beta_nz);
+        case kPairZC: return tile_fn<kPairZC>(p.vecA, p.vecB, p.same != 0, c.beta_nz);
     }
     return nullptr;
 }
 
-static DirectFn get_direct_fn(ttc_dtype dt, const Candidate& c) {
+static DirectFn get_direct_fn(int dt, const Candidate& c) {
     switch (dt) {
         case TTC_F32: return direct_fn<TTC_F32>(c.dp.vec, c.beta_nz, c.idx64);
         case TTC_F64: return direct_fn<TTC_F64>(c.dp.vec, c.beta_nz, c.idx64);
         case TTC_C64: return direct_fn<TTC_C64>(c.dp.vec, c.beta_nz, c.idx64);
         case TTC_C128: return direct_fn<TTC_C128>(c.dp.vec, c.beta_nz, c.idx64);
+        case kPairSD: return direct_fn<kPairSD>(c.dp.vec, c.beta_nz, c.idx64);
+        case kPairDS: return direct_fn<kPairDS>(c.dp.vec, c.beta_nz, c.idx64);
+        case kPairCZ: return direct_fn<kPairCZ>(c.dp.vec, c.beta_nz, c.idx64);
+        case kPairZC: return direct_fn<kPairZC>(c.dp.vec, c.beta_nz, c.idx64);
     }
     return nullptr;
 }
 
-int prepare_candidate(Candidate* cand, ttc_dtype dtype, int sm_count) {
+int prepare_candidate(Candidate* cand, ttc_dtype dtype, ttc_dtype dtype_a, int sm_count) {
+    const int pair = pair_id(dtype, dtype_a);
+    if (pair < 0) return (int)cudaErrorInvalidValue;
     if (cand->info.kernel == TTC_KERNEL_COPY) {
-        DirectFn fn = get_direct_fn(dtype, *cand);
+        DirectFn fn = get_direct_fn(pair, *cand);
         if (!fn) return (int)cudaErrorInvalidValue;
         int occ = 0;
         cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kDirectThreads, 0);
@@ -864,7 +926,7 @@ int prepare_candidate(Candidate* cand, ttc_dtype dtype, int sm_count) {
         cand->info.grid = (int)(cand->dp.dyn || need < cap ? need : cap);
         return 0;
     }
-    TileFn fn = get_tile_fn(dtype, *cand);
+    TileFn fn = get_tile_fn(pair, *cand);
     if (!fn) return (int)cudaErrorInvalidValue;
     const int smem = (int)tile_smem_layout(cand->tp, elem_size(dtype)).total;
     // The attribute belongs to the kernel function, which many candidates share: raise it once
@@ -891,16 +953,18 @@ int prepare_candidate(Candidate* cand, ttc_dtype dtype, int sm_count) {
     return 0;
 }
 
-int launch_candidate(const Candidate& cand, ttc_dtype dtype, const Scalar& alpha, const Scalar& beta,
-                     const void* A, void* B, void* stream) {
+int launch_candidate(const Candidate& cand, ttc_dtype dtype, ttc_dtype dtype_a, const Scalar& alpha,
+                     const Scalar& beta, const void* A, void* B, void* stream) {
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int pair = pair_id(dtype, dtype_a);
+    if (pair < 0) return (int)cudaErrorInvalidValue;
     if (cand.info.grid <= 0) return (int)cudaErrorInvalidConfiguration;
     if (cand.info.kernel == TTC_KERNEL_COPY) {
-        DirectFn fn = get_direct_fn(dtype, cand);
+        DirectFn fn = get_direct_fn(pair, cand);
         if (!fn) return (int)cudaErrorInvalidValue;
         fn<<<cand.info.grid, kDirectThreads, 0, st>>>(cand.dp, A, B, alpha, beta);
     } else {
-        TileFn fn = get_tile_fn(dtype, cand);
+        TileFn fn = get_tile_fn(pair, cand);
         if (!fn) return (int)cudaErrorInvalidValue;
         fn<<<cand.info.grid, cand.tp.threads, cand.info.smem_bytes, st>>>(cand.tp, A, B, alpha, beta);
     }

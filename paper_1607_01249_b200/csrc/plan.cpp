@@ -149,10 +149,14 @@ int legal_vec(const Canon& c, int lead, bool sideA, int32_t t_lead, int mv) {
 }
 
 // Build one tile-kernel candidate.  Returns false if the combination is not legal.
-bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const TileSpec& spec,
+bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, const TileSpec& spec,
                           int loop_order, int want_va, int want_vb, int max_smem, int sched, int ring, Candidate* out) {
-    const int es = elem_size(dtype);
-    const int mv = 16 / es;
+    // es: B's element and the tile's (the planner's world is B-typed); esA differs from it only for
+    // the mixed-precision pairs, where A is converted in the load phase and the ring kernel (raw
+    // bulk copies of A's bytes) does not apply.
+    const int es = elem_size(dtype), esA = elem_size(dtype_a);
+    const int mv = max_vec(dtype, dtype_a);
+    if (ring && dtype_a != dtype) return false;
     Candidate cand;
     cand.beta_nz = beta_nz;
     TileParams& P = cand.tp;
@@ -416,7 +420,7 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
     I.grid = 0;
     I.n_tiles = n_tiles;
     for (int i = 0; i < kMaxRank; ++i) I.tile_ext[i] = i < c.rank ? spec.t[i] : 0;
-    cand.align_a = P.row_pairs ? 8 : want_va * es;
+    cand.align_a = P.row_pairs ? 8 : want_va * esA;
     cand.align_b = peelB ? es : want_vb * es;
 
     // Cost heuristic: long contiguous runs on both sides, small remainders,
@@ -428,7 +432,7 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, bool beta_nz, const T
         waste *= nt * spec.t[i] / (double)c.d[i].e;
     }
     const double tile_bytes = (double)itemsA * want_va * es;
-    const double rd = 1.0 / run_eff((double)runA * es) * (want_va * es >= 16 ? 1.0 : 1.15);
+    const double rd = 1.0 / run_eff((double)runA * esA) * (want_va * esA >= 16 ? 1.0 : 1.15);
     // short runs cost much less on the B side than on the A side: the 126 MB L2 merges the writes of
     // neighbouring tiles before they reach DRAM (measured: 64-byte B runs win several c2 permutations)
     const double wr = (beta_nz ? 2.0 : 1.0) / run_eff((double)runB * es, 12.0) * (want_vb * es >= 16 ? 1.0 : 1.10);
@@ -508,10 +512,10 @@ void side_options(const Canon& c, const std::vector<int>& order, const int32_t* 
     }
 }
 
-void add_direct(const Canon& c, ttc_dtype dtype, bool beta_nz, int loop_order, bool vector, int sched,
-                std::vector<Candidate>* out) {
-    const int es = elem_size(dtype);
-    const int mv = 16 / es;
+void add_direct(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, int loop_order, bool vector,
+                int sched, std::vector<Candidate>* out) {
+    const int es = elem_size(dtype), esA = elem_size(dtype_a);
+    const int mv = max_vec(dtype, dtype_a);
     Candidate cand;
     cand.beta_nz = beta_nz;
     DirectParams& P = cand.dp;
@@ -556,7 +560,8 @@ void add_direct(const Canon& c, ttc_dtype dtype, bool beta_nz, int loop_order, b
     if (n_items >= (uint64_t)kInt31 / 2) idx64 = true;
     if (c.spanA >= kInt31 || c.spanB >= kInt31) idx64 = true;   // 32-bit element offsets otherwise
     cand.idx64 = idx64;
-    cand.align_a = cand.align_b = vec * es;
+    cand.align_a = vec * esA;
+    cand.align_b = vec * es;
     ttc_candidate_info& I = cand.info;
     I.kernel = TTC_KERNEL_COPY;
     I.vec_a = I.vec_b = vec;
@@ -578,10 +583,10 @@ void add_direct(const Canon& c, ttc_dtype dtype, bool beta_nz, int loop_order, b
         }
         return run;
     };
-    const double ra = (double)run_of(true) * es, rb = (double)run_of(false) * es;
+    const double ra = (double)run_of(true) * esA, rb = (double)run_of(false) * es;
     auto eff = [&](double r) { return r <= es ? es / 32.0 * 0.5 : run_eff(r); };
     double cost = 1.0 / eff(ra) + (beta_nz ? 2.0 : 1.0) / eff(rb);
-    if (vec * es < 16) cost *= 1.25;
+    if (vec * std::max(es, esA) < 16) cost *= 1.25;
     if (idx64) cost *= 1.5;
     I.est_cost = (float)cost;
     I.tile_u = (int)std::min<int64_t>(run_of(true), INT32_MAX);
@@ -591,13 +596,13 @@ void add_direct(const Canon& c, ttc_dtype dtype, bool beta_nz, int loop_order, b
 
 }  // namespace
 
-void generate_candidates(const Canon& c, ttc_dtype dtype, bool beta_nz, int sm_count,
+void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, int sm_count,
                          int max_smem_optin, std::vector<Candidate>* out) {
     (void)sm_count;
     out->clear();
     if (c.empty || c.rank == 0) return;
     const int es = elem_size(dtype);
-    const int mv = 16 / es;
+    const int mv = max_vec(dtype, dtype_a);
     const int max_smem = std::min(max_smem_optin > 0 ? max_smem_optin : 48 * 1024, 160 * 1024);
 
     // Work distribution (row H6): dynamic (cluster launch control) unless TTC_SCHED says
@@ -613,8 +618,8 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, bool beta_nz, int sm_c
     // K1 / fallback: direct kernels (always at least the scalar one, valid for any strides).
     for (int sched : scheds)
         for (int lo = 0; lo < 2; ++lo) {
-            add_direct(c, dtype, beta_nz, lo, true, sched, out);
-            add_direct(c, dtype, beta_nz, lo, false, sched, out);
+            add_direct(c, dtype, dtype_a, beta_nz, lo, true, sched, out);
+            add_direct(c, dtype, dtype_a, beta_nz, lo, false, sched, out);
         }
 
     // K2 / K3: tiles.  A side = leading indices of A, B side = leading indices of B.
@@ -650,7 +655,7 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, bool beta_nz, int sm_c
                             for (int ring = 0; ring <= ring_max; ring += 2) {
                                 if (ring && bytes * ring > 64 * 1024) continue;   // 2 buffers <= 32 KB, 4 <= 16 KB
                                 Candidate cand;
-                                if (build_tile_candidate(c, dtype, beta_nz, spec, lo, va, vb, max_smem, sched, ring, &cand))
+                                if (build_tile_candidate(c, dtype, dtype_a, beta_nz, spec, lo, va, vb, max_smem, sched, ring, &cand))
                                     out->push_back(cand);
                             }
                     }

@@ -189,14 +189,17 @@ struct Scalar {         // alpha or beta, as doubles (re, im); narrowed in the l
     double re, im;
 };
 
-void generate_candidates(const Canon& c, ttc_dtype dtype, bool beta_nz, int sm_count,
+// `dtype` is B's element type -- the type Eq. 1 is evaluated in and the type of the shared-memory
+// tile; `dtype_a` is A's.  They differ only for the mixed-precision pairs sd, ds, cz, zc
+// (PAPER.md:75, 87): A's elements are then converted as they are loaded (reading M1).
+void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, int sm_count,
                          int max_smem_optin, std::vector<Candidate>* out);
 
 // Launch one candidate.  Returns the CUDA error code (0 = success) as int.
-int launch_candidate(const Candidate& cand, ttc_dtype dtype, const Scalar& alpha, const Scalar& beta,
-                     const void* A, void* B, void* stream);
+int launch_candidate(const Candidate& cand, ttc_dtype dtype, ttc_dtype dtype_a, const Scalar& alpha,
+                     const Scalar& beta, const void* A, void* B, void* stream);
 // Configure dynamic shared memory / occupancy-derived grid for a candidate (needs a device).
-int prepare_candidate(Candidate* cand, ttc_dtype dtype, int sm_count);
+int prepare_candidate(Candidate* cand, ttc_dtype dtype, ttc_dtype dtype_a, int sm_count);
 
 inline int elem_size(ttc_dtype t) {
     switch (t) {
@@ -205,6 +208,20 @@ inline int elem_size(ttc_dtype t) {
         case TTC_C64: return 8;
         default: return 16;
     }
+}
+
+// Mixed-precision pairs the library accepts: sd, ds, cz, zc; equal types always.
+inline bool valid_pair(ttc_dtype a, ttc_dtype b) {
+    if ((int)a < 0 || (int)a > 3 || (int)b < 0 || (int)b > 3) return false;
+    if (a == b) return true;
+    return (a == TTC_F32 && b == TTC_F64) || (a == TTC_F64 && b == TTC_F32) ||
+           (a == TTC_C64 && b == TTC_C128) || (a == TTC_C128 && b == TTC_C64);
+}
+
+// Elements per vector access: a vector is at most 16 bytes in A, in B and in the tile.
+inline int max_vec(ttc_dtype dtype, ttc_dtype dtype_a) {
+    const int ea = elem_size(dtype_a), eb = elem_size(dtype);
+    return 16 / (ea > eb ? ea : eb);
 }
 
 }  // namespace ttc

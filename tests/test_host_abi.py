@@ -167,3 +167,51 @@ def test_copy_class_configs_rank_a_vector_copy_first():
         c = ttc.ttc_plan_candidate(p, 0, 0)
         assert c.vec_a * 8 == 16 and c.vec_b * 8 == 16
         ttc.ttc_destroy(p)
+
+
+# --------------------------------------------------------------------- mixed precision
+MIXED_PAIRS = ((0, 1), (1, 0), (2, 3), (3, 2))     # sd, ds, cz, zc
+
+
+@pytest.mark.parametrize("da,db", MIXED_PAIRS)
+def test_mixed_plan_reports_both_types_and_has_no_ring_candidates(da, db):
+    """ttc_plan_mixed: dtype of the plan is B's, ttc_plan_dtype_a gives A's; vectors are at most 16
+    bytes on the wider side; the ring kernel (raw bulk copies of A's bytes) is never a candidate."""
+    w = wl.config2((2, 0, 3, 1))
+    p = ttc.ttc_plan_mixed(da, db, w.n, w.sizes, w.perm)
+    try:
+        info = ttc.ttc_plan_info(p)
+        assert info.dtype == db and ttc.ttc_plan_dtype_a(p) == da
+        assert info.numel == w.numel
+        wide = max(wl.ELEM_SIZE[da], wl.ELEM_SIZE[db])
+        for which in (0, 1):
+            n = ttc.ttc_plan_num_candidates(p, which)
+            cs = [ttc.ttc_plan_candidate(p, which, i) for i in range(n)]
+            assert any(c.kernel == 1 and c.vec_a == 1 for c in cs)          # scalar fallback
+            assert any(c.kernel in (2, 3, 4) for c in cs)                   # tiled transposes
+            assert all(c.kernel != 5 for c in cs)                           # no ring kernel
+            assert all(c.vec_a * wide <= 16 and c.vec_b * wide <= 16 for c in cs)
+    finally:
+        ttc.ttc_destroy(p)
+
+
+def test_mixed_plan_of_equal_types_is_the_plain_plan():
+    w = wl.config1()
+    p = ttc.ttc_plan_mixed(w.dtype, w.dtype, w.n, w.sizes, w.perm)
+    q = ttc.ttc_plan(w.dtype, w.n, w.sizes, w.perm)
+    try:
+        assert ttc.ttc_plan_dtype_a(p) == ttc.ttc_plan_dtype_a(q) == w.dtype
+        assert ttc.ttc_plan_num_candidates(p, 0) == ttc.ttc_plan_num_candidates(q, 0)
+    finally:
+        ttc.ttc_destroy(p)
+        ttc.ttc_destroy(q)
+
+
+@pytest.mark.parametrize("da,db", [(0, 2), (2, 0), (1, 3), (0, 3), (2, 1)])
+def test_real_complex_pairs_are_unsupported(da, db):
+    with pytest.raises(ttc.TTCError) as ei:
+        ttc.ttc_plan_mixed(da, db, 2, (4, 4), (1, 0))
+    assert ttc.STATUS_NAMES[ei.value.status] == "TTC_ERR_UNSUPPORTED"
+    with pytest.raises(ttc.TTCError) as ei:
+        ttc.ttc_plan_mixed(7, 0, 2, (4, 4), (1, 0))
+    assert ttc.STATUS_NAMES[ei.value.status] == "TTC_ERR_INVALID_ARG"
