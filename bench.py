@@ -180,8 +180,60 @@ def detail_all_configs(torch, ttc, wl, path: str, peak: float, profile: bool = F
                      "n_candidates": info.n_candidates[which]})
         ttc.ttc_destroy(plan)
         del a_dev, b_dev
+    rows.extend(detail_mixed(torch, ttc, wl, flush, peak, profile))
     with open(path, "w") as fh:
         json.dump(rows, fh, indent=1)
+
+
+def detail_mixed(torch, ttc, wl, flush, peak: float, profile: bool = False) -> list:
+    """Mixed-precision transpositions on configs[1]'s tensor:
+    A of one type, B of the other.  Algorithmic bytes = |A| * (sizeof(A) + (1 | 2) * sizeof(B))."""
+    import numpy as np
+    rows = []
+    pairs = (("sd", wl.F32, wl.F64), ("ds", wl.F64, wl.F32), ("cz", wl.C64, wl.C128), ("zc", wl.C128, wl.C64))
+    cases = [(p, perm, 0.0) for p in pairs[:2] for perm in ((0, 2, 1, 3), (2, 3, 0, 1), (3, 1, 0, 2))]
+    cases += [(pairs[0], (2, 3, 0, 1), 0.5), (pairs[1], (2, 3, 0, 1), 0.5), (pairs[2], (3, 1, 0, 2), 0.0),
+              (pairs[3], (3, 1, 0, 2), 0.0)]
+    for (name, da, db), perm, beta in cases:
+        w = wl.config2(perm)
+        numel = w.numel
+        plan = ttc.ttc_plan_mixed(da, db, w.n, w.sizes, perm)
+        info = ttc.ttc_plan_info(plan)
+        a_dev = torch.from_numpy(wl.uniform_values(wl.SEED_A, numel, da)).cuda()
+        b_dev = torch.from_numpy(wl.uniform_values(wl.SEED_B, numel, db)).cuda()
+        alpha = 1.5
+        for _ in range(3):
+            ttc.ttc_execute(plan, alpha, a_dev, beta, b_dev)
+        ts = []
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for _ in range(21):
+            flush.zero_()
+            e0.record()
+            ttc.ttc_execute(plan, alpha, a_dev, beta, b_dev)
+            e1.record()
+            e1.synchronize()
+            ts.append(e0.elapsed_time(e1) * 1e3)
+        if profile and beta == 0 and name in ("sd", "ds") and perm != (3, 1, 0, 2):   # 4 launches for ncu
+            torch.cuda.synchronize()
+            torch.cuda.cudart().cudaProfilerStart()
+            ttc.ttc_execute(plan, alpha, a_dev, beta, b_dev)
+            torch.cuda.synchronize()
+            torch.cuda.cudart().cudaProfilerStop()
+        which = 1 if beta != 0 else 0
+        cand = ttc.ttc_plan_candidate(plan, which, info.chosen[which])
+        nbytes = numel * (wl.ELEM_SIZE[da] + (2 if which else 1) * wl.ELEM_SIZE[db])
+        t3, tm = min(ts[:3]), statistics.median(ts)
+        rows.append({"config": "mixed-%s %s on configs[1]'s tensor, beta=%g" % (name, wl.DTYPE_NAME[da] + "->" + wl.DTYPE_NAME[db], beta),
+                     "perm": list(perm), "bytes": nbytes, "us_min_of_3": t3, "us_median_21": tm, "us_min_21": min(ts),
+                     "gbs_min_of_3": nbytes / t3 / 1e3, "gbs_median": nbytes / tm / 1e3, "gbs_best": nbytes / min(ts) / 1e3,
+                     "gibs_median": nbytes / tm / 1e3 * 1e9 / 2 ** 30,
+                     "frac_of_8TBs": nbytes / tm / 1e3 / NOMINAL_HBM_GBS,
+                     "frac_of_measured_copy": nbytes / tm / 1e3 / peak,
+                     "chosen": ttc.describe_candidate(cand, info.canon_rank),
+                     "n_candidates": info.n_candidates[which]})
+        ttc.ttc_destroy(plan)
+        del a_dev, b_dev
+    return rows
 
 
 def whole_job_value(step_bytes: int, steps: int, world: int, ms_local: float, dist, device) -> tuple:

@@ -87,6 +87,8 @@ template <int BYTES> struct RawT;
 template <> struct RawT<4>  { using T = uint32_t; };
 template <> struct RawT<8>  { using T = uint2; };
 template <> struct RawT<16> { using T = uint4; };
+struct __align__(16) Raw32 { uint4 lo, hi; };      // tile side only: a converted vector of a narrower A type
+template <> struct RawT<32> { using T = Raw32; };
 
 template <typename T, int V>
 union Pack {
@@ -832,13 +834,25 @@ static TileFn tile_fn_beta(bool beta) {
 
 template <int DT>
 static TileFn tile_fn(int va, int vb, bool same, bool beta) {
-    constexpr int MV = max_vec_of<DT>();   // elements per vector access
-    if constexpr (MV > 1) {
-        if (same && va == MV && vb == MV) return tile_fn_beta<DT, MV, MV, true>(beta);
-        if (same) return nullptr;
-        if (va == MV && vb == MV) return tile_fn_beta<DT, MV, MV, false>(beta);
-        if (va == MV && vb == 1) return tile_fn_beta<DT, MV, 1, false>(beta);
-        if (va == 1 && vb == MV) return tile_fn_beta<DT, 1, MV, false>(beta);
+    // 16-byte vectors of each side's own type; MS: the one width that fits both (wide class, and the
+    // extra equal-width variant of the mixed-precision pairs)
+    constexpr int MVA = 16 / (int)sizeof(typename ElemT<DT>::TA), MVB = 16 / ElemT<DT>::ES;
+    constexpr int MS = MVA < MVB ? MVA : MVB;
+    if constexpr (MS > 1) {
+        if (same && va == MS && vb == MS) return tile_fn_beta<DT, MS, MS, true>(beta);
+    }
+    if (same) return nullptr;
+    if constexpr (MVA > 1 && MVB > 1) {
+        if (va == MVA && vb == MVB) return tile_fn_beta<DT, MVA, MVB, false>(beta);
+    }
+    if constexpr (MVA != MVB && MS > 1) {
+        if (va == MS && vb == MS) return tile_fn_beta<DT, MS, MS, false>(beta);
+    }
+    if constexpr (MVA > 1) {
+        if (va == MVA && vb == 1) return tile_fn_beta<DT, MVA, 1, false>(beta);
+    }
+    if constexpr (MVB > 1) {
+        if (va == 1 && vb == MVB) return tile_fn_beta<DT, 1, MVB, false>(beta);
     }
     if (va == 1 && vb == 1) return tile_fn_beta<DT, 1, 1, false>(beta);
     return nullptr;

@@ -154,8 +154,11 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
     // es: B's element and the tile's (the planner's world is B-typed); esA differs from it only for
     // the mixed-precision pairs, where A is converted in the load phase and the ring kernel (raw
     // bulk copies of A's bytes) does not apply.
+    // Vectors are 16 bytes of the side's own element type (mvA elements in A, mvB in B); where one
+    // vector has to serve both sides (the wide class) it has mvS = min of the two.
     const int es = elem_size(dtype), esA = elem_size(dtype_a);
-    const int mv = max_vec(dtype, dtype_a);
+    const int mvA = 16 / esA, mvB = 16 / es, mvS = std::min(mvA, mvB);
+    const int mv = mvB;   // the ring kernel's peeled store phase (same-type pairs only: mvA == mvB)
     if (ring && dtype_a != dtype) return false;
     Candidate cand;
     cand.beta_nz = beta_nz;
@@ -169,8 +172,8 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
         if (spec.t[c.orderB[k]] > 1) tb.push_back(c.orderB[k]);
     if (ta.empty()) return false;
     const int A0 = ta[0], B0 = tb[0];
-    int va = legal_vec(c, A0, true, spec.t[A0], mv);
-    const int vb = legal_vec(c, B0, false, spec.t[B0], mv);
+    int va = legal_vec(c, A0, true, spec.t[A0], want_va > 1 ? want_va : mvA);
+    const int vb = legal_vec(c, B0, false, spec.t[B0], want_vb > 1 ? want_vb : mvB);
     // K3 for a tiny/odd stride-1 extent of A (c5: 7 complex64 = 56 bytes): when the tile takes the
     // leading index whole and the next one continues it in memory, the two are ONE contiguous run
     // for the load phase (7 x t1 elements), which can be vectorised although the leading extent
@@ -179,19 +182,19 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
     // straddle the end of the second index (its extent is a multiple of its tile extent), so no
     // vector is cut by a tile edge.
     bool fuseA = false;
-    if (want_va > va && want_va == mv && ta.size() >= 2 && A0 != B0) {
+    if (want_va > va && want_va == mvA && ta.size() >= 2 && A0 != B0) {
         const int A1 = ta[1];
         bool ok = c.d[A0].sA == 1 && spec.t[A0] == c.d[A0].e && c.d[A1].sA == c.d[A0].e &&
-                  ((int64_t)spec.t[A0] * spec.t[A1]) % mv == 0 && c.d[A1].e % spec.t[A1] == 0 && A1 != B0;
+                  ((int64_t)spec.t[A0] * spec.t[A1]) % mvA == 0 && c.d[A1].e % spec.t[A1] == 0 && A1 != B0;
         for (int i = 0; i < c.rank && ok; ++i)
-            if (i != A0 && i != A1 && c.d[i].sA % mv != 0) ok = false;
-        if (ok) { fuseA = true; va = mv; }
+            if (i != A0 && i != A1 && c.d[i].sA % mvA != 0) ok = false;
+        if (ok) { fuseA = true; va = mvA; }
     }
     // Ring kernel, peeled store phase: the B-leading index is stride-1 but its rows are not
     // 16-byte aligned (odd extent or stride): rows are cut into aligned 16-byte windows of B.
     const bool peelB = ring && mv > 1 && want_vb == mv && vb < mv && c.d[B0].sB == 1 && A0 != B0;
     if (want_va > va || (want_vb > vb && !peelB)) return false;
-    const bool same = (A0 == B0) && want_va == mv && want_vb == mv && mv > 1;
+    const bool same = (A0 == B0) && want_va == mvS && want_vb == mvS && mvS > 1;
     if (A0 == B0 && want_va != want_vb) return false;   // nothing gained by mixing widths on one index
     P.vecA = want_va;
     P.vecB = want_vb;
@@ -287,7 +290,7 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
     int combos = 1;
     for (int i = 0; i < search_levels; ++i) combos *= n_opts;
     for (int split = 0; split < ((want_va > 1 && !same && !ring) ? 2 : 1); ++split) {
-    const int unit = split ? 1 : std::max(std::max(want_va, same ? mv : 1), P.row_pairs ? 2 : 1);
+    const int unit = split ? 1 : std::max(std::max(want_va, same ? mvS : 1), P.row_pairs ? 2 : 1);
     for (int combo = 0; combo < combos; ++combo) {
         int cc = combo;
         int64_t stride = 1;
@@ -602,7 +605,7 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, boo
     out->clear();
     if (c.empty || c.rank == 0) return;
     const int es = elem_size(dtype);
-    const int mv = max_vec(dtype, dtype_a);
+    const int mvA = 16 / elem_size(dtype_a), mvB = 16 / es, mvS = std::min(mvA, mvB);
     const int max_smem = std::min(max_smem_optin > 0 ? max_smem_optin : 48 * 1024, 160 * 1024);
 
     // Work distribution (row H6): dynamic (cluster launch control) unless TTC_SCHED says
@@ -630,13 +633,13 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, boo
     if (fits32 && c.rank >= 2) {
         std::vector<SideOpt> optsA;
         int32_t none[kMaxRank] = {0};
-        side_options(c, orderA, none, mv, es, &optsA);
+        side_options(c, orderA, none, mvA, es, &optsA);
         std::set<std::string> seen;
         for (const SideOpt& ua : optsA) {
             int32_t taken[kMaxRank] = {0};
             for (auto& d : ua.dims) taken[d.first] = d.second;
             std::vector<SideOpt> optsB;
-            side_options(c, orderB, taken, mv, es, &optsB);
+            side_options(c, orderB, taken, mvB, es, &optsB);
             for (const SideOpt& wb : optsB) {
                 const int64_t bytes = ua.elems * wb.elems * es;
                 if (bytes < 2048 || bytes > max_smem) continue;
@@ -646,11 +649,13 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, boo
                 for (auto& d : wb.dims) spec.t[d.first] = d.second;
                 std::string key((const char*)spec.t, sizeof(int32_t) * c.rank);
                 if (!seen.insert(key).second) continue;
-                static const int vopts[4][2] = {{16, 16}, {16, 1}, {1, 16}, {1, 1}};
+                // {8, 8}: mixed precision only -- one vector width (mvS elements) on both sides
+                static const int vopts[5][2] = {{16, 16}, {16, 1}, {1, 16}, {1, 1}, {8, 8}};
                 for (int lo = 0; lo < 2; ++lo) {
                     for (auto& vo : vopts) {
-                        const int va = vo[0] == 16 ? mv : 1, vb = vo[1] == 16 ? mv : 1;
-                        if (mv == 1 && (vo[0] == 16 || vo[1] == 16)) continue;
+                        const int va = vo[0] == 16 ? mvA : vo[0] == 8 ? mvS : 1, vb = vo[1] == 16 ? mvB : vo[1] == 8 ? mvS : 1;
+                        if ((mvA == 1 && vo[0] == 16) || (mvB == 1 && vo[1] == 16)) continue;
+                        if (vo[0] == 8 && (mvA == mvB || mvS == 1)) continue;
                         for (int sched : scheds)
                             for (int ring = 0; ring <= ring_max; ring += 2) {
                                 if (ring && bytes * ring > 64 * 1024) continue;   // 2 buffers <= 32 KB, 4 <= 16 KB

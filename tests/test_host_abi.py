@@ -176,21 +176,22 @@ MIXED_PAIRS = ((0, 1), (1, 0), (2, 3), (3, 2))     # sd, ds, cz, zc
 @pytest.mark.parametrize("da,db", MIXED_PAIRS)
 def test_mixed_plan_reports_both_types_and_has_no_ring_candidates(da, db):
     """ttc_plan_mixed: dtype of the plan is B's, ttc_plan_dtype_a gives A's; vectors are at most 16
-    bytes on the wider side; the ring kernel (raw bulk copies of A's bytes) is never a candidate."""
+    bytes of each side's own type; the ring kernel (raw bulk copies of A's bytes) is never a candidate."""
     w = wl.config2((2, 0, 3, 1))
     p = ttc.ttc_plan_mixed(da, db, w.n, w.sizes, w.perm)
     try:
         info = ttc.ttc_plan_info(p)
         assert info.dtype == db and ttc.ttc_plan_dtype_a(p) == da
         assert info.numel == w.numel
-        wide = max(wl.ELEM_SIZE[da], wl.ELEM_SIZE[db])
         for which in (0, 1):
             n = ttc.ttc_plan_num_candidates(p, which)
             cs = [ttc.ttc_plan_candidate(p, which, i) for i in range(n)]
             assert any(c.kernel == 1 and c.vec_a == 1 for c in cs)          # scalar fallback
             assert any(c.kernel in (2, 3, 4) for c in cs)                   # tiled transposes
             assert all(c.kernel != 5 for c in cs)                           # no ring kernel
-            assert all(c.vec_a * wide <= 16 and c.vec_b * wide <= 16 for c in cs)
+            assert all(c.vec_a * wl.ELEM_SIZE[da] <= 16 and c.vec_b * wl.ELEM_SIZE[db] <= 16 for c in cs)
+            if wl.ELEM_SIZE[da] < 16 and wl.ELEM_SIZE[db] < 16:   # 16-byte vectors on both sides exist
+                assert any(c.vec_a * wl.ELEM_SIZE[da] == 16 and c.vec_b * wl.ELEM_SIZE[db] == 16 for c in cs)
     finally:
         ttc.ttc_destroy(p)
 
