@@ -462,8 +462,10 @@ tile_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
 // wait for a full buffer, run the store phase of tile_kernel on it (gather from the tile in
 // B order, alpha/beta, 16-byte stores) and hand the buffer back.  The load of the next tiles is
 // therefore in flight for the whole store phase of the current one, inside ONE CTA, instead of
-// relying on many resident CTAs to overlap the two streams.  Only for tilings without edge tiles
-// (every tile extent divides its index extent) and 16-byte rows.
+// relying on many resident CTAs to overlap the two streams.  Rows that are not 16-byte multiples
+// are copied with element-sized cp.async instead (P.row_async); edge tiles get shorter and fewer
+// rows.  Mixed precision (DT = a type pair): the bulk copies land A's bytes, so the tile holds
+// A's type and the consumers convert each element to B's type as they read it (reading M1).
 // ------------------------------------------------------------------------------------------
 // cp.async: global -> shared without a register stop (LDGSTS), BYTES = 4, 8 or 16.
 template <int BYTES>
@@ -489,11 +491,14 @@ template <int DT, int VB, bool BETA, bool PEEL>
 __global__ void __launch_bounds__(kRingThreads, PEEL ? 3 : BETA ? 4 : 5)
 ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, void* __restrict__ Bout,
             const Scalar alpha, const Scalar beta) {
-    using T = typename ElemT<DT>::T;
-    constexpr int ES = (int)sizeof(T);
+    using T = typename ElemT<DT>::T;         // B
+    using TA = typename ElemT<DT>::TA;       // A and the tile: bulk copies land A's bytes unconverted,
+    constexpr int ES = (int)sizeof(T);       // the consumers convert (mixed precision, reading M1)
+    constexpr int ESA = (int)sizeof(TA);
+    constexpr bool MIXED = !std::is_same<T, TA>::value;
     using RawB = typename RawT<ES * VB>::T;
     extern __shared__ __align__(16) unsigned char smem[];
-    const TileSmemLayout L = tile_smem_layout(P, ES);
+    const TileSmemLayout L = tile_smem_layout(P, ESA);
     int2* tabs[4];
 #pragma unroll
     for (int i = 0; i < 4; ++i) tabs[i] = reinterpret_cast<int2*>(smem + L.tab[i]);
@@ -575,7 +580,7 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
                     if (lane == 0) vx[g] = left < P.g[g].t ? left : P.g[g].t;
                 }
             }
-            const char* Ab = A + baseA * ES;
+            const char* Ab = A + baseA * ESA;
             unsigned char* tile = smem + L.tile + (uint32_t)s * L.tile_stride;
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             uint32_t row_bytes = P.row_bytes;
@@ -583,7 +588,7 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
             uint32_t n_rows = (uint32_t)rows;
             if (edge) {   // remainder tile: shorter rows, fewer rows
                 __syncwarp();
-                const int valid = vx[P.lead_gslot] * P.lead_vmul * ES;
+                const int valid = vx[P.lead_gslot] * P.lead_vmul * ESA;
                 row_bytes = (uint32_t)valid < row_bytes ? (uint32_t)valid : row_bytes;
                 row_ok = 0;
                 const Table& tb = P.tab[1];
@@ -610,36 +615,36 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
                     tile_of[s] = tile_id;
                     edge_of[s] = edge ? 1u : 0u;
                 }
-                const int len = (int)(row_bytes / ES);
+                const int len = (int)(row_bytes / ESA);
                 for (int row = 0; row < rows; ++row) {
                     if (edge && !((__shfl_sync(0xFFFFFFFFu, (unsigned)(row_ok >> (row >> 5)), row & 31)) & 1u)) continue;
                     const int2 e = tabs[1][row];
                     // one warp instruction copies 32 consecutive elements; pointers advance by constants
-                    if (ES == 4 && P.row_pairs) {   // 4-byte elements whose rows are all 8-byte aligned: pairs
-                        const char* src = Ab + ((int64_t)e.x + 2 * lane) * ES;
-                        uint32_t dst = (uint32_t)__cvta_generic_to_shared(tile + (e.y + 2 * lane) * ES);
+                    if (ESA == 4 && P.row_pairs) {   // 4-byte elements whose rows are all 8-byte aligned: pairs
+                        const char* src = Ab + ((int64_t)e.x + 2 * lane) * ESA;
+                        uint32_t dst = (uint32_t)__cvta_generic_to_shared(tile + (e.y + 2 * lane) * ESA);
                         const int n = ((len >> 1) - lane + 31) >> 5;
 #pragma unroll 4
                         for (int i = 0; i < n; ++i) {
                             asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
-                            dst += 64 * ES;
-                            src += 64 * ES;
+                            dst += 64 * ESA;
+                            src += 64 * ESA;
                         }
                         continue;
                     }
-                    const char* src = Ab + ((int64_t)e.x + lane) * ES;
-                    uint32_t dst = (uint32_t)__cvta_generic_to_shared(tile + (e.y + lane) * ES);
+                    const char* src = Ab + ((int64_t)e.x + lane) * ESA;
+                    uint32_t dst = (uint32_t)__cvta_generic_to_shared(tile + (e.y + lane) * ESA);
                     const int n = (len - lane + 31) >> 5;
 #pragma unroll 4
                     for (int i = 0; i < n; ++i) {
-                        if constexpr (ES == 4)
+                        if constexpr (ESA == 4)
                             asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(src) : "memory");
-                        else if constexpr (ES == 8)
+                        else if constexpr (ESA == 8)
                             asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
                         else
                             asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
-                        dst += 32 * ES;
-                        src += 32 * ES;
+                        dst += 32 * ESA;
+                        src += 32 * ESA;
                     }
                 }
                 asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(full_a) : "memory");
@@ -656,9 +661,9 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
                 for (int row = lane; row < rows; row += 32, ++j) {
                     if (!((row_ok >> j) & 1ull)) continue;
                     const int2 e = tabs[1][row];
-                    const uint32_t dst = (uint32_t)__cvta_generic_to_shared(tile + e.y * ES);
+                    const uint32_t dst = (uint32_t)__cvta_generic_to_shared(tile + e.y * ESA);
                     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                                 ::"r"(dst), "l"(Ab + (int64_t)e.x * ES), "r"(row_bytes), "r"(full_a) : "memory");
+                                 ::"r"(dst), "l"(Ab + (int64_t)e.x * ESA), "r"(row_bytes), "r"(full_a) : "memory");
                 }
             }
             }
@@ -670,7 +675,7 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
     // ---------------- consumer warps ----------------
     const int ctid = tid - 32;
     const int NC = NT - 32;
-    const int sstep = P.sstepB * ES;
+    const int sstep = P.sstepB * ESA;
     const bool same = P.same != 0;
     const FastDiv dlo = P.divBlo;
     for (uint32_t it = 0;; ++it) {
@@ -737,7 +742,7 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
                         const int m = (bmis + (int)((baseB + eh.x) & (VB - 1))) & (VB - 1);
                         s0[k] = (int)(p - row * nch) * VB - m;          // first element of the window, row-relative
                         ok[k] = ok[k] && s0[k] + VB > 0 && s0[k] < len;
-                        so[k] = eh.y * ES;
+                        so[k] = eh.y * ESA;
                         go[k] = eh.x;
                         if (BETA && ok[k]) {
                             const char* src = Bb + ((int64_t)go[k] + s0[k]) * ES;
@@ -759,7 +764,7 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
 #pragma unroll
                         for (int j = 0; j < VB; ++j) {
                             if (full || (s0[k] + j >= 0 && s0[k] + j < len)) {
-                                T x = scale(alpha, *reinterpret_cast<const T*>(tile + so[k] + (s0[k] + j) * sstep));
+                                T x = scale(alpha, cvt_to(T(), *reinterpret_cast<const TA*>(tile + so[k] + (s0[k] + j) * sstep)));
                                 if (BETA) x = add(x, scale(beta, bv[k].e[j]));
                                 o.e[j] = x;
                             }
@@ -790,7 +795,7 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
                     const uint32_t lo = p - hi * dlo.d;
                     const int2 el = tabs[2][lo], eh = tabs[3][hi];
                     if (edge) ok[k] = v2[lo] & v3[hi];
-                    so[k] = (el.y + eh.y) * ES;
+                    so[k] = (el.y + eh.y) * ESA;
                     go[k] = el.x + eh.x;
                     if (BETA && ok[k]) bv[k].raw = ld_plain<RawB>(Bb + (int64_t)go[k] * ES);
                 }
@@ -799,7 +804,10 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
             for (int k = 0; k < kTileUnroll; ++k) {
                 if (ok[k]) {
                     Pack<T, VB> a, o;
-                    if (VB == 1 || same) {   // same: the vector leads A and B, chunks move unchanged
+                    if constexpr (MIXED) {   // the tile holds A's type: convert element by element
+#pragma unroll
+                        for (int j = 0; j < VB; ++j) a.e[j] = cvt_to(T(), *reinterpret_cast<const TA*>(tile + so[k] + j * sstep));
+                    } else if (VB == 1 || same) {   // same: the vector leads A and B, chunks move unchanged
                         a.raw = *reinterpret_cast<const RawB*>(tile + so[k]);
                     } else {
 #pragma unroll
@@ -877,9 +885,12 @@ static DirectFn direct_fn(int vec, bool beta, bool idx64) {
 template <int DT>
 static TileFn ring_fn(int vb, bool beta, bool peel) {
     constexpr int MV = 16 / ElemT<DT>::ES;
-    if constexpr (MV > 1) {
+    constexpr bool kSameType = std::is_same<typename ElemT<DT>::T, typename ElemT<DT>::TA>::value;
+    if constexpr (MV > 1 && kSameType) {   // the peeled store phase exists for same-type pairs only
         if (vb == MV && peel) return beta ? (TileFn)ring_kernel<DT, MV, true, true> : (TileFn)ring_kernel<DT, MV, false, true>;
-        if (vb == MV) return beta ? (TileFn)ring_kernel<DT, MV, true, false> : (TileFn)ring_kernel<DT, MV, false, false>;
+    }
+    if constexpr (MV > 1) {
+        if (vb == MV && !peel) return beta ? (TileFn)ring_kernel<DT, MV, true, false> : (TileFn)ring_kernel<DT, MV, false, false>;
     }
     if (vb == 1 && !peel) return beta ? (TileFn)ring_kernel<DT, 1, true, false> : (TileFn)ring_kernel<DT, 1, false, false>;
     return nullptr;
@@ -887,8 +898,13 @@ static TileFn ring_fn(int vb, bool beta, bool peel) {
 
 static TileFn get_tile_fn(int dt, const Candidate& c) {
     const TileParams& p = c.tp;
-    if (p.ring > 0) {   // same-type pairs only: the bulk copies move A's bytes unconverted
+    if (p.ring > 0) {   // mixed pairs: no peeled store phase (the planner builds none)
+        if (dt > TTC_C128 && p.peel) return nullptr;
         switch (dt) {
+            case kPairSD: return ring_fn<kPairSD>(p.vecB, c.beta_nz, false);
+            case kPairDS: return ring_fn<kPairDS>(p.vecB, c.beta_nz, false);
+            case kPairCZ: return ring_fn<kPairCZ>(p.vecB, c.beta_nz, false);
+            case kPairZC: return ring_fn<kPairZC>(p.vecB, c.beta_nz, false);
             case TTC_F32: return ring_fn<TTC_F32>(p.vecB, c.beta_nz, p.peel != 0);
             case TTC_F64: return ring_fn<TTC_F64>(p.vecB, c.beta_nz, p.peel != 0);
             case TTC_C64: return ring_fn<TTC_C64>(p.vecB, c.beta_nz, p.peel != 0);
@@ -942,7 +958,8 @@ int prepare_candidate(Candidate* cand, ttc_dtype dtype, ttc_dtype dtype_a, int s
     }
     TileFn fn = get_tile_fn(pair, *cand);
     if (!fn) return (int)cudaErrorInvalidValue;
-    const int smem = (int)tile_smem_layout(cand->tp, elem_size(dtype)).total;
+    // the ring kernel's tile holds A's type (bulk copies), the tile kernel's B's
+    const int smem = (int)tile_smem_layout(cand->tp, elem_size(cand->tp.ring > 0 ? dtype_a : dtype)).total;
     // The attribute belongs to the kernel function, which many candidates share: raise it once
     // to the device's opt-in maximum instead of per candidate.
     int dev = 0, optin = 0;

@@ -152,14 +152,17 @@ int legal_vec(const Canon& c, int lead, bool sideA, int32_t t_lead, int mv) {
 bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, const TileSpec& spec,
                           int loop_order, int want_va, int want_vb, int max_smem, int sched, int ring, Candidate* out) {
     // es: B's element and the tile's (the planner's world is B-typed); esA differs from it only for
-    // the mixed-precision pairs, where A is converted in the load phase and the ring kernel (raw
-    // bulk copies of A's bytes) does not apply.
+    // the mixed-precision pairs.  There the tile kernel converts A in its load phase (the tile holds
+    // B's type), while the ring kernel's bulk copies land A's bytes unconverted: its tile holds A's
+    // type (esT = esA) and the consumers convert in the store phase.  Mixed ring candidates exist
+    // for 16-byte bulk rows only (no cp.async rows, no peeled store phase).
     // Vectors are 16 bytes of the side's own element type (mvA elements in A, mvB in B); where one
     // vector has to serve both sides (the wide class) it has mvS = min of the two.
     const int es = elem_size(dtype), esA = elem_size(dtype_a);
     const int mvA = 16 / esA, mvB = 16 / es, mvS = std::min(mvA, mvB);
     const int mv = mvB;   // the ring kernel's peeled store phase (same-type pairs only: mvA == mvB)
-    if (ring && dtype_a != dtype) return false;
+    const bool mixed = dtype_a != dtype;
+    const int esT = ring ? esA : es;   // element size of the shared-memory tile
     Candidate cand;
     cand.beta_nz = beta_nz;
     TileParams& P = cand.tp;
@@ -192,10 +195,12 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
     }
     // Ring kernel, peeled store phase: the B-leading index is stride-1 but its rows are not
     // 16-byte aligned (odd extent or stride): rows are cut into aligned 16-byte windows of B.
-    const bool peelB = ring && mv > 1 && want_vb == mv && vb < mv && c.d[B0].sB == 1 && A0 != B0;
+    const bool peelB = ring && !mixed && mv > 1 && want_vb == mv && vb < mv && c.d[B0].sB == 1 && A0 != B0;
     if (want_va > va || (want_vb > vb && !peelB)) return false;
     const bool same = (A0 == B0) && want_va == mvS && want_vb == mvS && mvS > 1;
-    if (A0 == B0 && want_va != want_vb) return false;   // nothing gained by mixing widths on one index
+    // nothing gained by mixing widths on one index -- except for a mixed ring, whose 16-byte rows of
+    // A's type and 16-byte stores of B's type have different element counts
+    if (A0 == B0 && want_va != want_vb && !(ring && mixed)) return false;
     P.vecA = want_va;
     P.vecB = want_vb;
     P.same = same ? 1 : 0;
@@ -225,8 +230,9 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
     // table of the A side.  Edge tiles get shorter and fewer rows.
     int row_dims = 1;
     if (ring) {
-        if (same && want_vb * es != 16) return false;
-        if (want_va * es != 16) {
+        if (same && (want_vb * es != 16 || mixed)) return false;
+        if (mixed && (want_va * esA != 16 || (want_vb != mvB && want_vb != 1))) return false;   // instances: VB = mvB or 1
+        if (want_va * esA != 16) {
             // rows that cannot be 16-byte bulk copies: element-sized cp.async rows, only where the
             // vector form is not legal (otherwise the bulk twin of this candidate is the better one)
             if (want_va != 1 || mv == 1 || legal_vec(c, A0, true, spec.t[A0] / mv * mv, mv) == mv || same ||
@@ -255,10 +261,10 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
         int64_t row_items = 1, hi = 1;
         for (int k = 0; k < row_dims; ++k) row_items *= phA[k].n;
         for (size_t k = row_dims; k < phA.size(); ++k) hi *= phA[k].n;
-        if (hi > kMaxTabEntries || (int)phA.size() - row_dims > kMaxTab || row_items * want_va * es >= (1 << 20)) return false;
+        if (hi > kMaxTabEntries || (int)phA.size() - row_dims > kMaxTab || row_items * want_va * esA >= (1 << 20)) return false;
         splitA = row_dims;
         P.ring = ring;
-        P.row_bytes = (uint32_t)(row_items * want_va * es);
+        P.row_bytes = (uint32_t)(row_items * want_va * esA);
         P.threads = 32 + (itemsB <= 4 * 256 ? 128 : 256);
     }
     if (peelB) {
@@ -310,10 +316,10 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
         }
         if (!ok) continue;
         const int64_t elems = (int64_t)ss[ta.back()] * spec.t[ta.back()];
-        if (elems * es * (ring ? ring : 1) > max_smem) continue;
-        const double conf = smem_conflict_cost(phA, phB, ss, es, want_va, want_vb, same, ss[B0], itemsA, itemsB, split != 0);
+        if (elems * esT * (ring ? ring : 1) > max_smem) continue;
+        const double conf = smem_conflict_cost(phA, phB, ss, esT, want_va, want_vb, same, ss[B0], itemsA, itemsB, split != 0);
         // a split store costs want_va - 1 extra instructions per item: worth it only for a real gain
-        const double cost = conf + 1e-3 * (double)elems * es / 1024.0 + (split ? 0.08 : 0.0);
+        const double cost = conf + 1e-3 * (double)elems * esT / 1024.0 + (split ? 0.08 : 0.0);
         if (cost < best_cost) {
             best_cost = cost;
             best_elems = elems;
@@ -391,7 +397,7 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
         P.divBlo = make_fastdiv((uint32_t)((spec.t[B0] + mv - 1) / mv + 1));
         P.peel_gslot = gslot_of[B0];
     }
-    if ((int)tile_smem_layout(P, es).total > max_smem) return false;
+    if ((int)tile_smem_layout(P, esT).total > max_smem) return false;
 
     // Contiguous runs the tile touches in A and in B (elements): leading tile indices that are
     // whole and contiguous extend the run.
@@ -417,7 +423,7 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
     I.n_u = (int)ta.size();
     I.n_w = (int)tb.size();
     I.threads = P.threads;
-    I.smem_bytes = (int)tile_smem_layout(P, es).total;
+    I.smem_bytes = (int)tile_smem_layout(P, esT).total;
     I.loop_order = loop_order;
     I.sched = sched;
     I.grid = 0;
@@ -434,7 +440,7 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
         const double nt = std::ceil((double)c.d[i].e / spec.t[i]);
         waste *= nt * spec.t[i] / (double)c.d[i].e;
     }
-    const double tile_bytes = (double)itemsA * want_va * es;
+    const double tile_bytes = (double)itemsA * want_va * esT;
     const double rd = 1.0 / run_eff((double)runA * esA) * (want_va * esA >= 16 ? 1.0 : 1.15);
     // short runs cost much less on the B side than on the A side: the 126 MB L2 merges the writes of
     // neighbouring tiles before they reach DRAM (measured: 64-byte B runs win several c2 permutations)

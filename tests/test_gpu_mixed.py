@@ -136,6 +136,31 @@ def test_mid_size_candidates(da, db, sizes, perm):
             ttc.ttc_destroy(plan)
 
 
+# ------------------------------------------------------------------ ring kernel (class tma) with conversion
+@pytest.mark.parametrize("da,db", PAIRS)
+@pytest.mark.parametrize("sizes,perm,lda,ldb", [
+    ((128, 72, 20), (2, 1, 0), None, None),                          # whole tiles
+    ((132, 50, 9), (1, 2, 0), None, None),                           # remainder tiles
+    ((8, 40, 36), (0, 2, 1), (8, 44, 36), None),                     # packing shape: short rows joined into bulk rows
+    ((24, 10, 8, 12), (3, 1, 0, 2), (24, 12, 8, 12), (12, 10, 28, 8)),   # leading dimensions on both sides
+])
+def test_ring_candidates_mixed(da, db, sizes, perm, lda, ldb):
+    """Every ring-kernel candidate of a mixed plan: the bulk copies land A's bytes, the consumer warps
+    convert (reading M1) while they store.  Bit-exact, beta = 0 and beta != 0."""
+    seen = 0
+    for beta_nz in (False, True):
+        plan = ttc.ttc_plan_mixed(da, db, len(sizes), sizes, perm, lda, ldb)
+        try:
+            which = 1 if beta_nz else 0
+            for i in range(ttc.ttc_plan_num_candidates(plan, which)):
+                if ttc.ttc_plan_candidate(plan, which, i).kernel == 5:
+                    check(da, db, sizes, perm, lda, ldb, beta_nz, plan=plan, candidate=i)
+                    seen += 1
+        finally:
+            ttc.ttc_destroy(plan)
+    assert seen > 0, "no ring candidate generated"
+
+
 # ------------------------------------------------------------------ edge cases
 @pytest.mark.parametrize("da,db", PAIRS)
 def test_beta_zero_never_reads_b_and_misaligned_pointers_fall_back(da, db):

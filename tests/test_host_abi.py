@@ -174,9 +174,10 @@ MIXED_PAIRS = ((0, 1), (1, 0), (2, 3), (3, 2))     # sd, ds, cz, zc
 
 
 @pytest.mark.parametrize("da,db", MIXED_PAIRS)
-def test_mixed_plan_reports_both_types_and_has_no_ring_candidates(da, db):
+def test_mixed_plan_reports_both_types_and_has_ring_candidates(da, db):
     """ttc_plan_mixed: dtype of the plan is B's, ttc_plan_dtype_a gives A's; vectors are at most 16
-    bytes of each side's own type; the ring kernel (raw bulk copies of A's bytes) is never a candidate."""
+    bytes of each side's own type; the ring kernel is a candidate with 16-byte bulk rows of A's type
+    only (its tile holds A's bytes, the consumers convert)."""
     w = wl.config2((2, 0, 3, 1))
     p = ttc.ttc_plan_mixed(da, db, w.n, w.sizes, w.perm)
     try:
@@ -188,7 +189,8 @@ def test_mixed_plan_reports_both_types_and_has_no_ring_candidates(da, db):
             cs = [ttc.ttc_plan_candidate(p, which, i) for i in range(n)]
             assert any(c.kernel == 1 and c.vec_a == 1 for c in cs)          # scalar fallback
             assert any(c.kernel in (2, 3, 4) for c in cs)                   # tiled transposes
-            assert all(c.kernel != 5 for c in cs)                           # no ring kernel
+            ring = [c for c in cs if c.kernel == 5]
+            assert ring and all(c.vec_a * wl.ELEM_SIZE[da] == 16 for c in ring)   # bulk rows only
             assert all(c.vec_a * wl.ELEM_SIZE[da] <= 16 and c.vec_b * wl.ELEM_SIZE[db] <= 16 for c in cs)
             if wl.ELEM_SIZE[da] < 16 and wl.ELEM_SIZE[db] < 16:   # 16-byte vectors on both sides exist
                 assert any(c.vec_a * wl.ELEM_SIZE[da] == 16 and c.vec_b * wl.ELEM_SIZE[db] == 16 for c in cs)
