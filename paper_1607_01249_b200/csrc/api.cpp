@@ -566,6 +566,6 @@ int64_t ttc_launch_count(void) { return g_launches.load(); }
 
 uint32_t ttc_debug_fastdiv(uint32_t n, uint32_t d) { return fd_div(n, make_fastdiv(d)); }
 
-const char* ttc_version(void) { return "ttc-b200 0.1 (sm_100a)"; }
+const char* ttc_version(void) { return "ttc-b200 0.2 (sm_100a)"; }
 
 }  // extern "C"
