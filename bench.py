@@ -194,13 +194,17 @@ def detail_mixed(torch, ttc, wl, flush, peak: float, profile: bool = False) -> l
     cases = [(p, perm, 0.0) for p in pairs[:2] for perm in ((0, 2, 1, 3), (2, 3, 0, 1), (3, 1, 0, 2))]
     cases += [(pairs[0], (2, 3, 0, 1), 0.5), (pairs[1], (2, 3, 0, 1), 0.5), (pairs[2], (3, 1, 0, 2), 0.0),
               (pairs[3], (3, 1, 0, 2), 0.0)]
+    # the paper's mixed-precision use case is packing for GEMM: configs[3]'s shape and lda
+    cases += [(pairs[0], "c4", 0.0), (pairs[1], "c4", 0.0)]
     for (name, da, db), perm, beta in cases:
-        w = wl.config2(perm)
+        w = wl.config4() if perm == "c4" else wl.config2(perm)
+        perm = w.perm
         numel = w.numel
-        plan = ttc.ttc_plan_mixed(da, db, w.n, w.sizes, perm)
+        plan = ttc.ttc_plan_mixed(da, db, w.n, w.sizes, perm, w.lda, w.ldb)
         info = ttc.ttc_plan_info(plan)
-        a_dev = torch.from_numpy(wl.uniform_values(wl.SEED_A, numel, da)).cuda()
-        b_dev = torch.from_numpy(wl.uniform_values(wl.SEED_B, numel, db)).cuda()
+        szb = tuple(w.sizes[q] for q in perm)
+        a_dev = torch.from_numpy(wl.embed(wl.uniform_values(wl.SEED_A, numel, da), w.sizes, w.lda)).cuda()
+        b_dev = torch.from_numpy(wl.embed(wl.uniform_values(wl.SEED_B, numel, db), szb, w.ldb)).cuda()
         alpha = 1.5
         for _ in range(3):
             ttc.ttc_execute(plan, alpha, a_dev, beta, b_dev)
@@ -213,7 +217,7 @@ def detail_mixed(torch, ttc, wl, flush, peak: float, profile: bool = False) -> l
             e1.record()
             e1.synchronize()
             ts.append(e0.elapsed_time(e1) * 1e3)
-        if profile and beta == 0 and name in ("sd", "ds") and perm != (3, 1, 0, 2):   # 4 launches for ncu
+        if profile and beta == 0 and name in ("sd", "ds") and perm != (3, 1, 0, 2) and w.name.startswith("c2"):   # 4 launches for ncu
             torch.cuda.synchronize()
             torch.cuda.cudart().cudaProfilerStart()
             ttc.ttc_execute(plan, alpha, a_dev, beta, b_dev)
@@ -223,7 +227,8 @@ def detail_mixed(torch, ttc, wl, flush, peak: float, profile: bool = False) -> l
         cand = ttc.ttc_plan_candidate(plan, which, info.chosen[which])
         nbytes = numel * (wl.ELEM_SIZE[da] + (2 if which else 1) * wl.ELEM_SIZE[db])
         t3, tm = min(ts[:3]), statistics.median(ts)
-        rows.append({"config": "mixed-%s %s on configs[1]'s tensor, beta=%g" % (name, wl.DTYPE_NAME[da] + "->" + wl.DTYPE_NAME[db], beta),
+        rows.append({"config": "mixed-%s %s on configs[%d]'s tensor, beta=%g" % (name, wl.DTYPE_NAME[da] + "->" + wl.DTYPE_NAME[db],
+                                                                               3 if w.name.startswith("c4") else 1, beta),
                      "perm": list(perm), "bytes": nbytes, "us_min_of_3": t3, "us_median_21": tm, "us_min_21": min(ts),
                      "gbs_min_of_3": nbytes / t3 / 1e3, "gbs_median": nbytes / tm / 1e3, "gbs_best": nbytes / min(ts) / 1e3,
                      "gibs_median": nbytes / tm / 1e3 * 1e9 / 2 ** 30,
