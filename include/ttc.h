@@ -19,9 +19,12 @@
  *   lda[N-1] / ldb[N-1] are validated but never used for addressing.
  *
  * Ownership: the caller owns A, B and the stream.  A plan owns only its own small host
- * state (and, for ttc_execute_host, a private pair of device staging buffers).  While
+ * state.  ttc_execute_host uses ONE pair of device staging buffers per process, grown to the
+ * largest request and freed by ttc_release_host_staging().  While
  * ttc_plan auto-tunes it allocates scratch device buffers of the real spans of A and B
  * and frees them before it returns; the caller's tensors are never touched by tuning.
+ * A candidate that fails to launch during tuning is skipped and counted in ttc_info.tune_errors
+ * (the error of that scratch launch is cleared; nothing else clears CUDA errors).
  *
  * Thread safety: distinct plans may be used from distinct threads.  One plan must not be
  * executed, re-tuned or destroyed concurrently from two threads.
@@ -87,6 +90,10 @@ typedef struct {
     int      n_candidates[2];             /* [0]: beta == 0 variants, [1]: beta != 0               */
     int      chosen[2];                   /* index of the winner in each list                      */
     float    chosen_us[2];                /* its tuned time in microseconds (0 if not tuned)       */
+    int      tune_errors;                 /* candidates that failed to configure or launch while tuning
+                                             (skipped, never chosen; 0 on a healthy device)         */
+    float    plan_ms;                     /* wall time ttc_plan spent building this plan (ms)      */
+    float    tune_ms;                     /* the part of it spent timing candidates on the device  */
 } ttc_info;
 
 /* One candidate implementation (loop order x blocking; here also kernel class). */
@@ -155,10 +162,14 @@ int ttc_plan_dtype_a(ttc_plan_t plan);
  *   A            DEVICE pointer, span_a elements; never written; padding never read.
  *   B            DEVICE pointer, span_b elements; only the elements Pi maps onto are
  *                written; padding never touched.  A and B must not overlap.
- * Pointers only have to be aligned to the element size; when they are not 16-byte aligned
- * a narrower-vector candidate of the same plan is launched instead of the tuned one.
+ * Pointers only have to be aligned to the element size (16 bytes for complex128); when they
+ * are less aligned than the tuned candidate needs, the best candidate of the same plan whose
+ * vector widths fit the actual alignment is launched instead (a tile / ring candidate with
+ * narrower vectors on the misaligned side; the scalar copy kernel only if nothing else fits).
  * Errors: TTC_ERR_INVALID_ARG (NULL plan/alpha/beta, NULL A or B for a non-empty tensor),
- * TTC_ERR_MISALIGNED, TTC_ERR_CUDA (launch failed; the CUDA error state is left as is).
+ * TTC_ERR_MISALIGNED, TTC_ERR_CUDA (the launch failed: the code cudaLaunchKernelEx returned;
+ * the library neither reads nor clears the thread's CUDA error state here, so an error left
+ * by the caller's earlier work is still there afterwards).
  */
 ttc_status ttc_execute(ttc_plan_t plan, const void* alpha, const void* A,
                        const void* beta, void* B, void* cuda_stream);
@@ -175,8 +186,12 @@ ttc_status ttc_execute(ttc_plan_t plan, const void* alpha, const void* A,
 ttc_status ttc_execute_host(ttc_plan_t plan, const void* alpha, const void* A_host,
                             const void* beta, void* B_host, void* cuda_stream);
 
-/* ttc_destroy -- frees the plan (and its staging buffers).  NULL is allowed. */
+/* ttc_destroy -- frees the plan.  NULL is allowed. */
 ttc_status ttc_destroy(ttc_plan_t plan);
+
+/* Frees the process-wide device staging buffers of ttc_execute_host (they are re-allocated on
+ * the next call that needs them).  Must not run concurrently with ttc_execute_host. */
+ttc_status ttc_release_host_staging(void);
 
 /* Thread-local status of the last ttc_plan / ttc_canonicalize call on this thread. */
 ttc_status ttc_last_error(void);

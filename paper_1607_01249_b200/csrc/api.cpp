@@ -32,8 +32,9 @@ struct ttc_plan_s {
     bool have_device = false;
     int sm_count = 148;
     int max_smem = 227 * 1024;
-    void* stage_a = nullptr;
-    void* stage_b = nullptr;
+    int tune_errors = 0;               // candidates that could not be prepared or launched while tuning
+    float plan_ms = 0.f, tune_ms = 0.f;  // wall time of building the plan / of timing candidates inside it
+    int fallback[2][25];               // [which][5 * log2(align of A) + log2(align of B)] -> candidate, -2 = not looked up
     // ttc_execute_host pipeline (contiguous tensors): the transposition is cut into `pipe_n` slabs
     // along canonical index `pipe_d`; slab c is copied in, transposed by `pipe_sub` and copied out
     // while slab c + 1 is on its way in (PCIe is full duplex).
@@ -48,6 +49,22 @@ namespace {
 
 thread_local ttc_status g_last_error = TTC_OK;
 std::atomic<int64_t> g_launches{0};
+
+// One pair of device staging buffers per process for ttc_execute_host (grown to the largest
+// request, released by ttc_release_host_staging); the call is synchronous, so it holds the lock.
+std::mutex g_stage_mu;
+void* g_stage[2] = {nullptr, nullptr};
+size_t g_stage_cap[2] = {0, 0};
+
+bool stage_reserve(int i, size_t bytes) {
+    if (g_stage_cap[i] >= bytes) return true;
+    if (g_stage[i]) cudaFree(g_stage[i]);
+    g_stage[i] = nullptr;
+    g_stage_cap[i] = 0;
+    if (cudaMalloc(&g_stage[i], bytes) != cudaSuccess) { cudaGetLastError(); return false; }
+    g_stage_cap[i] = bytes;
+    return true;
+}
 
 struct CacheEntry { int winner[2]; float us[2]; };
 std::mutex g_cache_mu;
@@ -66,6 +83,7 @@ std::string cache_key(const ttc_plan_s* p) {
     k.append((const char*)&n1, sizeof(int));
     if (const char* e = std::getenv("TTC_SCHED")) k.append(e);
     if (const char* e = std::getenv("TTC_RING")) { k.append("|ring"); k.append(e); }
+    if (const char* e = std::getenv("TTC_VARIANTS")) { k.append("|var"); k.append(e); }
     return k;
 }
 
@@ -158,17 +176,37 @@ bool ensure_prepared(ttc_plan_s* p, int which, int idx) {
 ttc_status tune(ttc_plan_s* p, int top_k, int reps, int budget_ms) {
     if (!p->have_device) return TTC_ERR_CUDA;
     if (p->canon.empty) return TTC_OK;
+    const auto t_tune0 = std::chrono::steady_clock::now();
     const size_t es = (size_t)elem_size(p->dtype), esA = (size_t)elem_size(p->dtype_a);
+    // Scratch of the real spans.  Tensors that would fit the 126 MB L2 are timed on a ROTATION of
+    // copies whose total exceeds it (caches are cleared before each run), so that
+    // candidates are ranked on DRAM traffic, as they will run, not on L2-resident data.
+    const size_t bytes_a = ((size_t)p->canon.spanA * esA + 255) & ~(size_t)255;
+    const size_t bytes_b = ((size_t)p->canon.spanB * es + 255) & ~(size_t)255;
+    int nrot = 1;
+    if (env_int("TTC_TUNE_COLD", 1) != 0 && bytes_a + bytes_b < ((size_t)300 << 20))
+        nrot = (int)std::min<size_t>(24, (((size_t)300 << 20) + bytes_a + bytes_b - 1) / (bytes_a + bytes_b));
     void *a = nullptr, *b = nullptr;
-    if (cudaMalloc(&a, (size_t)p->canon.spanA * esA) != cudaSuccess) { cudaGetLastError(); return TTC_ERR_ALLOC; }
-    if (cudaMalloc(&b, (size_t)p->canon.spanB * es) != cudaSuccess) { cudaGetLastError(); cudaFree(a); return TTC_ERR_ALLOC; }
+    while (nrot >= 1) {
+        if (cudaMalloc(&a, bytes_a * nrot) == cudaSuccess) {
+            if (cudaMalloc(&b, bytes_b * nrot) == cudaSuccess) break;
+            cudaFree(a);
+        }
+        cudaGetLastError();
+        a = b = nullptr;
+        nrot = nrot > 1 ? 1 : 0;
+    }
+    if (!a || !b) return TTC_ERR_ALLOC;
+    int rot = 0;
+    auto next_a = [&]() { return (const void*)((const char*)a + bytes_a * (size_t)(rot % nrot)); };
+    auto next_b = [&]() { void* q = (char*)b + bytes_b * (size_t)(rot % nrot); ++rot; return q; };
     cudaStream_t st;
     cudaEvent_t e0, e1;
     cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
     cudaEventCreate(&e0);
     cudaEventCreate(&e1);
-    cudaMemsetAsync(a, 0, (size_t)p->canon.spanA * esA, st);
-    cudaMemsetAsync(b, 0, (size_t)p->canon.spanB * es, st);
+    cudaMemsetAsync(a, 0, bytes_a * nrot, st);
+    cudaMemsetAsync(b, 0, bytes_b * nrot, st);
     const Scalar alpha{1.0, 0.0};
     ttc_status rc = TTC_OK;
     if (reps < 1) reps = 3;
@@ -188,13 +226,17 @@ ttc_status tune(ttc_plan_s* p, int top_k, int reps, int budget_ms) {
             }
             // the scalar fallback is always timed so that it is known to work
             if ((i >= n || over_budget) && i != p->scalar[which]) continue;
-            if (!ensure_prepared(p, which, i)) continue;
-            if (launch_candidate(cs[i], p->dtype, p->dtype_a, alpha, beta, a, b, st) != 0) { cudaGetLastError(); continue; }
+            if (!ensure_prepared(p, which, i)) { ++p->tune_errors; continue; }
+            if (launch_candidate(cs[i], p->dtype, p->dtype_a, alpha, beta, next_a(), next_b(), st) != 0) {
+                cudaGetLastError();   // a failed launch of OUR scratch run: cleared, and counted in ttc_info.tune_errors
+                ++p->tune_errors;
+                continue;
+            }
             float us = 1e30f;
             bool ok = true;
             for (int g = 0; g < 3 && ok; ++g) {   // minimum over groups (min of 3 runs)
                 cudaEventRecord(e0, st);
-                for (int r = 0; r < reps; ++r) ok &= launch_candidate(cs[i], p->dtype, p->dtype_a, alpha, beta, a, b, st) == 0;
+                for (int r = 0; r < reps; ++r) ok &= launch_candidate(cs[i], p->dtype, p->dtype_a, alpha, beta, next_a(), next_b(), st) == 0;
                 cudaEventRecord(e1, st);
                 if (cudaEventSynchronize(e1) != cudaSuccess) { ok = false; break; }
                 float ms = 0.f;
@@ -202,7 +244,7 @@ ttc_status tune(ttc_plan_s* p, int top_k, int reps, int budget_ms) {
                 us = std::min(us, ms * 1000.f / reps);
             }
             g_launches += 1 + 3 * reps;
-            if (!ok) { cudaGetLastError(); continue; }
+            if (!ok) { cudaGetLastError(); ++p->tune_errors; continue; }
             cs[i].info.tuned_us = us;
             if (best < 0 || us < best_us) { best = i; best_us = us; }
         }
@@ -222,7 +264,7 @@ ttc_status tune(ttc_plan_s* p, int top_k, int reps, int budget_ms) {
                 for (int r = 0; r < rounds && ok; ++r)
                     for (size_t f = 0; f < fin.size() && ok; ++f) {
                         cudaEventRecord(e0, st);
-                        for (int k = 0; k < per; ++k) ok &= launch_candidate(cs[fin[f]], p->dtype, p->dtype_a, alpha, beta, a, b, st) == 0;
+                        for (int k = 0; k < per; ++k) ok &= launch_candidate(cs[fin[f]], p->dtype, p->dtype_a, alpha, beta, next_a(), next_b(), st) == 0;
                         cudaEventRecord(e1, st);
                         if (cudaEventSynchronize(e1) != cudaSuccess) { ok = false; break; }
                         float ms = 0.f;
@@ -240,6 +282,7 @@ ttc_status tune(ttc_plan_s* p, int top_k, int reps, int budget_ms) {
                     }
                 } else {
                     cudaGetLastError();
+                    ++p->tune_errors;
                 }
             }
             p->winner[which] = best;
@@ -252,6 +295,7 @@ ttc_status tune(ttc_plan_s* p, int top_k, int reps, int budget_ms) {
     cudaFree(a);
     cudaFree(b);
     if (rc == TTC_OK) p->tuned = true;
+    p->tune_ms += (float)std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_tune0).count();
     return rc;
 }
 
@@ -286,6 +330,12 @@ ttc_plan_t ttc_plan_mixed(ttc_dtype dtype_a, ttc_dtype dtype, int N, const int64
 
 // Stages 2-6 for an already canonical transposition (also used for the slabs of ttc_execute_host).
 static void finish_plan(ttc_plan_s* p) {
+    const auto t_plan0 = std::chrono::steady_clock::now();
+    struct Stamp {
+        ttc_plan_s* p; std::chrono::steady_clock::time_point t0;
+        ~Stamp() { p->plan_ms = (float)std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count(); }
+    } stamp{p, t_plan0};
+    for (auto& w : p->fallback) for (int& x : w) x = -2;
     const ttc_dtype dtype = p->dtype;
     int dev = 0, count = 0;
     if (cudaGetDeviceCount(&count) == cudaSuccess && count > 0 && cudaGetDevice(&dev) == cudaSuccess) {
@@ -345,18 +395,34 @@ ttc_status ttc_execute(ttc_plan_t p, const void* alpha, const void* A, const voi
     if (p->canon.empty) return TTC_OK;
     if (!A || !B) return TTC_ERR_INVALID_ARG;
     const int es = elem_size(p->dtype), esA = elem_size(p->dtype_a);
-    const int al_b = es > 8 ? 8 : es, al_a = esA > 8 ? 8 : esA;   // complex128 only needs the alignment of its parts
-    if (((uintptr_t)A % al_a) != 0 || ((uintptr_t)B % al_b) != 0) return TTC_ERR_MISALIGNED;
+    if (((uintptr_t)A % esA) != 0 || ((uintptr_t)B % es) != 0) return TTC_ERR_MISALIGNED;
     if (!p->have_device) return TTC_ERR_CUDA;
     const int which = is_zero(p->dtype, beta) ? 0 : 1;
     int idx = p->forced[which] >= 0 ? p->forced[which] : p->winner[which];
     if (idx < 0) return TTC_ERR_UNSUPPORTED;
     const Candidate* c = &p->cands[which][idx];
     if (((uintptr_t)A % c->align_a) != 0 || ((uintptr_t)B % c->align_b) != 0) {
-        idx = p->scalar[which];
+        // Pointers that are element-aligned but not as aligned as the chosen candidate needs: the
+        // best candidate of the same list whose accesses fit (a timed one if there is one, else the
+        // best-ranked): normally a tile or ring candidate with narrower vectors on the misaligned
+        // side, the scalar direct kernel only as the last resort.  Looked up once per alignment class.
+        auto lg = [](uintptr_t x) { int l = 0; while (l < 4 && !((x >> l) & 1)) ++l; return l; };
+        const int la = lg((uintptr_t)A), lb = lg((uintptr_t)B);
+        int& slot = p->fallback[which][5 * la + lb];
+        if (slot == -2) {
+            slot = -1;
+            float best_us = 0.f;
+            const std::vector<Candidate>& cs = p->cands[which];
+            for (int i = 0; i < (int)cs.size(); ++i) {
+                if ((1 << la) % cs[i].align_a != 0 || (1 << lb) % cs[i].align_b != 0) continue;
+                const float us = cs[i].info.tuned_us;
+                if (slot < 0) { slot = i; best_us = us; continue; }       // best-ranked fitting candidate
+                if (us > 0.f && (best_us <= 0.f || us < best_us)) { slot = i; best_us = us; }
+            }
+        }
+        idx = slot;
         if (idx < 0) return TTC_ERR_MISALIGNED;
         c = &p->cands[which][idx];
-        if (((uintptr_t)A % c->align_a) != 0 || ((uintptr_t)B % c->align_b) != 0) return TTC_ERR_MISALIGNED;
     }
     if (!ensure_prepared(p, which, idx)) return TTC_ERR_CUDA;
     const int rc = launch_candidate(*c, p->dtype, p->dtype_a, to_scalar(p->dtype, alpha), to_scalar(p->dtype, beta), A, B, cuda_stream);
@@ -426,8 +492,10 @@ ttc_status ttc_execute_host(ttc_plan_t p, const void* alpha, const void* A_host,
     if (!p->have_device) return TTC_ERR_CUDA;
     const size_t es = (size_t)elem_size(p->dtype), esA = (size_t)elem_size(p->dtype_a);
     const size_t bytes_a = (size_t)p->canon.spanA * esA, bytes_b = (size_t)p->canon.spanB * es;
-    if (!p->stage_a && cudaMalloc(&p->stage_a, bytes_a) != cudaSuccess) { cudaGetLastError(); return TTC_ERR_ALLOC; }
-    if (!p->stage_b && cudaMalloc(&p->stage_b, bytes_b) != cudaSuccess) { cudaGetLastError(); return TTC_ERR_ALLOC; }
+    std::lock_guard<std::mutex> stage_lock(g_stage_mu);
+    if (!stage_reserve(0, bytes_a) || !stage_reserve(1, bytes_b)) return TTC_ERR_ALLOC;
+    void* const stage_a = g_stage[0];
+    void* const stage_b = g_stage[1];
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     // B travels to the device when it is read (beta != 0) or has padding that must survive
     const bool b_in = !is_zero(p->dtype, beta) || p->canon.spanB != p->canon.numel;
@@ -442,8 +510,8 @@ ttc_status ttc_execute_host(ttc_plan_t p, const void* alpha, const void* A_host,
                   cudaStreamWaitEvent(p->pipe_in, p->pipe_ev[2 * n], 0) == cudaSuccess &&
                   cudaStreamWaitEvent(p->pipe_out, p->pipe_ev[2 * n], 0) == cudaSuccess;
         for (int c = 0; c < n && ok; ++c) {
-            char* da = (char*)p->stage_a + c * wa;
-            char* db = (char*)p->stage_b + c * wb;
+            char* da = (char*)stage_a + c * wa;
+            char* db = (char*)stage_b + c * wb;
             ok = cudaMemcpy2DAsync(da, pa, (const char*)A_host + c * wa, pa, wa, ha, cudaMemcpyHostToDevice, p->pipe_in) == cudaSuccess;
             if (ok && b_in)
                 ok = cudaMemcpy2DAsync(db, pb, (const char*)B_host + c * wb, pb, wb, hb, cudaMemcpyHostToDevice, p->pipe_in) == cudaSuccess;
@@ -460,19 +528,17 @@ ttc_status ttc_execute_host(ttc_plan_t p, const void* alpha, const void* A_host,
         const bool s3 = cudaStreamSynchronize(p->pipe_out) == cudaSuccess;
         return ok && s1 && s2 && s3 ? TTC_OK : TTC_ERR_CUDA;
     }
-    if (cudaMemcpyAsync(p->stage_a, A_host, bytes_a, cudaMemcpyHostToDevice, st) != cudaSuccess) return TTC_ERR_CUDA;
-    if (b_in && cudaMemcpyAsync(p->stage_b, B_host, bytes_b, cudaMemcpyHostToDevice, st) != cudaSuccess) return TTC_ERR_CUDA;
-    ttc_status rc = ttc_execute(p, alpha, p->stage_a, beta, p->stage_b, cuda_stream);
+    if (cudaMemcpyAsync(stage_a, A_host, bytes_a, cudaMemcpyHostToDevice, st) != cudaSuccess) return TTC_ERR_CUDA;
+    if (b_in && cudaMemcpyAsync(stage_b, B_host, bytes_b, cudaMemcpyHostToDevice, st) != cudaSuccess) return TTC_ERR_CUDA;
+    ttc_status rc = ttc_execute(p, alpha, stage_a, beta, stage_b, cuda_stream);
     if (rc != TTC_OK) return rc;
-    if (cudaMemcpyAsync(B_host, p->stage_b, bytes_b, cudaMemcpyDeviceToHost, st) != cudaSuccess) return TTC_ERR_CUDA;
+    if (cudaMemcpyAsync(B_host, stage_b, bytes_b, cudaMemcpyDeviceToHost, st) != cudaSuccess) return TTC_ERR_CUDA;
     if (cudaStreamSynchronize(st) != cudaSuccess) return TTC_ERR_CUDA;
     return TTC_OK;
 }
 
 ttc_status ttc_destroy(ttc_plan_t p) {
     if (!p) return TTC_OK;
-    if (p->stage_a) cudaFree(p->stage_a);
-    if (p->stage_b) cudaFree(p->stage_b);
     if (p->pipe_sub) ttc_destroy(p->pipe_sub);
     if (p->pipe_in) cudaStreamDestroy(p->pipe_in);
     if (p->pipe_out) cudaStreamDestroy(p->pipe_out);
@@ -512,6 +578,9 @@ ttc_status ttc_plan_info(ttc_plan_t p, ttc_info* out) {
     out->span_a = p->canon.spanA;
     out->span_b = p->canon.spanB;
     out->tuned = p->tuned ? 1 : 0;
+    out->tune_errors = p->tune_errors;
+    out->plan_ms = p->plan_ms;
+    out->tune_ms = p->tune_ms;
     for (int w = 0; w < 2; ++w) {
         out->n_candidates[w] = (int)p->cands[w].size();
         const int idx = p->forced[w] >= 0 ? p->forced[w] : p->winner[w];
@@ -542,6 +611,7 @@ ttc_status ttc_plan_select(ttc_plan_t p, int which, int index) {
 
 ttc_status ttc_plan_tune(ttc_plan_t p, int top_k, int reps) {
     if (!p) return TTC_ERR_INVALID_ARG;
+    for (auto& w : p->fallback) for (int& x : w) x = -2;
     return tune(p, top_k, reps, 0);
 }
 
@@ -566,6 +636,16 @@ int64_t ttc_launch_count(void) { return g_launches.load(); }
 
 uint32_t ttc_debug_fastdiv(uint32_t n, uint32_t d) { return fd_div(n, make_fastdiv(d)); }
 
-const char* ttc_version(void) { return "ttc-b200 0.2 (sm_100a)"; }
+const char* ttc_version(void) { return "ttc-b200 0.3 (sm_100a)"; }
+
+ttc_status ttc_release_host_staging(void) {
+    std::lock_guard<std::mutex> lk(g_stage_mu);
+    for (int i = 0; i < 2; ++i) {
+        if (g_stage[i]) cudaFree(g_stage[i]);
+        g_stage[i] = nullptr;
+        g_stage_cap[i] = 0;
+    }
+    return TTC_OK;
+}
 
 }  // extern "C"

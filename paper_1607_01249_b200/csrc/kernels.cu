@@ -990,16 +990,23 @@ int launch_candidate(const Candidate& cand, ttc_dtype dtype, ttc_dtype dtype_a, 
     const int pair = pair_id(dtype, dtype_a);
     if (pair < 0) return (int)cudaErrorInvalidValue;
     if (cand.info.grid <= 0) return (int)cudaErrorInvalidConfiguration;
+    // cudaLaunchKernelEx returns the launch error itself: the caller's CUDA error state is not
+    // read (no cudaGetLastError, which would clear errors that are not ours).
+    cudaLaunchConfig_t cfg{};
+    cfg.stream = st;
+    cfg.gridDim = dim3((unsigned)cand.info.grid, 1, 1);
     if (cand.info.kernel == TTC_KERNEL_COPY) {
         DirectFn fn = get_direct_fn(pair, cand);
         if (!fn) return (int)cudaErrorInvalidValue;
-        fn<<<cand.info.grid, kDirectThreads, 0, st>>>(cand.dp, A, B, alpha, beta);
-    } else {
-        TileFn fn = get_tile_fn(pair, cand);
-        if (!fn) return (int)cudaErrorInvalidValue;
-        fn<<<cand.info.grid, cand.tp.threads, cand.info.smem_bytes, st>>>(cand.tp, A, B, alpha, beta);
+        cfg.blockDim = dim3(kDirectThreads, 1, 1);
+        cfg.dynamicSmemBytes = 0;
+        return (int)cudaLaunchKernelEx(&cfg, fn, cand.dp, A, B, alpha, beta);
     }
-    return (int)cudaGetLastError();   // launch-configuration errors only; clears them
+    TileFn fn = get_tile_fn(pair, cand);
+    if (!fn) return (int)cudaErrorInvalidValue;
+    cfg.blockDim = dim3((unsigned)cand.tp.threads, 1, 1);
+    cfg.dynamicSmemBytes = (size_t)cand.info.smem_bytes;
+    return (int)cudaLaunchKernelEx(&cfg, fn, cand.tp, A, B, alpha, beta);
 }
 
 }  // namespace ttc

@@ -622,7 +622,7 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, boo
         else if (!std::strcmp(e, "both")) scheds = {1, 0};
     }
 
-    static const int ring_max = std::getenv("TTC_RING") ? std::atoi(std::getenv("TTC_RING")) : 4;
+    const int ring_max = std::getenv("TTC_RING") ? std::atoi(std::getenv("TTC_RING")) : 4;
 
     // K1 / fallback: direct kernels (always at least the scalar one, valid for any strides).
     for (int sched : scheds)

@@ -27,7 +27,7 @@ NP_DTYPE = {TTC_F32: np.float32, TTC_F64: np.float64, TTC_C64: np.complex64, TTC
 EXPORTS = ["ttc_plan", "ttc_plan_mixed", "ttc_plan_dtype_a", "ttc_execute", "ttc_execute_host", "ttc_destroy", "ttc_last_error",
            "ttc_status_string", "ttc_plan_info", "ttc_plan_num_candidates", "ttc_plan_candidate",
            "ttc_plan_select", "ttc_plan_tune", "ttc_canonicalize", "ttc_launch_count",
-           "ttc_debug_fastdiv", "ttc_version"]
+           "ttc_debug_fastdiv", "ttc_version", "ttc_release_host_staging"]
 
 
 class ttc_info(ctypes.Structure):
@@ -37,7 +37,8 @@ class ttc_info(ctypes.Structure):
                 ("canon_stride_b", ctypes.c_int64 * TTC_MAX_RANK),
                 ("numel", ctypes.c_int64), ("span_a", ctypes.c_int64), ("span_b", ctypes.c_int64),
                 ("tuned", ctypes.c_int), ("n_candidates", ctypes.c_int * 2),
-                ("chosen", ctypes.c_int * 2), ("chosen_us", ctypes.c_float * 2)]
+                ("chosen", ctypes.c_int * 2), ("chosen_us", ctypes.c_float * 2),
+                ("tune_errors", ctypes.c_int), ("plan_ms", ctypes.c_float), ("tune_ms", ctypes.c_float)]
 
 
 class ttc_candidate_info(ctypes.Structure):
@@ -50,9 +51,9 @@ class ttc_candidate_info(ctypes.Structure):
 
 
 def _load() -> ctypes.CDLL:
-    path = _build.LIB_PATH
-    if not os.path.exists(path):
-        path = _build.build()           # raises if nvcc is missing: there is no other path
+    # always through build(): its mtime check makes this cheap and a stale library can never
+    # survive a source edit.  Raises if nvcc is missing and the library is out of date: there is no other path.
+    path = _build.build()
     lib = ctypes.CDLL(path)
     i64p = ctypes.POINTER(ctypes.c_int64)
     i32p = ctypes.POINTER(ctypes.c_int)
@@ -88,6 +89,7 @@ def _load() -> ctypes.CDLL:
     lib.ttc_debug_fastdiv.restype = ctypes.c_uint32
     lib.ttc_debug_fastdiv.argtypes = [ctypes.c_uint32, ctypes.c_uint32]
     lib.ttc_version.restype = ctypes.c_char_p
+    lib.ttc_release_host_staging.restype = ctypes.c_int
     return lib
 
 
@@ -238,6 +240,10 @@ def ttc_launch_count() -> int:
 
 def ttc_version() -> str:
     return lib.ttc_version().decode()
+
+
+def ttc_release_host_staging() -> None:
+    lib.ttc_release_host_staging()
 
 
 def describe_candidate(c: ttc_candidate_info, rank: int) -> str:

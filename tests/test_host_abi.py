@@ -30,9 +30,16 @@ def test_library_exports_every_declared_symbol():
     assert "sm_100a" in ttc.ttc_version()
 
 
+def test_versions_agree():
+    """Package __version__ and ttc_version() name the same release."""
+    import paper_1607_01249_b200 as pkg
+    major_minor = ".".join(pkg.__version__.split(".")[:2])
+    assert ("ttc-b200 %s " % major_minor) in ttc.ttc_version()
+
+
 def test_struct_layouts_match_header():
     """The ctypes mirrors must have the C sizes (int64 alignment included)."""
-    assert ctypes.sizeof(ttc.ttc_info) == 4 * 4 + 3 * 16 * 8 + 3 * 8 + 4 + 2 * 4 + 2 * 4 + 2 * 4 + 4
+    assert ctypes.sizeof(ttc.ttc_info) == 4 * 4 + 3 * 16 * 8 + 3 * 8 + 4 + 2 * 4 + 2 * 4 + 2 * 4 + 3 * 4
     assert ctypes.sizeof(ttc.ttc_candidate_info) % 8 == 0
 
 

@@ -273,6 +273,35 @@ def test_p9_numpy_transpose(dtype, n):
         assert np.array_equal(got, want)
 
 
+@pytest.mark.parametrize("dtype", [wl.F32, wl.C64, wl.F64])
+@pytest.mark.parametrize("n", [10, 16])
+def test_p9_numpy_transpose_high_rank(dtype, n):
+    """P9 at rank 10 and at the library's maximum rank 16 (extents 1..3, with and without leading
+    dimensions, general alpha/beta by small integers): the oracle is the checker of the GPU's
+    ``test_high_rank``, so it is pinned at those ranks too.  P1's closed form at the same ranks."""
+    rng = np.random.default_rng(1000 + n)
+    for trial in range(4):
+        sizes = tuple(int(x) for x in rng.choice([1, 2, 2, 3], size=n))
+        perm = tuple(int(x) for x in rng.permutation(n))
+        szb = sizes_b(sizes, perm)
+        lda = tuple(int(e + rng.integers(0, 2)) for e in sizes) if trial % 2 else None
+        ldb = tuple(int(e + rng.integers(0, 2)) for e in szb) if trial >= 2 else None
+        numel = int(np.prod(sizes))
+        a = small_int_values(numel, dtype, trial)
+        b0 = small_int_values(numel, dtype, 50 + trial)
+        _, got = run(dtype, sizes, perm, lda, ldb, 2.0, -3.0, a, b0)
+        want = 2 * np.transpose(a.reshape(sizes, order="F"), perm).reshape(-1, order="F") - 3 * b0
+        assert np.array_equal(got, want.astype(NP[dtype]))
+        # P1: A holds its logical linear index; B decoded from its own position
+        if dtype == wl.F64:
+            _, gotL = run(dtype, sizes, perm, lda, ldb, 1.0, 0.0, np.arange(numel, dtype=np.float64))
+            j = np.unravel_index(np.arange(numel), szb, order="F")
+            L = np.zeros(numel, dtype=np.int64)
+            for k in range(n):
+                L += j[k].astype(np.int64) * int(np.prod(sizes[:perm[k]], dtype=np.int64))
+            assert np.array_equal(gotL, L.astype(np.float64))
+
+
 # ------------------------------------------------------------- P10: linearity
 @pytest.mark.parametrize("dtype", ALL_DTYPES)
 def test_p10_linearity(dtype):
