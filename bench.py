@@ -102,6 +102,39 @@ def time_oracle(perms, A, B) -> float:
     return time.perf_counter() - t0
 
 
+def time_ref_omp(works, A_host) -> dict:
+    """The paper's OpenMP reference loop nest -- BASELINE.md section 3's timed CPU baseline --
+    built with -O3 -march=native -fopenmp on this box, all host cores, arrays first-touched in parallel
+    (PAPER.md:147, 183), minimum of 3 runs per permutation; its result is compared with the oracle's."""
+    import oracle
+    A = oracle.first_touch_copy(A_host)
+    B = oracle.first_touch_zeros(A_host)
+    secs = 0.0
+    for w in works:
+        best = None
+        for _ in range(3):
+            t0 = time.perf_counter()
+            oracle.ref_omp_native_transpose(w.dtype, w.sizes, w.perm, None, None, 1.0, A, 0.0, B)
+            dt = time.perf_counter() - t0
+            best = dt if best is None or dt < best else best
+        secs += best
+    last = works[-1]
+    B_or = np.zeros_like(A_host)
+    oracle.transpose(last.dtype, last.sizes, last.perm, None, None, 1.0, A_host, 0.0, B_or)
+    if not np.array_equal(B_or.view(np.uint8), B.view(np.uint8)):
+        raise SystemExit("bench.py: the OpenMP reference loop differs from the oracle")
+    step_bytes = sum(w.algorithmic_bytes for w in works)
+    try:
+        affinity = len(os.sched_getaffinity(0))
+    except Exception:
+        affinity = None
+    return {"value": step_bytes / secs / 1e9, "unit": UNIT, "cores": oracle.ref_omp_native_threads(),
+            "nproc": os.cpu_count(), "affinity_cores": affinity, "kind": "paper's OpenMP reference loop nest (PAPER.md:167)",
+            "flags": oracle.NATIVE_FLAGS, "seconds": secs,
+            "sample": "one whole step: all %d permutations, min of 3 runs each, whole 198 MB tensors" % len(works),
+            "checked": "bit-identical to the oracle on the last permutation"}
+
+
 def run_reference(args) -> None:
     """--impl reference: the oracle on the host cores, same metric/config; a step is a bounded
     sample (3 of the 23 permutations: canonical rank 2, 3 and 4)."""
@@ -133,62 +166,173 @@ def run_reference(args) -> None:
 
 
 # ------------------------------------------------------------------------------ GPU arm
-def cold_times(torch, ttc, plan, w, a_dev, b_dev, flush, reps: int):
-    """Per-launch device times (us) with L2 flushed before every run."""
+class Evictor:
+    """Puts the 126 MB L2 into a known state before a timed launch (the paper clears the
+    caches before every run).  Two ways, reported side by side so that their difference is attributed:
+      read   -- a reduction READS a 256 MB buffer: L2 ends up full of CLEAN lines of that buffer, the timed
+                kernel pays nothing for the eviction (the clean-cold figure);
+      memset -- the buffer is WRITTEN: L2 ends up full of DIRTY lines whose write-back to HBM is
+                charged to the timed kernel (what round 1 reported as "cold")."""
+    METHODS = ("read", "memset")
+
+    def __init__(self, torch, nbytes: int = 256 << 20):
+        self.torch = torch
+        self.buf = torch.zeros(nbytes // 4, dtype=torch.int32, device="cuda")
+
+    def __call__(self, method: str) -> None:
+        if method == "read":
+            self.buf.max()
+        elif method == "memset":
+            self.buf.zero_()
+        else:
+            raise ValueError(method)
+
+
+def cold_times(torch, ttc, plan, alpha, beta, a_dev, b_dev, evict, method: str, reps: int):
+    """Per-launch device times (us), L2 evicted before every run."""
     out = []
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     for _ in range(reps):
-        flush.zero_()
+        evict(method)
         e0.record()
-        ttc.ttc_execute(plan, w.alpha, a_dev, w.beta, b_dev)
+        ttc.ttc_execute(plan, alpha, a_dev, beta, b_dev)
         e1.record()
         e1.synchronize()
         out.append(e0.elapsed_time(e1) * 1e3)
     return out
 
 
+def cold_row(torch, ttc, plan, w, nbytes, alpha, beta, a_dev, b_dev, evict, peak, reps: int = 21) -> dict:
+    """min of 3 (the paper's statistic) and median of `reps`, for both eviction methods."""
+    for _ in range(3):
+        ttc.ttc_execute(plan, alpha, a_dev, beta, b_dev)
+    row = {"config": w.name, "perm": "".join(map(str, w.perm)), "bytes": nbytes}
+    for m in Evictor.METHODS:
+        ts = cold_times(torch, ttc, plan, alpha, beta, a_dev, b_dev, evict, m, reps)
+        t3, tm = min(ts[:3]), statistics.median(ts)
+        row[m] = {"us_min_of_3": t3, "us_median": tm, "gbs_min_of_3": nbytes / t3 / 1e3, "gbs_median": nbytes / tm / 1e3,
+                  "frac_of_measured_copy": nbytes / tm / 1e3 / peak, "frac_of_8TBs": nbytes / tm / 1e3 / NOMINAL_HBM_GBS}
+    return row
+
+
+def cold_block(torch, ttc, wl, peak, works, plans, a_dev, b_dev) -> dict:
+    """SURVEY.md 8(d) protocol inside the driver-run line: every permutation of configs[1] and
+    configs[0], [2], [3], [4], L2 evicted before EVERY timed launch, min of 3 and median of 21."""
+    evict = Evictor(torch)
+    rows = []
+    for p, w in zip(plans, works):
+        rows.append(cold_row(torch, ttc, p, w, w.algorithmic_bytes, w.alpha, w.beta, a_dev, b_dev, evict, peak))
+    others = {}
+    for w in (wl.config1(), wl.config3(), wl.config4(), wl.config5()):
+        plan = ttc.ttc_plan(w.dtype, w.n, w.sizes, w.perm, w.lda, w.ldb)
+        info = ttc.ttc_plan_info(plan)
+        xa = torch.from_numpy(w.make_a()).cuda()
+        xb = torch.from_numpy(w.make_b()).cuda()
+        row = cold_row(torch, ttc, plan, w, w.algorithmic_bytes, w.alpha, w.beta, xa, xb, evict, peak)
+        which = 1 if w.beta_nonzero else 0
+        row["chosen"] = ttc.describe_candidate(ttc.ttc_plan_candidate(plan, which, info.chosen[which]), info.canon_rank)
+        row["plan_ms"] = info.plan_ms
+        if w.name.startswith("c1"):      # small tensor (23.6 MB): also the warm, L2-resident figure
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            ts = []
+            for _ in range(21):
+                e0.record()
+                ttc.ttc_execute(plan, w.alpha, xa, w.beta, xb)
+                e1.record()
+                e1.synchronize()
+                ts.append(e0.elapsed_time(e1) * 1e3)
+            row["warm_l2_resident"] = {"us_median": statistics.median(ts),
+                                       "gbs_median": w.algorithmic_bytes / statistics.median(ts) / 1e3}
+        rows.append(row)
+        others[w.name.split("_")[0]] = row
+        ttc.ttc_destroy(plan)
+        del xa, xb
+    c2 = rows[:len(works)]
+
+    def summary(method):
+        g = [r[method]["gbs_median"] for r in c2]
+        return {"min": min(g), "median": statistics.median(g), "max": max(g),
+                "min_frac_of_measured_copy": min(g) / peak, "median_frac_of_measured_copy": statistics.median(g) / peak,
+                "median_frac_of_8TBs": statistics.median(g) / NOMINAL_HBM_GBS}
+    per_config = {"c2": {"gbs_median_over_perms": summary("read")["median"], "gbs_min_over_perms": summary("read")["min"],
+                         "frac_of_measured_copy": summary("read")["median_frac_of_measured_copy"],
+                         "frac_of_8TBs": summary("read")["median_frac_of_8TBs"]}}
+    for k, r in others.items():
+        per_config[k] = {"gbs_median": r["read"]["gbs_median"], "gbs_min_of_3": r["read"]["gbs_min_of_3"],
+                         "frac_of_measured_copy": r["read"]["frac_of_measured_copy"], "frac_of_8TBs": r["read"]["frac_of_8TBs"]}
+    return {"protocol": "L2 evicted before every timed launch (PAPER.md:147); min of 3 and median of 21 per case; "
+                        "read = 256 MB read sweep (clean lines), memset = 256 MB write (dirty lines, their write-back "
+                        "is charged to the timed kernel); per_config quotes the read-evicted medians",
+            "c2_read": summary("read"), "c2_memset": summary("memset"), "per_config": per_config, "rows": rows}
+
+
+def _legacy_fields(row: dict, peak: float) -> dict:
+    """Flat keys of the round-1 detail table, taken from the read-evicted (clean-cold) measurement."""
+    r = row["read"]
+    row.update({"us_min_of_3": r["us_min_of_3"], "us_median_21": r["us_median"], "gbs_min_of_3": r["gbs_min_of_3"],
+                "gbs_median": r["gbs_median"], "gibs_median": r["gbs_median"] * 1e9 / 2 ** 30,
+                "frac_of_8TBs": r["frac_of_8TBs"], "frac_of_measured_copy": r["frac_of_measured_copy"],
+                "gbs_median_memset_evicted": row["memset"]["gbs_median"]})
+    return row
+
+
+def profiled_launch(torch, ttc, plan, alpha, beta, a_dev, b_dev) -> None:
+    """One launch inside a cudaProfilerStart/Stop range (for ncu --profile-from-start off)."""
+    torch.cuda.synchronize()
+    torch.cuda.cudart().cudaProfilerStart()
+    ttc.ttc_execute(plan, alpha, a_dev, beta, b_dev)
+    torch.cuda.synchronize()
+    torch.cuda.cudart().cudaProfilerStop()
+
+
 def detail_all_configs(torch, ttc, wl, path: str, peak: float, profile: bool = False) -> None:
     """Per-config report of all five BASELINE.json configs (north_star: 'reported per config')."""
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    evict = Evictor(torch)
     rows = []
     for w in wl.baseline_configs():
         plan = ttc.ttc_plan(w.dtype, w.n, w.sizes, w.perm, w.lda, w.ldb)
         info = ttc.ttc_plan_info(plan)
         a_dev = torch.from_numpy(w.make_a()).cuda()
         b_dev = torch.from_numpy(w.make_b()).cuda()
-        for _ in range(3):
-            ttc.ttc_execute(plan, w.alpha, a_dev, w.beta, b_dev)
-        ts = cold_times(torch, ttc, plan, w, a_dev, b_dev, flush, 21)
-        if profile and not w.name.startswith("c2"):     # one launch per config for ncu --profile-from-start off
-            torch.cuda.synchronize()
-            torch.cuda.cudart().cudaProfilerStart()
-            ttc.ttc_execute(plan, w.alpha, a_dev, w.beta, b_dev)
-            torch.cuda.synchronize()
-            torch.cuda.cudart().cudaProfilerStop()
+        row = cold_row(torch, ttc, plan, w, w.algorithmic_bytes, w.alpha, w.beta, a_dev, b_dev, evict, peak)
+        if profile and not w.name.startswith("c2"):
+            profiled_launch(torch, ttc, plan, w.alpha, w.beta, a_dev, b_dev)
         which = 1 if w.beta_nonzero else 0
         cand = ttc.ttc_plan_candidate(plan, which, info.chosen[which])
-        t3, tm = min(ts[:3]), statistics.median(ts)
-        gbs = w.algorithmic_bytes / (min(ts) * 1e-6) / 1e9
-        rows.append({"config": w.name, "perm": list(w.perm), "bytes": w.algorithmic_bytes,
-                     "us_min_of_3": t3, "us_median_21": tm, "us_min_21": min(ts),
-                     "gbs_min_of_3": w.algorithmic_bytes / t3 / 1e3,
-                     "gbs_median": w.algorithmic_bytes / tm / 1e3, "gbs_best": gbs,
-                     "gibs_median": w.algorithmic_bytes / tm / 1e3 * 1e9 / 2 ** 30,
-                     "frac_of_8TBs": w.algorithmic_bytes / tm / 1e3 / NOMINAL_HBM_GBS,
-                     "frac_of_measured_copy": w.algorithmic_bytes / tm / 1e3 / peak,
-                     "chosen": ttc.describe_candidate(cand, info.canon_rank),
-                     "n_candidates": info.n_candidates[which]})
+        row.update({"chosen": ttc.describe_candidate(cand, info.canon_rank), "n_candidates": info.n_candidates[which],
+                    "plan_ms": info.plan_ms, "tune_ms": info.tune_ms})
+        rows.append(_legacy_fields(row, peak))
         ttc.ttc_destroy(plan)
         del a_dev, b_dev
-    rows.extend(detail_mixed(torch, ttc, wl, flush, peak, profile))
+    rows.extend(detail_misaligned(torch, ttc, wl, evict, peak))
+    rows.extend(detail_mixed(torch, ttc, wl, evict, peak, profile))
     with open(path, "w") as fh:
         json.dump(rows, fh, indent=1)
 
 
-def detail_mixed(torch, ttc, wl, flush, peak: float, profile: bool = False) -> list:
+def detail_misaligned(torch, ttc, wl, evict, peak: float) -> list:
+    """Element-aligned but not 16-byte aligned pointers: the alignment-aware fallback
+    candidate of the same plan, timed on three permutations of configs[1]'s tensor."""
+    rows = []
+    for perm in ((0, 2, 1, 3), (2, 3, 0, 1), (3, 1, 0, 2)):
+        w = wl.config2(perm)
+        plan = ttc.ttc_plan(w.dtype, w.n, w.sizes, w.perm)
+        a_all = torch.zeros(w.numel + 2, dtype=torch.float64, device="cuda")
+        b_all = torch.zeros(w.numel + 2, dtype=torch.float64, device="cuda")
+        a_all[1:1 + w.numel] = torch.from_numpy(w.make_a()).cuda()
+        for ma, mb in ((1, 0), (0, 1), (1, 1)):
+            name = "misaligned A+%d B+%d elements, %s" % (ma, mb, w.name)
+            row = cold_row(torch, ttc, plan, wl.Workload(name, w.dtype, w.sizes, w.perm), w.algorithmic_bytes, 1.0, 0.0,
+                           a_all[ma:ma + w.numel], b_all[mb:mb + w.numel], evict, peak)
+            rows.append(_legacy_fields(row, peak))
+        ttc.ttc_destroy(plan)
+        del a_all, b_all
+    return rows
+
+
+def detail_mixed(torch, ttc, wl, evict, peak: float, profile: bool = False) -> list:
     """Mixed-precision transpositions on configs[1]'s tensor:
     A of one type, B of the other.  Algorithmic bytes = |A| * (sizeof(A) + (1 | 2) * sizeof(B))."""
-    import numpy as np
     rows = []
     pairs = (("sd", wl.F32, wl.F64), ("ds", wl.F64, wl.F32), ("cz", wl.C64, wl.C128), ("zc", wl.C128, wl.C64))
     cases = [(p, perm, 0.0) for p in pairs[:2] for perm in ((0, 2, 1, 3), (2, 3, 0, 1), (3, 1, 0, 2))]
@@ -206,36 +350,17 @@ def detail_mixed(torch, ttc, wl, flush, peak: float, profile: bool = False) -> l
         a_dev = torch.from_numpy(wl.embed(wl.uniform_values(wl.SEED_A, numel, da), w.sizes, w.lda)).cuda()
         b_dev = torch.from_numpy(wl.embed(wl.uniform_values(wl.SEED_B, numel, db), szb, w.ldb)).cuda()
         alpha = 1.5
-        for _ in range(3):
-            ttc.ttc_execute(plan, alpha, a_dev, beta, b_dev)
-        ts = []
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        for _ in range(21):
-            flush.zero_()
-            e0.record()
-            ttc.ttc_execute(plan, alpha, a_dev, beta, b_dev)
-            e1.record()
-            e1.synchronize()
-            ts.append(e0.elapsed_time(e1) * 1e3)
-        if profile and beta == 0 and name in ("sd", "ds") and perm != (3, 1, 0, 2) and w.name.startswith("c2"):   # 4 launches for ncu
-            torch.cuda.synchronize()
-            torch.cuda.cudart().cudaProfilerStart()
-            ttc.ttc_execute(plan, alpha, a_dev, beta, b_dev)
-            torch.cuda.synchronize()
-            torch.cuda.cudart().cudaProfilerStop()
         which = 1 if beta != 0 else 0
-        cand = ttc.ttc_plan_candidate(plan, which, info.chosen[which])
         nbytes = numel * (wl.ELEM_SIZE[da] + (2 if which else 1) * wl.ELEM_SIZE[db])
-        t3, tm = min(ts[:3]), statistics.median(ts)
-        rows.append({"config": "mixed-%s %s on configs[%d]'s tensor, beta=%g" % (name, wl.DTYPE_NAME[da] + "->" + wl.DTYPE_NAME[db],
-                                                                               3 if w.name.startswith("c4") else 1, beta),
-                     "perm": list(perm), "bytes": nbytes, "us_min_of_3": t3, "us_median_21": tm, "us_min_21": min(ts),
-                     "gbs_min_of_3": nbytes / t3 / 1e3, "gbs_median": nbytes / tm / 1e3, "gbs_best": nbytes / min(ts) / 1e3,
-                     "gibs_median": nbytes / tm / 1e3 * 1e9 / 2 ** 30,
-                     "frac_of_8TBs": nbytes / tm / 1e3 / NOMINAL_HBM_GBS,
-                     "frac_of_measured_copy": nbytes / tm / 1e3 / peak,
-                     "chosen": ttc.describe_candidate(cand, info.canon_rank),
-                     "n_candidates": info.n_candidates[which]})
+        label = "mixed-%s %s on configs[%d]'s tensor, beta=%g" % (name, wl.DTYPE_NAME[da] + "->" + wl.DTYPE_NAME[db],
+                                                                   3 if w.name.startswith("c4") else 1, beta)
+        row = cold_row(torch, ttc, plan, wl.Workload(label, db, w.sizes, perm), nbytes, alpha, beta, a_dev, b_dev, evict, peak)
+        if profile and beta == 0 and name in ("sd", "ds") and perm != (3, 1, 0, 2) and w.name.startswith("c2"):   # 4 launches for ncu
+            profiled_launch(torch, ttc, plan, alpha, beta, a_dev, b_dev)
+        cand = ttc.ttc_plan_candidate(plan, which, info.chosen[which])
+        row.update({"chosen": ttc.describe_candidate(cand, info.canon_rank), "n_candidates": info.n_candidates[which],
+                    "plan_ms": info.plan_ms})
+        rows.append(_legacy_fields(row, peak))
         ttc.ttc_destroy(plan)
         del a_dev, b_dev
     return rows
@@ -273,21 +398,24 @@ def run_ours(args) -> None:
     if args.perms:     # profiling aid (ncu captures of single permutations); not the headline workload
         keep = {tuple(int(ch) for ch in x) for x in args.perms.split(",")}
         works = [w for w in works if w.perm in keep]
+    t_plan0 = time.perf_counter()
     plans = [ttc.ttc_plan(w.dtype, w.n, w.sizes, w.perm) for w in works]      # tuned here, untimed
+    plan_wall_s = time.perf_counter() - t_plan0
     A_host = works[0].make_a()
     a_dev = torch.from_numpy(A_host).cuda()
     b_dev = torch.zeros_like(a_dev)
     step_bytes = sum(w.algorithmic_bytes for w in works)
     stream = torch.cuda.current_stream()
 
-    def one_step(events=None):
+    def one_step(events=None, st=None):
         # one event between consecutive launches: events[i] .. events[i + 1] brackets launch i
+        st = st or stream
         for i, (p, w) in enumerate(zip(plans, works)):
             if events is not None:
-                events[i].record(stream)
-            ttc.ttc_execute(p, 1.0, a_dev, 0.0, b_dev, stream)
+                events[i].record(st)
+            ttc.ttc_execute(p, 1.0, a_dev, 0.0, b_dev, st)
         if events is not None:
-            events[len(plans)].record(stream)
+            events[len(plans)].record(st)
 
     def barrier():
         torch.cuda.synchronize()
@@ -295,29 +423,70 @@ def run_ours(args) -> None:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(warmup):
+    # A step is launched as ONE CUDA graph replay: the 23 ttc_execute calls are captured once
+    # (untimed) and replayed -- ttc_execute is a single asynchronous kernel launch with no library
+    # state, so it captures as one kernel node.  Kernel-to-kernel edges of a graph cost ~2.5 us less
+    # than stream launches on this machine and let programmatic dependent launch overlap a kernel's
+    # prologue with its predecessor's tail.  --no-graph: plain stream launches.
+    use_graph = not args.no_graph
+    n_ev = 0 if args.no_launch_events else min(8, max(1, steps // 4))
+    ev_steps = list(range(0, steps, 4))[:n_ev]
+    ev = {s: [torch.cuda.Event(enable_timing=True, external=use_graph) for _ in range(len(works) + 1)]
+          for s in ev_steps} if n_ev else None
+    side = torch.cuda.Stream()
+
+    def capture(events=None):
+        g = torch.cuda.CUDAGraph()
+        side.wait_stream(stream)
+        with torch.cuda.stream(side):
+            with torch.cuda.graph(g, stream=side):
+                one_step(events, side)
+        return g
+
+    for _ in range(warmup if not use_graph else 1):
         one_step()
-    # per-launch events for the roofline of the dominant kernel, live in the timed region
-    # per-launch events in every 4th timed step (each event costs ~0.3 us of stream time)
-    ev_steps = list(range(0, steps, 4))
-    ev = {s: [torch.cuda.Event(enable_timing=True) for _ in range(len(works) + 1)]
-          for s in ev_steps} if not args.no_launch_events else None
+    graph_plain = graph_ev = None
+    if use_graph:
+        graph_plain = capture()
+        # per-launch events for the roofline of the dominant kernel, live in the timed region: every
+        # 4th of the first steps replays a twin graph with an (external) event node between the launches
+        graph_ev = {s: capture(ev[s]) for s in ev_steps} if ev else {}
+        for _ in range(warmup):
+            graph_plain.replay()
     sampler = ClockSampler(local)
     sampler.start()
     time.sleep(0.25)
     barrier()
-    launches0 = ttc.ttc_launch_count()
     t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.cudart().cudaProfilerStart()     # ncu --profile-from-start off sees only the timed region
     t0.record(stream)
     for s in range(steps):
-        one_step(ev.get(s) if ev else None)
+        if use_graph:
+            (graph_ev.get(s) or graph_plain).replay()
+        else:
+            one_step(ev.get(s) if ev else None)
     t1.record(stream)
     barrier()
     torch.cuda.cudart().cudaProfilerStop()
-    launches = ttc.ttc_launch_count() - launches0
+    launches = steps * len(plans)               # kernels of libttc.so launched inside the timed region
     clocks = sampler.stop()
     value, ms_total = whole_job_value(step_bytes, steps, world, t0.elapsed_time(t1), dist, "cuda")
+
+    # the same step as plain stream launches (what round 1 timed), for comparison
+    stream_launch = None
+    if use_graph:
+        k = min(steps, 20)
+        for _ in range(3):
+            one_step()
+        barrier()
+        t0.record(stream)
+        for _ in range(k):
+            one_step()
+        t1.record(stream)
+        barrier()
+        v2, ms2 = whole_job_value(step_bytes, k, world, t0.elapsed_time(t1), dist, "cuda")
+        stream_launch = {"value": v2, "unit": UNIT, "ms_per_step": ms2 / k, "steps": k,
+                         "note": "23 ttc_execute calls per step issued on the stream, no graph"}
 
     # per-permutation launch durations (median over steps) and the roofline of the tile kernel
     per_perm, infos = [], []
@@ -328,6 +497,9 @@ def run_ours(args) -> None:
         infos.append((w, cand, info))
         per_perm.append({"perm": "".join(map(str, w.perm)), "kernel": ttc.KERNEL_NAMES[cand.kernel],
                          "us": us, "gbs": (w.algorithmic_bytes / us / 1e3) if us else None,
+                         "frac_of_measured_copy": (w.algorithmic_bytes / us / 1e3 / peak) if us else None,
+                         "plan_ms": info.plan_ms, "tune_ms": info.tune_ms, "tune_errors": info.tune_errors,
+                         "n_candidates": info.n_candidates[0],
                          "chosen": ttc.describe_candidate(cand, info.canon_rank)})
     roofline = None
     if ev:
@@ -341,12 +513,20 @@ def run_ours(args) -> None:
                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                     "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
                     "avg_launch_us": dom_us / len(dom), "algorithmic_bytes_per_launch": works[0].algorithmic_bytes,
-                    "share_of_step": dom_us / sum(r["us"] for r in per_perm), "traffic": None}
-        tr = os.path.join(ROOT, "profiles", "traffic_r01.csv")     # from the ncu --set full capture
-        if os.path.exists(tr):
+                    "share_of_step": dom_us / sum(r["us"] for r in per_perm),
+                    "per_launch_gbs": {"min": min(r["gbs"] for r in dom), "median": statistics.median(r["gbs"] for r in dom),
+                                       "max": max(r["gbs"] for r in dom)},
+                    "traffic": None, "traffic_source": None}
+        # dram__bytes_read.sum + dram__bytes_write.sum per launch of that kernel, from the committed
+        # ncu --set full capture of this round (a run under ncu cannot be the timed run)
+        import glob
+        for tr in sorted(glob.glob(os.path.join(ROOT, "profiles", "traffic_r*.csv")), reverse=True):
             for ln in open(tr):
                 if ln.startswith("transpose_kernel_dram_bytes_per_launch,"):
                     roofline["traffic"] = int(ln.split(",")[1])
+                    roofline["traffic_source"] = "profiles/" + os.path.basename(tr)
+            if roofline["traffic"] is not None:
+                break
 
     # ---- end to end through the public host-buffer call: pinned host A -> device, kernel,
     # device -> pinned host B, every permutation, inside the timed region
@@ -383,7 +563,13 @@ def run_ours(args) -> None:
     if args.detail and rank == 0:
         detail_all_configs(torch, ttc, wl, args.detail, peak, args.profile_detail)
 
-    cpu = None
+    cold = None
+    if rank == 0 and world == 1 and not args.no_cold:
+        cold = cold_block(torch, ttc, wl, peak, works, plans, a_dev, b_dev)
+
+    cpu = cpu_omp = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu_omp = time_ref_omp(works, A_host)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         B_or = np.zeros_like(A_host)
         perms = [w.perm for w in works]
@@ -404,12 +590,21 @@ def run_ours(args) -> None:
                 "data": "synthetic (seeded SplitMix64 uniform [-1,1))",
                 "config": {"workload": WORKLOAD if not args.perms else WORKLOAD + " -- SUBSET " + args.perms,
                            "parallelism": "replicas only (no collective)",
-                           "l2": "inputs larger than L2: A and B are 198 MB each, L2 is 126 MB; "
-                                 "no explicit flush between launches",
-                           "launches_per_step": len(plans)},
+                           "l2": "inputs larger than L2: A and B are 198 MB each, L2 is 126 MB; no explicit flush "
+                                 "between the 23 back-to-back launches of a step (the `cold` block holds the "
+                                 "flush-before-every-launch figures of SURVEY.md 8(d))",
+                           "launches_per_step": len(plans),
+                           "launch_mode": "one CUDA graph replay per step (23 kernel nodes, captured once before "
+                                          "the timed region)" if use_graph else "stream launches"},
+                "stream_launch": stream_launch,
                 "frac_of_measured_copy": value / world / peak, "frac_of_nominal_8TBs": value / world / NOMINAL_HBM_GBS,
                 "per_perm_gbs": {"min": min(gbs), "median": statistics.median(gbs), "max": max(gbs)} if gbs else None,
-                "per_perm": per_perm, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
+                "per_perm": per_perm, "roofline": roofline, "cold": cold,
+                "per_config": cold["per_config"] if cold else None,
+                "plan_ms": {"median": statistics.median(r["plan_ms"] for r in per_perm),
+                            "max": max(r["plan_ms"] for r in per_perm), "total_wall_s": plan_wall_s,
+                            "note": "ttc_plan incl. on-device tuning of the beta=0 and beta!=0 lists; untimed, once per transposition"},
+                "cpu_baseline": cpu, "cpu_baseline_omp": cpu_omp, "e2e": e2e,
                 "gpu_launches": launches, "clocks": clocks}
         print(json.dumps(line))
     if dist is not None:
@@ -429,7 +624,9 @@ def main() -> None:
     ap.add_argument("--profile-detail", action="store_true", help="with --detail: one extra launch of c1, c3, c4, c5 "
                     "inside a cudaProfilerStart/Stop range (for ncu --profile-from-start off)")
     ap.add_argument("--no-launch-events", action="store_true")
+    ap.add_argument("--no-graph", action="store_true", help="issue the 23 launches of a step on the stream instead of replaying a CUDA graph")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-cold", action="store_true", help="skip the cold-L2 block (profiling runs)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

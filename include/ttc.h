@@ -36,6 +36,7 @@
  *   TTC_CACHE_FILE=path   solution store on disk (winners appended, reloaded by later processes)
  *   TTC_SCHED=static|both work distribution: persistent grid-stride instead of / beside the default,
  *                         dynamic distribution by cluster launch control
+ *   TTC_PDL=0             launch without programmatic dependent launch (default: with)
  *   TTC_RING=0|2|4        largest ring of tile buffers of the warp-specialised kernel (0: none; default 4)
  */
 #ifndef TTC_H_

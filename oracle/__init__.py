@@ -113,6 +113,75 @@ def ref_omp_threads() -> int:
     return int(_load().ttc_ref_omp_threads())
 
 
+# ------------------------------------------------------------------ the timed CPU baseline
+# BASELINE.md section 3 item 2 / SURVEY.md 8(d): the paper's reference loop nest built with
+# ``-O3 -march=native -fopenmp`` (Table 2's compiler flags), all host cores.
+# -march=native binds the object to the CPU it was compiled on, so it is compiled on the box that
+# runs it, into a file named after that CPU's flags.  -ffp-contract=off keeps the separate
+# roundings (reading A7), so the result can still be compared with the oracle bit for bit; it
+# does not slow a bandwidth-bound loop.
+_NATIVE_CFLAGS = ["-O3", "-march=native", "-fopenmp", "-std=c11", "-ffp-contract=off", "-fPIC", "-shared"]
+_native = None
+
+
+def _cpu_tag() -> str:
+    import hashlib
+    try:
+        with open("/proc/cpuinfo") as fh:
+            flags = next((ln for ln in fh if ln.startswith("flags")), "")
+    except OSError:
+        flags = ""
+    return hashlib.sha1(flags.encode()).hexdigest()[:10]
+
+
+def _load_native():
+    global _native
+    if _native is None:
+        path = os.path.join(_HERE, "libttc_ref_omp_native.%s.so" % _cpu_tag())
+        src = _SOURCES[1]
+        if not os.path.exists(path) or os.path.getmtime(path) < os.path.getmtime(src):
+            tmp = path + ".tmp.%d" % os.getpid()
+            subprocess.check_call(["gcc", *_NATIVE_CFLAGS, "-o", tmp, src])
+            os.replace(tmp, path)
+        lib = ctypes.CDLL(path)
+        i64p = ctypes.POINTER(ctypes.c_int64)
+        i32p = ctypes.POINTER(ctypes.c_int)
+        lib.ttc_ref_omp_transpose.restype = ctypes.c_int
+        lib.ttc_ref_omp_transpose.argtypes = [ctypes.c_int, ctypes.c_int, i64p, i32p, i64p, i64p,
+                                              ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+        lib.ttc_ref_omp_parallel_copy.restype = None
+        lib.ttc_ref_omp_parallel_copy.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64]
+        lib.ttc_ref_omp_threads.restype = ctypes.c_int
+        _native = lib
+    return _native
+
+
+NATIVE_FLAGS = "gcc " + " ".join(_NATIVE_CFLAGS)
+
+
+def ref_omp_native_transpose(dtype: int, sizes, perm, lda, ldb, alpha, A: np.ndarray, beta, B: np.ndarray) -> None:
+    """The same loop nest as :func:`ref_omp_transpose`, built with ``NATIVE_FLAGS`` on this machine."""
+    _call(_load_native().ttc_ref_omp_transpose, dtype, sizes, perm, lda, ldb, alpha, A, beta, B)
+
+
+def ref_omp_native_threads() -> int:
+    return int(_load_native().ttc_ref_omp_threads())
+
+
+def first_touch_copy(src: np.ndarray) -> np.ndarray:
+    """A copy of ``src`` whose pages are first touched by the OpenMP threads."""
+    dst = np.empty_like(src)
+    _load_native().ttc_ref_omp_parallel_copy(dst.ctypes.data_as(ctypes.c_void_p), src.ctypes.data_as(ctypes.c_void_p),
+                                             int(src.nbytes))
+    return dst
+
+
+def first_touch_zeros(like: np.ndarray) -> np.ndarray:
+    dst = np.empty_like(like)
+    _load_native().ttc_ref_omp_parallel_copy(dst.ctypes.data_as(ctypes.c_void_p), None, int(like.nbytes))
+    return dst
+
+
 def offsets(sizes, perm, lda, ldb, index):
     """(offA, offB) in elements of the logical element with A multi-index ``index``."""
     n = len(sizes)

@@ -104,6 +104,20 @@ int ttc_ref_omp_transpose(int dtype, int N, const int64_t *sizes, const int *per
     return 0;
 }
 
+/* Parallel copy with the same static schedule as the loop nest: a freshly mmap'ed destination is
+ * thereby FIRST TOUCHED by the threads that will use it (the arrays of the
+ * paper's measurements are initialised in parallel).  No arithmetic of the method in here. */
+void ttc_ref_omp_parallel_copy(void *dst, const void *src, int64_t bytes)
+{
+    const int64_t chunk = 1 << 20;
+    const int64_t n = (bytes + chunk - 1) / chunk;
+    _Pragma("omp parallel for schedule(static)")
+    for (int64_t c = 0; c < n; ++c) {
+        const int64_t lo = c * chunk, hi = lo + chunk < bytes ? lo + chunk : bytes;
+        for (int64_t i = lo; i < hi; ++i) ((unsigned char *)dst)[i] = src ? ((const unsigned char *)src)[i] : 0;
+    }
+}
+
 int ttc_ref_omp_threads(void)
 {
     int n = 1;

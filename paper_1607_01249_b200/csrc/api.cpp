@@ -32,6 +32,7 @@ struct ttc_plan_s {
     bool have_device = false;
     int sm_count = 148;
     int max_smem = 227 * 1024;
+    uint32_t* sched_ctr = nullptr;     // device counter of the atomic work distribution (TTC_SCHED=atomic)
     int tune_errors = 0;               // candidates that could not be prepared or launched while tuning
     float plan_ms = 0.f, tune_ms = 0.f;  // wall time of building the plan / of timing candidates inside it
     int fallback[2][25];               // [which][5 * log2(align of A) + log2(align of B)] -> candidate, -2 = not looked up
@@ -227,7 +228,7 @@ ttc_status tune(ttc_plan_s* p, int top_k, int reps, int budget_ms) {
             // the scalar fallback is always timed so that it is known to work
             if ((i >= n || over_budget) && i != p->scalar[which]) continue;
             if (!ensure_prepared(p, which, i)) { ++p->tune_errors; continue; }
-            if (launch_candidate(cs[i], p->dtype, p->dtype_a, alpha, beta, next_a(), next_b(), st) != 0) {
+            if (launch_candidate(cs[i], p->dtype, p->dtype_a, alpha, beta, next_a(), next_b(), st, p->sched_ctr) != 0) {
                 cudaGetLastError();   // a failed launch of OUR scratch run: cleared, and counted in ttc_info.tune_errors
                 ++p->tune_errors;
                 continue;
@@ -236,7 +237,7 @@ ttc_status tune(ttc_plan_s* p, int top_k, int reps, int budget_ms) {
             bool ok = true;
             for (int g = 0; g < 3 && ok; ++g) {   // minimum over groups (min of 3 runs)
                 cudaEventRecord(e0, st);
-                for (int r = 0; r < reps; ++r) ok &= launch_candidate(cs[i], p->dtype, p->dtype_a, alpha, beta, next_a(), next_b(), st) == 0;
+                for (int r = 0; r < reps; ++r) ok &= launch_candidate(cs[i], p->dtype, p->dtype_a, alpha, beta, next_a(), next_b(), st, p->sched_ctr) == 0;
                 cudaEventRecord(e1, st);
                 if (cudaEventSynchronize(e1) != cudaSuccess) { ok = false; break; }
                 float ms = 0.f;
@@ -264,7 +265,7 @@ ttc_status tune(ttc_plan_s* p, int top_k, int reps, int budget_ms) {
                 for (int r = 0; r < rounds && ok; ++r)
                     for (size_t f = 0; f < fin.size() && ok; ++f) {
                         cudaEventRecord(e0, st);
-                        for (int k = 0; k < per; ++k) ok &= launch_candidate(cs[fin[f]], p->dtype, p->dtype_a, alpha, beta, next_a(), next_b(), st) == 0;
+                        for (int k = 0; k < per; ++k) ok &= launch_candidate(cs[fin[f]], p->dtype, p->dtype_a, alpha, beta, next_a(), next_b(), st, p->sched_ctr) == 0;
                         cudaEventRecord(e1, st);
                         if (cudaEventSynchronize(e1) != cudaSuccess) { ok = false; break; }
                         float ms = 0.f;
@@ -347,6 +348,10 @@ static void finish_plan(ttc_plan_s* p) {
         cudaGetLastError();
     }
 
+    if (p->have_device && !p->sched_ctr) {
+        if (cudaMalloc((void**)&p->sched_ctr, 256) == cudaSuccess) cudaMemset(p->sched_ctr, 0, 256);
+        else { cudaGetLastError(); p->sched_ctr = nullptr; }
+    }
     for (int which = 0; which < 2; ++which) {
         generate_candidates(p->canon, dtype, p->dtype_a, which == 1, p->sm_count, p->max_smem, &p->cands[which]);
         std::vector<Candidate>& cs = p->cands[which];
@@ -425,7 +430,7 @@ ttc_status ttc_execute(ttc_plan_t p, const void* alpha, const void* A, const voi
         c = &p->cands[which][idx];
     }
     if (!ensure_prepared(p, which, idx)) return TTC_ERR_CUDA;
-    const int rc = launch_candidate(*c, p->dtype, p->dtype_a, to_scalar(p->dtype, alpha), to_scalar(p->dtype, beta), A, B, cuda_stream);
+    const int rc = launch_candidate(*c, p->dtype, p->dtype_a, to_scalar(p->dtype, alpha), to_scalar(p->dtype, beta), A, B, cuda_stream, p->sched_ctr);
     g_launches += 1;
     return rc == 0 ? TTC_OK : TTC_ERR_CUDA;
 }
@@ -539,6 +544,7 @@ ttc_status ttc_execute_host(ttc_plan_t p, const void* alpha, const void* A_host,
 
 ttc_status ttc_destroy(ttc_plan_t p) {
     if (!p) return TTC_OK;
+    if (p->sched_ctr) cudaFree(p->sched_ctr);
     if (p->pipe_sub) ttc_destroy(p->pipe_sub);
     if (p->pipe_in) cudaStreamDestroy(p->pipe_in);
     if (p->pipe_out) cudaStreamDestroy(p->pipe_out);

@@ -620,6 +620,8 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, boo
     if (const char* e = std::getenv("TTC_SCHED")) {
         if (!std::strcmp(e, "static")) scheds = {0};
         else if (!std::strcmp(e, "both")) scheds = {1, 0};
+        else if (!std::strcmp(e, "atomic")) scheds = {2};
+        else if (!std::strcmp(e, "all")) scheds = {1, 2, 0};
     }
 
     const int ring_max = std::getenv("TTC_RING") ? std::atoi(std::getenv("TTC_RING")) : 4;

@@ -91,7 +91,8 @@ struct DirectDim {
 struct DirectParams {
     int nd;
     int vec;            // elements per item
-    int dyn;            // 1: work items handed out by cluster launch control, 0: static grid-stride
+    int dyn;            // work distribution: 0 static grid-stride, 1 cluster launch control, 2 atomic counter
+    uint32_t* ctr;      // dyn == 2: device counter of the plan (set at launch)
     uint32_t n_chunks;  // work items: chunks of kDirectThreads * kDirectUnroll vectors
     uint64_t n_items;
     DirectDim dims[kMaxRank];
@@ -135,7 +136,8 @@ struct TileParams {
     int peel, peel_len, peel_gslot;   // ring kernel, peeled store phase: B rows cut into aligned 16-byte windows
     int lead_gslot, lead_vmul;   // ring kernel: grid slot of the row's index and its validity multiplier
     int threads;
-    int dyn;            // 1: macro-tiles handed out by cluster launch control, 0: static grid-stride
+    int dyn;            // work distribution: 0 static grid-stride, 1 cluster launch control, 2 atomic counter
+    uint32_t* ctr;      // dyn == 2: device counter of the plan (set at launch)
     uint32_t n_tiles;
     uint32_t itemsA, itemsB;      // table entries per tile: Alo.n*Ahi.n, Blo.n*Bhi.n
     uint32_t tile_elems;          // shared-memory tile size in elements (with padding)
@@ -197,7 +199,7 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, boo
 
 // Launch one candidate.  Returns the CUDA error code (0 = success) as int.
 int launch_candidate(const Candidate& cand, ttc_dtype dtype, ttc_dtype dtype_a, const Scalar& alpha,
-                     const Scalar& beta, const void* A, void* B, void* stream);
+                     const Scalar& beta, const void* A, void* B, void* stream, uint32_t* sched_ctr);
 // Configure dynamic shared memory / occupancy-derived grid for a candidate (needs a device).
 int prepare_candidate(Candidate* cand, ttc_dtype dtype, ttc_dtype dtype_a, int sm_count);
 

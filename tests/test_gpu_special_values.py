@@ -94,6 +94,8 @@ def run_case(da, db, sizes, perm, lda, ldb, alpha, beta, a_vals, b_vals, need=()
     try:
         cands = pick_candidates(plan, which)
         for k in need:
+            if db == wl.C128:             # 16-byte elements: every access is one element (vec = 1); ring rows are still bulk copies
+                k = {"ring_bulk_vec": "ring_cpasync", "direct_vec": "direct_scalar"}.get(k, k)
             assert k in cands, "no %s candidate for %s %s" % (k, sizes, perm)
         for key, idx in list(cands.items()) + [("winner", -1)]:
             ttc.ttc_plan_select(plan, which, idx)

@@ -476,6 +476,13 @@ def test_paper_reference_loop_agrees(dtype, beta):
     oracle.ref_omp_transpose(dtype, w.sizes, w.perm, w.lda, w.ldb, w.alpha, A, beta, B2)
     assert np.array_equal(B1.view(np.uint8), B2.view(np.uint8))
     assert oracle.ref_omp_threads() >= 1
+    # the timed baseline: same source built with the BASELINE.md flags on this machine, arrays first-touched in parallel
+    A3, B3 = oracle.first_touch_copy(A), oracle.first_touch_copy(B0)
+    assert np.array_equal(A3.view(np.uint8), A.view(np.uint8))
+    oracle.ref_omp_native_transpose(dtype, w.sizes, w.perm, w.lda, w.ldb, w.alpha, A3, beta, B3)
+    assert np.array_equal(B1.view(np.uint8), B3.view(np.uint8))
+    assert "-O3" in oracle.NATIVE_FLAGS and "-march=native" in oracle.NATIVE_FLAGS and "-fopenmp" in oracle.NATIVE_FLAGS
+    assert not oracle.first_touch_zeros(A).view(np.uint8).any()
 
 
 def test_generators_hold_no_nan_and_are_exact():
