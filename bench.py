@@ -236,6 +236,7 @@ def cold_block(torch, ttc, wl, peak, works, plans, a_dev, b_dev) -> dict:
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             ts = []
             for _ in range(21):
+                torch.cuda._sleep(40000)        # ~20 us of device spin: the launch below is queued before e0 is reached
                 e0.record()
                 ttc.ttc_execute(plan, w.alpha, xa, w.beta, xb)
                 e1.record()
@@ -429,8 +430,8 @@ def run_ours(args) -> None:
     # than stream launches on this machine and let programmatic dependent launch overlap a kernel's
     # prologue with its predecessor's tail.  --no-graph: plain stream launches.
     use_graph = not args.no_graph
-    n_ev = 0 if args.no_launch_events else min(8, max(1, steps // 4))
-    ev_steps = list(range(0, steps, 4))[:n_ev]
+    n_ev = 0 if args.no_launch_events else min(8, max(1, steps // 10))
+    ev_steps = list(range(0, steps, 10))[:n_ev]
     ev = {s: [torch.cuda.Event(enable_timing=True, external=use_graph) for _ in range(len(works) + 1)]
           for s in ev_steps} if n_ev else None
     side = torch.cuda.Stream()
@@ -449,7 +450,7 @@ def run_ours(args) -> None:
     if use_graph:
         graph_plain = capture()
         # per-launch events for the roofline of the dominant kernel, live in the timed region: every
-        # 4th of the first steps replays a twin graph with an (external) event node between the launches
+        # 10th of the first steps replays a twin graph with an (external) event node between the launches
         graph_ev = {s: capture(ev[s]) for s in ev_steps} if ev else {}
         for _ in range(warmup):
             graph_plain.replay()

@@ -97,6 +97,9 @@ typedef struct {
     float    tune_ms;                     /* the part of it spent timing candidates on the device  */
 } ttc_info;
 
+#define TTC_CAND_STAGGERED 1   /* ring kernel: bank-conflict-free "staggered" gather from the tile      */
+#define TTC_CAND_TENSORMAP 2   /* tiles moved by TMA tensor-map loads / stores (cp.async.bulk.tensor)  */
+
 /* One candidate implementation (loop order x blocking; here also kernel class). */
 typedef struct {
     int      kernel;          /* ttc_kernel_class                                              */
@@ -106,7 +109,9 @@ typedef struct {
     int      threads;         /* CTA size                                                      */
     int      smem_bytes;      /* dynamic shared memory per CTA                                 */
     int      loop_order;      /* 0: macro-tiles walk A linearly, 1: walk B linearly            */
-    int      sched;           /* 0: static persistent grid-stride, 1: dynamic (cluster launch control) */
+    int      sched;           /* 0: static persistent grid-stride, 1: dynamic (cluster launch control),
+                                 2: dynamic (atomic counter of the plan; TTC_SCHED=atomic)   */
+    int      flags;           /* TTC_CAND_* bits                                               */
     int      grid;            /* CTAs launched, 0 if not yet fixed (dynamic: one per work item, most of
                                  which are cancelled and taken over by the resident CTAs)      */
     float    est_cost;        /* heuristic cost used for ranking (lower is better)             */

@@ -717,6 +717,7 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
     const int NC = NT - 32;
     const int sstep = P.sstepB * ESA;
     const bool same = P.same != 0;
+    const int rot = P.xp ? ((tid >> 3) & (VB - 1)) : 0;   // staggered gather: this lane's row rotation
     const FastDiv dlo = P.divBlo;
     for (uint32_t it = 0;; ++it) {
         const int s = (int)(it % (uint32_t)S);
@@ -849,9 +850,23 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
                         for (int j = 0; j < VB; ++j) a.e[j] = cvt_to(T(), *reinterpret_cast<const TA*>(tile + so[k] + j * sstep));
                     } else if (VB == 1 || same) {   // same: the vector leads A and B, chunks move unchanged
                         a.raw = *reinterpret_cast<const RawB*>(tile + so[k]);
+                    } else if constexpr (VB == 2) {
+                        // Staggered gather (P.xp): the warp reads 2 columns x 8 row pairs per instruction; lanes
+                        // 8..15 and 24..31 take their two rows in the opposite order (rot), which spreads the 16
+                        // rows over all banks when the row pitch is an odd multiple of 16 bytes.  rot = 0: plain.
+                        const T v0 = *reinterpret_cast<const T*>(tile + so[k] + rot * sstep);
+                        const T v1 = *reinterpret_cast<const T*>(tile + so[k] + (1 - rot) * sstep);
+                        a.e[0] = rot ? v1 : v0;
+                        a.e[1] = rot ? v0 : v1;
                     } else {
+                        T v[VB], u[VB];
 #pragma unroll
-                        for (int j = 0; j < VB; ++j) a.e[j] = *reinterpret_cast<const T*>(tile + so[k] + j * sstep);
+                        for (int j = 0; j < VB; ++j) v[j] = *reinterpret_cast<const T*>(tile + so[k] + ((j + rot) & (VB - 1)) * sstep);
+                        // v[j] holds row (j + rot) mod 4: rotate back in two conditional stages
+#pragma unroll
+                        for (int j = 0; j < VB; ++j) u[j] = (rot & 1) ? v[(j + VB - 1) & (VB - 1)] : v[j];
+#pragma unroll
+                        for (int j = 0; j < VB; ++j) a.e[j] = (rot & 2) ? u[(j + VB - 2) & (VB - 1)] : u[j];
                     }
 #pragma unroll
                     for (int j = 0; j < VB; ++j) {

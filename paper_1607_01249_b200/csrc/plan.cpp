@@ -63,7 +63,7 @@ int64_t phase_smem_offset(const std::vector<PhaseDim>& ph, const int32_t* ss, in
 // Relative smem cost (>= 1) of both phases for the given tile strides.
 double smem_conflict_cost(const std::vector<PhaseDim>& phA, const std::vector<PhaseDim>& phB,
                           const int32_t* ss, int es, int vecA, int vecB, bool same, int sstepB,
-                          int64_t itemsA, int64_t itemsB, bool splitA) {
+                          int64_t itemsA, int64_t itemsB, bool splitA, bool skipA = false, bool xp = false) {
     double got = 0, ideal = 0;
     const int warps = 8;
     int64_t addr[32];
@@ -72,7 +72,7 @@ double smem_conflict_cost(const std::vector<PhaseDim>& phA, const std::vector<Ph
         const int64_t startA = (itemsA / 32) * w / warps * 32;
         int n = 0;
         for (int l = 0; l < 32 && startA + l < itemsA; ++l) addr[n++] = phase_smem_offset(phA, ss, startA + l) * es;
-        if (n) {
+        if (n && !skipA) {
             if (!splitA) {
                 got += smem_wavefronts(addr, n, es * vecA);
             } else {   // the vecA elements of a global vector are stored one by one
@@ -94,7 +94,9 @@ double smem_conflict_cost(const std::vector<PhaseDim>& phA, const std::vector<Ph
             } else {
                 for (int j = 0; j < vecB; ++j) {
                     int64_t a2[32];
-                    for (int l = 0; l < n; ++l) a2[l] = addr[l] + (int64_t)j * sstepB * es;
+                    // xp: lane l reads its vecB rows in the rotated order (j + (l >> 3)) mod vecB
+                    for (int l = 0; l < n; ++l)
+                        a2[l] = addr[l] + (int64_t)(xp ? ((j + (l >> 3)) & (vecB - 1)) : j) * sstepB * es;
                     got += smem_wavefronts(a2, n, es);
                     ideal += std::max(1.0, n * es / 128.0);
                 }
@@ -150,7 +152,7 @@ int legal_vec(const Canon& c, int lead, bool sideA, int32_t t_lead, int mv) {
 
 // Build one tile-kernel candidate.  Returns false if the combination is not legal.
 bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, const TileSpec& spec,
-                          int loop_order, int want_va, int want_vb, int max_smem, int sched, int ring, Candidate* out) {
+                          int loop_order, int want_va, int want_vb, int max_smem, int sched, int ring, int xp, Candidate* out) {
     // es: B's element and the tile's (the planner's world is B-typed); esA differs from it only for
     // the mixed-precision pairs.  There the tile kernel converts A in its load phase (the tile holds
     // B's type), while the ring kernel's bulk copies land A's bytes unconverted: its tile holds A's
@@ -216,6 +218,25 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
         for (int i : ta) phA.push_back(PhaseDim{i, spec.t[i] / (i == A0 ? want_va : 1), i == A0 ? want_va : 1});
     }
     const int step_b = peelB ? 1 : want_vb;   // peeled: the tables enumerate single elements of the leading index
+    // xp ("staggered gather", ring kernel): the store phase's fastest digit is a pair / quad of
+    // COLUMNS -- neighbouring elements of a tile index X with an odd tile stride (A's leading index, or
+    // the second one behind an odd fused leading extent) -- followed by the vectors of B's leading
+    // index.  A warp then reads, per instruction, vecB columns x 8 rows; with the rows taken in a
+    // lane-dependent rotation (kernel) and a row pitch that is an odd multiple of 16 bytes these hit
+    // 32 distinct banks, which a plain gather down ONE column of 16-byte-granular rows cannot (8-byte
+    // elements would need an odd element pitch).  Stores stay coalesced: 32 / vecB vectors per column.
+    int X = -1;
+    if (xp) {
+        if (!ring || mixed || same || peelB || want_vb != mvB || mvB < 2 || ta.size() < 2) return false;
+        if (spec.t[A0] % want_vb == 0 && c.d[A0].e % want_vb == 0 && A0 != B0) X = A0;
+        else if (fuseA && spec.t[ta[1]] % want_vb == 0 && (spec.t[A0] & 1) && ta[1] != B0) X = ta[1];
+        if (X < 0) return false;
+        phB.push_back(PhaseDim{X, want_vb, 1});
+        for (int i : tb) {
+            if (i == X) phB.push_back(PhaseDim{i, spec.t[i] / want_vb, want_vb});
+            else phB.push_back(PhaseDim{i, spec.t[i] / (i == B0 ? step_b : 1), i == B0 ? step_b : 1});
+        }
+    } else
     for (int i : tb) phB.push_back(PhaseDim{i, spec.t[i] / (i == B0 ? step_b : 1), i == B0 ? step_b : 1});
     int64_t itemsA = 1, itemsB = 1;
     for (auto& p : phA) itemsA *= p.n;
@@ -317,7 +338,8 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
         if (!ok) continue;
         const int64_t elems = (int64_t)ss[ta.back()] * spec.t[ta.back()];
         if (elems * esT * (ring ? ring : 1) > max_smem) continue;
-        const double conf = smem_conflict_cost(phA, phB, ss, esT, want_va, want_vb, same, ss[B0], itemsA, itemsB, split != 0);
+        const double conf = smem_conflict_cost(phA, phB, ss, esT, want_va, want_vb, same, ss[B0], itemsA, itemsB, split != 0,
+                                               ring != 0 && !P.row_async, xp != 0);
         // a split store costs want_va - 1 extra instructions per item: worth it only for a real gain
         const double cost = conf + 1e-3 * (double)elems * esT / 1024.0 + (split ? 0.08 : 0.0);
         if (cost < best_cost) {
@@ -332,6 +354,7 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
     std::memcpy(ss, best_ss, sizeof(ss));
     P.tile_elems = (uint32_t)best_elems;
     P.sstepB = ss[B0];
+    P.xp = xp ? 1 : 0;
     P.splitA = best_split;
     P.itemsA = (uint32_t)itemsA;
     P.itemsB = (uint32_t)itemsB;
@@ -426,6 +449,7 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
     I.smem_bytes = (int)tile_smem_layout(P, esT).total;
     I.loop_order = loop_order;
     I.sched = sched;
+    I.flags = xp ? TTC_CAND_STAGGERED : 0;
     I.grid = 0;
     I.n_tiles = n_tiles;
     for (int i = 0; i < kMaxRank; ++i) I.tile_ext[i] = i < c.rank ? spec.t[i] : 0;
@@ -624,6 +648,9 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, boo
         else if (!std::strcmp(e, "all")) scheds = {1, 2, 0};
     }
 
+    // TTC_VARIANTS: bit 0 = staggered-gather ring candidates (default on)
+    const int variants = std::getenv("TTC_VARIANTS") ? std::atoi(std::getenv("TTC_VARIANTS")) : 1;
+    const int xp_max = (variants & 1) ? 1 : 0;
     const int ring_max = std::getenv("TTC_RING") ? std::atoi(std::getenv("TTC_RING")) : 4;
 
     // K1 / fallback: direct kernels (always at least the scalar one, valid for any strides).
@@ -667,9 +694,11 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, boo
                         for (int sched : scheds)
                             for (int ring = 0; ring <= ring_max; ring += 2) {
                                 if (ring && bytes * ring > 64 * 1024) continue;   // 2 buffers <= 32 KB, 4 <= 16 KB
-                                Candidate cand;
-                                if (build_tile_candidate(c, dtype, dtype_a, beta_nz, spec, lo, va, vb, max_smem, sched, ring, &cand))
-                                    out->push_back(cand);
+                                for (int xp = 0; xp <= (ring ? xp_max : 0); ++xp) {
+                                    Candidate cand;
+                                    if (build_tile_candidate(c, dtype, dtype_a, beta_nz, spec, lo, va, vb, max_smem, sched, ring, xp, &cand))
+                                        out->push_back(cand);
+                                }
                             }
                     }
                 }

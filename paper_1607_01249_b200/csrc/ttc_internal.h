@@ -129,6 +129,7 @@ struct TileParams {
     int same;           // 1: the vectorised index leads A and B (chunks move unchanged)
     int sstepB;         // smem stride between the vecB elements one store gathers (!same)
     int splitA;         // 1: a loaded vector is written to the tile as vecA element stores
+    int xp;             // ring kernel: 1 = staggered gather (rows of a store vector read in a lane-dependent rotation)
     int ring;           // > 0: ring kernel with this many tile buffers (producer warp + consumer warps)
     uint32_t row_bytes; // ring kernel: bytes of one tile row (one cp.async.bulk each); rows = tab[1].n
     int row_pairs;      // ring kernel, cp.async rows of 4-byte elements: 1 = every row is 8-byte aligned (copy pairs)

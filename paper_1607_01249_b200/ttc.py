@@ -45,7 +45,7 @@ class ttc_candidate_info(ctypes.Structure):
     _fields_ = [("kernel", ctypes.c_int), ("vec_a", ctypes.c_int), ("vec_b", ctypes.c_int),
                 ("tile_u", ctypes.c_int), ("tile_w", ctypes.c_int), ("n_u", ctypes.c_int),
                 ("n_w", ctypes.c_int), ("threads", ctypes.c_int), ("smem_bytes", ctypes.c_int),
-                ("loop_order", ctypes.c_int), ("sched", ctypes.c_int), ("grid", ctypes.c_int), ("est_cost", ctypes.c_float),
+                ("loop_order", ctypes.c_int), ("sched", ctypes.c_int), ("flags", ctypes.c_int), ("grid", ctypes.c_int), ("est_cost", ctypes.c_float),
                 ("tuned_us", ctypes.c_float), ("n_tiles", ctypes.c_int64),
                 ("tile_ext", ctypes.c_int * TTC_MAX_RANK)]
 
@@ -248,6 +248,6 @@ def ttc_release_host_staging() -> None:
 
 def describe_candidate(c: ttc_candidate_info, rank: int) -> str:
     ext = "x".join(str(c.tile_ext[i]) for i in range(rank))
-    return "%s tile=%s vec=%d/%d run=%d/%d loop=%s sched=%s smem=%d grid=%d cost=%.2f us=%.1f" % (
-        KERNEL_NAMES.get(c.kernel, "?"), ext, c.vec_a, c.vec_b, c.tile_u, c.tile_w,
+    return "%s%s tile=%s vec=%d/%d run=%d/%d loop=%s sched=%s smem=%d grid=%d cost=%.2f us=%.1f" % (
+        KERNEL_NAMES.get(c.kernel, "?"), "+stag" if c.flags & 1 else "", ext, c.vec_a, c.vec_b, c.tile_u, c.tile_w,
         "AB"[c.loop_order], ("static", "dynamic", "atomic")[c.sched], c.smem_bytes, c.grid, c.est_cost, c.tuned_us)

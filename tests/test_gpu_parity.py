@@ -299,6 +299,12 @@ def test_ring_kernel_is_covered():
                     assert ring, "no ring candidate for %s dtype %d" % (w.name, dtype)
                     for i in ring[:12] + ring[12::5]:
                         check_bit_exact(w, plan=plan, candidate=i)
+                    # the staggered (bank-conflict-free) gather of the store phase: every 3rd such candidate
+                    stag = [i for i in ring if ttc.ttc_plan_candidate(plan, which, i).flags & 1]
+                    if dtype != wl.C128 and w.name == "ring":
+                        assert stag, "no staggered ring candidate for %s dtype %d" % (w.name, dtype)
+                    for i in stag[::3]:
+                        check_bit_exact(w, plan=plan, candidate=i)
                     if w.name == "ringodd" and dtype != wl.C128:
                         # cp.async rows (vec_a = 1) with the peeled, vector store phase (vec_b > 1)
                         peeled = [i for i in ring if ttc.ttc_plan_candidate(plan, which, i).vec_a == 1

@@ -66,6 +66,8 @@ def pick_candidates(plan, which):
         c = ttc.ttc_plan_candidate(plan, which, i)
         if c.kernel == 1:
             key = "direct_vec" if c.vec_a > 1 else "direct_scalar"
+        elif c.kernel == 5 and c.flags & 1:
+            key = "ring_staggered"
         elif c.kernel == 5:
             if c.vec_a > 1:
                 key = "ring_bulk_vec" if c.vec_b > 1 else "ring_bulk_scalar"
@@ -138,6 +140,8 @@ def test_special_values_same_type(dtype, shape):
         seen |= run_case(dtype, dtype, sizes, perm, lda, ldb, alpha, beta, a_vals, b_vals, need)
     if shape[0][0] == 131 and dtype != wl.C128:
         assert "ring_cpasync" in seen and "ring_cpasync_peeled" in seen, seen
+    if shape[0][0] == 64 and dtype != wl.C128:
+        assert "ring_staggered" in seen, seen
 
 
 MP2_INPUTS = [1.0 + 2.0 ** -24, 1.0 + 2.0 ** -24 + 2.0 ** -50, 1.0 + 3 * 2.0 ** -24, 1.0 - 2.0 ** -25,
