@@ -98,6 +98,7 @@ typedef struct {
 } ttc_info;
 
 #define TTC_CAND_STAGGERED 1   /* ring kernel: bank-conflict-free "staggered" gather from the tile      */
+#define TTC_CAND_SHIFTED_ROWS 4 /* ring kernel, rows not 16-byte aligned: aligned bodies by bulk copy, skewed tile */
 #define TTC_CAND_TENSORMAP 2   /* tiles moved by TMA tensor-map loads / stores (cp.async.bulk.tensor)  */
 
 /* One candidate implementation (loop order x blocking; here also kernel class). */

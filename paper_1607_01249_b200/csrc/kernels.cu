@@ -67,14 +67,25 @@ __device__ __forceinline__ float   cvt_to(float,   double a)  { return __double2
 __device__ __forceinline__ double2 cvt_to(double2, float2 a)  { return make_double2((double)a.x, (double)a.y); }
 __device__ __forceinline__ float2  cvt_to(float2,  double2 a) { return make_float2(__double2float_rn(a.x), __double2float_rn(a.y)); }
 
-__device__ __forceinline__ float scale(const Scalar& s, float a) { return __fmul_rn((float)s.re, a); }
-__device__ __forceinline__ double scale(const Scalar& s, double a) { return __dmul_rn(s.re, a); }
-__device__ __forceinline__ float2 scale(const Scalar& s, float2 a) {
-    const float sr = (float)s.re, si = (float)s.im;
-    return make_float2(__fsub_rn(__fmul_rn(sr, a.x), __fmul_rn(si, a.y)),
-                       __fadd_rn(__fmul_rn(sr, a.y), __fmul_rn(si, a.x)));
+// alpha / beta in the element type, converted ONCE per thread at kernel entry (the launcher passes
+// doubles; converting at every use costs an F2F per element in the inner loops).
+template <typename T> struct TScal;
+template <> struct TScal<float>   { float re; };
+template <> struct TScal<double>  { double re; };
+template <> struct TScal<float2>  { float re, im; };
+template <> struct TScal<double2> { double re, im; };
+__device__ __forceinline__ void typed(const Scalar& s, TScal<float>& o)   { o.re = (float)s.re; }
+__device__ __forceinline__ void typed(const Scalar& s, TScal<double>& o)  { o.re = s.re; }
+__device__ __forceinline__ void typed(const Scalar& s, TScal<float2>& o)  { o.re = (float)s.re; o.im = (float)s.im; }
+__device__ __forceinline__ void typed(const Scalar& s, TScal<double2>& o) { o.re = s.re; o.im = s.im; }
+
+__device__ __forceinline__ float scale(const TScal<float>& s, float a) { return __fmul_rn(s.re, a); }
+__device__ __forceinline__ double scale(const TScal<double>& s, double a) { return __dmul_rn(s.re, a); }
+__device__ __forceinline__ float2 scale(const TScal<float2>& s, float2 a) {
+    return make_float2(__fsub_rn(__fmul_rn(s.re, a.x), __fmul_rn(s.im, a.y)),
+                       __fadd_rn(__fmul_rn(s.re, a.y), __fmul_rn(s.im, a.x)));
 }
-__device__ __forceinline__ double2 scale(const Scalar& s, double2 a) {
+__device__ __forceinline__ double2 scale(const TScal<double2>& s, double2 a) {
     return make_double2(__dsub_rn(__dmul_rn(s.re, a.x), __dmul_rn(s.im, a.y)),
                         __dadd_rn(__dmul_rn(s.re, a.y), __dmul_rn(s.im, a.x)));
 }
@@ -218,8 +229,11 @@ __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;"
 template <int DT, int V, bool BETA, bool IDX64>
 __global__ void __launch_bounds__(kDirectThreads)
 direct_kernel(const __grid_constant__ DirectParams P, const void* __restrict__ Ain, void* __restrict__ Bout,
-              const Scalar alpha, const Scalar beta) {
+              const Scalar alpha_in, const Scalar beta_in) {
     using T = typename ElemT<DT>::T;
+    TScal<T> alpha, beta;
+    typed(alpha_in, alpha);
+    typed(beta_in, beta);
     using TA = typename ElemT<DT>::TA;
     using PackT = Pack<T, V>;
     using PackA = Pack<TA, V>;
@@ -315,8 +329,11 @@ constexpr int kTileMinCtas = 6;
 template <int DT, int VA, int VB, bool SAME, bool BETA>
 __global__ void __launch_bounds__(kTileThreads, BETA ? 4 : kTileMinCtas)
 tile_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, void* __restrict__ Bout,
-            const Scalar alpha, const Scalar beta) {
+            const Scalar alpha_in, const Scalar beta_in) {
     using T = typename ElemT<DT>::T;
+    TScal<T> alpha, beta;
+    typed(alpha_in, alpha);
+    typed(beta_in, beta);
     using TA = typename ElemT<DT>::TA;
     constexpr int ES = (int)sizeof(T);       // B and the tile
     constexpr int ESA = (int)sizeof(TA);     // A
@@ -526,10 +543,13 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 }
 
 template <int DT, int VB, bool BETA, bool PEEL>
-__global__ void __launch_bounds__(kRingThreads, PEEL ? 3 : BETA ? 4 : 5)
+__global__ void __launch_bounds__(kRingThreads, (PEEL || (BETA && VB == 1)) ? 3 : BETA ? 4 : 5)
 ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, void* __restrict__ Bout,
-            const Scalar alpha, const Scalar beta) {
-    using T = typename ElemT<DT>::T;         // B
+            const Scalar alpha_in, const Scalar beta_in) {
+    using T = typename ElemT<DT>::T;
+    TScal<T> alpha, beta;
+    typed(alpha_in, alpha);
+    typed(beta_in, beta);         // B
     using TA = typename ElemT<DT>::TA;       // A and the tile: bulk copies land A's bytes unconverted,
     constexpr int ES = (int)sizeof(T);       // the consumers convert (mixed precision, reading M1)
     constexpr int ESA = (int)sizeof(TA);
@@ -551,6 +571,7 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
     __shared__ __align__(8) uint64_t full_bar[kRingMaxStages], empty_bar[kRingMaxStages];
     __shared__ uint32_t tile_of[kRingMaxStages];
     __shared__ uint32_t edge_of[kRingMaxStages];
+    __shared__ uint32_t shift_of[kRingMaxStages];   // shifted rows: misalignment of the tile origin in A, << 30
     WorkSched sched;
     sched.init(P.dyn, &sched_bar, &sched_resp, P.ctr);
     pdl_launch_dependents();
@@ -570,6 +591,7 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
         for (int idx = tid; idx < tb.n; idx += NT) {
             uint32_t r = (uint32_t)idx;
             int32_t g = 0, s = 0;
+            uint32_t a = 0;
 #pragma unroll 1
             for (int k = 0; k < tb.nd; ++k) {
                 const uint32_t qq = fd_div(r, tb.d[k].div);
@@ -577,8 +599,11 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
                 r = qq;
                 g += (int32_t)c * (int32_t)tb.d[k].sG;
                 s += (int32_t)c * tb.d[k].sS;
+                a += c * (uint32_t)tb.d[k].aS;
             }
-            tabs[i][idx] = make_int2(g, s);
+            // shifted rows: bits 30-31 carry the entry's contribution to its tile row's misalignment
+            // in A (mod 4 elements); the sum of lo + hi + tile origin wraps mod 4 by itself
+            tabs[i][idx] = make_int2(g, s | (int32_t)(a << 30));
         }
     }
     __syncthreads();
@@ -647,7 +672,48 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
                 }
                 n_rows = __reduce_add_sync(0xFFFFFFFFu, (uint32_t)__popcll(row_ok));
             }
-            if (P.row_async) {
+            if (P.row_async == 2) {
+                // Shifted rows: lane handles rows lane, lane + 32, ...  The 16-byte aligned body of a row is one
+                // bulk copy that lands at the row's own misalignment sk (elements) behind its 16-byte aligned
+                // slot; the < 16-byte head and tail are element-sized cp.async.  Nothing outside the row is read.
+                constexpr int MVE = 16 / ESA;
+                const uint32_t org = (uint32_t)((reinterpret_cast<uintptr_t>(A) / ESA + (uint64_t)baseA) & (MVE - 1));
+                if (lane == 0) {
+                    tile_of[s] = tile_id;
+                    edge_of[s] = edge ? 1u : 0u;
+                    shift_of[s] = org << 30;
+                }
+                const int len = (int)(row_bytes / ESA);
+                int j = 0;
+                for (int row = lane; row < rows; row += 32, ++j) {
+                    if (!((row_ok >> j) & 1ull)) continue;
+                    const int2 e = tabs[1][row];
+                    const int sk = (int)((org + (uint32_t)e.x) & (MVE - 1));
+                    int h = (MVE - sk) & (MVE - 1);
+                    h = h < len ? h : len;
+                    const int body = (len - h) & ~(MVE - 1);
+                    const char* src = Ab + (int64_t)e.x * ESA;
+                    const uint32_t dst = (uint32_t)__cvta_generic_to_shared(tile + (e.y + sk) * ESA);
+                    if (body > 0) {
+                        asm volatile("mbarrier.expect_tx.relaxed.cta.shared::cta.b64 [%0], %1;" ::"r"(full_a), "r"(body * ESA) : "memory");
+                        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                                     ::"r"(dst + h * ESA), "l"(src + h * ESA), "r"(body * ESA), "r"(full_a) : "memory");
+                    }
+#pragma unroll
+                    for (int i = 0; i < MVE - 1; ++i) {
+                        if (i < h) {
+                            if constexpr (ESA == 4) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst + i * ESA), "l"(src + i * ESA) : "memory");
+                            else asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst + i * ESA), "l"(src + i * ESA) : "memory");
+                        }
+                        const int t = h + body + i;
+                        if (t < len) {
+                            if constexpr (ESA == 4) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst + t * ESA), "l"(src + t * ESA) : "memory");
+                            else asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst + t * ESA), "l"(src + t * ESA) : "memory");
+                        }
+                    }
+                }
+                asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(full_a) : "memory");
+            } else if (P.row_async) {
                 // Rows that are not 16-byte aligned (odd extents of 4/8-byte elements): the warp copies
                 // each row with element-sized cp.async (LDGSTS), 32 elements per instruction; each lane
                 // then lets the mbarrier track its copies (cp.async.mbarrier.arrive.noinc).
@@ -718,7 +784,19 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
     const int sstep = P.sstepB * ESA;
     const bool same = P.same != 0;
     const int rot = P.xp ? ((tid >> 3) & (VB - 1)) : 0;   // staggered gather: this lane's row rotation
+    // Shifted rows (P.row_async == 2): tile row r sits sk(r) = 0..MVE-1 elements behind its slot, sk = the row's
+    // misalignment in A.  Bits 30-31 of the table entries' tile offsets and of shift_of[] add up to it (mod 4);
+    // all of them are 0 for every other kind of tile, so the decoding below is unconditional.
+    constexpr uint32_t MVE = 16 / ESA, kOffMask = 0x3FFFFFFFu;
+    constexpr int U = (VB == 1 && BETA && ES <= 8) ? 8 : kTileUnroll;
+    const bool shifted = P.row_async == 2;
+    const int ldm = P.shift_ld;
     const FastDiv dlo = P.divBlo;
+    // division-free enumeration of the store phase (see the loop): needs |lo table| to divide the consumer threads
+    const bool lofix = !PEEL && (uint32_t)NC % dlo.d == 0;
+    const uint32_t my_lo = lofix ? (uint32_t)ctid % dlo.d : 0u, hi_first = lofix ? (uint32_t)ctid / dlo.d : 0u;
+    const uint32_t hi_step = lofix ? (uint32_t)NC / dlo.d : 0u;
+    const int2 el_fixed = lofix ? tabs[2][my_lo] : make_int2(0, 0);
     for (uint32_t it = 0;; ++it) {
         const int s = (int)(it % (uint32_t)S);
         mbar_wait((uint32_t)__cvta_generic_to_shared(&full_bar[s]), (it / (uint32_t)S) & 1u);
@@ -738,6 +816,7 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
         char* Bb = B + baseB * ES;
         const unsigned char* tile = smem + L.tile + (uint32_t)s * L.tile_stride;
         const bool edge = edge_of[s] != 0;
+        const uint32_t org = shifted ? shift_of[s] : 0u;
         uint8_t* v2 = smem + L.rval + (uint32_t)s * L.rval_stride;
         uint8_t* v3 = v2 + (((uint32_t)P.tab[2].n + 3u) & ~3u);
         if (edge) {   // mark which B-side table entries are inside the tensor (consumers only)
@@ -768,6 +847,14 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
             const int len = edge ? reinterpret_cast<const int32_t*>(smem + L.rvext)[s * kMaxRank + P.peel_gslot] : P.peel_len;
             const uint32_t nch = dlo.d;                                  // windows per row (divBlo is set to it)
             const int bmis = (int)((reinterpret_cast<uintptr_t>(B) / ES) & (uintptr_t)(VB - 1));
+            // element e of the B row whose table entry decodes to (base, sk): tile row (.. + e), whose skew advances by ldm
+            auto tile_elem = [&](int32_t sok, int e) -> T {
+                const int sk = sok & (int)(MVE - 1);
+                return cvt_to(T(), *reinterpret_cast<const TA*>(tile + (sok & ~(int)(MVE - 1)) + e * sstep +
+                                                                ((sk + e * ldm) & (int)(MVE - 1)) * ESA));
+            };
+            // pass 1: the windows that lie inside their row -- one vector load of B (beta), VB gathers, one vector
+            // store; every lane of a warp takes the same path
             for (uint32_t p0 = ctid; p0 < P.itemsB; p0 += NC * kTileUnroll) {
                 Pack<T, VB> bv[kTileUnroll];
                 int32_t so[kTileUnroll], go[kTileUnroll], s0[kTileUnroll];
@@ -782,67 +869,94 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
                         if (edge) ok[k] = v3[row] != 0;
                         const int m = (bmis + (int)((baseB + eh.x) & (VB - 1))) & (VB - 1);
                         s0[k] = (int)(p - row * nch) * VB - m;          // first element of the window, row-relative
-                        ok[k] = ok[k] && s0[k] + VB > 0 && s0[k] < len;
-                        so[k] = eh.y * ESA;
-                        go[k] = eh.x;
-                        if (BETA && ok[k]) {
-                            const char* src = Bb + ((int64_t)go[k] + s0[k]) * ES;
-                            if (s0[k] >= 0 && s0[k] + VB <= len) {
-                                bv[k].raw = ld_plain<RawB>(src);
-                            } else {
-#pragma unroll
-                                for (int j = 0; j < VB; ++j)
-                                    if (s0[k] + j >= 0 && s0[k] + j < len) bv[k].e[j] = *reinterpret_cast<const T*>(src + j * ES);
-                            }
-                        }
+                        ok[k] = ok[k] && s0[k] >= 0 && s0[k] + VB <= len;
+                        const uint32_t t = (uint32_t)eh.y + org;
+                        so[k] = (int32_t)((t & kOffMask) * ESA | ((t >> 30) & (MVE - 1)));   // low bits: the row's skew
+                        go[k] = eh.x + s0[k];
+                        if (BETA && ok[k]) bv[k].raw = ld_plain<RawB>(Bb + (int64_t)go[k] * ES);
                     }
                 }
 #pragma unroll
                 for (int k = 0; k < kTileUnroll; ++k) {
                     if (ok[k]) {
                         Pack<T, VB> o;
-                        const bool full = s0[k] >= 0 && s0[k] + VB <= len;
 #pragma unroll
                         for (int j = 0; j < VB; ++j) {
-                            if (full || (s0[k] + j >= 0 && s0[k] + j < len)) {
-                                T x = scale(alpha, cvt_to(T(), *reinterpret_cast<const TA*>(tile + so[k] + (s0[k] + j) * sstep)));
-                                if (BETA) x = add(x, scale(beta, bv[k].e[j]));
-                                o.e[j] = x;
-                            }
+                            T x = scale(alpha, tile_elem(so[k], s0[k] + j));
+                            if (BETA) x = add(x, scale(beta, bv[k].e[j]));
+                            o.e[j] = x;
                         }
-                        char* dst = Bb + ((int64_t)go[k] + s0[k]) * ES;
-                        if (full) {
-                            st_global<RawB>(dst, o.raw);
-                        } else {
+                        st_global<RawB>(Bb + (int64_t)go[k] * ES, o.raw);
+                    }
+                }
+            }
+            // pass 2: the two ends of every row (< VB elements each), element by element.  Item = (row, end).
+            const uint32_t n_rows_b = (uint32_t)P.tab[3].n;
+            for (uint32_t q = ctid; q < 2u * n_rows_b; q += NC) {
+                const uint32_t row = q >> 1;
+                if (edge && v3[row] == 0) continue;
+                const int2 eh = tabs[3][row];
+                const int m = (bmis + (int)((baseB + eh.x) & (VB - 1))) & (VB - 1);
+                const int wl = (len + m - 1) / VB;                       // last window that touches the row
+                int s0;
+                if ((q & 1u) == 0) {           // head: window 0, partial when the row starts inside it
+                    if (m == 0 && len >= VB) continue;
+                    s0 = -m;
+                } else {                       // tail: the last window, unless it is full or is the head's window
+                    s0 = wl * VB - m;
+                    if (wl == 0 || s0 + VB <= len) continue;
+                }
+                const uint32_t t = (uint32_t)eh.y + org;
+                const int32_t sok = (int32_t)((t & kOffMask) * ESA | ((t >> 30) & (MVE - 1)));
 #pragma unroll
-                            for (int j = 0; j < VB; ++j)
-                                if (s0[k] + j >= 0 && s0[k] + j < len) *reinterpret_cast<T*>(dst + j * ES) = o.e[j];
-                        }
+                for (int j = 0; j < VB; ++j) {
+                    const int e = s0 + j;
+                    if (e >= 0 && e < len) {
+                        T* dst = reinterpret_cast<T*>(Bb + ((int64_t)eh.x + e) * ES);
+                        T x = scale(alpha, tile_elem(sok, e));
+                        if (BETA) x = add(x, scale(beta, *dst));
+                        *dst = x;
                     }
                 }
             }
         } else
         // store phase: tile -> B, enumerated in ascending B-stride (as in tile_kernel)
-        for (uint32_t p0 = ctid; p0 < P.itemsB; p0 += NC * kTileUnroll) {
-            Pack<T, VB> bv[kTileUnroll];
-            int32_t so[kTileUnroll], go[kTileUnroll];
-            bool ok[kTileUnroll];
+        // U items per thread in flight; the element-wise beta path needs 8 (4-byte loads of B: 4 of them per
+        // thread cover too little of the DRAM latency -- profiles/: the first use of the loaded B stalls)
+        for (uint32_t p0 = ctid, hb = hi_first; p0 < P.itemsB; p0 += NC * U, hb += hi_step * U) {
+            Pack<T, VB> bv[U];
+            int32_t so[U], go[U];
+            bool ok[U];
 #pragma unroll
-            for (int k = 0; k < kTileUnroll; ++k) {
+            for (int k = 0; k < U; ++k) {
                 const uint32_t p = p0 + k * NC;
                 ok[k] = p < P.itemsB;
                 if (ok[k]) {
-                    const uint32_t hi = fd_div(p, dlo);
-                    const uint32_t lo = p - hi * dlo.d;
-                    const int2 el = tabs[2][lo], eh = tabs[3][hi];
+                    // item p = hi * |lo table| + lo.  When the lo table divides the consumer threads, lo is the
+                    // same for every item of a thread (its entry sits in registers) and hi advances by a constant
+                    uint32_t hi, lo;
+                    int2 el;
+                    if (lofix) {
+                        hi = hb + k * hi_step;
+                        lo = my_lo;
+                        el = el_fixed;
+                    } else {
+                        hi = fd_div(p, dlo);
+                        lo = p - hi * dlo.d;
+                        el = tabs[2][lo];
+                    }
+                    const int2 eh = tabs[3][hi];
                     if (edge) ok[k] = v2[lo] & v3[hi];
-                    so[k] = (el.y + eh.y) * ESA;
+                    const uint32_t t = (uint32_t)(el.y + eh.y) + org;
+                    so[k] = (int32_t)((t & kOffMask) * ESA);
+                    if (VB == 1) so[k] += (int32_t)(((t >> 30) & (MVE - 1)) * ESA);     // the row's skew
+                    else so[k] |= (int32_t)((t >> 30) & (MVE - 1));                      // kept in the low bits (VB > 1)
                     go[k] = el.x + eh.x;
                     if (BETA && ok[k]) bv[k].raw = ld_plain<RawB>(Bb + (int64_t)go[k] * ES);
                 }
             }
 #pragma unroll
-            for (int k = 0; k < kTileUnroll; ++k) {
+            for (int k = 0; k < U; ++k) {
                 if (ok[k]) {
                     Pack<T, VB> a, o;
                     if constexpr (MIXED) {   // the tile holds A's type: convert element by element
@@ -850,6 +964,11 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
                         for (int j = 0; j < VB; ++j) a.e[j] = cvt_to(T(), *reinterpret_cast<const TA*>(tile + so[k] + j * sstep));
                     } else if (VB == 1 || same) {   // same: the vector leads A and B, chunks move unchanged
                         a.raw = *reinterpret_cast<const RawB*>(tile + so[k]);
+                    } else if (shifted) {      // vector of VB tile rows, each behind its slot by its own skew
+                        const int sk = so[k] & (int)(MVE - 1), base = so[k] & ~(int)(MVE - 1);
+#pragma unroll
+                        for (int j = 0; j < VB; ++j)
+                            a.e[j] = *reinterpret_cast<const T*>(tile + base + j * sstep + ((sk + j * ldm) & (int)(MVE - 1)) * ESA);
                     } else if constexpr (VB == 2) {
                         // Staggered gather (P.xp): the warp reads 2 columns x 8 row pairs per instruction; lanes
                         // 8..15 and 24..31 take their two rows in the opposite order (rot), which spreads the 16

@@ -112,12 +112,14 @@ double run_eff(double bytes, double knee = 48.0) {
     return bytes / (bytes + knee) / (4096.0 / (4096.0 + knee));
 }
 
-bool split_tables(const std::vector<PhaseDim>& ph, int* split_out) {
+bool split_tables(const std::vector<PhaseDim>& ph, int* split_out, int threads = 0) {
     // lo = ph[0..k), hi = ph[k..): both <= kMaxTabEntries entries and <= kMaxTab dims;
-    // choose k that minimises lo.n + hi.n.
+    // choose k that minimises lo.n + hi.n.  `threads` > 0 (ring kernel, B side): a lo table whose size
+    // divides the consumer threads is preferred (the largest such) -- the kernel then enumerates the
+    // store phase without a division, each thread keeping its lo entry in registers.
     const int n = (int)ph.size();
-    int best = -1;
-    int64_t best_sum = 0;
+    int best = -1, best_fix = -1;
+    int64_t best_sum = 0, best_fix_lo = 0;
     for (int k = 1; k <= n; ++k) {
         int64_t lo = 1, hi = 1;
         for (int i = 0; i < k; ++i) lo *= ph[i].n;
@@ -125,8 +127,9 @@ bool split_tables(const std::vector<PhaseDim>& ph, int* split_out) {
         if (k > kMaxTab || n - k > kMaxTab) continue;
         if (lo > kMaxTabEntries || hi > kMaxTabEntries) continue;
         if (best < 0 || lo + hi < best_sum) { best = k; best_sum = lo + hi; }
+        if (threads > 0 && lo <= threads && threads % lo == 0 && lo > best_fix_lo) { best_fix = k; best_fix_lo = lo; }
     }
-    *split_out = best;
+    *split_out = best_fix >= 0 ? best_fix : best;
     return best >= 0;
 }
 
@@ -152,7 +155,7 @@ int legal_vec(const Canon& c, int lead, bool sideA, int32_t t_lead, int mv) {
 
 // Build one tile-kernel candidate.  Returns false if the combination is not legal.
 bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, const TileSpec& spec,
-                          int loop_order, int want_va, int want_vb, int max_smem, int sched, int ring, int xp, Candidate* out) {
+                          int loop_order, int want_va, int want_vb, int max_smem, int sched, int ring, int xp, int rowmode, Candidate* out) {
     // es: B's element and the tile's (the planner's world is B-typed); esA differs from it only for
     // the mixed-precision pairs.  There the tile kernel converts A in its load phase (the tile holds
     // B's type), while the ring kernel's bulk copies land A's bytes unconverted: its tile holds A's
@@ -244,7 +247,7 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
     // small tiles run in 128-thread CTAs: the same threads per SM, shorter barrier waits
     if (std::max(itemsA, itemsB) <= 4 * 256) P.threads = 128;
     int splitA, splitB;
-    if (!split_tables(phA, &splitA) || !split_tables(phB, &splitB)) return false;
+    if (!split_tables(phA, &splitA) || !split_tables(phB, &splitB, ring ? (itemsB <= 4 * 256 ? 128 : 256) : 0)) return false;
     // Ring kernel (producer warp + consumer warps, `ring` tile buffers): every tile row along the
     // (vectorised, possibly fused) leading A index is one cp.async.bulk, so rows and addresses must
     // be 16-byte multiples, the tile layout 16-byte granular (no split stores) and the rows the hi
@@ -258,16 +261,22 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
             // vector form is not legal (otherwise the bulk twin of this candidate is the better one)
             if (want_va != 1 || mv == 1 || legal_vec(c, A0, true, spec.t[A0] / mv * mv, mv) == mv || same ||
                 c.d[A0].sA != 1) return false;
-            P.row_async = 1;
+            // rowmode 2, "shifted rows": the 16-byte aligned body of every row is ONE bulk copy that lands in
+            // the tile at the row's own misalignment (0 .. mv-1 elements, a per-row skew the consumers add),
+            // only the < 16-byte head and tail are element copies; nothing outside the row is touched.
+            P.row_async = rowmode == 2 ? 2 : 1;
+            if (rowmode == 2 && xp) return false;
             // 4-byte elements: rows can be copied as 8-byte pairs when every row start and length is
             // even (all other A strides, the leading extent and tile extent) -- the tile rows then
             // must start at even offsets too (pitches rounded to 2 below)
-            if (es == 4 && c.d[A0].e % 2 == 0 && spec.t[A0] % 2 == 0) {
+            if (P.row_async == 1 && es == 4 && c.d[A0].e % 2 == 0 && spec.t[A0] % 2 == 0) {
                 bool even = true;
                 for (int i = 0; i < c.rank; ++i)
                     if (i != A0 && c.d[i].sA % 2 != 0) even = false;
                 P.row_pairs = even ? 1 : 0;
             }
+        } else if (rowmode == 2) {
+            return false;     // only rows that are not 16-byte aligned have a shifted twin
         }
         // A row = the leading A indices of the tile that form ONE contiguous run in A: an index
         // extends the row when the previous one is taken whole and continues in memory; the tile
@@ -316,8 +325,9 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
     const int n_opts = 5;
     int combos = 1;
     for (int i = 0; i < search_levels; ++i) combos *= n_opts;
+    const bool shifted = P.row_async == 2;
     for (int split = 0; split < ((want_va > 1 && !same && !ring) ? 2 : 1); ++split) {
-    const int unit = split ? 1 : std::max(std::max(want_va, same ? mvS : 1), P.row_pairs ? 2 : 1);
+    const int unit = split ? 1 : std::max(std::max(std::max(want_va, same ? mvS : 1), P.row_pairs ? 2 : 1), shifted ? mv : 1);
     for (int combo = 0; combo < combos; ++combo) {
         int cc = combo;
         int64_t stride = 1;
@@ -328,6 +338,7 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
                 int pad = 0;
                 if ((int)k <= search_levels) { pad = pad_opts[cc % n_opts] * unit; cc /= n_opts; }
                 stride = stride * spec.t[ta[k - 1]];
+                if (shifted && (int)k == dense_levels) stride += mv - 1;   // room for the row's skew
                 if ((int)k < dense_levels) pad = 0;                  // a fused pair / a bulk row stays dense
                 else stride = (stride + unit - 1) / unit * unit;
                 stride += pad;
@@ -336,7 +347,8 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
             ss[ta[k]] = (int32_t)stride;
         }
         if (!ok) continue;
-        const int64_t elems = (int64_t)ss[ta.back()] * spec.t[ta.back()];
+        int64_t elems = (int64_t)ss[ta.back()] * spec.t[ta.back()];
+        if (shifted && (int)ta.size() <= dense_levels) elems = (elems + 2 * mv - 1) / mv * mv;   // a one-row tile
         if (elems * esT * (ring ? ring : 1) > max_smem) continue;
         const double conf = smem_conflict_cost(phA, phB, ss, esT, want_va, want_vb, same, ss[B0], itemsA, itemsB, split != 0,
                                                ring != 0 && !P.row_async, xp != 0);
@@ -354,6 +366,12 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
     std::memcpy(ss, best_ss, sizeof(ss));
     P.tile_elems = (uint32_t)best_elems;
     P.sstepB = ss[B0];
+    P.shift_ld = 0;
+    if (shifted) {     // skew step per element of B's leading index: its A-stride mod the vector, unless a row runs along it
+        bool in_row = false;
+        for (int r = 0; r < row_dims; ++r) in_row |= phA[r].dim == B0;
+        if (!in_row) P.shift_ld = (int)(c.d[B0].sA % mv);
+    }
     P.xp = xp ? 1 : 0;
     P.splitA = best_split;
     P.itemsA = (uint32_t)itemsA;
@@ -398,6 +416,12 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
             d.gslot = gslot_of[p.dim];
             d.vmul = 1;
             d.sS = ss[p.dim] * p.step;
+            d.aS = 0;
+            if (shifted && !sideA) {       // does this index select the tile row?  (the row runs along phA[0..row_dims))
+                bool in_row = false;
+                for (int r = 0; r < row_dims; ++r) in_row |= phA[r].dim == p.dim;
+                if (!in_row) d.aS = (int32_t)((c.d[p.dim].sA * p.step) % mv);
+            }
             d.sG = (sideA ? c.d[p.dim].sA : c.d[p.dim].sB) * p.step;
             if (p.fused) {   // one run over (A0, A1): stride 1 in A and in the tile; valid up to e(A0) * vext(A1)
                 d.vmul = spec.t[A0];
@@ -449,7 +473,7 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
     I.smem_bytes = (int)tile_smem_layout(P, esT).total;
     I.loop_order = loop_order;
     I.sched = sched;
-    I.flags = xp ? TTC_CAND_STAGGERED : 0;
+    I.flags = (xp ? TTC_CAND_STAGGERED : 0) | (shifted ? TTC_CAND_SHIFTED_ROWS : 0);
     I.grid = 0;
     I.n_tiles = n_tiles;
     for (int i = 0; i < kMaxRank; ++i) I.tile_ext[i] = i < c.rank ? spec.t[i] : 0;
@@ -475,7 +499,9 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
     if (tile_bytes > 48 * 1024) cost *= 1.0 + (tile_bytes - 48 * 1024) / (256.0 * 1024);   // occupancy
     if (n_tiles < 148 * 2) cost *= 1.0 + (148.0 * 2 - n_tiles) / (148.0 * 2);
     if (ring) cost *= 0.95;   // read and write streams overlap inside the CTA
-    if (P.row_async) {
+    if (P.row_async == 2) {
+        cost *= 1.04;     // heads and tails; skewed reads
+    } else if (P.row_async) {
         // one producer warp copies the rows 32 elements per instruction plus ~6 instructions per
         // row: short rows make the producer the bottleneck (measured: 32-element rows 2.7x, 64-element
         // rows 1.6x the time of rows of 128 and more)
@@ -648,8 +674,8 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, boo
         else if (!std::strcmp(e, "all")) scheds = {1, 2, 0};
     }
 
-    // TTC_VARIANTS: bit 0 = staggered-gather ring candidates (default on)
-    const int variants = std::getenv("TTC_VARIANTS") ? std::atoi(std::getenv("TTC_VARIANTS")) : 1;
+    // TTC_VARIANTS: bit 0 = staggered-gather ring candidates, bit 1 = shifted-row ring candidates (default: both)
+    const int variants = std::getenv("TTC_VARIANTS") ? std::atoi(std::getenv("TTC_VARIANTS")) : 3;
     const int xp_max = (variants & 1) ? 1 : 0;
     const int ring_max = std::getenv("TTC_RING") ? std::atoi(std::getenv("TTC_RING")) : 4;
 
@@ -694,11 +720,13 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, boo
                         for (int sched : scheds)
                             for (int ring = 0; ring <= ring_max; ring += 2) {
                                 if (ring && bytes * ring > 64 * 1024) continue;   // 2 buffers <= 32 KB, 4 <= 16 KB
-                                for (int xp = 0; xp <= (ring ? xp_max : 0); ++xp) {
-                                    Candidate cand;
-                                    if (build_tile_candidate(c, dtype, dtype_a, beta_nz, spec, lo, va, vb, max_smem, sched, ring, xp, &cand))
-                                        out->push_back(cand);
-                                }
+                                for (int xp = 0; xp <= (ring ? xp_max : 0); ++xp)
+                                    for (int rowmode = 1; rowmode <= (ring && !xp && (variants & 2) ? 2 : 1); ++rowmode) {
+                                        Candidate cand;
+                                        if (build_tile_candidate(c, dtype, dtype_a, beta_nz, spec, lo, va, vb, max_smem, sched, ring, xp,
+                                                                 rowmode, &cand))
+                                            out->push_back(cand);
+                                    }
                             }
                     }
                 }

@@ -110,6 +110,8 @@ struct TabDim {
     int32_t gslot;      // position of this index in TileParams::g (for edge-tile validity)
     int32_t vmul;       // entry c is valid iff c * step < vext[gslot] * vmul (vmul > 1: fused leading pair)
     int32_t sS;         // shared-memory stride per entry step (elements)
+    int32_t aS;         // shifted rows (row_async == 2), B-side tables: stride in A per entry step, mod the vector
+                        // width, of an index that selects the tile ROW (0 for the indices a row runs along)
     int64_t sG;         // global stride per entry step (elements)
 };
 struct Table {
@@ -133,7 +135,10 @@ struct TileParams {
     int ring;           // > 0: ring kernel with this many tile buffers (producer warp + consumer warps)
     uint32_t row_bytes; // ring kernel: bytes of one tile row (one cp.async.bulk each); rows = tab[1].n
     int row_pairs;      // ring kernel, cp.async rows of 4-byte elements: 1 = every row is 8-byte aligned (copy pairs)
-    int row_async;      // ring kernel: 1 = rows are copied with element-sized cp.async (rows not 16-byte aligned)
+    int row_async;      // ring kernel, rows not 16-byte aligned: 1 = copied with element-sized cp.async; 2 = "shifted
+                        // rows": the 16-byte aligned body of a row is one bulk copy, landed at the row's own
+                        // misalignment (0..3 elements) in the tile, the < 16-byte head and tail are element cp.async
+    int shift_ld;       // row_async == 2: A-stride of B's leading index mod the vector width (skew step per B element)
     int peel, peel_len, peel_gslot;   // ring kernel, peeled store phase: B rows cut into aligned 16-byte windows
     int lead_gslot, lead_vmul;   // ring kernel: grid slot of the row's index and its validity multiplier
     int threads;

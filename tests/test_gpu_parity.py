@@ -305,6 +305,14 @@ def test_ring_kernel_is_covered():
                         assert stag, "no staggered ring candidate for %s dtype %d" % (w.name, dtype)
                     for i in stag[::3]:
                         check_bit_exact(w, plan=plan, candidate=i)
+                    if (w.name == "ringodd" and dtype != wl.C128) or (w.name == "ringeven" and dtype == wl.F32):
+                        # shifted rows: aligned row bodies by bulk copy at the row's skew, heads/tails by cp.async
+                        shifted = [i for i in ring if ttc.ttc_plan_candidate(plan, which, i).flags & 4]
+                        assert shifted, "no shifted-row ring candidate for %s dtype %d" % (w.name, dtype)
+                        for i in shifted[:10] + shifted[10::4]:
+                            check_bit_exact(w, plan=plan, candidate=i)
+                        for i in shifted[:3]:          # and with pointers that are only element-aligned
+                            check_bit_exact(w, plan=plan, candidate=i, misalign_a=1, misalign_b=1)
                     if w.name == "ringodd" and dtype != wl.C128:
                         # cp.async rows (vec_a = 1) with the peeled, vector store phase (vec_b > 1)
                         peeled = [i for i in ring if ttc.ttc_plan_candidate(plan, which, i).vec_a == 1

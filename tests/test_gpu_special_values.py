@@ -68,6 +68,8 @@ def pick_candidates(plan, which):
             key = "direct_vec" if c.vec_a > 1 else "direct_scalar"
         elif c.kernel == 5 and c.flags & 1:
             key = "ring_staggered"
+        elif c.kernel == 5 and c.flags & 4:
+            key = "ring_shifted_peeled" if c.vec_b > 1 else "ring_shifted"
         elif c.kernel == 5:
             if c.vec_a > 1:
                 key = "ring_bulk_vec" if c.vec_b > 1 else "ring_bulk_scalar"
@@ -140,6 +142,7 @@ def test_special_values_same_type(dtype, shape):
         seen |= run_case(dtype, dtype, sizes, perm, lda, ldb, alpha, beta, a_vals, b_vals, need)
     if shape[0][0] == 131 and dtype != wl.C128:
         assert "ring_cpasync" in seen and "ring_cpasync_peeled" in seen, seen
+        assert "ring_shifted" in seen and "ring_shifted_peeled" in seen, seen
     if shape[0][0] == 64 and dtype != wl.C128:
         assert "ring_staggered" in seen, seen
 
