@@ -311,6 +311,57 @@ def detail_all_configs(torch, ttc, wl, path: str, peak: float, profile: bool = F
         json.dump(rows, fh, indent=1)
 
 
+def batched_block(torch, ttc, wl, peak: float) -> dict:
+    """ttc_execute_batched: many small transpositions that share a plan in one launch.
+    (a) 256 BLAS A-panel packs of 8 x 32 x 1024 fp64 blocks (2 MB each) cut out of one padded
+    operand; (b) 24 copies of configs[0] (the 23.6 MB, launch-bound case).  Each against the same work issued
+    as one ttc_execute per block; L2 evicted (read sweep) before every timed run, median of 11."""
+    evict = Evictor(torch)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    out = {}
+    c1 = wl.config1()
+    cases = (("a_panel_packs_256x2MB", wl.F64, (8, 32, 1024), (0, 2, 1), (8, 40, 1024), 256),
+             ("configs0_x24", c1.dtype, c1.sizes, c1.perm, None, 24))
+    for name, dtype, sizes, perm, lda, batch in cases:
+        plan = ttc.ttc_plan(dtype, len(sizes), sizes, perm, lda, None)
+        info = ttc.ttc_plan_info(plan)
+        tdt = torch.float64 if dtype == wl.F64 else torch.float32
+        la, lb = info.span_a + 8, info.numel + 8
+        big_a = torch.rand(batch * la, dtype=tdt, device="cuda")
+        big_b = torch.zeros(batch * lb, dtype=tdt, device="cuda")
+        As = [big_a[i * la:i * la + info.span_a] for i in range(batch)]
+        Bs = [big_b[i * lb:i * lb + info.numel] for i in range(batch)]
+        nbytes = 2 * info.numel * wl.ELEM_SIZE[dtype] * batch
+
+        def looped():
+            for a, b in zip(As, Bs):
+                ttc.ttc_execute(plan, 1.0, a, 0.0, b)
+
+        def batched():
+            ttc.ttc_execute_batched(plan, 1.0, As, 0.0, Bs)
+        res = {}
+        for label, fn in (("batched", batched), ("one_launch_per_block", looped)):
+            fn()
+            ts = []
+            for _ in range(11):
+                evict("read")
+                torch.cuda._sleep(200000)       # the (slow, Python-issued) launches are queued before the timer starts
+                e0.record()
+                fn()
+                e1.record()
+                e1.synchronize()
+                ts.append(e0.elapsed_time(e1) * 1e3)
+            us = statistics.median(ts)
+            res[label] = {"us_median": us, "gbs": nbytes / us / 1e3, "frac_of_measured_copy": nbytes / us / 1e3 / peak}
+        res["blocks"] = batch
+        res["bytes"] = nbytes
+        res["launches_batched"] = (batch + 63) // 64
+        out[name] = res
+        ttc.ttc_destroy(plan)
+        del big_a, big_b, As, Bs
+    return out
+
+
 def detail_misaligned(torch, ttc, wl, evict, peak: float) -> list:
     """Element-aligned but not 16-byte aligned pointers: the alignment-aware fallback
     candidate of the same plan, timed on three permutations of configs[1]'s tensor."""
@@ -568,6 +619,10 @@ def run_ours(args) -> None:
     if rank == 0 and world == 1 and not args.no_cold:
         cold = cold_block(torch, ttc, wl, peak, works, plans, a_dev, b_dev)
 
+    batched = None
+    if rank == 0 and world == 1 and not args.no_cold:
+        batched = batched_block(torch, ttc, wl, peak)
+
     cpu = cpu_omp = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu_omp = time_ref_omp(works, A_host)
@@ -601,7 +656,7 @@ def run_ours(args) -> None:
                 "frac_of_measured_copy": value / world / peak, "frac_of_nominal_8TBs": value / world / NOMINAL_HBM_GBS,
                 "per_perm_gbs": {"min": min(gbs), "median": statistics.median(gbs), "max": max(gbs)} if gbs else None,
                 "per_perm": per_perm, "roofline": roofline, "cold": cold,
-                "per_config": cold["per_config"] if cold else None,
+                "per_config": cold["per_config"] if cold else None, "batched": batched,
                 "plan_ms": {"median": statistics.median(r["plan_ms"] for r in per_perm),
                             "max": max(r["plan_ms"] for r in per_perm), "total_wall_s": plan_wall_s,
                             "note": "ttc_plan incl. on-device tuning of the beta=0 and beta!=0 lists; untimed, once per transposition"},

@@ -31,7 +31,9 @@
  *
  * Environment (read when a plan is built):
  *   TTC_TUNE=0            do not time anything: the heuristic's first choice is used
- *   TTC_TUNE_TOPK=k       time only the k best-ranked candidates of each list (default 0 = all)
+ *   TTC_TUNE_TOPK=k       time only the k best-ranked candidates of each list (default 32; 0 = all, the
+ *                         paper's exhaustive mode)
+ *   TTC_COST=legacy       rank candidates with the hand-written round-1 cost formula instead of the fitted one
  *   TTC_TUNE_BUDGET_MS=t  after the first 16 candidates, stop timing a list after t ms (default 400)
  *   TTC_CACHE_FILE=path   solution store on disk (winners appended, reloaded by later processes)
  *   TTC_SCHED=static|both work distribution: persistent grid-stride instead of / beside the default,
@@ -127,8 +129,9 @@ typedef struct {
  * rank candidate kernels and, if a CUDA device is present and the
  * environment does not say TTC_TUNE=0, time them in rank order on the device, for beta == 0
  * and for beta != 0, and keep the fastest of each.  The search of one list ends
- * after TTC_TUNE_TOPK candidates (default 0 = all, the paper's exhaustive mode) or, once 16
- * have been timed, when TTC_TUNE_BUDGET_MS (default 400) milliseconds have passed.
+ * after TTC_TUNE_TOPK candidates (default 32, enough for 0.995 of the exhaustive search's result with
+ * the fitted ranking; 0 = all, the paper's exhaustive mode) or, once 16 have been timed, when
+ * TTC_TUNE_BUDGET_MS (default 400) milliseconds have passed.
  * Winners are remembered per process; if the environment names a file in TTC_CACHE_FILE they
  * are also appended to it and loaded by later processes (the paper's database of known
  * solutions), so that planning the same transposition again times nothing.
@@ -182,6 +185,19 @@ ttc_status ttc_execute(ttc_plan_t plan, const void* alpha, const void* A,
                        const void* beta, void* B, void* cuda_stream);
 
 /*
+ * ttc_execute_batched -- Eq. 1 for `batch` independent tensor pairs (A_list[i], B_list[i]) that share one
+ * plan (same sizes, permutation, leading dimensions, types), in ONE kernel launch per 64 pairs: the
+ * macro-tiles of all pairs form one work list for the resident CTAs.  This is how a GEMM's packing routine
+ * ("packing kernels ... used by level 3 BLAS") moves many small mc x kc blocks without
+ * paying a launch and a machine fill-and-drain per block.  A_list and B_list are HOST arrays of DEVICE
+ * pointers, read before the call returns; the pairs must not overlap one another.  alpha, beta, alignment
+ * rules (the least aligned pointer decides the candidate), errors and asynchrony are those of ttc_execute;
+ * batch == 0 is a no-op, batch < 0 is TTC_ERR_INVALID_ARG.
+ */
+ttc_status ttc_execute_batched(ttc_plan_t plan, const void* alpha, const void* const* A_list,
+                               const void* beta, void* const* B_list, int batch, void* cuda_stream);
+
+/*
  * ttc_execute_host -- the same operation for HOST buffers A (span_a elements) and B
  * (span_b elements): copies A (and B when beta != 0, or when B has padding that has to
  * survive) to the plan's private device staging buffers, runs ttc_execute, copies B back
@@ -210,6 +226,12 @@ ttc_status ttc_plan_info(ttc_plan_t plan, ttc_info* out);
 /* Candidate lists of a plan: which = 0 for the beta == 0 list, 1 for beta != 0. */
 int        ttc_plan_num_candidates(ttc_plan_t plan, int which);
 ttc_status ttc_plan_candidate(ttc_plan_t plan, int which, int index, ttc_candidate_info* out);
+/* The 16 raw inputs of the ranking heuristic for one candidate (contiguous bytes per tile in A and in B,
+ * remainder waste, bank-conflict factor, tile bytes, number of tiles, ring depth, row mode, peel, staggered,
+ * vector bytes on each side, beta != 0, kernel class, row bytes, store items): what
+ * `python -m paper_1607_01249_b200.fit_cost` regresses measured times on when the heuristic is re-fitted
+ * for another device (PAPER.md:141-143 leaves the cost function to the implementation). */
+ttc_status ttc_plan_candidate_features(ttc_plan_t plan, int which, int index, float* out16);
 /* Force a candidate (tests, search-quality experiments).  index = -1 restores the winner. */
 ttc_status ttc_plan_select(ttc_plan_t plan, int which, int index);
 /*

@@ -104,6 +104,16 @@ def transpose_mixed(dtype_a: int, dtype_b: int, sizes, perm, lda, ldb, alpha, A:
         raise ValueError("oracle rejected its arguments (code %d)" % rc)
 
 
+def transpose_batched(dtype: int, sizes, perm, lda, ldb, alpha, A_list, beta, B_list) -> None:
+    """Eq. 1 for a list of independent tensor pairs that share sizes, permutation and leading dimensions
+    (the packing of many GEMM blocks): BY DEFINITION the single-pair operation applied
+    to each pair in turn.  The oracle of ``ttc_execute_batched``."""
+    if len(A_list) != len(B_list):
+        raise ValueError("A_list and B_list differ in length")
+    for A, B in zip(A_list, B_list):
+        transpose(dtype, sizes, perm, lda, ldb, alpha, A, beta, B)
+
+
 def ref_omp_transpose(dtype: int, sizes, perm, lda, ldb, alpha, A: np.ndarray, beta, B: np.ndarray) -> None:
     """The paper's OpenMP reference loop nest, all host cores."""
     _call(_load().ttc_ref_omp_transpose, dtype, sizes, perm, lda, ldb, alpha, A, beta, B)

@@ -210,7 +210,8 @@ ttc_status tune(ttc_plan_s* p, int top_k, int reps, int budget_ms) {
     cudaMemsetAsync(b, 0, bytes_b * nrot, st);
     const Scalar alpha{1.0, 0.0};
     ttc_status rc = TTC_OK;
-    if (reps < 1) reps = 3;
+    const int n_groups = reps < 1 ? 2 : 3;     // reps < 1: the quick protocol of ttc_plan (2 groups of 2 launches)
+    if (reps < 1) reps = 2;
     for (int which = 0; which < 2; ++which) {
         const Scalar beta{which ? 1.0 : 0.0, 0.0};
         std::vector<Candidate>& cs = p->cands[which];
@@ -235,7 +236,9 @@ ttc_status tune(ttc_plan_s* p, int top_k, int reps, int budget_ms) {
             }
             float us = 1e30f;
             bool ok = true;
-            for (int g = 0; g < 3 && ok; ++g) {   // minimum over groups (min of 3 runs)
+            // minimum over groups of `reps` launches (min of 3 runs); this first pass only has to
+            // find the 6 candidates of the interleaved final below, which re-times them (2 groups suffice)
+            for (int g = 0; g < n_groups && ok; ++g) {
                 cudaEventRecord(e0, st);
                 for (int r = 0; r < reps; ++r) ok &= launch_candidate(cs[i], p->dtype, p->dtype_a, alpha, beta, next_a(), next_b(), st, p->sched_ctr) == 0;
                 cudaEventRecord(e1, st);
@@ -244,7 +247,7 @@ ttc_status tune(ttc_plan_s* p, int top_k, int reps, int budget_ms) {
                 cudaEventElapsedTime(&ms, e0, e1);
                 us = std::min(us, ms * 1000.f / reps);
             }
-            g_launches += 1 + 3 * reps;
+            g_launches += 1 + n_groups * reps;
             if (!ok) { cudaGetLastError(); ++p->tune_errors; continue; }
             cs[i].info.tuned_us = us;
             if (best < 0 || us < best_us) { best = i; best_us = us; }
@@ -298,6 +301,33 @@ ttc_status tune(ttc_plan_s* p, int top_k, int reps, int budget_ms) {
     if (rc == TTC_OK) p->tuned = true;
     p->tune_ms += (float)std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_tune0).count();
     return rc;
+}
+
+// The candidate to launch for pointers A and B (only their low 4 bits matter): the forced or tuned one, or --
+// for pointers that are element-aligned but less aligned than it needs -- the best candidate of the same
+// list whose accesses fit (a timed one if there is one, else the best-ranked): normally a tile or ring
+// candidate with narrower vectors on the misaligned side, the scalar direct kernel only as the last resort.
+// Looked up once per alignment class.  -1: the plan has no candidate, -2: nothing fits the alignment.
+int choose_candidate(ttc_plan_s* p, int which, uintptr_t A, uintptr_t B) {
+    int idx = p->forced[which] >= 0 ? p->forced[which] : p->winner[which];
+    if (idx < 0) return -1;
+    const Candidate* c = &p->cands[which][idx];
+    if ((A % c->align_a) == 0 && (B % c->align_b) == 0) return idx;
+    auto lg = [](uintptr_t x) { int l = 0; while (l < 4 && !((x >> l) & 1)) ++l; return l; };
+    const int la = lg(A), lb = lg(B);
+    int& slot = p->fallback[which][5 * la + lb];
+    if (slot == -2) {
+        slot = -1;
+        float best_us = 0.f;
+        const std::vector<Candidate>& cs = p->cands[which];
+        for (int i = 0; i < (int)cs.size(); ++i) {
+            if ((1 << la) % cs[i].align_a != 0 || (1 << lb) % cs[i].align_b != 0) continue;
+            const float us = cs[i].info.tuned_us;
+            if (slot < 0) { slot = i; best_us = us; continue; }       // best-ranked fitting candidate
+            if (us > 0.f && (best_us <= 0.f || us < best_us)) { slot = i; best_us = us; }
+        }
+    }
+    return slot < 0 ? -2 : slot;
 }
 
 }  // namespace
@@ -379,7 +409,7 @@ static void finish_plan(ttc_plan_s* p) {
                 p->tuned = true;
             }
         }
-        if (!hit && tune(p, env_int("TTC_TUNE_TOPK", 0), 3, env_int("TTC_TUNE_BUDGET_MS", 400)) == TTC_OK) {
+        if (!hit && tune(p, env_int("TTC_TUNE_TOPK", 32), 0, env_int("TTC_TUNE_BUDGET_MS", 400)) == TTC_OK) {
             std::lock_guard<std::mutex> lk(g_cache_mu);
             CacheEntry e;
             for (int w = 0; w < 2; ++w) {
@@ -403,36 +433,51 @@ ttc_status ttc_execute(ttc_plan_t p, const void* alpha, const void* A, const voi
     if (((uintptr_t)A % esA) != 0 || ((uintptr_t)B % es) != 0) return TTC_ERR_MISALIGNED;
     if (!p->have_device) return TTC_ERR_CUDA;
     const int which = is_zero(p->dtype, beta) ? 0 : 1;
-    int idx = p->forced[which] >= 0 ? p->forced[which] : p->winner[which];
-    if (idx < 0) return TTC_ERR_UNSUPPORTED;
+    const int idx = choose_candidate(p, which, (uintptr_t)A, (uintptr_t)B);
+    if (idx == -1) return TTC_ERR_UNSUPPORTED;
+    if (idx < 0) return TTC_ERR_MISALIGNED;
     const Candidate* c = &p->cands[which][idx];
-    if (((uintptr_t)A % c->align_a) != 0 || ((uintptr_t)B % c->align_b) != 0) {
-        // Pointers that are element-aligned but not as aligned as the chosen candidate needs: the
-        // best candidate of the same list whose accesses fit (a timed one if there is one, else the
-        // best-ranked): normally a tile or ring candidate with narrower vectors on the misaligned
-        // side, the scalar direct kernel only as the last resort.  Looked up once per alignment class.
-        auto lg = [](uintptr_t x) { int l = 0; while (l < 4 && !((x >> l) & 1)) ++l; return l; };
-        const int la = lg((uintptr_t)A), lb = lg((uintptr_t)B);
-        int& slot = p->fallback[which][5 * la + lb];
-        if (slot == -2) {
-            slot = -1;
-            float best_us = 0.f;
-            const std::vector<Candidate>& cs = p->cands[which];
-            for (int i = 0; i < (int)cs.size(); ++i) {
-                if ((1 << la) % cs[i].align_a != 0 || (1 << lb) % cs[i].align_b != 0) continue;
-                const float us = cs[i].info.tuned_us;
-                if (slot < 0) { slot = i; best_us = us; continue; }       // best-ranked fitting candidate
-                if (us > 0.f && (best_us <= 0.f || us < best_us)) { slot = i; best_us = us; }
-            }
-        }
-        idx = slot;
-        if (idx < 0) return TTC_ERR_MISALIGNED;
-        c = &p->cands[which][idx];
-    }
     if (!ensure_prepared(p, which, idx)) return TTC_ERR_CUDA;
     const int rc = launch_candidate(*c, p->dtype, p->dtype_a, to_scalar(p->dtype, alpha), to_scalar(p->dtype, beta), A, B, cuda_stream, p->sched_ctr);
     g_launches += 1;
     return rc == 0 ? TTC_OK : TTC_ERR_CUDA;
+}
+
+ttc_status ttc_execute_batched(ttc_plan_t p, const void* alpha, const void* const* A_list, const void* beta,
+                               void* const* B_list, int batch, void* cuda_stream) {
+    if (!p || !alpha || !beta || batch < 0) return TTC_ERR_INVALID_ARG;
+    if (p->canon.empty || batch == 0) return TTC_OK;
+    if (!A_list || !B_list) return TTC_ERR_INVALID_ARG;
+    if (!p->have_device) return TTC_ERR_CUDA;
+    const int es = elem_size(p->dtype), esA = elem_size(p->dtype_a);
+    uintptr_t oa = 0, ob = 0;      // the OR of all addresses is as aligned as the least aligned of them
+    for (int i = 0; i < batch; ++i) {
+        if (!A_list[i] || !B_list[i]) return TTC_ERR_INVALID_ARG;
+        oa |= (uintptr_t)A_list[i];
+        ob |= (uintptr_t)B_list[i];
+    }
+    if ((oa % esA) != 0 || (ob % es) != 0) return TTC_ERR_MISALIGNED;
+    const int which = is_zero(p->dtype, beta) ? 0 : 1;
+    const int idx = choose_candidate(p, which, oa, ob);
+    if (idx == -1) return TTC_ERR_UNSUPPORTED;
+    if (idx < 0) return TTC_ERR_MISALIGNED;
+    const Candidate& c = p->cands[which][idx];
+    if (!ensure_prepared(p, which, idx)) return TTC_ERR_CUDA;
+    const uint32_t per = c.info.kernel == TTC_KERNEL_COPY ? c.dp.n_chunks : c.tp.n_tiles;
+    // one launch per kMaxBatch problems (the pointers travel as kernel parameters)
+    for (int first = 0; first < batch; first += kMaxBatch) {
+        BatchPtrs bt{};
+        bt.n = std::min(kMaxBatch, batch - first);
+        bt.per = per;
+        bt.div = make_fastdiv(per);
+        if ((uint64_t)per * (uint64_t)bt.n >= (1ull << 31)) return TTC_ERR_UNSUPPORTED;
+        for (int i = 0; i < bt.n; ++i) { bt.a[i] = A_list[first + i]; bt.b[i] = B_list[first + i]; }
+        const int rc = launch_candidate(c, p->dtype, p->dtype_a, to_scalar(p->dtype, alpha), to_scalar(p->dtype, beta),
+                                        bt.a[0], bt.b[0], cuda_stream, p->sched_ctr, &bt);
+        g_launches += 1;
+        if (rc != 0) return TTC_ERR_CUDA;
+    }
+    return TTC_OK;
 }
 
 }  // extern "C"
@@ -608,6 +653,13 @@ ttc_status ttc_plan_candidate(ttc_plan_t p, int which, int index, ttc_candidate_
     return TTC_OK;
 }
 
+ttc_status ttc_plan_candidate_features(ttc_plan_t p, int which, int index, float* out16) {
+    if (!p || !out16 || which < 0 || which > 1) return TTC_ERR_INVALID_ARG;
+    if (index < 0 || index >= (int)p->cands[which].size()) return TTC_ERR_INVALID_ARG;
+    std::memcpy(out16, p->cands[which][index].feat, sizeof(float) * 16);
+    return TTC_OK;
+}
+
 ttc_status ttc_plan_select(ttc_plan_t p, int which, int index) {
     if (!p || which < 0 || which > 1) return TTC_ERR_INVALID_ARG;
     if (index < -1 || index >= (int)p->cands[which].size()) return TTC_ERR_INVALID_ARG;
@@ -618,7 +670,7 @@ ttc_status ttc_plan_select(ttc_plan_t p, int which, int index) {
 ttc_status ttc_plan_tune(ttc_plan_t p, int top_k, int reps) {
     if (!p) return TTC_ERR_INVALID_ARG;
     for (auto& w : p->fallback) for (int& x : w) x = -2;
-    return tune(p, top_k, reps, 0);
+    return tune(p, top_k, reps < 1 ? 3 : reps, 0);
 }
 
 int ttc_canonicalize(int N, const int64_t* sizes, const int* perm, const int64_t* lda,

@@ -222,6 +222,15 @@ struct WorkSched {
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
+// Batched launch: work item `w` of the whole launch -> (problem, item inside it); A and B of that problem.
+__device__ __forceinline__ uint32_t batch_item(const BatchPtrs& Bt, uint32_t w, const char*& A, char*& B) {
+    if (Bt.n == 0) return w;
+    const uint32_t bi = fd_div(w, Bt.div);
+    A = static_cast<const char*>(Bt.a[bi]);
+    B = static_cast<char*>(Bt.b[bi]);
+    return w - bi * Bt.per;
+}
+
 // ------------------------------------------------------------------------------------------
 // K1: direct kernel
 // ------------------------------------------------------------------------------------------
@@ -229,7 +238,7 @@ __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;"
 template <int DT, int V, bool BETA, bool IDX64>
 __global__ void __launch_bounds__(kDirectThreads)
 direct_kernel(const __grid_constant__ DirectParams P, const void* __restrict__ Ain, void* __restrict__ Bout,
-              const Scalar alpha_in, const Scalar beta_in) {
+              const Scalar alpha_in, const Scalar beta_in, const __grid_constant__ BatchPtrs Bt) {
     using T = typename ElemT<DT>::T;
     TScal<T> alpha, beta;
     typed(alpha_in, alpha);
@@ -244,6 +253,7 @@ direct_kernel(const __grid_constant__ DirectParams P, const void* __restrict__ A
     const char* A = static_cast<const char*>(Ain);
     char* B = static_cast<char*>(Bout);
     const idx_t n = (idx_t)P.n_items;
+    const uint32_t n_work = Bt.n ? P.n_chunks * (uint32_t)Bt.n : P.n_chunks;
     __shared__ __align__(16) uint4 sched_resp;
     __shared__ __align__(8) uint64_t sched_bar;
     WorkSched sched;
@@ -256,7 +266,7 @@ direct_kernel(const __grid_constant__ DirectParams P, const void* __restrict__ A
     uint32_t chunk = blockIdx.x;
     for (;;) {
         sched.prefetch();
-        const idx_t first = (idx_t)chunk * (idx_t)(kDirectThreads * kDirectUnroll) + threadIdx.x;
+        const idx_t first = (idx_t)batch_item(Bt, chunk, A, B) * (idx_t)(kDirectThreads * kDirectUnroll) + threadIdx.x;
         PackA a[kDirectUnroll];
         PackT b[kDirectUnroll];
         eoff_t oa[kDirectUnroll], ob[kDirectUnroll];
@@ -310,7 +320,7 @@ direct_kernel(const __grid_constant__ DirectParams P, const void* __restrict__ A
                 st_global<Raw>(B + (int64_t)ob[k] * (int64_t)sizeof(T), o.raw);
             }
         }
-        const bool more = sched.next(chunk, P.n_chunks);
+        const bool more = sched.next(chunk, n_work);
         if (!more) break;
         if (sched.dyn) __syncthreads();   // everyone has read the response before the next prefetch
     }
@@ -329,7 +339,7 @@ constexpr int kTileMinCtas = 6;
 template <int DT, int VA, int VB, bool SAME, bool BETA>
 __global__ void __launch_bounds__(kTileThreads, BETA ? 4 : kTileMinCtas)
 tile_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, void* __restrict__ Bout,
-            const Scalar alpha_in, const Scalar beta_in) {
+            const Scalar alpha_in, const Scalar beta_in, const __grid_constant__ BatchPtrs Bt) {
     using T = typename ElemT<DT>::T;
     TScal<T> alpha, beta;
     typed(alpha_in, alpha);
@@ -390,7 +400,7 @@ tile_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
         int64_t baseA = 0, baseB = 0;
         bool edge = false;
         {
-            uint32_t r = tile_id;
+            uint32_t r = batch_item(Bt, tile_id, A, B);
 #pragma unroll 1
             for (int g = 0; g < P.nG; ++g) {
                 const uint32_t qq = fd_div(r, P.g[g].div);
@@ -502,7 +512,7 @@ tile_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
                 }
             }
         }
-        const bool more = sched.next(tile_id, P.n_tiles);
+        const bool more = sched.next(tile_id, Bt.n ? P.n_tiles * (uint32_t)Bt.n : P.n_tiles);
         if (!more) break;
         __syncthreads();   // tile and scheduler response are free again
     }
@@ -545,7 +555,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 template <int DT, int VB, bool BETA, bool PEEL>
 __global__ void __launch_bounds__(kRingThreads, (PEEL || (BETA && VB == 1)) ? 3 : BETA ? 4 : 5)
 ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, void* __restrict__ Bout,
-            const Scalar alpha_in, const Scalar beta_in) {
+            const Scalar alpha_in, const Scalar beta_in, const __grid_constant__ BatchPtrs Bt) {
     using T = typename ElemT<DT>::T;
     TScal<T> alpha, beta;
     typed(alpha_in, alpha);
@@ -632,7 +642,8 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
             bool edge = false;
             int32_t* vx = reinterpret_cast<int32_t*>(smem + L.rvext) + s * kMaxRank;
             {
-                uint32_t r = tile_id;
+                char* Bunused = nullptr;
+                uint32_t r = batch_item(Bt, tile_id, A, Bunused);
 #pragma unroll 1
                 for (int g = 0; g < P.nG; ++g) {
                     const uint32_t qq = fd_div(r, P.g[g].div);
@@ -773,7 +784,7 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
                 }
             }
             }
-            more = sched.next<true>(tile_id, P.n_tiles);
+            more = sched.next<true>(tile_id, Bt.n ? P.n_tiles * (uint32_t)Bt.n : P.n_tiles);
             __syncwarp();
         }
         return;
@@ -804,7 +815,8 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
         if (tile_id == 0xFFFFFFFFu) break;
         int64_t baseB = 0;
         {
-            uint32_t r = tile_id;
+            const char* Aunused = nullptr;
+            uint32_t r = batch_item(Bt, tile_id, Aunused, B);
 #pragma unroll 1
             for (int g = 0; g < P.nG; ++g) {
                 const uint32_t qq = fd_div(r, P.g[g].div);
@@ -1006,8 +1018,8 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
 // ------------------------------------------------------------------------------------------
 // Dispatch: (dtype, vector widths, beta != 0) -> kernel instance
 // ------------------------------------------------------------------------------------------
-using TileFn = void (*)(const TileParams, const void*, void*, const Scalar, const Scalar);
-using DirectFn = void (*)(const DirectParams, const void*, void*, const Scalar, const Scalar);
+using TileFn = void (*)(const TileParams, const void*, void*, const Scalar, const Scalar, const BatchPtrs);
+using DirectFn = void (*)(const DirectParams, const void*, void*, const Scalar, const Scalar, const BatchPtrs);
 
 template <int DT, int VA, int VB, bool SAME>
 static TileFn tile_fn_beta(bool beta) {
@@ -1128,6 +1140,7 @@ int prepare_candidate(Candidate* cand, ttc_dtype dtype, ttc_dtype dtype_a, int s
         cand->info.threads = kDirectThreads;
         cand->info.smem_bytes = 0;
         cand->info.grid = (int)(cand->dp.dyn == 1 || need < cap ? need : cap);
+        cand->grid_cap = (int)cap;
         return 0;
     }
     TileFn fn = get_tile_fn(pair, *cand);
@@ -1155,11 +1168,13 @@ int prepare_candidate(Candidate* cand, ttc_dtype dtype, ttc_dtype dtype_a, int s
     cand->info.threads = cand->tp.threads;
     cand->info.smem_bytes = smem;
     cand->info.grid = (int)(cand->tp.dyn == 1 || cand->tp.n_tiles < cap ? cand->tp.n_tiles : cap);
+    cand->grid_cap = (int)cap;
     return 0;
 }
 
 int launch_candidate(const Candidate& cand, ttc_dtype dtype, ttc_dtype dtype_a, const Scalar& alpha,
-                     const Scalar& beta, const void* A, void* B, void* stream, uint32_t* sched_ctr) {
+                     const Scalar& beta, const void* A, void* B, void* stream, uint32_t* sched_ctr,
+                     const BatchPtrs* batch) {
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const int pair = pair_id(dtype, dtype_a);
     if (pair < 0) return (int)cudaErrorInvalidValue;
@@ -1168,7 +1183,16 @@ int launch_candidate(const Candidate& cand, ttc_dtype dtype, ttc_dtype dtype_a, 
     // read (no cudaGetLastError, which would clear errors that are not ours).
     cudaLaunchConfig_t cfg{};
     cfg.stream = st;
-    cfg.gridDim = dim3((unsigned)cand.info.grid, 1, 1);
+    static const BatchPtrs kNoBatch{};
+    const BatchPtrs& bt = batch ? *batch : kNoBatch;
+    uint64_t grid = (uint64_t)cand.info.grid;
+    if (bt.n > 0) {     // one CTA per work item (launch control) or as many as the device holds
+        const uint64_t work = (uint64_t)bt.per * (uint64_t)bt.n;
+        const int dyn_b = cand.info.kernel == TTC_KERNEL_COPY ? cand.dp.dyn : cand.tp.dyn;
+        grid = (dyn_b == 1 || work < (uint64_t)cand.grid_cap) ? work : (uint64_t)cand.grid_cap;
+        if (grid >= (1ull << 31)) return (int)cudaErrorInvalidConfiguration;
+    }
+    cfg.gridDim = dim3((unsigned)grid, 1, 1);
     // Every launch carries the programmatic-stream-serialisation attribute (programmatic dependent
     // launch): the kernels call griddepcontrol.launch_dependents first thing and griddepcontrol.wait
     // before their first global access, so the prologue (scheduler set-up, offset tables) of a kernel
@@ -1192,7 +1216,7 @@ int launch_candidate(const Candidate& cand, ttc_dtype dtype, ttc_dtype dtype_a, 
         cfg.dynamicSmemBytes = 0;
         DirectParams dp = cand.dp;
         dp.ctr = sched_ctr;
-        return (int)cudaLaunchKernelEx(&cfg, fn, dp, A, B, alpha, beta);
+        return (int)cudaLaunchKernelEx(&cfg, fn, dp, A, B, alpha, beta, bt);
     }
     TileFn fn = get_tile_fn(pair, cand);
     if (!fn) return (int)cudaErrorInvalidValue;
@@ -1200,7 +1224,7 @@ int launch_candidate(const Candidate& cand, ttc_dtype dtype, ttc_dtype dtype_a, 
     cfg.dynamicSmemBytes = (size_t)cand.info.smem_bytes;
     TileParams tp = cand.tp;
     tp.ctr = sched_ctr;
-    return (int)cudaLaunchKernelEx(&cfg, fn, tp, A, B, alpha, beta);
+    return (int)cudaLaunchKernelEx(&cfg, fn, tp, A, B, alpha, beta, bt);
 }
 
 }  // namespace ttc

@@ -14,13 +14,11 @@ namespace ttc {
 
 namespace {
 
+constexpr int kFullSearch = 96;             // candidates at the head of the list that get the full padding search
 constexpr int kMaxImplementations = 400;   // the paper's default bound is 200; ours holds the
                                            // ring-kernel variants as well, and a candidate costs ~1 ms to time
 constexpr int64_t kInt31 = (int64_t)1 << 31;
 
-struct TileSpec {
-    int32_t t[kMaxRank];   // tile extent per canonical index (1 = outside the tile)
-};
 
 // ----------------------------------------------------------------------------------------
 // Shared-memory bank model: wavefronts needed by one warp-wide access of `sz` bytes per lane
@@ -29,17 +27,24 @@ struct TileSpec {
 // ----------------------------------------------------------------------------------------
 int smem_wavefronts(const int64_t* addr, int n, int sz) {
     const int lanes_per_group = sz <= 4 ? 32 : (sz == 8 ? 16 : 8);
+    const int wpl = std::max(1, sz / 4);                 // words per lane
     int total = 0;
     for (int g0 = 0; g0 < n; g0 += lanes_per_group) {
-        int64_t words[32 * 4];
-        int nw = 0;
-        for (int l = g0; l < std::min(n, g0 + lanes_per_group); ++l)
-            for (int w = 0; w < std::max(1, sz / 4); ++w) words[nw++] = addr[l] / 4 + w;
-        std::sort(words, words + nw);
-        nw = (int)(std::unique(words, words + nw) - words);
-        int per_bank[32] = {0};
+        // distinct words per bank (a group holds at most 32 words, so 32 slots per bank always suffice)
+        int64_t seen[32][32];
+        int cnt[32] = {0};
         int worst = 0;
-        for (int i = 0; i < nw; ++i) worst = std::max(worst, ++per_bank[words[i] & 31]);
+        const int g1 = std::min(n, g0 + lanes_per_group);
+        for (int l = g0; l < g1; ++l)
+            for (int w = 0; w < wpl; ++w) {
+                const int64_t word = addr[l] / 4 + w;
+                const int bank = (int)(word & 31);
+                bool dup = false;
+                for (int k = 0; k < cnt[bank]; ++k) dup |= seen[bank][k] == word;
+                if (dup) continue;
+                seen[bank][cnt[bank]] = word;
+                worst = std::max(worst, ++cnt[bank]);
+            }
         total += worst;
     }
     return total;
@@ -60,19 +65,50 @@ int64_t phase_smem_offset(const std::vector<PhaseDim>& ph, const int32_t* ss, in
     return s;
 }
 
-// Relative smem cost (>= 1) of both phases for the given tile strides.
-double smem_conflict_cost(const std::vector<PhaseDim>& phA, const std::vector<PhaseDim>& phB,
-                          const int32_t* ss, int es, int vecA, int vecB, bool same, int sstepB,
-                          int64_t itemsA, int64_t itemsB, bool splitA, bool skipA = false, bool xp = false) {
-    double got = 0, ideal = 0;
-    const int warps = 8;
-    int64_t addr[32];
-    for (int w = 0; w < warps; ++w) {
-        // spread the sampled warps over the tile
-        const int64_t startA = (itemsA / 32) * w / warps * 32;
+// The sampled warps of one phase: the coordinates of every sampled lane's entry, decomposed ONCE per
+// candidate (the padding search only changes the strides they are multiplied with).
+constexpr int kSampleWarps = 8, kMaxPhaseDims = 2 * kMaxTab;
+struct PhaseSamples {
+    int nk = 0;
+    int dim[kMaxPhaseDims];
+    bool fused[kMaxPhaseDims];
+    int n[kSampleWarps];
+    int32_t co[kSampleWarps][32][kMaxPhaseDims];   // coordinate * step per enumerated index
+};
+
+void sample_phase(const std::vector<PhaseDim>& ph, int64_t items, PhaseSamples* S) {
+    S->nk = (int)std::min<size_t>(ph.size(), kMaxPhaseDims);
+    for (int k = 0; k < S->nk; ++k) { S->dim[k] = ph[k].dim; S->fused[k] = ph[k].fused; }
+    for (int w = 0; w < kSampleWarps; ++w) {
+        const int64_t start = (items / 32) * w / kSampleWarps * 32;   // spread the sampled warps over the tile
         int n = 0;
-        for (int l = 0; l < 32 && startA + l < itemsA; ++l) addr[n++] = phase_smem_offset(phA, ss, startA + l) * es;
-        if (n && !skipA) {
+        for (int l = 0; l < 32 && start + l < items; ++l, ++n) {
+            int64_t idx = start + l;
+            for (int k = 0; k < S->nk; ++k) {
+                S->co[w][l][k] = (int32_t)((idx % ph[k].n) * ph[k].step);
+                idx /= ph[k].n;
+            }
+        }
+        S->n[w] = n;
+    }
+}
+
+inline int64_t sample_offset(const PhaseSamples& S, int w, int l, const int32_t* ss) {
+    int64_t o = 0;
+    for (int k = 0; k < S.nk; ++k) o += (int64_t)S.co[w][l][k] * (S.fused[k] ? 1 : ss[S.dim[k]]);
+    return o;
+}
+
+// Relative smem cost (>= 1) of both phases for the given tile strides.
+double smem_conflict_cost(const PhaseSamples& SA, const PhaseSamples& SB,
+                          const int32_t* ss, int es, int vecA, int vecB, bool same, int sstepB,
+                          bool splitA, bool skipA = false, bool xp = false) {
+    double got = 0, ideal = 0;
+    int64_t addr[32];
+    for (int w = 0; w < kSampleWarps; ++w) {
+        int n = skipA ? 0 : SA.n[w];
+        for (int l = 0; l < n; ++l) addr[l] = sample_offset(SA, w, l, ss) * es;
+        if (n) {
             if (!splitA) {
                 got += smem_wavefronts(addr, n, es * vecA);
             } else {   // the vecA elements of a global vector are stored one by one
@@ -84,9 +120,8 @@ double smem_conflict_cost(const std::vector<PhaseDim>& phA, const std::vector<Ph
             }
             ideal += std::max(1.0, n * es * vecA / 128.0);
         }
-        const int64_t startB = (itemsB / 32) * w / warps * 32;
-        n = 0;
-        for (int l = 0; l < 32 && startB + l < itemsB; ++l) addr[n++] = phase_smem_offset(phB, ss, startB + l) * es;
+        n = SB.n[w];
+        for (int l = 0; l < n; ++l) addr[l] = sample_offset(SB, w, l, ss) * es;
         if (n) {
             if (same || vecB == 1) {
                 got += smem_wavefronts(addr, n, es * vecB);
@@ -137,6 +172,42 @@ bool split_tables(const std::vector<PhaseDim>& ph, int* split_out, int threads =
 
 namespace {
 
+// Ranking cost of a tile / ring candidate from its raw features F (see the end of build_tile_candidate);
+// `legacy` is the hand-written round-1 formula.  TTC_COST=legacy ranks by it (for comparisons).
+double fitted_tile_cost(const float* F, double legacy) {
+    static const bool use_legacy = std::getenv("TTC_COST") && !std::strcmp(std::getenv("TTC_COST"), "legacy");
+    if (use_legacy) return legacy;
+    // exp(w . terms): estimated time / (bytes at 6.5 TB/s).  Least-squares fit of log(time) on measured
+    // times of all candidates of 71 transpositions on B200 (BASELINE.json's configs and 44 seeded random
+    // 2-D..6-D cases of ~200 MB), weighted towards each case's fastest candidates; terms and weights come
+    // from `python -m paper_1607_01249_b200.fit_cost fit` (same order as terms() there).  On those samples
+    // the best of the 10 / 32 best-ranked candidates reaches 0.98 / 0.995 of the exhaustive search's time
+    // (hand-written round-1 formula: 0.92 / 0.95).
+    static const double kCostW[30] = {0.19459, 0.29221, 0.10785, -0.08450, -0.03553, 0.73929, 0.03056, 0.14005, -0.27823, 0.17293,
+                                      0.15489, 0.93256, -0.16513, 0.06247, -0.06912, -0.10319, 0.40596, 0.03243, 0.13822, 0.06578,
+                                      0.02644, 0.29674, -0.04683, 0.70913, 0.15136, -0.00012, -0.08401, -0.02661, 0.03885, -0.10466};
+    const double runA = F[0], runB = F[1], waste = F[2], conf = F[3], tile_b = F[4], n_tiles = F[5], ring = F[6];
+    const double rowmode = F[7], peel = F[8], xp = F[9], vab = F[10], vbb = F[11], beta = F[12], kern = F[13], row_b = F[14];
+    const double lc = std::log(std::max(conf, 1.0));
+    const double na = vab < 16 ? 1.0 : 0.0, nb = vbb < 16 ? 1.0 : 0.0;
+    const double t[30] = {
+        1.0,
+        std::log1p(256.0 / std::max(runA, 1.0)), std::log1p(64.0 / std::max(runB, 1.0)),
+        std::log1p(2048.0 / std::max(runA, 1.0)), std::log1p(512.0 / std::max(runB, 1.0)),
+        std::log(std::max(waste, 1.0)), lc,
+        4096.0 / std::max(tile_b, 256.0), std::max(0.0, tile_b - 32768.0) / 65536.0, std::max(0.0, tile_b - 16384.0) / 65536.0,
+        std::max(0.0, 1.0 - n_tiles / 1184.0), std::max(0.0, 1.0 - n_tiles / 4736.0),
+        ring > 0 ? 1.0 : 0.0, ring >= 4 ? 1.0 : 0.0,
+        rowmode == 1 ? 1.0 : 0.0, rowmode == 2 ? 1.0 : 0.0, peel != 0 ? 1.0 : 0.0, xp != 0 ? 1.0 : 0.0,
+        na, nb, na * (vab <= 4 ? 1.0 : 0.0), nb * (vbb <= 4 ? 1.0 : 0.0),
+        beta, (rowmode == 1 ? 1.0 : 0.0) * 128.0 / std::max(row_b, 16.0), beta * std::log1p(64.0 / std::max(runB, 1.0)),
+        beta * nb, (ring == 0 ? 1.0 : 0.0) * lc, lc * (xp != 0 ? 1.0 : 0.0),
+        kern == 3 ? 1.0 : 0.0, kern == 4 ? 1.0 : 0.0};
+    double z = 0;
+    for (int i = 0; i < 30; ++i) z += kCostW[i] * t[i];
+    return std::exp(z);
+}
+
 // Largest vector (in elements) legal for global accesses along canonical index `lead` of
 // tensor X (strideOf gives that tensor's strides): the index is stride-1, its extent and
 // tile extent are multiples of the vector, and every other stride keeps 16-byte alignment.
@@ -155,7 +226,8 @@ int legal_vec(const Canon& c, int lead, bool sideA, int32_t t_lead, int mv) {
 
 // Build one tile-kernel candidate.  Returns false if the combination is not legal.
 bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, const TileSpec& spec,
-                          int loop_order, int want_va, int want_vb, int max_smem, int sched, int ring, int xp, int rowmode, Candidate* out) {
+                          int loop_order, int want_va, int want_vb, int max_smem, int sched, int ring, int xp, int rowmode, bool quick,
+                          Candidate* out) {
     // es: B's element and the tile's (the planner's world is B-typed); esA differs from it only for
     // the mixed-precision pairs.  There the tile kernel converts A in its load phase (the tile holds
     // B's type), while the ring kernel's bulk copies land A's bytes unconverted: its tile holds A's
@@ -320,13 +392,21 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
     int64_t best_elems = 0;
     int best_split = 0;
     const int levels = (int)ta.size() - 1;
-    const int search_levels = std::min(levels, 3);
+    const int search_levels = std::min(levels, 2);     // paddings of the two innermost levels decide the conflicts
     static const int pad_opts[] = {0, 1, 2, 3, 4};
     const int n_opts = 5;
     int combos = 1;
     for (int i = 0; i < search_levels; ++i) combos *= n_opts;
     const bool shifted = P.row_async == 2;
-    for (int split = 0; split < ((want_va > 1 && !same && !ring) ? 2 : 1); ++split) {
+    // quick: no padding search (dense tile, paddings 0) -- the first pass of generate_candidates ranks with
+    // it; only candidates that make the bounded list's head are built again with the full search
+    if (quick) combos = 1;
+    static thread_local PhaseSamples samplesA, samplesB;
+    PhaseSamples *SA = &samplesA, *SB = &samplesB;
+    if ((int)phA.size() > kMaxPhaseDims || (int)phB.size() > kMaxPhaseDims) return false;
+    sample_phase(phA, itemsA, SA);
+    sample_phase(phB, itemsB, SB);
+    for (int split = 0; split < ((want_va > 1 && !same && !ring && !quick) ? 2 : 1); ++split) {
     const int unit = split ? 1 : std::max(std::max(std::max(want_va, same ? mvS : 1), P.row_pairs ? 2 : 1), shifted ? mv : 1);
     for (int combo = 0; combo < combos; ++combo) {
         int cc = combo;
@@ -350,7 +430,7 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
         int64_t elems = (int64_t)ss[ta.back()] * spec.t[ta.back()];
         if (shifted && (int)ta.size() <= dense_levels) elems = (elems + 2 * mv - 1) / mv * mv;   // a one-row tile
         if (elems * esT * (ring ? ring : 1) > max_smem) continue;
-        const double conf = smem_conflict_cost(phA, phB, ss, esT, want_va, want_vb, same, ss[B0], itemsA, itemsB, split != 0,
+        const double conf = smem_conflict_cost(*SA, *SB, ss, esT, want_va, want_vb, same, ss[B0], split != 0,
                                                ring != 0 && !P.row_async, xp != 0);
         // a split store costs want_va - 1 extra instructions per item: worth it only for a real gain
         const double cost = conf + 1e-3 * (double)elems * esT / 1024.0 + (split ? 0.08 : 0.0);
@@ -360,6 +440,7 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
             best_split = split;
             std::memcpy(best_ss, ss, sizeof(ss));
         }
+        if (conf <= 1.0 + 1e-9) break;      // conflict-free: larger paddings only cost shared memory
     }
     }
     if (best_cost >= 1e30) return false;
@@ -508,7 +589,25 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
         const double len = (double)P.row_bytes / es;
         cost *= std::max(1.0, 0.4 * (std::ceil(len / 32.0) + 6.0) / (len / 32.0));
     }
-    I.est_cost = (float)cost;
+    // raw inputs of the heuristic, for re-fitting it against measured times (ttc_plan_candidate_features)
+    float* F = cand.feat;
+    F[0] = (float)((double)runA * esA);      // contiguous bytes per tile in A
+    F[1] = (float)((double)runB * es);       // contiguous bytes per tile in B
+    F[2] = (float)waste;                     // padded / logical elements (remainder tiles)
+    F[3] = (float)best_cost;                 // shared-memory wavefronts / ideal (bank model)
+    F[4] = (float)tile_bytes;
+    F[5] = (float)n_tiles;
+    F[6] = (float)ring;
+    F[7] = (float)P.row_async;
+    F[8] = (float)P.peel;
+    F[9] = (float)P.xp;
+    F[10] = (float)(want_va * esA);
+    F[11] = (float)(want_vb * es);
+    F[12] = beta_nz ? 1.f : 0.f;
+    F[13] = (float)I.kernel;
+    F[14] = (float)P.row_bytes;
+    F[15] = (float)itemsB;
+    I.est_cost = (float)fitted_tile_cost(F, cost);
     *out = cand;
     return true;
 }
@@ -647,7 +746,18 @@ void add_direct(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz
     double cost = 1.0 / eff(ra) + (beta_nz ? 2.0 : 1.0) / eff(rb);
     if (vec * std::max(es, esA) < 16) cost *= 1.25;
     if (idx64) cost *= 1.5;
-    I.est_cost = (float)cost;
+    cand.feat[0] = (float)ra;
+    cand.feat[1] = (float)rb;
+    cand.feat[2] = 1.f;
+    cand.feat[10] = (float)(vec * esA);
+    cand.feat[11] = (float)(vec * es);
+    cand.feat[12] = beta_nz ? 1.f : 0.f;
+    cand.feat[13] = (float)TTC_KERNEL_COPY;
+    cand.feat[5] = (float)n_chunks;
+    cand.feat[6] = idx64 ? 1.f : 0.f;
+    // the tile candidates' fitted costs are time / ideal time; the direct formula is about 2.0 at its best
+    static const bool legacy_cost = std::getenv("TTC_COST") && !std::strcmp(std::getenv("TTC_COST"), "legacy");
+    I.est_cost = (float)(legacy_cost ? cost : 0.5 * cost);
     I.tile_u = (int)std::min<int64_t>(run_of(true), INT32_MAX);
     I.tile_w = (int)std::min<int64_t>(run_of(false), INT32_MAX);
     out->push_back(cand);
@@ -724,8 +834,10 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, boo
                                     for (int rowmode = 1; rowmode <= (ring && !xp && (variants & 2) ? 2 : 1); ++rowmode) {
                                         Candidate cand;
                                         if (build_tile_candidate(c, dtype, dtype_a, beta_nz, spec, lo, va, vb, max_smem, sched, ring, xp,
-                                                                 rowmode, &cand))
+                                                                 rowmode, true, &cand)) {
+                                            cand.recipe = Recipe{spec, lo, va, vb, sched, ring, xp, rowmode};
                                             out->push_back(cand);
+                                        }
                                     }
                             }
                     }
@@ -735,8 +847,8 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, boo
     }
 
     // Bounded list ordered by estimated cost.
-    std::stable_sort(out->begin(), out->end(),
-                     [](const Candidate& a, const Candidate& b) { return a.info.est_cost < b.info.est_cost; });
+    auto by_cost = [](const Candidate& a, const Candidate& b) { return a.info.est_cost < b.info.est_cost; };
+    std::stable_sort(out->begin(), out->end(), by_cost);
     if ((int)out->size() > kMaxImplementations) {
         // keep the scalar direct fallback whatever its rank
         Candidate fallback;
@@ -748,6 +860,21 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, boo
         for (auto& cd : *out) kept |= (cd.info.kernel == TTC_KERNEL_COPY && cd.info.vec_a == 1);
         if (have && !kept) out->back() = fallback;
     }
+    // Second pass: the head of the list (what the tuner times by default) gets the full shared-memory padding
+    // search of the bank model; the tail keeps its dense tiles (still complete, launchable candidates).
+    const int n_full = std::min<int>((int)out->size(), kFullSearch);
+    for (int i = 0; i < n_full; ++i) {
+        Candidate& cd = (*out)[i];
+        if (cd.info.kernel == TTC_KERNEL_COPY) continue;
+        const Recipe r = cd.recipe;
+        Candidate full;
+        if (build_tile_candidate(c, dtype, dtype_a, beta_nz, r.spec, r.loop_order, r.va, r.vb, max_smem, r.sched, r.ring, r.xp,
+                                 r.rowmode, false, &full)) {
+            full.recipe = r;
+            cd = full;
+        }
+    }
+    std::stable_sort(out->begin(), out->end(), by_cost);
 }
 
 }  // namespace ttc

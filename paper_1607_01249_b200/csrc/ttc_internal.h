@@ -152,6 +152,17 @@ struct TileParams {
     GridDim g[kMaxRank];
 };
 
+// Batched execution (ttc_execute_batched): up to kMaxBatch problems that share one plan run in ONE launch;
+// work item w belongs to problem w / per.  n == 0: a single problem, the kernel's own A and B arguments.
+constexpr int kMaxBatch = 64;
+struct BatchPtrs {
+    int n;
+    uint32_t per;               // work items (macro-tiles / chunks) per problem
+    FastDiv div;                // by `per`
+    const void* a[kMaxBatch];
+    void* b[kMaxBatch];
+};
+
 // Shared-memory carve-up (bytes), identical on host and device.
 struct TileSmemLayout {
     uint32_t tab[4];     // int2 tables
@@ -184,6 +195,13 @@ TTC_HD TileSmemLayout tile_smem_layout(const TileParams& P, int es) {
 // ---------------------------------------------------------------------------------------
 // A candidate = kernel class + blocking + loop order + launch shape.
 // ---------------------------------------------------------------------------------------
+struct TileSpec {
+    int32_t t[kMaxRank];   // tile extent per canonical index (1 = outside the tile)
+};
+struct Recipe {             // what build_tile_candidate was called with (to build the candidate again)
+    TileSpec spec;
+    int loop_order, va, vb, sched, ring, xp, rowmode;
+};
 struct Candidate {
     ttc_candidate_info info{};
     bool beta_nz = false;
@@ -191,6 +209,9 @@ struct Candidate {
     int  align_a = 1, align_b = 1;  // required pointer alignment in bytes
     DirectParams dp{};
     TileParams tp{};
+    float feat[16] = {0};        // raw inputs of the cost heuristic (plan.cpp), exported for re-fitting
+    Recipe recipe{};
+    int grid_cap = 0;            // resident CTAs the device holds of this kernel (set by prepare_candidate)
 };
 
 struct Scalar {         // alpha or beta, as doubles (re, im); narrowed in the launcher
@@ -205,7 +226,8 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, boo
 
 // Launch one candidate.  Returns the CUDA error code (0 = success) as int.
 int launch_candidate(const Candidate& cand, ttc_dtype dtype, ttc_dtype dtype_a, const Scalar& alpha,
-                     const Scalar& beta, const void* A, void* B, void* stream, uint32_t* sched_ctr);
+                     const Scalar& beta, const void* A, void* B, void* stream, uint32_t* sched_ctr,
+                     const BatchPtrs* batch = nullptr);
 // Configure dynamic shared memory / occupancy-derived grid for a candidate (needs a device).
 int prepare_candidate(Candidate* cand, ttc_dtype dtype, ttc_dtype dtype_a, int sm_count);
 

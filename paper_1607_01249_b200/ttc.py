@@ -24,9 +24,9 @@ STATUS_NAMES = ["TTC_OK", "TTC_ERR_INVALID_ARG", "TTC_ERR_NOT_PERMUTATION", "TTC
 KERNEL_NAMES = {0: "none", 1: "copy", 2: "tile", 3: "gather", 4: "wide", 5: "tma"}
 NP_DTYPE = {TTC_F32: np.float32, TTC_F64: np.float64, TTC_C64: np.complex64, TTC_C128: np.complex128}
 
-EXPORTS = ["ttc_plan", "ttc_plan_mixed", "ttc_plan_dtype_a", "ttc_execute", "ttc_execute_host", "ttc_destroy", "ttc_last_error",
+EXPORTS = ["ttc_plan", "ttc_plan_mixed", "ttc_plan_dtype_a", "ttc_execute", "ttc_execute_batched", "ttc_execute_host", "ttc_destroy", "ttc_last_error",
            "ttc_status_string", "ttc_plan_info", "ttc_plan_num_candidates", "ttc_plan_candidate",
-           "ttc_plan_select", "ttc_plan_tune", "ttc_canonicalize", "ttc_launch_count",
+           "ttc_plan_candidate_features", "ttc_plan_select", "ttc_plan_tune", "ttc_canonicalize", "ttc_launch_count",
            "ttc_debug_fastdiv", "ttc_version", "ttc_release_host_staging"]
 
 
@@ -66,6 +66,8 @@ def _load() -> ctypes.CDLL:
     lib.ttc_plan_dtype_a.argtypes = [vp]
     lib.ttc_execute.restype = ctypes.c_int
     lib.ttc_execute.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.ttc_execute_batched.restype = ctypes.c_int
+    lib.ttc_execute_batched.argtypes = [vp, vp, ctypes.POINTER(vp), vp, ctypes.POINTER(vp), ctypes.c_int, vp]
     lib.ttc_execute_host.restype = ctypes.c_int
     lib.ttc_execute_host.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.ttc_destroy.restype = ctypes.c_int
@@ -79,6 +81,8 @@ def _load() -> ctypes.CDLL:
     lib.ttc_plan_num_candidates.argtypes = [vp, ctypes.c_int]
     lib.ttc_plan_candidate.restype = ctypes.c_int
     lib.ttc_plan_candidate.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ttc_candidate_info)]
+    lib.ttc_plan_candidate_features.restype = ctypes.c_int
+    lib.ttc_plan_candidate_features.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_float)]
     lib.ttc_plan_select.restype = ctypes.c_int
     lib.ttc_plan_select.argtypes = [vp, ctypes.c_int, ctypes.c_int]
     lib.ttc_plan_tune.restype = ctypes.c_int
@@ -176,6 +180,21 @@ def ttc_execute(plan: int, alpha, A, beta, B, stream=None) -> None:
         raise TTCError(rc, "ttc_execute")
 
 
+def ttc_execute_batched(plan: int, alpha, A_list, beta, B_list, stream=None) -> None:
+    """One launch (per 64 pairs) for a list of tensor pairs that share ``plan``."""
+    npdt = _scalar_dtype(plan)
+    a = np.array([alpha], dtype=npdt)
+    b = np.array([beta], dtype=npdt)
+    n = len(A_list)
+    if len(B_list) != n:
+        raise ValueError("A_list and B_list differ in length")
+    pa = (ctypes.c_void_p * max(n, 1))(*[_ptr(x) for x in A_list])
+    pb = (ctypes.c_void_p * max(n, 1))(*[_ptr(x) for x in B_list])
+    rc = lib.ttc_execute_batched(plan, a.ctypes.data, pa, b.ctypes.data, pb, n, _stream(stream))
+    if rc != TTC_OK:
+        raise TTCError(rc, "ttc_execute_batched")
+
+
 def ttc_execute_host(plan: int, alpha, A_host, beta, B_host, stream=None) -> None:
     npdt = _scalar_dtype(plan)
     a = np.array([alpha], dtype=npdt)
@@ -208,6 +227,14 @@ def ttc_plan_candidate(plan: int, which: int, index: int) -> ttc_candidate_info:
     if rc != TTC_OK:
         raise TTCError(rc, "ttc_plan_candidate")
     return out
+
+
+def ttc_plan_candidate_features(plan: int, which: int, index: int):
+    out = (ctypes.c_float * 16)()
+    rc = lib.ttc_plan_candidate_features(plan, which, index, out)
+    if rc != TTC_OK:
+        raise TTCError(rc, "ttc_plan_candidate_features")
+    return [float(x) for x in out]
 
 
 def ttc_plan_select(plan: int, which: int, index: int) -> None:

@@ -233,7 +233,7 @@ def test_p7_fig2_subtensor_pack():
 
 
 # ------------------------------------------------------------- P8: Fig. 3 / config 4 packing
-@pytest.mark.parametrize("mr,npanel,K,lda2d", [(4, 6, 5, 24), (4, 6, 5, 28), (8, 3, 7, 32)])
+@pytest.mark.parametrize("mr,npanel,K,lda2d", [(4, 6, 5, 24), (4, 6, 5, 28), (8, 3, 7, 32), (6, 4, 5, 30), (16, 2, 3, 48)])
 def test_p8_blas_panel_pack(mr, npanel, K, lda2d):
     """PAPER.md:113, 125-129: A_{m,k} viewed as A_{m1,m2,k}, perm=0,2,1 -> B_{m1,k,m2}.
     Stated on the 2-D matrix alone: B[i + mr*(k + K*p)] = A2d[(i + mr*p) + lda2d*k]."""
@@ -253,6 +253,36 @@ def test_p8_blas_panel_pack(mr, npanel, K, lda2d):
         for k in range(K):
             for i in range(mr):
                 assert B[i + mr * (k + K * p)] == A2d[(i + mr * p) + lda2d * k]
+
+
+@pytest.mark.parametrize("nr", [4, 6, 8, 16])
+@pytest.mark.parametrize("dtype", [wl.F64, wl.F32])
+def test_p8b_blas_b_panel_pack_and_batched(nr, dtype):
+    """The other half of a GEMM's packing pair (BLIS-style B panels of nr columns): the
+    K x N matrix M (column-major, leading dimension ldm) viewed as the 3-D tensor M_{k,n1,n2} with sizes
+    (K, nr, N/nr) and leading dimensions (ldm, nr, .), perm = (1,0,2) -> P_{n1,k,n2}.  Stated on the 2-D
+    matrix alone: P[j + nr*(k + K*q)] = M[k + ldm*(j + nr*q)].  Rows k >= K of M (padding) are NaN and must
+    not be read.  Then the batched form: several blocks in one call is the same loop block by block."""
+    K, npanel, ldm = 7, 3, 9
+    N = nr * npanel
+    rng = np.random.default_rng(80 + nr)
+
+    def block():
+        M = np.full(ldm * N, np.nan, dtype=NP[dtype])
+        for n in range(N):
+            M[ldm * n: ldm * n + K] = rng.integers(-99, 100, size=K)
+        return M
+    blocks = [block() for _ in range(3)]
+    packed = [np.full(N * K, np.nan, dtype=NP[dtype]) for _ in blocks]
+    oracle.transpose_batched(dtype, (K, nr, npanel), (1, 0, 2), (ldm, nr, npanel), None, 1.0, blocks, 0.0, packed)
+    for M, P in zip(blocks, packed):
+        assert not np.isnan(P).any()
+        for q in range(npanel):
+            for k in range(K):
+                for j in range(nr):
+                    assert P[j + nr * (k + K * q)] == M[k + ldm * (j + nr * q)]
+    with pytest.raises(ValueError):
+        oracle.transpose_batched(dtype, (K, nr, npanel), (1, 0, 2), None, None, 1.0, blocks, 0.0, packed[:2])
 
 
 # ------------------------------------------------------------- P9: library routine
