@@ -19,6 +19,8 @@
 
 #include <cstdio>
 #include <cstdlib>
+#include <mutex>
+#include <set>
 #include <type_traits>
 
 #include "ttc_internal.h"
@@ -222,6 +224,10 @@ struct WorkSched {
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
+// The kernels are instantiated twice: for a single problem (BT = NoBatch: no pointer table among the kernel
+// parameters, nothing to decode) and for ttc_execute_batched (BT = BatchPtrs).
+struct NoBatch { static constexpr int n = 0; };
+__device__ __forceinline__ uint32_t batch_item(const NoBatch&, uint32_t w, const char*&, char*&) { return w; }
 // Batched launch: work item `w` of the whole launch -> (problem, item inside it); A and B of that problem.
 __device__ __forceinline__ uint32_t batch_item(const BatchPtrs& Bt, uint32_t w, const char*& A, char*& B) {
     if (Bt.n == 0) return w;
@@ -235,10 +241,10 @@ __device__ __forceinline__ uint32_t batch_item(const BatchPtrs& Bt, uint32_t w, 
 // K1: direct kernel
 // ------------------------------------------------------------------------------------------
 
-template <int DT, int V, bool BETA, bool IDX64>
+template <int DT, int V, bool BETA, bool IDX64, typename BT>
 __global__ void __launch_bounds__(kDirectThreads)
 direct_kernel(const __grid_constant__ DirectParams P, const void* __restrict__ Ain, void* __restrict__ Bout,
-              const Scalar alpha_in, const Scalar beta_in, const __grid_constant__ BatchPtrs Bt) {
+              const Scalar alpha_in, const Scalar beta_in, const __grid_constant__ BT Bt) {
     using T = typename ElemT<DT>::T;
     TScal<T> alpha, beta;
     typed(alpha_in, alpha);
@@ -336,10 +342,10 @@ constexpr int kTileUnroll = 4;
 // The beta != 0 instances need more registers (the B vectors in flight) and are left alone.
 constexpr int kTileMinCtas = 6;
 
-template <int DT, int VA, int VB, bool SAME, bool BETA>
+template <int DT, int VA, int VB, bool SAME, bool BETA, typename BT>
 __global__ void __launch_bounds__(kTileThreads, BETA ? 4 : kTileMinCtas)
 tile_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, void* __restrict__ Bout,
-            const Scalar alpha_in, const Scalar beta_in, const __grid_constant__ BatchPtrs Bt) {
+            const Scalar alpha_in, const Scalar beta_in, const __grid_constant__ BT Bt) {
     using T = typename ElemT<DT>::T;
     TScal<T> alpha, beta;
     typed(alpha_in, alpha);
@@ -552,10 +558,10 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     }
 }
 
-template <int DT, int VB, bool BETA, bool PEEL>
-__global__ void __launch_bounds__(kRingThreads, (PEEL || (BETA && VB == 1)) ? 3 : BETA ? 4 : 5)
+template <int DT, int VB, bool BETA, bool PEEL, bool SHIFT, typename BT>
+__global__ void __launch_bounds__(kRingThreads, (PEEL || (BETA && VB == 1 && SHIFT)) ? 3 : BETA ? 4 : 5)
 ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, void* __restrict__ Bout,
-            const Scalar alpha_in, const Scalar beta_in, const __grid_constant__ BatchPtrs Bt) {
+            const Scalar alpha_in, const Scalar beta_in, const __grid_constant__ BT Bt) {
     using T = typename ElemT<DT>::T;
     TScal<T> alpha, beta;
     typed(alpha_in, alpha);
@@ -683,7 +689,7 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
                 }
                 n_rows = __reduce_add_sync(0xFFFFFFFFu, (uint32_t)__popcll(row_ok));
             }
-            if (P.row_async == 2) {
+            if constexpr (SHIFT) {
                 // Shifted rows: lane handles rows lane, lane + 32, ...  The 16-byte aligned body of a row is one
                 // bulk copy that lands at the row's own misalignment sk (elements) behind its 16-byte aligned
                 // slot; the < 16-byte head and tail are element-sized cp.async.  Nothing outside the row is read.
@@ -799,9 +805,9 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
     // misalignment in A.  Bits 30-31 of the table entries' tile offsets and of shift_of[] add up to it (mod 4);
     // all of them are 0 for every other kind of tile, so the decoding below is unconditional.
     constexpr uint32_t MVE = 16 / ESA, kOffMask = 0x3FFFFFFFu;
-    constexpr int U = (VB == 1 && BETA && ES <= 8) ? 8 : kTileUnroll;
-    const bool shifted = P.row_async == 2;
-    const int ldm = P.shift_ld;
+    constexpr int U = (VB == 1 && BETA && SHIFT && ES <= 8) ? 8 : kTileUnroll;
+    constexpr bool shifted = SHIFT;
+    const int ldm = SHIFT ? P.shift_ld : 0;
     const FastDiv dlo = P.divBlo;
     // division-free enumeration of the store phase (see the loop): needs |lo table| to divide the consumer threads
     const bool lofix = !PEEL && (uint32_t)NC % dlo.d == 0;
@@ -861,6 +867,7 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
             const int bmis = (int)((reinterpret_cast<uintptr_t>(B) / ES) & (uintptr_t)(VB - 1));
             // element e of the B row whose table entry decodes to (base, sk): tile row (.. + e), whose skew advances by ldm
             auto tile_elem = [&](int32_t sok, int e) -> T {
+                if constexpr (!SHIFT) return cvt_to(T(), *reinterpret_cast<const TA*>(tile + sok + e * sstep));
                 const int sk = sok & (int)(MVE - 1);
                 return cvt_to(T(), *reinterpret_cast<const TA*>(tile + (sok & ~(int)(MVE - 1)) + e * sstep +
                                                                 ((sk + e * ldm) & (int)(MVE - 1)) * ESA));
@@ -883,7 +890,8 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
                         s0[k] = (int)(p - row * nch) * VB - m;          // first element of the window, row-relative
                         ok[k] = ok[k] && s0[k] >= 0 && s0[k] + VB <= len;
                         const uint32_t t = (uint32_t)eh.y + org;
-                        so[k] = (int32_t)((t & kOffMask) * ESA | ((t >> 30) & (MVE - 1)));   // low bits: the row's skew
+                        so[k] = SHIFT ? (int32_t)((t & kOffMask) * ESA | ((t >> 30) & (MVE - 1)))   // low bits: the row's skew
+                                      : eh.y * ESA;
                         go[k] = eh.x + s0[k];
                         if (BETA && ok[k]) bv[k].raw = ld_plain<RawB>(Bb + (int64_t)go[k] * ES);
                     }
@@ -919,7 +927,7 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
                     if (wl == 0 || s0 + VB <= len) continue;
                 }
                 const uint32_t t = (uint32_t)eh.y + org;
-                const int32_t sok = (int32_t)((t & kOffMask) * ESA | ((t >> 30) & (MVE - 1)));
+                const int32_t sok = SHIFT ? (int32_t)((t & kOffMask) * ESA | ((t >> 30) & (MVE - 1))) : eh.y * ESA;
 #pragma unroll
                 for (int j = 0; j < VB; ++j) {
                     const int e = s0 + j;
@@ -959,10 +967,14 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
                     }
                     const int2 eh = tabs[3][hi];
                     if (edge) ok[k] = v2[lo] & v3[hi];
-                    const uint32_t t = (uint32_t)(el.y + eh.y) + org;
-                    so[k] = (int32_t)((t & kOffMask) * ESA);
-                    if (VB == 1) so[k] += (int32_t)(((t >> 30) & (MVE - 1)) * ESA);     // the row's skew
-                    else so[k] |= (int32_t)((t >> 30) & (MVE - 1));                      // kept in the low bits (VB > 1)
+                    if constexpr (SHIFT) {
+                        const uint32_t t = (uint32_t)(el.y + eh.y) + org;
+                        so[k] = (int32_t)((t & kOffMask) * ESA);
+                        if (VB == 1) so[k] += (int32_t)(((t >> 30) & (MVE - 1)) * ESA);     // the row's skew
+                        else so[k] |= (int32_t)((t >> 30) & (MVE - 1));                      // kept in the low bits (VB > 1)
+                    } else {
+                        so[k] = (el.y + eh.y) * ESA;
+                    }
                     go[k] = el.x + eh.x;
                     if (BETA && ok[k]) bv[k].raw = ld_plain<RawB>(Bb + (int64_t)go[k] * ES);
                 }
@@ -976,7 +988,7 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
                         for (int j = 0; j < VB; ++j) a.e[j] = cvt_to(T(), *reinterpret_cast<const TA*>(tile + so[k] + j * sstep));
                     } else if (VB == 1 || same) {   // same: the vector leads A and B, chunks move unchanged
                         a.raw = *reinterpret_cast<const RawB*>(tile + so[k]);
-                    } else if (shifted) {      // vector of VB tile rows, each behind its slot by its own skew
+                    } else if constexpr (SHIFT) {      // vector of VB tile rows, each behind its slot by its own skew
                         const int sk = so[k] & (int)(MVE - 1), base = so[k] & ~(int)(MVE - 1);
 #pragma unroll
                         for (int j = 0; j < VB; ++j)
@@ -1018,118 +1030,152 @@ ring_kernel(const __grid_constant__ TileParams P, const void* __restrict__ Ain, 
 // ------------------------------------------------------------------------------------------
 // Dispatch: (dtype, vector widths, beta != 0) -> kernel instance
 // ------------------------------------------------------------------------------------------
-using TileFn = void (*)(const TileParams, const void*, void*, const Scalar, const Scalar, const BatchPtrs);
-using DirectFn = void (*)(const DirectParams, const void*, void*, const Scalar, const Scalar, const BatchPtrs);
+// Kernel instances are handed around as untyped entry points (their last parameter's type differs between
+// the single-problem and the batched instantiation) and launched with cudaLaunchKernelExC.
+using KernelFn = const void*;
 
 template <int DT, int VA, int VB, bool SAME>
-static TileFn tile_fn_beta(bool beta) {
-    return beta ? (TileFn)tile_kernel<DT, VA, VB, SAME, true> : (TileFn)tile_kernel<DT, VA, VB, SAME, false>;
+static KernelFn tile_fn_beta(bool beta, bool batched) {
+    if (batched)
+        return beta ? (KernelFn)tile_kernel<DT, VA, VB, SAME, true, BatchPtrs> : (KernelFn)tile_kernel<DT, VA, VB, SAME, false, BatchPtrs>;
+    return beta ? (KernelFn)tile_kernel<DT, VA, VB, SAME, true, NoBatch> : (KernelFn)tile_kernel<DT, VA, VB, SAME, false, NoBatch>;
 }
 
 template <int DT>
-static TileFn tile_fn(int va, int vb, bool same, bool beta) {
+static KernelFn tile_fn(int va, int vb, bool same, bool beta, bool batched) {
     // 16-byte vectors of each side's own type; MS: the one width that fits both (wide class, and the
     // extra equal-width variant of the mixed-precision pairs)
     constexpr int MVA = 16 / (int)sizeof(typename ElemT<DT>::TA), MVB = 16 / ElemT<DT>::ES;
     constexpr int MS = MVA < MVB ? MVA : MVB;
     if constexpr (MS > 1) {
-        if (same && va == MS && vb == MS) return tile_fn_beta<DT, MS, MS, true>(beta);
+        if (same && va == MS && vb == MS) return tile_fn_beta<DT, MS, MS, true>(beta, batched);
     }
     if (same) return nullptr;
     if constexpr (MVA > 1 && MVB > 1) {
-        if (va == MVA && vb == MVB) return tile_fn_beta<DT, MVA, MVB, false>(beta);
+        if (va == MVA && vb == MVB) return tile_fn_beta<DT, MVA, MVB, false>(beta, batched);
     }
     if constexpr (MVA != MVB && MS > 1) {
-        if (va == MS && vb == MS) return tile_fn_beta<DT, MS, MS, false>(beta);
+        if (va == MS && vb == MS) return tile_fn_beta<DT, MS, MS, false>(beta, batched);
     }
     if constexpr (MVA > 1) {
-        if (va == MVA && vb == 1) return tile_fn_beta<DT, MVA, 1, false>(beta);
+        if (va == MVA && vb == 1) return tile_fn_beta<DT, MVA, 1, false>(beta, batched);
     }
     if constexpr (MVB > 1) {
-        if (va == 1 && vb == MVB) return tile_fn_beta<DT, 1, MVB, false>(beta);
+        if (va == 1 && vb == MVB) return tile_fn_beta<DT, 1, MVB, false>(beta, batched);
     }
-    if (va == 1 && vb == 1) return tile_fn_beta<DT, 1, 1, false>(beta);
+    if (va == 1 && vb == 1) return tile_fn_beta<DT, 1, 1, false>(beta, batched);
     return nullptr;
 }
 
 template <int DT, int V>
-static DirectFn direct_fn_v(bool beta, bool idx64) {
-    if (beta) return idx64 ? (DirectFn)direct_kernel<DT, V, true, true> : (DirectFn)direct_kernel<DT, V, true, false>;
-    return idx64 ? (DirectFn)direct_kernel<DT, V, false, true> : (DirectFn)direct_kernel<DT, V, false, false>;
+static KernelFn direct_fn_v(bool beta, bool idx64, bool batched) {
+    if (batched) {
+        if (beta) return idx64 ? (KernelFn)direct_kernel<DT, V, true, true, BatchPtrs> : (KernelFn)direct_kernel<DT, V, true, false, BatchPtrs>;
+        return idx64 ? (KernelFn)direct_kernel<DT, V, false, true, BatchPtrs> : (KernelFn)direct_kernel<DT, V, false, false, BatchPtrs>;
+    }
+    if (beta) return idx64 ? (KernelFn)direct_kernel<DT, V, true, true, NoBatch> : (KernelFn)direct_kernel<DT, V, true, false, NoBatch>;
+    return idx64 ? (KernelFn)direct_kernel<DT, V, false, true, NoBatch> : (KernelFn)direct_kernel<DT, V, false, false, NoBatch>;
 }
 
 template <int DT>
-static DirectFn direct_fn(int vec, bool beta, bool idx64) {
+static KernelFn direct_fn(int vec, bool beta, bool idx64, bool batched) {
     constexpr int MV = max_vec_of<DT>();
     if constexpr (MV > 1) {
-        if (vec == MV) return direct_fn_v<DT, MV>(beta, idx64);
+        if (vec == MV) return direct_fn_v<DT, MV>(beta, idx64, batched);
     }
-    if (vec == 1) return direct_fn_v<DT, 1>(beta, idx64);
+    if (vec == 1) return direct_fn_v<DT, 1>(beta, idx64, batched);
     return nullptr;
+}
+
+template <int DT, int VB, bool PEEL, bool SHIFT>
+static KernelFn ring_fn_inst(bool beta, bool batched) {
+    if (batched)
+        return beta ? (KernelFn)ring_kernel<DT, VB, true, PEEL, SHIFT, BatchPtrs> : (KernelFn)ring_kernel<DT, VB, false, PEEL, SHIFT, BatchPtrs>;
+    return beta ? (KernelFn)ring_kernel<DT, VB, true, PEEL, SHIFT, NoBatch> : (KernelFn)ring_kernel<DT, VB, false, PEEL, SHIFT, NoBatch>;
 }
 
 template <int DT>
-static TileFn ring_fn(int vb, bool beta, bool peel) {
+static KernelFn ring_fn(int vb, bool beta, bool peel, bool shift, bool batched) {
     constexpr int MV = 16 / ElemT<DT>::ES;
     constexpr bool kSameType = std::is_same<typename ElemT<DT>::T, typename ElemT<DT>::TA>::value;
-    if constexpr (MV > 1 && kSameType) {   // the peeled store phase exists for same-type pairs only
-        if (vb == MV && peel) return beta ? (TileFn)ring_kernel<DT, MV, true, true> : (TileFn)ring_kernel<DT, MV, false, true>;
+    // the peeled store phase and the shifted rows exist for same-type pairs of 4- and 8-byte elements only
+    if constexpr (MV > 1 && kSameType) {
+        if (vb == MV && peel) return shift ? ring_fn_inst<DT, MV, true, true>(beta, batched) : ring_fn_inst<DT, MV, true, false>(beta, batched);
+        if (vb == MV && shift) return ring_fn_inst<DT, MV, false, true>(beta, batched);
+        if (vb == 1 && shift && !peel) return ring_fn_inst<DT, 1, false, true>(beta, batched);
     }
+    if (peel || shift) return nullptr;
     if constexpr (MV > 1) {
-        if (vb == MV && !peel) return beta ? (TileFn)ring_kernel<DT, MV, true, false> : (TileFn)ring_kernel<DT, MV, false, false>;
+        if (vb == MV) return ring_fn_inst<DT, MV, false, false>(beta, batched);
     }
-    if (vb == 1 && !peel) return beta ? (TileFn)ring_kernel<DT, 1, true, false> : (TileFn)ring_kernel<DT, 1, false, false>;
+    if (vb == 1) return ring_fn_inst<DT, 1, false, false>(beta, batched);
     return nullptr;
 }
 
-static TileFn get_tile_fn(int dt, const Candidate& c) {
+static KernelFn get_tile_fn(int dt, const Candidate& c, bool batched) {
     const TileParams& p = c.tp;
-    if (p.ring > 0) {   // mixed pairs: no peeled store phase (the planner builds none)
-        if (dt > TTC_C128 && p.peel) return nullptr;
+    if (p.ring > 0) {
+        const bool peel = p.peel != 0, shift = p.row_async == 2;
         switch (dt) {
-            case kPairSD: return ring_fn<kPairSD>(p.vecB, c.beta_nz, false);
-            case kPairDS: return ring_fn<kPairDS>(p.vecB, c.beta_nz, false);
-            case kPairCZ: return ring_fn<kPairCZ>(p.vecB, c.beta_nz, false);
-            case kPairZC: return ring_fn<kPairZC>(p.vecB, c.beta_nz, false);
-            case TTC_F32: return ring_fn<TTC_F32>(p.vecB, c.beta_nz, p.peel != 0);
-            case TTC_F64: return ring_fn<TTC_F64>(p.vecB, c.beta_nz, p.peel != 0);
-            case TTC_C64: return ring_fn<TTC_C64>(p.vecB, c.beta_nz, p.peel != 0);
-            case TTC_C128: return ring_fn<TTC_C128>(p.vecB, c.beta_nz, p.peel != 0);
+            case kPairSD: return ring_fn<kPairSD>(p.vecB, c.beta_nz, peel, shift, batched);
+            case kPairDS: return ring_fn<kPairDS>(p.vecB, c.beta_nz, peel, shift, batched);
+            case kPairCZ: return ring_fn<kPairCZ>(p.vecB, c.beta_nz, peel, shift, batched);
+            case kPairZC: return ring_fn<kPairZC>(p.vecB, c.beta_nz, peel, shift, batched);
+            case TTC_F32: return ring_fn<TTC_F32>(p.vecB, c.beta_nz, peel, shift, batched);
+            case TTC_F64: return ring_fn<TTC_F64>(p.vecB, c.beta_nz, peel, shift, batched);
+            case TTC_C64: return ring_fn<TTC_C64>(p.vecB, c.beta_nz, peel, shift, batched);
+            case TTC_C128: return ring_fn<TTC_C128>(p.vecB, c.beta_nz, peel, shift, batched);
         }
         return nullptr;
     }
     switch (dt) {
-        case TTC_F32: return tile_fn<TTC_F32>(p.vecA, p.vecB, p.same != 0, c.beta_nz);
-        case TTC_F64: return tile_fn<TTC_F64>(p.vecA, p.vecB, p.same != 0, c.beta_nz);
-        case TTC_C64: return tile_fn<TTC_C64>(p.vecA, p.vecB, p.same != 0, c.beta_nz);
-        case TTC_C128: return tile_fn<TTC_C128>(p.vecA, p.vecB, p.same != 0, c.beta_nz);
-        case kPairSD: return tile_fn<kPairSD>(p.vecA, p.vecB, p.same != 0, c.beta_nz);
-        case kPairDS: return tile_fn<kPairDS>(p.vecA, p.vecB, p.same != 0, c.beta_nz);
-        case kPairCZ: return tile_fn<kPairCZ>(p.vecA, p.vecB, p.same != 0, c.beta_nz);
-        case kPairZC: return tile_fn<kPairZC>(p.vecA, p.vecB, p.same != 0, c.beta_nz);
+        case TTC_F32: return tile_fn<TTC_F32>(p.vecA, p.vecB, p.same != 0, c.beta_nz, batched);
+        case TTC_F64: return tile_fn<TTC_F64>(p.vecA, p.vecB, p.same != 0, c.beta_nz, batched);
+        case TTC_C64: return tile_fn<TTC_C64>(p.vecA, p.vecB, p.same != 0, c.beta_nz, batched);
+        case TTC_C128: return tile_fn<TTC_C128>(p.vecA, p.vecB, p.same != 0, c.beta_nz, batched);
+        case kPairSD: return tile_fn<kPairSD>(p.vecA, p.vecB, p.same != 0, c.beta_nz, batched);
+        case kPairDS: return tile_fn<kPairDS>(p.vecA, p.vecB, p.same != 0, c.beta_nz, batched);
+        case kPairCZ: return tile_fn<kPairCZ>(p.vecA, p.vecB, p.same != 0, c.beta_nz, batched);
+        case kPairZC: return tile_fn<kPairZC>(p.vecA, p.vecB, p.same != 0, c.beta_nz, batched);
     }
     return nullptr;
 }
 
-static DirectFn get_direct_fn(int dt, const Candidate& c) {
+static KernelFn get_direct_fn(int dt, const Candidate& c, bool batched) {
     switch (dt) {
-        case TTC_F32: return direct_fn<TTC_F32>(c.dp.vec, c.beta_nz, c.idx64);
-        case TTC_F64: return direct_fn<TTC_F64>(c.dp.vec, c.beta_nz, c.idx64);
-        case TTC_C64: return direct_fn<TTC_C64>(c.dp.vec, c.beta_nz, c.idx64);
-        case TTC_C128: return direct_fn<TTC_C128>(c.dp.vec, c.beta_nz, c.idx64);
-        case kPairSD: return direct_fn<kPairSD>(c.dp.vec, c.beta_nz, c.idx64);
-        case kPairDS: return direct_fn<kPairDS>(c.dp.vec, c.beta_nz, c.idx64);
-        case kPairCZ: return direct_fn<kPairCZ>(c.dp.vec, c.beta_nz, c.idx64);
-        case kPairZC: return direct_fn<kPairZC>(c.dp.vec, c.beta_nz, c.idx64);
+        case TTC_F32: return direct_fn<TTC_F32>(c.dp.vec, c.beta_nz, c.idx64, batched);
+        case TTC_F64: return direct_fn<TTC_F64>(c.dp.vec, c.beta_nz, c.idx64, batched);
+        case TTC_C64: return direct_fn<TTC_C64>(c.dp.vec, c.beta_nz, c.idx64, batched);
+        case TTC_C128: return direct_fn<TTC_C128>(c.dp.vec, c.beta_nz, c.idx64, batched);
+        case kPairSD: return direct_fn<kPairSD>(c.dp.vec, c.beta_nz, c.idx64, batched);
+        case kPairDS: return direct_fn<kPairDS>(c.dp.vec, c.beta_nz, c.idx64, batched);
+        case kPairCZ: return direct_fn<kPairCZ>(c.dp.vec, c.beta_nz, c.idx64, batched);
+        case kPairZC: return direct_fn<kPairZC>(c.dp.vec, c.beta_nz, c.idx64, batched);
     }
     return nullptr;
+}
+
+// Opt the instance in to the device's maximum of dynamic shared memory (the attribute belongs to the kernel
+// function, which many candidates share); returns that maximum less the kernel's static shared memory.
+static int raise_smem_limit(KernelFn fn, int* optin_out) {
+    int dev = 0, optin = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    if (e != cudaSuccess) return (int)e;
+    cudaFuncAttributes fa;
+    e = cudaFuncGetAttributes(&fa, fn);
+    if (e != cudaSuccess) return (int)e;
+    optin -= (int)fa.sharedSizeBytes;   // the scheduler's mbarrier and response are static shared memory
+    e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+    *optin_out = optin;
+    return (int)e;
 }
 
 int prepare_candidate(Candidate* cand, ttc_dtype dtype, ttc_dtype dtype_a, int sm_count) {
     const int pair = pair_id(dtype, dtype_a);
     if (pair < 0) return (int)cudaErrorInvalidValue;
     if (cand->info.kernel == TTC_KERNEL_COPY) {
-        DirectFn fn = get_direct_fn(pair, *cand);
+        KernelFn fn = get_direct_fn(pair, *cand, false);
         if (!fn) return (int)cudaErrorInvalidValue;
         int occ = 0;
         cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kDirectThreads, 0);
@@ -1143,25 +1189,16 @@ int prepare_candidate(Candidate* cand, ttc_dtype dtype, ttc_dtype dtype_a, int s
         cand->grid_cap = (int)cap;
         return 0;
     }
-    TileFn fn = get_tile_fn(pair, *cand);
+    KernelFn fn = get_tile_fn(pair, *cand, false);
     if (!fn) return (int)cudaErrorInvalidValue;
     // the ring kernel's tile holds A's type (bulk copies), the tile kernel's B's
     const int smem = (int)tile_smem_layout(cand->tp, elem_size(cand->tp.ring > 0 ? dtype_a : dtype)).total;
-    // The attribute belongs to the kernel function, which many candidates share: raise it once
-    // to the device's opt-in maximum instead of per candidate.
-    int dev = 0, optin = 0;
-    cudaError_t e = cudaGetDevice(&dev);
-    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-    if (e != cudaSuccess) return (int)e;
-    cudaFuncAttributes fa;
-    e = cudaFuncGetAttributes(&fa, fn);
-    if (e != cudaSuccess) return (int)e;
-    optin -= (int)fa.sharedSizeBytes;   // the scheduler's mbarrier and response are static shared memory
+    int optin = 0;
+    int rc = raise_smem_limit(fn, &optin);
+    if (rc != 0) return rc;
     if (smem > optin) return (int)cudaErrorInvalidConfiguration;
-    e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
-    if (e != cudaSuccess) return (int)e;
     int occ = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, cand->tp.threads, smem);
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, cand->tp.threads, smem);
     if (e != cudaSuccess) return (int)e;
     if (occ < 1) return (int)cudaErrorInvalidConfiguration;
     const uint64_t cap = (uint64_t)sm_count * (uint64_t)occ;
@@ -1179,15 +1216,14 @@ int launch_candidate(const Candidate& cand, ttc_dtype dtype, ttc_dtype dtype_a, 
     const int pair = pair_id(dtype, dtype_a);
     if (pair < 0) return (int)cudaErrorInvalidValue;
     if (cand.info.grid <= 0) return (int)cudaErrorInvalidConfiguration;
-    // cudaLaunchKernelEx returns the launch error itself: the caller's CUDA error state is not
+    // cudaLaunchKernelExC returns the launch error itself: the caller's CUDA error state is not
     // read (no cudaGetLastError, which would clear errors that are not ours).
     cudaLaunchConfig_t cfg{};
     cfg.stream = st;
-    static const BatchPtrs kNoBatch{};
-    const BatchPtrs& bt = batch ? *batch : kNoBatch;
+    const bool batched = batch != nullptr && batch->n > 0;
     uint64_t grid = (uint64_t)cand.info.grid;
-    if (bt.n > 0) {     // one CTA per work item (launch control) or as many as the device holds
-        const uint64_t work = (uint64_t)bt.per * (uint64_t)bt.n;
+    if (batched) {     // one CTA per work item (launch control) or as many as the device holds
+        const uint64_t work = (uint64_t)batch->per * (uint64_t)batch->n;
         const int dyn_b = cand.info.kernel == TTC_KERNEL_COPY ? cand.dp.dyn : cand.tp.dyn;
         grid = (dyn_b == 1 || work < (uint64_t)cand.grid_cap) ? work : (uint64_t)cand.grid_cap;
         if (grid >= (1ull << 31)) return (int)cudaErrorInvalidConfiguration;
@@ -1209,22 +1245,38 @@ int launch_candidate(const Candidate& cand, ttc_dtype dtype, ttc_dtype dtype_a, 
         cfg.attrs = attr;
         cfg.numAttrs = 1;
     }
+    NoBatch none;
+    Scalar al = alpha, be = beta;
+    void* args[6] = {nullptr, (void*)&A, (void*)&B, (void*)&al, (void*)&be, batched ? (void*)batch : (void*)&none};
     if (cand.info.kernel == TTC_KERNEL_COPY) {
-        DirectFn fn = get_direct_fn(pair, cand);
+        KernelFn fn = get_direct_fn(pair, cand, batched);
         if (!fn) return (int)cudaErrorInvalidValue;
         cfg.blockDim = dim3(kDirectThreads, 1, 1);
         cfg.dynamicSmemBytes = 0;
         DirectParams dp = cand.dp;
         dp.ctr = sched_ctr;
-        return (int)cudaLaunchKernelEx(&cfg, fn, dp, A, B, alpha, beta, bt);
+        args[0] = &dp;
+        return (int)cudaLaunchKernelExC(&cfg, fn, args);
     }
-    TileFn fn = get_tile_fn(pair, cand);
+    KernelFn fn = get_tile_fn(pair, cand, batched);
     if (!fn) return (int)cudaErrorInvalidValue;
+    if (batched) {      // the batched twin of the instance has its own shared-memory attribute: set it once
+        static std::mutex mu;
+        static std::set<KernelFn> raised;
+        std::lock_guard<std::mutex> lk(mu);
+        if (!raised.count(fn)) {
+            int optin = 0;
+            const int rc = raise_smem_limit(fn, &optin);
+            if (rc != 0) return rc;
+            raised.insert(fn);
+        }
+    }
     cfg.blockDim = dim3((unsigned)cand.tp.threads, 1, 1);
     cfg.dynamicSmemBytes = (size_t)cand.info.smem_bytes;
     TileParams tp = cand.tp;
     tp.ctr = sched_ctr;
-    return (int)cudaLaunchKernelEx(&cfg, fn, tp, A, B, alpha, beta, bt);
+    args[0] = &tp;
+    return (int)cudaLaunchKernelExC(&cfg, fn, args);
 }
 
 }  // namespace ttc

@@ -862,7 +862,7 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, boo
     }
     // Second pass: the head of the list (what the tuner times by default) gets the full shared-memory padding
     // search of the bank model; the tail keeps its dense tiles (still complete, launchable candidates).
-    const int n_full = std::min<int>((int)out->size(), kFullSearch);
+    const int n_full = std::min<int>((int)out->size(), std::getenv("TTC_FULL_SEARCH") ? std::atoi(std::getenv("TTC_FULL_SEARCH")) : kFullSearch);
     for (int i = 0; i < n_full; ++i) {
         Candidate& cd = (*out)[i];
         if (cd.info.kernel == TTC_KERNEL_COPY) continue;
