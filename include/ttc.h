@@ -160,6 +160,19 @@ ttc_plan_t ttc_plan(ttc_dtype dtype, int N, const int64_t* sizes, const int* per
 ttc_plan_t ttc_plan_mixed(ttc_dtype dtype_a, ttc_dtype dtype_b, int N, const int64_t* sizes,
                           const int* perm, const int64_t* lda, const int64_t* ldb);
 
+/*
+ * ttc_plan_strided -- ttc_plan_mixed for tensors described by explicit ELEMENT STRIDES instead of leading
+ * dimensions (an extension: the paper's interface has leading dimensions only, which cannot
+ * express an outer stride that is not a multiple of the inner ones -- BASELINE.json describes configs[3] by
+ * "outer stride 6208").  stride_a[k] is the stride of A's index k, stride_b[k] the stride of B's POSITION k
+ * (as ldb).  Every stride must be >= 1 and each tensor must be "nested": sorted by stride, each stride is at
+ * least the previous stride times the previous extent (so that no two elements of B share an address);
+ * otherwise NULL / TTC_ERR_BAD_LD.  A's indices need not be given in ascending stride.  dtype_a == dtype_b
+ * gives a same-type plan.  Everything else is as for ttc_plan.
+ */
+ttc_plan_t ttc_plan_strided(ttc_dtype dtype_a, ttc_dtype dtype_b, int N, const int64_t* sizes, const int* perm,
+                            const int64_t* stride_a, const int64_t* stride_b);
+
 /* Element type of A for this plan (equals ttc_info.dtype unless the plan came from
  * ttc_plan_mixed); -1 for a NULL plan. */
 int ttc_plan_dtype_a(ttc_plan_t plan);

@@ -48,6 +48,9 @@ def _load():
         lib.ttc_oracle_transpose_mixed.restype = ctypes.c_int
         lib.ttc_oracle_transpose_mixed.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, i64p, i32p, i64p, i64p,
                                                    ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+        lib.ttc_oracle_transpose_strided.restype = ctypes.c_int
+        lib.ttc_oracle_transpose_strided.argtypes = [ctypes.c_int, ctypes.c_int, i64p, i32p, i64p, i64p,
+                                                     ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
         lib.ttc_oracle_offsets.restype = ctypes.c_int
         lib.ttc_oracle_offsets.argtypes = [ctypes.c_int, i64p, i32p, i64p, i64p, i64p, i64p, i64p]
         lib.ttc_ref_omp_threads.restype = ctypes.c_int
@@ -102,6 +105,12 @@ def transpose_mixed(dtype_a: int, dtype_b: int, sizes, perm, lda, ldb, alpha, A:
         b.ctypes.data_as(ctypes.c_void_p), B.ctypes.data_as(ctypes.c_void_p))
     if rc != 0:
         raise ValueError("oracle rejected its arguments (code %d)" % rc)
+
+
+def transpose_strided(dtype: int, sizes, perm, stride_a, stride_b, alpha, A: np.ndarray, beta, B: np.ndarray) -> None:
+    """Eq. 1 on tensors given by explicit element strides: ``stride_a[k]`` of A's index k, ``stride_b[k]`` of
+    B's position k (optional extension).  The oracle of ``ttc_plan_strided``."""
+    _call(_load().ttc_oracle_transpose_strided, dtype, sizes, perm, stride_a, stride_b, alpha, A, beta, B)
 
 
 def transpose_batched(dtype: int, sizes, perm, lda, ldb, alpha, A_list, beta, B_list) -> None:

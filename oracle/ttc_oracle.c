@@ -291,6 +291,84 @@ int ttc_oracle_transpose_mixed(int dtype_a, int dtype_b, int N, const int64_t *s
     return 0;
 }
 
+/* Eq. 1 on tensors given by explicit element strides instead of leading dimensions (the
+ * optional extension of SURVEY.md 8(b): config 4 is described "with outer stride 6208"): sA[k] is the stride
+ * of A's index k, tB[k] the stride of B's position k.  Same loop, same arithmetic as ttc_oracle_transpose;
+ * only where the strides come from differs.  Same-type dtypes only.  Strides must be positive. */
+int ttc_oracle_transpose_strided(int dtype, int N, const int64_t *sizes, const int *perm,
+                                 const int64_t *sA, const int64_t *tB,
+                                 const void *alpha, const void *A, const void *beta, void *B)
+{
+    int64_t i[ORACLE_MAX_RANK];
+    int k, rc;
+    rc = check_args(dtype, N, sizes, perm, NULL, NULL);
+    if (rc) return rc;
+    if (!alpha || !beta || !sA || !tB) return -8;
+    for (k = 0; k < N; ++k)
+        if (sA[k] < 1 || tB[k] < 1) return -12;
+    for (k = 0; k < N; ++k)
+        if (sizes[k] == 0) return 0;
+    if (!A || !B) return -9;
+    for (k = 0; k < N; ++k) i[k] = 0;
+    if (dtype == ORACLE_F32 || dtype == ORACLE_F64) {
+        do {
+            OFFSETS();
+            if (dtype == ORACLE_F32) {
+                const float a = *(const float *)alpha, b = *(const float *)beta;
+                float t = a * ((const float *)A)[offA];
+                if (b == 0.0f) ((float *)B)[offB] = t;
+                else { float u = b * ((float *)B)[offB]; ((float *)B)[offB] = t + u; }
+            } else {
+                const double a = *(const double *)alpha, b = *(const double *)beta;
+                double t = a * ((const double *)A)[offA];
+                if (b == 0.0) ((double *)B)[offB] = t;
+                else { double u = b * ((double *)B)[offB]; ((double *)B)[offB] = t + u; }
+            }
+        } while (next_index(N, sizes, i));
+    } else if (dtype == ORACLE_C64) {
+        const float ar = ((const float *)alpha)[0], ai = ((const float *)alpha)[1];
+        const float br = ((const float *)beta)[0], bi = ((const float *)beta)[1];
+        const float *pa = (const float *)A;
+        float *pb = (float *)B;
+        do {
+            OFFSETS();
+            float xr = pa[2 * offA], xi = pa[2 * offA + 1];
+            float p0 = ar * xr, p1 = ai * xi, p2 = ar * xi, p3 = ai * xr;   /* A9 */
+            float tr = p0 - p1, ti = p2 + p3;
+            if (!(br == 0.0f && bi == 0.0f)) {
+                float yr = pb[2 * offB], yi = pb[2 * offB + 1];
+                float q0 = br * yr, q1 = bi * yi, q2 = br * yi, q3 = bi * yr;
+                float ur = q0 - q1, ui = q2 + q3;
+                tr = tr + ur;
+                ti = ti + ui;
+            }
+            pb[2 * offB] = tr;
+            pb[2 * offB + 1] = ti;
+        } while (next_index(N, sizes, i));
+    } else {
+        const double ar = ((const double *)alpha)[0], ai = ((const double *)alpha)[1];
+        const double br = ((const double *)beta)[0], bi = ((const double *)beta)[1];
+        const double *pa = (const double *)A;
+        double *pb = (double *)B;
+        do {
+            OFFSETS();
+            double xr = pa[2 * offA], xi = pa[2 * offA + 1];
+            double p0 = ar * xr, p1 = ai * xi, p2 = ar * xi, p3 = ai * xr;
+            double tr = p0 - p1, ti = p2 + p3;
+            if (!(br == 0.0 && bi == 0.0)) {
+                double yr = pb[2 * offB], yi = pb[2 * offB + 1];
+                double q0 = br * yr, q1 = bi * yi, q2 = br * yi, q3 = bi * yr;
+                double ur = q0 - q1, ui = q2 + q3;
+                tr = tr + ur;
+                ti = ti + ui;
+            }
+            pb[2 * offB] = tr;
+            pb[2 * offB + 1] = ti;
+        } while (next_index(N, sizes, i));
+    }
+    return 0;
+}
+
 /* Offsets of one logical element, exported so that tests can sample single outputs of a
  * full-size problem: element with A multi-index i[] lives at A[*offA_out] and goes to
  * B[*offB_out].  Same formulas as above (reading A1, A3, A4). */

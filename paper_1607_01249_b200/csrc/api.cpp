@@ -357,6 +357,22 @@ ttc_plan_t ttc_plan_mixed(ttc_dtype dtype_a, ttc_dtype dtype, int N, const int64
     return p;
 }
 
+ttc_plan_t ttc_plan_strided(ttc_dtype dtype_a, ttc_dtype dtype, int N, const int64_t* sizes, const int* perm,
+                            const int64_t* stride_a, const int64_t* stride_b) {
+    if ((int)dtype < 0 || (int)dtype > 3 || (int)dtype_a < 0 || (int)dtype_a > 3) { g_last_error = TTC_ERR_INVALID_ARG; return nullptr; }
+    if (!valid_pair(dtype_a, dtype)) { g_last_error = TTC_ERR_UNSUPPORTED; return nullptr; }
+    ttc_plan_s* p = new (std::nothrow) ttc_plan_s();
+    if (!p) { g_last_error = TTC_ERR_ALLOC; return nullptr; }
+    p->dtype = dtype;
+    p->dtype_a = dtype_a;
+    p->rank = N;
+    ttc_status st = canonicalize_strided(N, sizes, perm, stride_a, stride_b, &p->canon);
+    if (st != TTC_OK) { delete p; g_last_error = st; return nullptr; }
+    finish_plan(p);
+    g_last_error = TTC_OK;
+    return p;
+}
+
 }  // extern "C"
 
 // Stages 2-6 for an already canonical transposition (also used for the slabs of ttc_execute_host).

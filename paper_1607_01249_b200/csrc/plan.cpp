@@ -326,6 +326,7 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
     // table of the A side.  Edge tiles get shorter and fewer rows.
     int row_dims = 1;
     if (ring) {
+        if (c.d[A0].sA != 1) return false;     // bulk rows are contiguous runs of A's leading index
         if (same && (want_vb * es != 16 || mixed)) return false;
         if (mixed && (want_va * esA != 16 || (want_vb != mvB && want_vb != 1))) return false;   // instances: VB = mvB or 1
         if (want_va * esA != 16) {

@@ -75,6 +75,8 @@ struct Canon {
 
 ttc_status canonicalize(int N, const int64_t* sizes, const int* perm, const int64_t* lda,
                         const int64_t* ldb, Canon* out);
+ttc_status canonicalize_strided(int N, const int64_t* sizes, const int* perm, const int64_t* stride_a,
+                                const int64_t* stride_b, Canon* out);
 
 // ---------------------------------------------------------------------------------------
 // Kernel parameter blocks (passed by value as __grid_constant__).

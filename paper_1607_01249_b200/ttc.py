@@ -24,7 +24,7 @@ STATUS_NAMES = ["TTC_OK", "TTC_ERR_INVALID_ARG", "TTC_ERR_NOT_PERMUTATION", "TTC
 KERNEL_NAMES = {0: "none", 1: "copy", 2: "tile", 3: "gather", 4: "wide", 5: "tma"}
 NP_DTYPE = {TTC_F32: np.float32, TTC_F64: np.float64, TTC_C64: np.complex64, TTC_C128: np.complex128}
 
-EXPORTS = ["ttc_plan", "ttc_plan_mixed", "ttc_plan_dtype_a", "ttc_execute", "ttc_execute_batched", "ttc_execute_host", "ttc_destroy", "ttc_last_error",
+EXPORTS = ["ttc_plan", "ttc_plan_mixed", "ttc_plan_strided", "ttc_plan_dtype_a", "ttc_execute", "ttc_execute_batched", "ttc_execute_host", "ttc_destroy", "ttc_last_error",
            "ttc_status_string", "ttc_plan_info", "ttc_plan_num_candidates", "ttc_plan_candidate",
            "ttc_plan_candidate_features", "ttc_plan_select", "ttc_plan_tune", "ttc_canonicalize", "ttc_launch_count",
            "ttc_debug_fastdiv", "ttc_version", "ttc_release_host_staging"]
@@ -62,6 +62,8 @@ def _load() -> ctypes.CDLL:
     lib.ttc_plan.argtypes = [ctypes.c_int, ctypes.c_int, i64p, i32p, i64p, i64p]
     lib.ttc_plan_mixed.restype = vp
     lib.ttc_plan_mixed.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, i64p, i32p, i64p, i64p]
+    lib.ttc_plan_strided.restype = vp
+    lib.ttc_plan_strided.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, i64p, i32p, i64p, i64p]
     lib.ttc_plan_dtype_a.restype = ctypes.c_int
     lib.ttc_plan_dtype_a.argtypes = [vp]
     lib.ttc_execute.restype = ctypes.c_int
@@ -154,6 +156,15 @@ def ttc_plan_mixed(dtype_a: int, dtype_b: int, N: int, sizes, perm, lda=None, ld
                            _i64(lda), _i64(ldb))
     if not h:
         raise TTCError(lib.ttc_last_error(), "ttc_plan_mixed")
+    return h
+
+
+def ttc_plan_strided(dtype_a: int, dtype_b: int, N: int, sizes, perm, stride_a, stride_b) -> int:
+    """Plan from explicit element strides (stride_a per A-index, stride_b per B-position)."""
+    h = lib.ttc_plan_strided(int(dtype_a), int(dtype_b), int(N), _i64(sizes), _i32(perm) if perm is not None else None,
+                             _i64(stride_a), _i64(stride_b))
+    if not h:
+        raise TTCError(lib.ttc_last_error(), "ttc_plan_strided")
     return h
 
 

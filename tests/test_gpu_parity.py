@@ -392,3 +392,34 @@ def test_execute_host_slab_pipeline(beta_nz):
                 assert np.array_equal(bits(b_pin.numpy()), bits(want))
         finally:
             ttc.ttc_destroy(plan)
+
+
+@pytest.mark.parametrize("dtype", ALL_DTYPES)
+def test_plan_strided_parity(dtype):
+    """ttc_plan_strided against the strided oracle (pin P9s): outer strides no leading dimension can express, A
+    indices out of stride order, beta on and off; the tuned winner and every 6th candidate."""
+    rng = np.random.default_rng(61)
+    for sizes, perm, sa, sb in (((40, 12, 25), (0, 2, 1), (1, 40, 485), (1, 40, 1003)),
+                                ((33, 20, 14), (2, 0, 1), (21, 1, 700), (1, 15, 500)),
+                                ((16, 6, 10, 8), (3, 1, 0, 2), (1, 18, 110, 1111), (1, 9, 55, 900))):
+        szb = tuple(sizes[p] for p in perm)
+        span_a = 1 + sum((e - 1) * s for e, s in zip(sizes, sa))
+        span_b = 1 + sum((e - 1) * s for e, s in zip(szb, sb))
+        A = wl.uniform_values(wl.SEED_A, span_a, dtype)
+        B0 = wl.uniform_values(wl.SEED_B, span_b, dtype)
+        for beta_nz in (False, True):
+            alpha, beta = scalars(dtype, beta_nz)
+            want = B0.copy()
+            oracle.transpose_strided(dtype, sizes, perm, sa, sb, alpha, A, beta, want)
+            plan = ttc.ttc_plan_strided(dtype, dtype, len(sizes), sizes, perm, sa, sb)
+            try:
+                which = 1 if beta_nz else 0
+                n = ttc.ttc_plan_num_candidates(plan, which)
+                for i in [-1] + list(range(0, n, 6)):
+                    ttc.ttc_plan_select(plan, which, i)
+                    b_dev = torch.from_numpy(B0).cuda()
+                    ttc.ttc_execute(plan, alpha, torch.from_numpy(A).cuda(), beta, b_dev)
+                    torch.cuda.synchronize()
+                    assert np.array_equal(bits(b_dev.cpu().numpy()), bits(want)), (sizes, perm, i)
+            finally:
+                ttc.ttc_destroy(plan)

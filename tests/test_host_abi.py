@@ -225,3 +225,35 @@ def test_real_complex_pairs_are_unsupported(da, db):
     with pytest.raises(ttc.TTCError) as ei:
         ttc.ttc_plan_mixed(7, 0, 2, (4, 4), (1, 0))
     assert ttc.STATUS_NAMES[ei.value.status] == "TTC_ERR_INVALID_ARG"
+
+
+def test_plan_strided_canonical_form_and_errors():
+    """ttc_plan_strided (SURVEY.md 8(b) optional extension): same canonical form as the leading-dimension call
+    where both can describe the tensors; configs[3] by its raw outer stride; rejected layouts."""
+    p1 = ttc.ttc_plan(ttc.TTC_F64, 3, (8, 768, 4096), (0, 2, 1), (8, 776, 4096), None)
+    p2 = ttc.ttc_plan_strided(ttc.TTC_F64, ttc.TTC_F64, 3, (8, 768, 4096), (0, 2, 1), (1, 8, 6208), (1, 8, 8 * 4096))
+    i1, i2 = ttc.ttc_plan_info(p1), ttc.ttc_plan_info(p2)
+    assert i1.canon_rank == i2.canon_rank == 3
+    for k in range(3):
+        assert (i1.canon_extent[k], i1.canon_stride_a[k], i1.canon_stride_b[k]) == \
+               (i2.canon_extent[k], i2.canon_stride_a[k], i2.canon_stride_b[k])
+    assert (i1.span_a, i1.span_b) == (i2.span_a, i2.span_b)
+    ttc.ttc_destroy(p1)
+    ttc.ttc_destroy(p2)
+    # an outer stride that no leading dimension can express (6209 is not a multiple of 8); A indices out of order
+    p = ttc.ttc_plan_strided(ttc.TTC_F32, ttc.TTC_F32, 3, (8, 4, 5), (0, 2, 1), (1, 8, 6209), (1, 8, 40))
+    assert ttc.ttc_plan_info(p).canon_stride_a[2] == 6209
+    ttc.ttc_destroy(p)
+    p = ttc.ttc_plan_strided(ttc.TTC_F32, ttc.TTC_F32, 2, (6, 4), (1, 0), (5, 1), (1, 4))     # A is row-major: a pure copy
+    info = ttc.ttc_plan_info(p)
+    assert info.canon_rank == 2 and info.canon_stride_a[0] == 1 and info.canon_extent[0] == 4
+    ttc.ttc_destroy(p)
+    for sa, sb in (((1, 3), (1, 6)),        # A overlaps itself: stride 3 < extent 6
+                   ((1, 6), (1, 3)),        # B would be written twice
+                   ((0, 6), (1, 4)), ((1, 6), (1, -4))):
+        with pytest.raises(ttc.TTCError) as ei:
+            ttc.ttc_plan_strided(ttc.TTC_F32, ttc.TTC_F32, 2, (6, 4), (1, 0), sa, sb)
+        assert ei.value.status == 3          # TTC_ERR_BAD_LD
+    with pytest.raises(ttc.TTCError) as ei:
+        ttc.ttc_plan_strided(ttc.TTC_F32, ttc.TTC_C64, 2, (6, 4), (1, 0), (1, 6), (1, 4))
+    assert ei.value.status == 4              # TTC_ERR_UNSUPPORTED: not one of the paper's type pairs

@@ -332,6 +332,41 @@ def test_p9_numpy_transpose_high_rank(dtype, n):
             assert np.array_equal(gotL, L.astype(np.float64))
 
 
+# ------------------------------------------------------------- P9s: explicit strides
+@pytest.mark.parametrize("dtype", ALL_DTYPES)
+def test_p9s_strided_oracle_against_numpy_as_strided(dtype):
+    """``ttc_oracle_transpose_strided`` (explicit element strides; SURVEY.md 8(b) optional extension): A and B
+    are numpy ``as_strided`` views of flat buffers -- numpy does the addressing -- and the result must be
+    ``B_view = 2*transpose(A_view) - 3*B_view`` (small integers: exact).  Includes config 4's description, an
+    outer stride (6208-like) that is NOT a multiple of the inner ones, and A indices given out of stride order."""
+    from numpy.lib.stride_tricks import as_strided
+    rng = np.random.default_rng(99)
+    isz = np.dtype(NP[dtype]).itemsize
+    for sizes, perm, sa, sb in (((4, 3, 5), (0, 2, 1), (1, 4, 13), (1, 4, 20)),          # outer stride 13 = 4*3 + 1
+                                ((3, 4, 2), (1, 0, 2), (8, 1, 30), (1, 5, 17)),          # A's index 1 is the stride-1 one
+                                ((2, 3, 2, 2), (3, 1, 0, 2), (1, 2, 7, 15), (1, 3, 10, 21))):
+        span_a = 1 + sum((e - 1) * s for e, s in zip(sizes, sa))
+        szb = sizes_b(sizes, perm)
+        span_b = 1 + sum((e - 1) * s for e, s in zip(szb, sb))
+        A = small_int_values(span_a, dtype, 7)
+        B = small_int_values(span_b, dtype, 8)
+        B0 = B.copy()
+        av = as_strided(A, shape=sizes, strides=[s * isz for s in sa])
+        want = B0.copy()
+        bv = as_strided(want, shape=szb, strides=[s * isz for s in sb])
+        bv[...] = 2 * np.transpose(av, perm) - 3 * bv
+        oracle.transpose_strided(dtype, sizes, perm, sa, sb, 2.0, A, -3.0, B)
+        assert np.array_equal(B, want)
+        # and it agrees with the leading-dimension oracle where both can describe the tensors
+    sizes, perm, lda, ldb = (3, 4, 5), (2, 0, 1), (4, 6, 5), (5, 3, 4)
+    A = small_int_values(4 * 6 * 5, dtype, 1)
+    B1 = small_int_values(5 * 3 * 4, dtype, 2)
+    B2 = B1.copy()
+    oracle.transpose(dtype, sizes, perm, lda, ldb, 2.0, A, -3.0, B1)
+    oracle.transpose_strided(dtype, sizes, perm, (1, 4, 24), (1, 5, 15), 2.0, A, -3.0, B2)
+    assert np.array_equal(B1, B2)
+
+
 # ------------------------------------------------------------- P10: linearity
 @pytest.mark.parametrize("dtype", ALL_DTYPES)
 def test_p10_linearity(dtype):
