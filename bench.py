@@ -232,6 +232,16 @@ def cold_block(torch, ttc, wl, peak, works, plans, a_dev, b_dev) -> dict:
         which = 1 if w.beta_nonzero else 0
         row["chosen"] = ttc.describe_candidate(ttc.ttc_plan_candidate(plan, which, info.chosen[which]), info.canon_rank)
         row["plan_ms"] = info.plan_ms
+        # the NVRTC size-specialised twin of the winner against the generic instance
+        t_sp = time.perf_counter()
+        st = ttc.ttc_plan_specialize(plan)
+        i2 = ttc.ttc_plan_info(plan)
+        row["specialize"] = {"status": ttc.STATUS_NAMES[st], "seconds": time.perf_counter() - t_sp,
+                             "generic_us": i2.generic_us[which], "specialized_us": i2.spec_us[which],
+                             "used": {0: "generic (no twin)", 1: "generic (twin slower)", 2: "specialised"}[i2.specialized[which]]}
+        if i2.specialized[which] == 2:
+            r2 = cold_row(torch, ttc, plan, w, w.algorithmic_bytes, w.alpha, w.beta, xa, xb, evict, peak)
+            row["specialize"]["gbs_median_cold"] = r2["read"]["gbs_median"]
         if w.name.startswith("c1"):      # small tensor (23.6 MB): also the warm, L2-resident figure
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             ts = []

@@ -38,6 +38,7 @@
  *   TTC_CACHE_FILE=path   solution store on disk (winners appended, reloaded by later processes)
  *   TTC_SCHED=static|both work distribution: persistent grid-stride instead of / beside the default,
  *                         dynamic distribution by cluster launch control
+ *   TTC_SPECIALIZE=1      ttc_plan also runs ttc_plan_specialize (NVRTC size-specialised winners)
  *   TTC_PDL=0             launch without programmatic dependent launch (default: with)
  *   TTC_RING=0|2|4        largest ring of tile buffers of the warp-specialised kernel (0: none; default 4)
  */
@@ -97,6 +98,9 @@ typedef struct {
                                              (skipped, never chosen; 0 on a healthy device)         */
     float    plan_ms;                     /* wall time ttc_plan spent building this plan (ms)      */
     float    tune_ms;                     /* the part of it spent timing candidates on the device  */
+    int      specialized[2];              /* 0: generic kernel; 1: a size-specialised twin exists but the generic
+                                             instance measured faster and is used; 2: the twin is used */
+    float    spec_us[2], generic_us[2];   /* their times from ttc_plan_specialize (0 if it was not run) */
 } ttc_info;
 
 #define TTC_CAND_STAGGERED 1   /* ring kernel: bank-conflict-free "staggered" gather from the tile      */
@@ -245,6 +249,20 @@ ttc_status ttc_plan_candidate(ttc_plan_t plan, int which, int index, ttc_candida
  * `python -m paper_1607_01249_b200.fit_cost` regresses measured times on when the heuristic is re-fitted
  * for another device (PAPER.md:141-143 leaves the cost function to the implementation). */
 ttc_status ttc_plan_candidate_features(ttc_plan_t plan, int which, int index, float* out16);
+/*
+ * ttc_plan_specialize -- re-compile the plan's two winners FOR THIS TRANSPOSITION (TTC generates
+ * and compiles code "for a specific size", the sizes being template parameters): NVRTC compiles the library's
+ * own kernel source with the winner's whole parameter block -- extents, strides, division constants, tile
+ * shape, table shapes -- as a compile-time constant, so that they become immediates and the loops over them
+ * unroll.  The twin is timed against the generic instance (interleaved, median of 5 x 4 launches on scratch
+ * buffers) and used by ttc_execute only if it is faster; ttc_info.specialized / spec_us / generic_us report the
+ * outcome.  Only warp-specialised (TTC_KERNEL_TMA) winners have a twin; ttc_execute_batched and misaligned
+ * pointers keep the generic kernels.  Costs about a second of compile time per winner (cubins are kept under
+ * <TTC_CACHE_FILE>.cubins/ when that variable is set); TTC_SPECIALIZE=1 makes ttc_plan call it.
+ * Returns TTC_ERR_UNSUPPORTED when libnvrtc cannot be loaded or no winner is specialisable -- the plan then
+ * simply keeps its generic kernels -- and TTC_ERR_CUDA / TTC_ERR_ALLOC on device trouble.
+ */
+ttc_status ttc_plan_specialize(ttc_plan_t plan);
 /* Force a candidate (tests, search-quality experiments).  index = -1 restores the winner. */
 ttc_status ttc_plan_select(ttc_plan_t plan, int which, int index);
 /*
@@ -271,6 +289,12 @@ int64_t ttc_launch_count(void);
  * returns n / d computed with the (multiplier, shift) pair the plan generator would build
  * for divisor d.  Valid for 0 <= n < 2^31, 1 <= d < 2^31. */
 uint32_t ttc_debug_fastdiv(uint32_t n, uint32_t d);
+
+/* Host-only self-check hook of the run-time specialisation: compiles (NVRTC, for sm_100a; no device needed) the
+ * specialised source of candidate `index` of list `which`; returns the cubin's size in bytes, -2 if the candidate
+ * has no specialisable instance (not a ring-kernel candidate), -3 if the compilation failed (`log` then holds the
+ * compiler's messages, truncated to log_len), -1 on bad arguments. */
+int64_t ttc_debug_specialize_compile(ttc_plan_t plan, int which, int index, char* log, int log_len);
 
 const char* ttc_version(void);
 

@@ -14,8 +14,9 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(ROOT, "include")
 LIB_PATH = os.path.join(HERE, "libttc.so")
-SOURCES = ["kernels.cu", "api.cpp", "plan.cpp", "canon.cpp"]
-HEADERS = [os.path.join(CSRC, "ttc_internal.h"), os.path.join(INCLUDE, "ttc.h")]
+SOURCES = ["kernels.cu", "api.cpp", "plan.cpp", "canon.cpp", "specialize.cpp"]
+HEADERS = [os.path.join(CSRC, "ttc_internal.h"), os.path.join(CSRC, "ttc_params.h"), os.path.join(CSRC, "ttc_device.cuh"),
+           os.path.join(INCLUDE, "ttc.h")]
 # Never -use_fast_math: it would flush denormals and contract roundings (reading A10).
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-I" + INCLUDE, "-I" + CSRC]
@@ -28,6 +29,25 @@ def _nvcc() -> str:
     return "nvcc"
 
 
+def _embed_device_source(objdir: str) -> str:
+    """The device code as a string constant of the library (specialize.cpp hands it to NVRTC): ttc_params.h, a
+    marker line, ttc_device.cuh -- without the #pragma once / #include lines that tie them together as files."""
+    def text(name):
+        with open(os.path.join(CSRC, name)) as fh:
+            return "".join(ln for ln in fh if not ln.startswith("#pragma once") and not ln.startswith('#include "ttc_params.h"'))
+    body = text("ttc_params.h") + "//@@TTC_DEVICE_CODE@@\n" + text("ttc_device.cuh")
+    assert ')TTCSRC"' not in body
+    out = os.path.join(objdir, "device_source.cpp")
+    chunks = [body[i:i + 8000] for i in range(0, len(body), 8000)]       # string literals of moderate length
+    code = "namespace ttc {\nextern const char* const kDeviceSource;\nconst char* const kDeviceSource =\n" + \
+        "\n".join('R"TTCSRC(' + c + ')TTCSRC"' for c in chunks) + ";\n}\n"
+    old = open(out).read() if os.path.exists(out) else None
+    if old != code:
+        with open(out, "w") as fh:
+            fh.write(code)
+    return out
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     srcs = [os.path.join(CSRC, s) for s in SOURCES]
     newest = max(os.path.getmtime(p) for p in srcs + HEADERS + [os.path.abspath(__file__)])
@@ -35,11 +55,15 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB_PATH
     objdir = os.path.join(HERE, "build")
     os.makedirs(objdir, exist_ok=True)
+    srcs = srcs + [_embed_device_source(objdir)]
     objs = []
     procs = []
+    hdr_time = max(os.path.getmtime(p) for p in HEADERS + [os.path.abspath(__file__)])
     for s in srcs:
         o = os.path.join(objdir, os.path.basename(s) + ".o")
         objs.append(o)
+        if not force and os.path.exists(o) and os.path.getmtime(o) >= max(os.path.getmtime(s), hdr_time):
+            continue                      # object is newer than its source and every header
         cmd = [_nvcc(), *NVCC_FLAGS, "-c", s, "-o", o]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
@@ -49,7 +73,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
             raise RuntimeError("nvcc failed: " + " ".join(cmd))
     tmp = LIB_PATH + ".tmp.%d" % os.getpid()
     subprocess.check_call([_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", tmp, *objs,
-                           "-cudart", "static"])
+                           "-cudart", "static", "-ldl"])
     os.replace(tmp, LIB_PATH)
     return LIB_PATH
 

@@ -32,6 +32,10 @@ struct ttc_plan_s {
     bool have_device = false;
     int sm_count = 148;
     int max_smem = 227 * 1024;
+    SpecKernel* spec[2] = {nullptr, nullptr};   // NVRTC size-specialised twin of candidate spec_idx[w] (ttc_plan_specialize)
+    int spec_idx[2] = {-1, -1};
+    bool spec_active[2] = {false, false};       // the twin measured faster than the generic instance and is launched
+    float spec_us[2] = {0.f, 0.f}, generic_us[2] = {0.f, 0.f};
     uint32_t* sched_ctr = nullptr;     // device counter of the atomic work distribution (TTC_SCHED=atomic)
     int tune_errors = 0;               // candidates that could not be prepared or launched while tuning
     float plan_ms = 0.f, tune_ms = 0.f;  // wall time of building the plan / of timing candidates inside it
@@ -435,6 +439,7 @@ static void finish_plan(ttc_plan_s* p) {
             g_cache[key] = e;
             disk_store(key, e);
         }
+        if (env_int("TTC_SPECIALIZE", 0) != 0) ttc_plan_specialize(p);
     }
 }
 
@@ -454,6 +459,11 @@ ttc_status ttc_execute(ttc_plan_t p, const void* alpha, const void* A, const voi
     if (idx < 0) return TTC_ERR_MISALIGNED;
     const Candidate* c = &p->cands[which][idx];
     if (!ensure_prepared(p, which, idx)) return TTC_ERR_CUDA;
+    if (p->spec_active[which] && idx == p->spec_idx[which] && p->forced[which] < 0) {
+        const int rs = launch_specialized(p->spec[which], *c, to_scalar(p->dtype, alpha), to_scalar(p->dtype, beta), A, B, cuda_stream);
+        g_launches += 1;
+        return rs == 0 ? TTC_OK : TTC_ERR_CUDA;
+    }
     const int rc = launch_candidate(*c, p->dtype, p->dtype_a, to_scalar(p->dtype, alpha), to_scalar(p->dtype, beta), A, B, cuda_stream, p->sched_ctr);
     g_launches += 1;
     return rc == 0 ? TTC_OK : TTC_ERR_CUDA;
@@ -605,6 +615,7 @@ ttc_status ttc_execute_host(ttc_plan_t p, const void* alpha, const void* A_host,
 
 ttc_status ttc_destroy(ttc_plan_t p) {
     if (!p) return TTC_OK;
+    for (int w = 0; w < 2; ++w) release_specialized(p->spec[w]);
     if (p->sched_ctr) cudaFree(p->sched_ctr);
     if (p->pipe_sub) ttc_destroy(p->pipe_sub);
     if (p->pipe_in) cudaStreamDestroy(p->pipe_in);
@@ -645,6 +656,11 @@ ttc_status ttc_plan_info(ttc_plan_t p, ttc_info* out) {
     out->span_a = p->canon.spanA;
     out->span_b = p->canon.spanB;
     out->tuned = p->tuned ? 1 : 0;
+    for (int w = 0; w < 2; ++w) {
+        out->specialized[w] = p->spec[w] ? (p->spec_active[w] ? 2 : 1) : 0;
+        out->spec_us[w] = p->spec_us[w];
+        out->generic_us[w] = p->generic_us[w];
+    }
     out->tune_errors = p->tune_errors;
     out->plan_ms = p->plan_ms;
     out->tune_ms = p->tune_ms;
@@ -674,6 +690,78 @@ ttc_status ttc_plan_candidate_features(ttc_plan_t p, int which, int index, float
     if (index < 0 || index >= (int)p->cands[which].size()) return TTC_ERR_INVALID_ARG;
     std::memcpy(out16, p->cands[which][index].feat, sizeof(float) * 16);
     return TTC_OK;
+}
+
+int64_t ttc_debug_specialize_compile(ttc_plan_t p, int which, int index, char* log, int log_len) {
+    if (!p || which < 0 || which > 1 || index < 0 || index >= (int)p->cands[which].size()) return -1;
+    std::string name, cubin, lowered, msg;
+    const std::string src = spec_source(p->cands[which][index], pair_id(p->dtype, p->dtype_a), &name);
+    if (src.empty()) return -2;
+    const bool ok = nvrtc_compile(src, name, "sm_100a", &cubin, &lowered, &msg);
+    if (log && log_len > 0) { std::strncpy(log, msg.c_str(), (size_t)log_len - 1); log[log_len - 1] = 0; }
+    return ok ? (int64_t)cubin.size() : -3;
+}
+
+ttc_status ttc_plan_specialize(ttc_plan_t p) {
+    if (!p) return TTC_ERR_INVALID_ARG;
+    if (!p->have_device) return TTC_ERR_CUDA;
+    if (p->canon.empty) return TTC_OK;
+    if (!nvrtc_available()) return TTC_ERR_UNSUPPORTED;
+    const int pair = pair_id(p->dtype, p->dtype_a);
+    const size_t es = (size_t)elem_size(p->dtype), esA = (size_t)elem_size(p->dtype_a);
+    void *a = nullptr, *b = nullptr;
+    if (cudaMalloc(&a, (size_t)p->canon.spanA * esA) != cudaSuccess) { cudaGetLastError(); return TTC_ERR_ALLOC; }
+    if (cudaMalloc(&b, (size_t)p->canon.spanB * es) != cudaSuccess) { cudaGetLastError(); cudaFree(a); return TTC_ERR_ALLOC; }
+    cudaMemset(a, 0, (size_t)p->canon.spanA * esA);
+    cudaMemset(b, 0, (size_t)p->canon.spanB * es);
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    ttc_status rc = TTC_ERR_UNSUPPORTED;      // stays so if neither list's winner is a ring-kernel candidate
+    for (int which = 0; which < 2; ++which) {
+        const int idx = p->winner[which];
+        if (idx < 0) continue;
+        Candidate& c = p->cands[which][idx];
+        if (c.info.kernel != TTC_KERNEL_TMA || !ensure_prepared(p, which, idx)) continue;
+        if (p->spec[which]) { release_specialized(p->spec[which]); p->spec[which] = nullptr; p->spec_active[which] = false; }
+        std::string err;
+        SpecKernel* k = specialize_candidate(c, pair, &err);
+        if (!k) {
+            if (std::getenv("TTC_VERBOSE")) std::fprintf(stderr, "ttc_plan_specialize: %s\n", err.c_str());
+            continue;
+        }
+        // generic against specialised, interleaved: median of 5 groups of 4 launches each
+        const Scalar alpha{1.0, 0.0}, beta{which ? 1.0 : 0.0, 0.0};
+        float t[2][5];
+        bool ok = true;
+        for (int r = 0; r < 6 && ok; ++r)
+            for (int v = 0; v < 2 && ok; ++v) {
+                cudaEventRecord(e0, nullptr);
+                for (int i = 0; i < 4 && ok; ++i)
+                    ok = (v ? launch_specialized(k, c, alpha, beta, a, b, nullptr)
+                            : launch_candidate(c, p->dtype, p->dtype_a, alpha, beta, a, b, nullptr, p->sched_ctr)) == 0;
+                cudaEventRecord(e1, nullptr);
+                if (cudaEventSynchronize(e1) != cudaSuccess) ok = false;
+                float ms = 0.f;
+                cudaEventElapsedTime(&ms, e0, e1);
+                if (r > 0) t[v][r - 1] = ms * 250.f;      // us per launch; round 0 is the warm-up
+                g_launches += 4;
+            }
+        if (!ok) { cudaGetLastError(); release_specialized(k); continue; }
+        std::sort(t[0], t[0] + 5);
+        std::sort(t[1], t[1] + 5);
+        p->spec[which] = k;
+        p->spec_idx[which] = idx;
+        p->generic_us[which] = t[0][2];
+        p->spec_us[which] = t[1][2];
+        p->spec_active[which] = t[1][2] < t[0][2] || env_int("TTC_SPECIALIZE", 0) == 2;   // 2: use the twin whatever its time (tests)
+        rc = TTC_OK;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(a);
+    cudaFree(b);
+    return rc;
 }
 
 ttc_status ttc_plan_select(ttc_plan_t p, int which, int index) {

@@ -26,8 +26,8 @@ NP_DTYPE = {TTC_F32: np.float32, TTC_F64: np.float64, TTC_C64: np.complex64, TTC
 
 EXPORTS = ["ttc_plan", "ttc_plan_mixed", "ttc_plan_strided", "ttc_plan_dtype_a", "ttc_execute", "ttc_execute_batched", "ttc_execute_host", "ttc_destroy", "ttc_last_error",
            "ttc_status_string", "ttc_plan_info", "ttc_plan_num_candidates", "ttc_plan_candidate",
-           "ttc_plan_candidate_features", "ttc_plan_select", "ttc_plan_tune", "ttc_canonicalize", "ttc_launch_count",
-           "ttc_debug_fastdiv", "ttc_version", "ttc_release_host_staging"]
+           "ttc_plan_candidate_features", "ttc_plan_specialize", "ttc_plan_select", "ttc_plan_tune", "ttc_canonicalize", "ttc_launch_count",
+           "ttc_debug_fastdiv", "ttc_debug_specialize_compile", "ttc_version", "ttc_release_host_staging"]
 
 
 class ttc_info(ctypes.Structure):
@@ -38,7 +38,8 @@ class ttc_info(ctypes.Structure):
                 ("numel", ctypes.c_int64), ("span_a", ctypes.c_int64), ("span_b", ctypes.c_int64),
                 ("tuned", ctypes.c_int), ("n_candidates", ctypes.c_int * 2),
                 ("chosen", ctypes.c_int * 2), ("chosen_us", ctypes.c_float * 2),
-                ("tune_errors", ctypes.c_int), ("plan_ms", ctypes.c_float), ("tune_ms", ctypes.c_float)]
+                ("tune_errors", ctypes.c_int), ("plan_ms", ctypes.c_float), ("tune_ms", ctypes.c_float),
+                ("specialized", ctypes.c_int * 2), ("spec_us", ctypes.c_float * 2), ("generic_us", ctypes.c_float * 2)]
 
 
 class ttc_candidate_info(ctypes.Structure):
@@ -85,6 +86,8 @@ def _load() -> ctypes.CDLL:
     lib.ttc_plan_candidate.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ttc_candidate_info)]
     lib.ttc_plan_candidate_features.restype = ctypes.c_int
     lib.ttc_plan_candidate_features.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_float)]
+    lib.ttc_plan_specialize.restype = ctypes.c_int
+    lib.ttc_plan_specialize.argtypes = [vp]
     lib.ttc_plan_select.restype = ctypes.c_int
     lib.ttc_plan_select.argtypes = [vp, ctypes.c_int, ctypes.c_int]
     lib.ttc_plan_tune.restype = ctypes.c_int
@@ -95,6 +98,8 @@ def _load() -> ctypes.CDLL:
     lib.ttc_debug_fastdiv.restype = ctypes.c_uint32
     lib.ttc_debug_fastdiv.argtypes = [ctypes.c_uint32, ctypes.c_uint32]
     lib.ttc_version.restype = ctypes.c_char_p
+    lib.ttc_debug_specialize_compile.restype = ctypes.c_int64
+    lib.ttc_debug_specialize_compile.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.c_char_p, ctypes.c_int]
     lib.ttc_release_host_staging.restype = ctypes.c_int
     return lib
 
@@ -248,6 +253,12 @@ def ttc_plan_candidate_features(plan: int, which: int, index: int):
     return [float(x) for x in out]
 
 
+def ttc_plan_specialize(plan: int) -> int:
+    """NVRTC size-specialised twins of the plan's winners; returns the status (TTC_ERR_UNSUPPORTED = 4 when
+    libnvrtc is missing or no winner is specialisable: the plan keeps its generic kernels)."""
+    return int(lib.ttc_plan_specialize(plan))
+
+
 def ttc_plan_select(plan: int, which: int, index: int) -> None:
     rc = lib.ttc_plan_select(plan, which, index)
     if rc != TTC_OK:
@@ -274,6 +285,13 @@ def ttc_canonicalize(sizes, perm, lda=None, ldb=None):
 
 def ttc_launch_count() -> int:
     return int(lib.ttc_launch_count())
+
+
+def ttc_debug_specialize_compile(plan: int, which: int, index: int):
+    """(cubin bytes or negative code, compiler log) of the NVRTC-specialised source of one candidate (host only)."""
+    buf = ctypes.create_string_buffer(8192)
+    n = int(lib.ttc_debug_specialize_compile(plan, which, index, buf, len(buf)))
+    return n, buf.value.decode(errors="replace")
 
 
 def ttc_version() -> str:

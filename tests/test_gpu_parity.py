@@ -423,3 +423,34 @@ def test_plan_strided_parity(dtype):
                     assert np.array_equal(bits(b_dev.cpu().numpy()), bits(want)), (sizes, perm, i)
             finally:
                 ttc.ttc_destroy(plan)
+
+
+def test_size_specialised_kernels(monkeypatch):
+    """ttc_plan_specialize: the NVRTC twin of the tuned winner, forced into
+    use (TTC_SPECIALIZE=2), is bit-exact -- whole tiles, remainder tiles, shifted rows, beta on and off."""
+    monkeypatch.setenv("TTC_SPECIALIZE", "2")
+    ran = 0
+    for w in (wl.Workload("sp_c2", wl.F64, (96, 72, 16, 14), (1, 0, 3, 2), 1.0, 0.0),
+              wl.Workload("sp_edge", wl.F32, (100, 37, 44), (1, 2, 0), 1.5, 0.5, lda=(104, 40, 44)),
+              wl.Workload("sp_odd", wl.F32, (131, 9, 67), (2, 0, 1), 1.5, 0.5),
+              wl.Workload("sp_c5", wl.C64, (7, 24, 5, 10, 16), (4, 2, 0, 3, 1), 0.5 - 0.25j, 0.0),
+              wl.Workload("sp_c3", wl.F32, (24, 10, 8, 12, 10, 8), (5, 2, 0, 4, 1, 3), 1.5, 0.5)):
+        plan = ttc.ttc_plan(w.dtype, w.n, w.sizes, w.perm, w.lda, w.ldb)      # TTC_SPECIALIZE: specialised inside
+        try:
+            info = ttc.ttc_plan_info(plan)
+            which = 1 if w.beta_nonzero else 0
+            kernel = ttc.ttc_plan_candidate(plan, which, info.chosen[which]).kernel
+            if kernel == 5:
+                assert info.specialized[which] == 2, "winner is a ring candidate but has no active twin"
+                assert info.spec_us[which] > 0 and info.generic_us[which] > 0
+                ran += 1
+            else:
+                assert info.specialized[which] == 0
+            check_bit_exact(w, plan=plan)
+            check_bit_exact(w, plan=plan, b_init="nan" if not w.beta_nonzero else "auto")
+            # a forced candidate and misaligned pointers go through the generic kernels
+            check_bit_exact(w, plan=plan, candidate=info.chosen[which])
+            check_bit_exact(w, plan=plan, misalign_a=1, misalign_b=1)
+        finally:
+            ttc.ttc_destroy(plan)
+    assert ran >= 3

@@ -39,7 +39,7 @@ def test_versions_agree():
 
 def test_struct_layouts_match_header():
     """The ctypes mirrors must have the C sizes (int64 alignment included)."""
-    assert ctypes.sizeof(ttc.ttc_info) == 4 * 4 + 3 * 16 * 8 + 3 * 8 + 4 + 2 * 4 + 2 * 4 + 2 * 4 + 3 * 4
+    assert ctypes.sizeof(ttc.ttc_info) == 4 * 4 + 3 * 16 * 8 + 3 * 8 + 4 + 2 * 4 + 2 * 4 + 2 * 4 + 3 * 4 + 6 * 4
     assert ctypes.sizeof(ttc.ttc_candidate_info) % 8 == 0
 
 
@@ -257,3 +257,36 @@ def test_plan_strided_canonical_form_and_errors():
     with pytest.raises(ttc.TTCError) as ei:
         ttc.ttc_plan_strided(ttc.TTC_F32, ttc.TTC_C64, 2, (6, 4), (1, 0), (1, 6), (1, 4))
     assert ei.value.status == 4              # TTC_ERR_UNSUPPORTED: not one of the paper's type pairs
+
+
+def test_specialised_source_compiles_with_nvrtc():
+    """the size-specialised twin of a ring-kernel candidate -- the library's own device
+    source with the candidate's parameter block as a constexpr object -- compiles with NVRTC for sm_100a (no
+    device needed).  One candidate per flavour (plain, staggered, shifted rows, peeled) of three shapes."""
+    import ctypes.util
+    try:
+        ctypes.CDLL("libnvrtc.so.12")
+    except OSError:
+        if not os.path.exists("/usr/local/cuda/lib64/libnvrtc.so"):
+            pytest.skip("libnvrtc not installed: ttc_plan_specialize reports TTC_ERR_UNSUPPORTED and plans stay generic")
+    compiled = 0
+    for w in (wl.config2((1, 0, 2, 3)), wl.Workload("odd", wl.F32, (131, 9, 67), (2, 0, 1), 1.5, 0.5), wl.config5()):
+        p = ttc.ttc_plan(w.dtype, w.n, w.sizes, w.perm, w.lda, w.ldb)
+        try:
+            which = 1 if w.beta_nonzero else 0
+            seen = set()
+            for i in range(ttc.ttc_plan_num_candidates(p, which)):
+                c = ttc.ttc_plan_candidate(p, which, i)
+                key = (c.kernel, c.flags, c.vec_b > 1)
+                if key in seen:
+                    continue
+                seen.add(key)
+                n, log = ttc.ttc_debug_specialize_compile(p, which, i)
+                if c.kernel == 5:
+                    assert n > 1000, log
+                    compiled += 1
+                else:
+                    assert n == -2          # only warp-specialised candidates have a twin
+        finally:
+            ttc.ttc_destroy(p)
+    assert compiled >= 5
