@@ -463,6 +463,12 @@ def run_ours(args) -> None:
     t_plan0 = time.perf_counter()
     plans = [ttc.ttc_plan(w.dtype, w.n, w.sizes, w.perm) for w in works]      # tuned here, untimed
     plan_wall_s = time.perf_counter() - t_plan0
+    # TTC compiles code for the specific size.  The tuned winners are re-compiled by NVRTC with
+    # their parameter blocks as compile-time constants (untimed, once per transposition, like the tuning) and
+    # used where they measure faster than the generic instances.
+    t_sp0 = time.perf_counter()
+    spec_status = [ttc.ttc_plan_specialize(p) for p in plans] if not args.no_specialize else []
+    specialize_wall_s = time.perf_counter() - t_sp0
     A_host = works[0].make_a()
     a_dev = torch.from_numpy(A_host).cuda()
     b_dev = torch.zeros_like(a_dev)
@@ -562,6 +568,8 @@ def run_ours(args) -> None:
                          "frac_of_measured_copy": (w.algorithmic_bytes / us / 1e3 / peak) if us else None,
                          "plan_ms": info.plan_ms, "tune_ms": info.tune_ms, "tune_errors": info.tune_errors,
                          "n_candidates": info.n_candidates[0],
+                         "kernel_used": {0: "generic", 1: "generic (specialised twin slower)", 2: "size-specialised (NVRTC)"}[info.specialized[0]],
+                         "generic_us": info.generic_us[0], "specialized_us": info.spec_us[0],
                          "chosen": ttc.describe_candidate(cand, info.canon_rank)})
     roofline = None
     if ev:
@@ -669,6 +677,8 @@ def run_ours(args) -> None:
                 "per_config": cold["per_config"] if cold else None, "batched": batched,
                 "plan_ms": {"median": statistics.median(r["plan_ms"] for r in per_perm),
                             "max": max(r["plan_ms"] for r in per_perm), "total_wall_s": plan_wall_s,
+                            "specialize_total_wall_s": specialize_wall_s,
+                            "specialized_plans": sum(1 for r in per_perm if r["kernel_used"].startswith("size-")),
                             "note": "ttc_plan incl. on-device tuning of the beta=0 and beta!=0 lists; untimed, once per transposition"},
                 "cpu_baseline": cpu, "cpu_baseline_omp": cpu_omp, "e2e": e2e,
                 "gpu_launches": launches, "clocks": clocks}
@@ -690,6 +700,7 @@ def main() -> None:
     ap.add_argument("--profile-detail", action="store_true", help="with --detail: one extra launch of c1, c3, c4, c5 "
                     "inside a cudaProfilerStart/Stop range (for ncu --profile-from-start off)")
     ap.add_argument("--no-launch-events", action="store_true")
+    ap.add_argument("--no-specialize", action="store_true", help="keep the generic kernel instances (no NVRTC)")
     ap.add_argument("--no-graph", action="store_true", help="issue the 23 launches of a step on the stream instead of replaying a CUDA graph")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-cold", action="store_true", help="skip the cold-L2 block (profiling runs)")

@@ -722,7 +722,7 @@ ttc_status ttc_plan_specialize(ttc_plan_t p) {
         const int idx = p->winner[which];
         if (idx < 0) continue;
         Candidate& c = p->cands[which][idx];
-        if (c.info.kernel != TTC_KERNEL_TMA || !ensure_prepared(p, which, idx)) continue;
+        if ((c.info.kernel != TTC_KERNEL_TMA && c.info.kernel != TTC_KERNEL_COPY) || !ensure_prepared(p, which, idx)) continue;
         if (p->spec[which]) { release_specialized(p->spec[which]); p->spec[which] = nullptr; p->spec_active[which] = false; }
         std::string err;
         SpecKernel* k = specialize_candidate(c, pair, &err);

@@ -9,12 +9,21 @@
 // parameter block of ONE tuned ring-kernel candidate as a constexpr object; the kernel then has no
 // TileParams argument, loops over the parameter block are unrolled and every extent, stride, divisor and
 // tile shape folds into the instruction stream.
+// TTC_SPECIALIZED == 1: a ring-kernel candidate (kSpecP); == 2: a direct-kernel candidate (ttc::kSpecD).
 #if defined(TTC_SPECIALIZED)
-#define TTC_RING_PARAMS
 #define TTC_LOOP_P _Pragma("unroll")
 #else
-#define TTC_RING_PARAMS const __grid_constant__ TileParams P,
 #define TTC_LOOP_P _Pragma("unroll 1")
+#endif
+#if defined(TTC_SPECIALIZED) && TTC_SPECIALIZED == 1
+#define TTC_RING_PARAMS
+#else
+#define TTC_RING_PARAMS const __grid_constant__ TileParams P,
+#endif
+#if defined(TTC_SPECIALIZED) && TTC_SPECIALIZED == 2
+#define TTC_DIRECT_PARAMS
+#else
+#define TTC_DIRECT_PARAMS const __grid_constant__ DirectParams P,
 #endif
 
 namespace ttc {
@@ -233,8 +242,11 @@ __device__ __forceinline__ uint32_t batch_item(const BatchPtrs& Bt, uint32_t w, 
 
 template <int DT, int V, bool BETA, bool IDX64, typename BT>
 __global__ void __launch_bounds__(kDirectThreads)
-direct_kernel(const __grid_constant__ DirectParams P, const void* __restrict__ Ain, void* __restrict__ Bout,
+direct_kernel(TTC_DIRECT_PARAMS const void* __restrict__ Ain, void* __restrict__ Bout,
               const Scalar alpha_in, const Scalar beta_in, const __grid_constant__ BT Bt) {
+#if defined(TTC_SPECIALIZED) && TTC_SPECIALIZED == 2
+    constexpr const DirectParams& P = kSpecD;
+#endif
     using T = typename ElemT<DT>::T;
     TScal<T> alpha, beta;
     typed(alpha_in, alpha);
@@ -276,7 +288,7 @@ direct_kernel(const __grid_constant__ DirectParams P, const void* __restrict__ A
             ob[k] = 0;
         }
         // item -> offsets: the kDirectUnroll decompositions advance together (independent chains)
-#pragma unroll 1
+TTC_LOOP_P
         for (int d = 0; d < P.nd; ++d) {
             const eoff_t sA = (eoff_t)P.dims[d].sA, sB = (eoff_t)P.dims[d].sB;
 #pragma unroll
@@ -552,7 +564,7 @@ template <int DT, int VB, bool BETA, bool PEEL, bool SHIFT, typename BT>
 __global__ void __launch_bounds__(kRingThreads, (PEEL || (BETA && VB == 1 && SHIFT)) ? 3 : BETA ? 4 : 5)
 ring_kernel(TTC_RING_PARAMS const void* __restrict__ Ain, void* __restrict__ Bout,
             const Scalar alpha_in, const Scalar beta_in, const __grid_constant__ BT Bt) {
-#if defined(TTC_SPECIALIZED)
+#if defined(TTC_SPECIALIZED) && TTC_SPECIALIZED == 1
     constexpr const TileParams& P = kSpecP;    // the tuned candidate's parameter block, a compile-time constant
 #endif
     using T = typename ElemT<DT>::T;

@@ -434,14 +434,15 @@ def test_size_specialised_kernels(monkeypatch):
               wl.Workload("sp_edge", wl.F32, (100, 37, 44), (1, 2, 0), 1.5, 0.5, lda=(104, 40, 44)),
               wl.Workload("sp_odd", wl.F32, (131, 9, 67), (2, 0, 1), 1.5, 0.5),
               wl.Workload("sp_c5", wl.C64, (7, 24, 5, 10, 16), (4, 2, 0, 3, 1), 0.5 - 0.25j, 0.0),
+              wl.Workload("sp_copy", wl.F64, (96, 18, 16, 14), (0, 2, 1, 3), 1.5, 0.5),
               wl.Workload("sp_c3", wl.F32, (24, 10, 8, 12, 10, 8), (5, 2, 0, 4, 1, 3), 1.5, 0.5)):
         plan = ttc.ttc_plan(w.dtype, w.n, w.sizes, w.perm, w.lda, w.ldb)      # TTC_SPECIALIZE: specialised inside
         try:
             info = ttc.ttc_plan_info(plan)
             which = 1 if w.beta_nonzero else 0
             kernel = ttc.ttc_plan_candidate(plan, which, info.chosen[which]).kernel
-            if kernel == 5:
-                assert info.specialized[which] == 2, "winner is a ring candidate but has no active twin"
+            if kernel in (1, 5):
+                assert info.specialized[which] == 2, "winner is a ring / direct candidate but has no active twin"
                 assert info.spec_us[which] > 0 and info.generic_us[which] > 0
                 ran += 1
             else:
