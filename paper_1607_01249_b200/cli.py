@@ -38,6 +38,8 @@ def main(argv=None) -> dict:
     ap.add_argument("--list", type=int, default=0, help="also print the N fastest timed candidates")
     ap.add_argument("--select", type=int, default=None, help="force candidate index (of the list beta selects)")
     ap.add_argument("--profile", action="store_true")
+    ap.add_argument("--specialize", action="store_true",
+                    help="also re-compile the winner for this size (ttc_plan_specialize, NVRTC) and time it")
     args = ap.parse_args(argv)
     if args.maxImplementations is not None:
         import os
@@ -79,12 +81,35 @@ def main(argv=None) -> dict:
         torch.cuda.cudart().cudaProfilerStop()
     nbytes = numel * (ES[da] + (2 if which else 1) * ES[db])
     us = statistics.median(ts)
+    spec = None
+    if args.specialize:
+        st = ttc.ttc_plan_specialize(plan)
+        i2 = ttc.ttc_plan_info(plan)
+        spec = {"status": ttc.STATUS_NAMES[st], "used": i2.specialized[which], "generic_us": i2.generic_us[which],
+                "specialized_us": i2.spec_us[which]}
+        if i2.specialized[which] == 2:
+            t2 = []
+            for _ in range(args.reps):
+                evict.max()
+                e0.record()
+                ttc.ttc_execute(plan, args.alpha, a, args.beta, b)
+                e1.record()
+                e1.synchronize()
+                t2.append(e0.elapsed_time(e1) * 1e3)
+            spec["us_median"] = statistics.median(t2)
+            spec["GB/s"] = nbytes / spec["us_median"] / 1e3
+            if args.profile:             # second profiled launch: the specialised twin
+                torch.cuda.synchronize()
+                torch.cuda.cudart().cudaProfilerStart()
+                ttc.ttc_execute(plan, args.alpha, a, args.beta, b)
+                torch.cuda.synchronize()
+                torch.cuda.cudart().cudaProfilerStop()
     out = {"perm": perm, "size": sizes, "dataType": t, "alpha": args.alpha, "beta": args.beta, "lda": lda, "ldb": ldb,
            "canonical": [(info.canon_extent[i], info.canon_stride_a[i], info.canon_stride_b[i]) for i in range(info.canon_rank)],
            "candidates": info.n_candidates[which], "plan_ms": info.plan_ms, "tune_ms": info.tune_ms,
            "chosen_index": chosen, "chosen": ttc.describe_candidate(ttc.ttc_plan_candidate(plan, which, chosen), info.canon_rank),
            "us_min_of_3": min(ts[:3]), "us_median": us, "bytes": nbytes, "GB/s": nbytes / us / 1e3,
-           "GiB/s": nbytes / us / 1e3 * 1e9 / 2 ** 30}
+           "GiB/s": nbytes / us / 1e3 * 1e9 / 2 ** 30, "specialize": spec}
     print(json.dumps(out))
     if args.list:
         rows = []
