@@ -89,6 +89,7 @@ std::string cache_key(const ttc_plan_s* p) {
     if (const char* e = std::getenv("TTC_SCHED")) k.append(e);
     if (const char* e = std::getenv("TTC_RING")) { k.append("|ring"); k.append(e); }
     if (const char* e = std::getenv("TTC_VARIANTS")) { k.append("|var"); k.append(e); }
+    if (const char* e = std::getenv("TTC_LOOP_ORDERS")) { k.append("|lo"); k.append(e); }
     return k;
 }
 

@@ -463,8 +463,25 @@ bool build_tile_candidate(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bo
     int gslot_of[kMaxRank];
     int64_t n_tiles = 1;
     P.nG = c.rank;
+    // Orders 2 and 3 (TTC_LOOP_ORDERS=4; PAPER.md:137 explores all d! orders): the plane of the two leading
+    // indices first -- 2: A's leading index, then B's, then the rest by A-stride; 3: B's, then A's, then the
+    // rest by B-stride -- so that consecutive macro-tiles stay inside one 2-D slab of both tensors.
+    int order[kMaxRank];
+    for (int k = 0; k < c.rank; ++k) order[k] = (loop_order & 1) == 0 ? k : c.orderB[k];
+    if (loop_order >= 2) {
+        const int first = loop_order == 2 ? A0 : B0, second = loop_order == 2 ? B0 : A0;
+        if (first == second) return false;
+        int w = 0, tmp[kMaxRank];
+        tmp[w++] = first;
+        tmp[w++] = second;
+        for (int k = 0; k < c.rank; ++k)
+            if (order[k] != first && order[k] != second) tmp[w++] = order[k];
+        bool same_as_base = true;
+        for (int k = 0; k < c.rank; ++k) { same_as_base &= tmp[k] == order[k]; order[k] = tmp[k]; }
+        if (same_as_base) return false;       // nothing new
+    }
     for (int k = 0; k < c.rank; ++k) {
-        const int i = loop_order == 0 ? k : c.orderB[k];
+        const int i = order[k];
         if (c.d[i].e >= kInt31) return false;
         const int64_t nt = (c.d[i].e + spec.t[i] - 1) / spec.t[i];
         GridDim& g = P.g[k];
@@ -788,6 +805,7 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, boo
     // TTC_VARIANTS: bit 0 = staggered-gather ring candidates, bit 1 = shifted-row ring candidates (default: both)
     const int variants = std::getenv("TTC_VARIANTS") ? std::atoi(std::getenv("TTC_VARIANTS")) : 3;
     const int xp_max = (variants & 1) ? 1 : 0;
+    const int n_loop_orders = std::getenv("TTC_LOOP_ORDERS") ? std::max(2, std::min(4, std::atoi(std::getenv("TTC_LOOP_ORDERS")))) : 2;
     const int ring_max = std::getenv("TTC_RING") ? std::atoi(std::getenv("TTC_RING")) : 4;
 
     // K1 / fallback: direct kernels (always at least the scalar one, valid for any strides).
@@ -823,7 +841,7 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, boo
                 if (!seen.insert(key).second) continue;
                 // {8, 8}: mixed precision only -- one vector width (mvS elements) on both sides
                 static const int vopts[5][2] = {{16, 16}, {16, 1}, {1, 16}, {1, 1}, {8, 8}};
-                for (int lo = 0; lo < 2; ++lo) {
+                for (int lo = 0; lo < n_loop_orders; ++lo) {
                     for (auto& vo : vopts) {
                         const int va = vo[0] == 16 ? mvA : vo[0] == 8 ? mvS : 1, vb = vo[1] == 16 ? mvB : vo[1] == 8 ? mvS : 1;
                         if ((mvA == 1 && vo[0] == 16) || (mvB == 1 && vo[1] == 16)) continue;

@@ -306,4 +306,4 @@ def describe_candidate(c: ttc_candidate_info, rank: int) -> str:
     ext = "x".join(str(c.tile_ext[i]) for i in range(rank))
     return "%s%s tile=%s vec=%d/%d run=%d/%d loop=%s sched=%s smem=%d grid=%d cost=%.2f us=%.1f" % (
         KERNEL_NAMES.get(c.kernel, "?"), ("+stag" if c.flags & 1 else "") + ("+shift" if c.flags & 4 else ""), ext, c.vec_a, c.vec_b, c.tile_u, c.tile_w,
-        "AB"[c.loop_order], ("static", "dynamic", "atomic")[c.sched], c.smem_bytes, c.grid, c.est_cost, c.tuned_us)
+        "ABab"[c.loop_order], ("static", "dynamic", "atomic")[c.sched], c.smem_bytes, c.grid, c.est_cost, c.tuned_us)
