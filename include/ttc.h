@@ -38,6 +38,7 @@
  *   TTC_CACHE_FILE=path   solution store on disk (winners appended, reloaded by later processes)
  *   TTC_SCHED=static|both work distribution: persistent grid-stride instead of / beside the default,
  *                         dynamic distribution by cluster launch control
+ *   TTC_LOOP_ORDERS=4     also generate the two plane-first macro-tile orders (default 2: A-linear, B-linear)
  *   TTC_SPECIALIZE=1      ttc_plan also runs ttc_plan_specialize (NVRTC size-specialised winners)
  *   TTC_PDL=0             launch without programmatic dependent launch (default: with)
  *   TTC_RING=0|2|4        largest ring of tile buffers of the warp-specialised kernel (0: none; default 4)
