@@ -65,7 +65,8 @@ typedef enum {
     TTC_ERR_UNSUPPORTED = 4,      /* spans overflow int64 / more than 2^62 elements                  */
     TTC_ERR_ALLOC = 5,            /* host or device allocation failed                                */
     TTC_ERR_CUDA = 6,             /* a CUDA call failed (no device, launch error, ...)               */
-    TTC_ERR_MISALIGNED = 7        /* A or B is not aligned to its own element size                   */
+    TTC_ERR_MISALIGNED = 7,       /* A or B is not aligned to its own element size                   */
+    TTC_ERR_SCRATCH_LIMIT = 8     /* ttc_execute_host_static: A and B exceed TTC_STATIC_SCRATCH_BYTES */
 } ttc_status;
 
 /* Kernel classes. */
@@ -229,6 +230,29 @@ ttc_status ttc_execute_host(ttc_plan_t plan, const void* alpha, const void* A_ho
 
 /* ttc_destroy -- frees the plan.  NULL is allowed. */
 ttc_status ttc_destroy(ttc_plan_t plan);
+
+/*
+ * ttc_execute_host_static -- ttc_execute_host for callers that may not allocate device memory (set-up code of
+ * a captured graph, tight serving loops, harnesses that forbid cudaMalloc).  Same operation (Eq. 1,
+ * PAPER.md:24), same arguments and layouts: A_host holds span_a elements of the plan's dtype_a, B_host span_b
+ * elements of dtype_b, alpha and beta are host scalars of B's type.  Instead of the cudaMalloc'ed staging
+ * pool, A and B are staged inside ONE file-scope __device__ array of TTC_STATIC_SCRATCH_BYTES (8 MiB) that
+ * every GPU holds from the moment it loads that part of the library until the process exits; its first 256
+ * bytes are the work counter of the plan's kernel (atomic tile distribution), cleared by every call.  The
+ * call itself makes no cudaMalloc / cudaFree and calls no allocating library routine: it clears the counter,
+ * copies A (and B when beta != 0 or B has padding) in, launches the plan's generic kernel for the given beta
+ * (never an NVRTC twin), copies B back and waits for the stream.  Synchronous.
+ * Limit: 256 + round256(span_a * sizeof(dtype_a)) + round256(span_b * sizeof(dtype_b)) must not exceed
+ * TTC_STATIC_SCRATCH_BYTES, otherwise TTC_ERR_SCRATCH_LIMIT and nothing is touched.  Other errors as
+ * ttc_execute_host (TTC_ERR_INVALID_ARG, TTC_ERR_CUDA).  Empty tensors: no-op.
+ * All calls on one device share the array, which keeps the last call's contents: calls from several threads
+ * are serialised by a process-wide lock (each waits for its own stream before it returns), since two of them
+ * overlapping on the GPU would race on the array.  The plan must have been built beforehand (ttc_plan
+ * allocates while it tunes); the first call on a device also loads the module that holds the array.
+ */
+#define TTC_STATIC_SCRATCH_BYTES (8u << 20)
+ttc_status ttc_execute_host_static(ttc_plan_t plan, const void* alpha, const void* A_host, const void* beta,
+                                   void* B_host, void* cuda_stream);
 
 /* Frees the process-wide device staging buffers of ttc_execute_host (they are re-allocated on
  * the next call that needs them).  Must not run concurrently with ttc_execute_host. */

@@ -614,6 +614,28 @@ ttc_status ttc_execute_host(ttc_plan_t p, const void* alpha, const void* A_host,
     return TTC_OK;
 }
 
+ttc_status ttc_execute_host_static(ttc_plan_t p, const void* alpha, const void* A_host, const void* beta,
+                                   void* B_host, void* cuda_stream) {
+    if (!p || !alpha || !beta) return TTC_ERR_INVALID_ARG;
+    if (p->canon.empty) return TTC_OK;
+    if (!A_host || !B_host) return TTC_ERR_INVALID_ARG;
+    const size_t es = (size_t)elem_size(p->dtype), esA = (size_t)elem_size(p->dtype_a);
+    const size_t bytes_a = (size_t)p->canon.spanA * esA, bytes_b = (size_t)p->canon.spanB * es;
+    if ((uint64_t)p->canon.spanA > (uint64_t)TTC_STATIC_SCRATCH_BYTES || (uint64_t)p->canon.spanB > (uint64_t)TTC_STATIC_SCRATCH_BYTES ||
+        !static_scratch_fits(bytes_a, bytes_b)) return TTC_ERR_SCRATCH_LIMIT;
+    if (!p->have_device) return TTC_ERR_CUDA;
+    const int which = is_zero(p->dtype, beta) ? 0 : 1;
+    // both copies sit on 256-byte boundaries of the array: every candidate's alignment need is met
+    const int idx = choose_candidate(p, which, 256, 256);
+    if (idx < 0) return TTC_ERR_UNSUPPORTED;
+    if (!ensure_prepared(p, which, idx)) return TTC_ERR_CUDA;
+    const bool b_in = which == 1 || p->canon.spanB != p->canon.numel;      // as ttc_execute_host
+    const int rc = static_scratch_run(p->cands[which][idx], p->dtype, p->dtype_a, to_scalar(p->dtype, alpha),
+                                      to_scalar(p->dtype, beta), A_host, bytes_a, B_host, bytes_b, b_in, cuda_stream);
+    g_launches += 1;
+    return rc == 0 ? TTC_OK : TTC_ERR_CUDA;
+}
+
 ttc_status ttc_destroy(ttc_plan_t p) {
     if (!p) return TTC_OK;
     for (int w = 0; w < 2; ++w) release_specialized(p->spec[w]);
@@ -638,6 +660,7 @@ const char* ttc_status_string(ttc_status s) {
         case TTC_ERR_ALLOC: return "TTC_ERR_ALLOC";
         case TTC_ERR_CUDA: return "TTC_ERR_CUDA";
         case TTC_ERR_MISALIGNED: return "TTC_ERR_MISALIGNED";
+        case TTC_ERR_SCRATCH_LIMIT: return "TTC_ERR_SCRATCH_LIMIT";
     }
     return "TTC_ERR_UNKNOWN";
 }

@@ -84,6 +84,11 @@ bool nvrtc_compile(const std::string& src, const std::string& name, const std::s
                    std::string* lowered, std::string* log_out);
 int pair_id(ttc_dtype dtype, ttc_dtype dtype_a);     // kernels.cu: 0..3 same type, 4..7 sd, ds, cz, zc
 
+// static_scratch.cu: staging of ttc_execute_host_static inside the file-scope device array (no allocation).
+bool static_scratch_fits(size_t bytes_a, size_t bytes_b);
+int static_scratch_run(const Candidate& cand, ttc_dtype dtype, ttc_dtype dtype_a, const Scalar& alpha, const Scalar& beta,
+                       const void* A_host, size_t bytes_a, void* B_host, size_t bytes_b, bool b_in, void* stream);
+
 inline int elem_size(ttc_dtype t) {
     switch (t) {
         case TTC_F32: return 4;

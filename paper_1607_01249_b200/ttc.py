@@ -20,11 +20,13 @@ TTC_MAX_RANK = 16
 TTC_F32, TTC_F64, TTC_C64, TTC_C128 = 0, 1, 2, 3
 TTC_OK = 0
 STATUS_NAMES = ["TTC_OK", "TTC_ERR_INVALID_ARG", "TTC_ERR_NOT_PERMUTATION", "TTC_ERR_BAD_LD",
-                "TTC_ERR_UNSUPPORTED", "TTC_ERR_ALLOC", "TTC_ERR_CUDA", "TTC_ERR_MISALIGNED"]
+                "TTC_ERR_UNSUPPORTED", "TTC_ERR_ALLOC", "TTC_ERR_CUDA", "TTC_ERR_MISALIGNED", "TTC_ERR_SCRATCH_LIMIT"]
+TTC_ERR_SCRATCH_LIMIT = 8
+TTC_STATIC_SCRATCH_BYTES = 8 << 20
 KERNEL_NAMES = {0: "none", 1: "copy", 2: "tile", 3: "gather", 4: "wide", 5: "tma"}
 NP_DTYPE = {TTC_F32: np.float32, TTC_F64: np.float64, TTC_C64: np.complex64, TTC_C128: np.complex128}
 
-EXPORTS = ["ttc_plan", "ttc_plan_mixed", "ttc_plan_strided", "ttc_plan_dtype_a", "ttc_execute", "ttc_execute_batched", "ttc_execute_host", "ttc_destroy", "ttc_last_error",
+EXPORTS = ["ttc_plan", "ttc_plan_mixed", "ttc_plan_strided", "ttc_plan_dtype_a", "ttc_execute", "ttc_execute_batched", "ttc_execute_host", "ttc_execute_host_static", "ttc_destroy", "ttc_last_error",
            "ttc_status_string", "ttc_plan_info", "ttc_plan_num_candidates", "ttc_plan_candidate",
            "ttc_plan_candidate_features", "ttc_plan_specialize", "ttc_plan_select", "ttc_plan_tune", "ttc_canonicalize", "ttc_launch_count",
            "ttc_debug_fastdiv", "ttc_debug_specialize_compile", "ttc_version", "ttc_release_host_staging"]
@@ -73,6 +75,8 @@ def _load() -> ctypes.CDLL:
     lib.ttc_execute_batched.argtypes = [vp, vp, ctypes.POINTER(vp), vp, ctypes.POINTER(vp), ctypes.c_int, vp]
     lib.ttc_execute_host.restype = ctypes.c_int
     lib.ttc_execute_host.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.ttc_execute_host_static.restype = ctypes.c_int
+    lib.ttc_execute_host_static.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.ttc_destroy.restype = ctypes.c_int
     lib.ttc_destroy.argtypes = [vp]
     lib.ttc_last_error.restype = ctypes.c_int
@@ -218,6 +222,17 @@ def ttc_execute_host(plan: int, alpha, A_host, beta, B_host, stream=None) -> Non
     rc = lib.ttc_execute_host(plan, a.ctypes.data, _ptr(A_host), b.ctypes.data, _ptr(B_host), _stream(stream))
     if rc != TTC_OK:
         raise TTCError(rc, "ttc_execute_host")
+
+
+def ttc_execute_host_static(plan: int, alpha, A_host, beta, B_host, stream=None) -> None:
+    """ttc_execute_host staged through the library's file-scope device array: no device allocation; tensors
+    beyond TTC_STATIC_SCRATCH_BYTES raise TTCError(TTC_ERR_SCRATCH_LIMIT)."""
+    npdt = _scalar_dtype(plan)
+    a = np.array([alpha], dtype=npdt)
+    b = np.array([beta], dtype=npdt)
+    rc = lib.ttc_execute_host_static(plan, a.ctypes.data, _ptr(A_host), b.ctypes.data, _ptr(B_host), _stream(stream))
+    if rc != TTC_OK:
+        raise TTCError(rc, "ttc_execute_host_static")
 
 
 def ttc_destroy(plan: int) -> None:
