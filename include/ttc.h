@@ -76,8 +76,11 @@ typedef enum {
     TTC_KERNEL_TILE = 2,    /* K2: shared-memory tiled transpose in the plane (stride-1 of A, of B)   */
     TTC_KERNEL_GATHER = 3,  /* K3: K2 whose tile sides are coarsened over several leading indices     */
     TTC_KERNEL_WIDE = 4,    /* K2 on "wide elements": a >=16-byte run that leads both A and B         */
-    TTC_KERNEL_TMA = 5      /* K2/K3 warp-specialised: a producer warp fetches the tile rows by TMA
+    TTC_KERNEL_TMA = 5,     /* K2/K3 warp-specialised: a producer warp fetches the tile rows by TMA
                                bulk copies (cp.async.bulk) into a ring of buffers, consumers store  */
+    TTC_KERNEL_TENSORMAP = 6 /* K1/K2/K3 through tensor maps: cp.async.bulk.tensor box loads AND stores
+                               (<= 5-D, strides multiples of 16 bytes, 16-byte aligned A and B, same
+                               element type), swizzled shared-memory boxes, in-register micro-tiles  */
 } ttc_kernel_class;
 
 typedef struct ttc_plan_s* ttc_plan_t;

@@ -40,6 +40,7 @@ struct ttc_plan_s {
     int tune_errors = 0;               // candidates that could not be prepared or launched while tuning
     float plan_ms = 0.f, tune_ms = 0.f;  // wall time of building the plan / of timing candidates inside it
     int fallback[2][25];               // [which][5 * log2(align of A) + log2(align of B)] -> candidate, -2 = not looked up
+    int nomap[2][25];                  // the same for ttc_execute_batched when the choice is a tensor-map candidate
     // ttc_execute_host pipeline (contiguous tensors): the transposition is cut into `pipe_n` slabs
     // along canonical index `pipe_d`; slab c is copied in, transposed by `pipe_sub` and copied out
     // while slab c + 1 is on its way in (PCIe is full duplex).
@@ -335,6 +336,28 @@ int choose_candidate(ttc_plan_s* p, int which, uintptr_t A, uintptr_t B) {
     return slot < 0 ? -2 : slot;
 }
 
+// ttc_execute_batched cannot launch a tensor-map candidate (its two maps hold ONE base address each): the best
+// other candidate whose accesses fit the pointers' alignment, looked up once per alignment class.
+int without_tensormap(ttc_plan_s* p, int which, int idx, uintptr_t A, uintptr_t B) {
+    if (idx < 0 || p->cands[which][idx].info.kernel != TTC_KERNEL_TENSORMAP) return idx;
+    auto lg = [](uintptr_t x) { int l = 0; while (l < 4 && !((x >> l) & 1)) ++l; return l; };
+    const int la = lg(A), lb = lg(B);
+    int& slot = p->nomap[which][5 * la + lb];
+    if (slot == -2) {
+        slot = -1;
+        float best_us = 0.f;
+        const std::vector<Candidate>& cs = p->cands[which];
+        for (int i = 0; i < (int)cs.size(); ++i) {
+            if (cs[i].info.kernel == TTC_KERNEL_TENSORMAP) continue;
+            if ((1 << la) % cs[i].align_a != 0 || (1 << lb) % cs[i].align_b != 0) continue;
+            const float us = cs[i].info.tuned_us;
+            if (slot < 0) { slot = i; best_us = us; continue; }
+            if (us > 0.f && (best_us <= 0.f || us < best_us)) { slot = i; best_us = us; }
+        }
+    }
+    return slot < 0 ? -2 : slot;
+}
+
 }  // namespace
 
 static void finish_plan(ttc_plan_s* p);
@@ -388,6 +411,7 @@ static void finish_plan(ttc_plan_s* p) {
         ~Stamp() { p->plan_ms = (float)std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count(); }
     } stamp{p, t_plan0};
     for (auto& w : p->fallback) for (int& x : w) x = -2;
+    for (auto& w : p->nomap) for (int& x : w) x = -2;
     const ttc_dtype dtype = p->dtype;
     int dev = 0, count = 0;
     if (cudaGetDeviceCount(&count) == cudaSuccess && count > 0 && cudaGetDevice(&dev) == cudaSuccess) {
@@ -485,7 +509,7 @@ ttc_status ttc_execute_batched(ttc_plan_t p, const void* alpha, const void* cons
     }
     if ((oa % esA) != 0 || (ob % es) != 0) return TTC_ERR_MISALIGNED;
     const int which = is_zero(p->dtype, beta) ? 0 : 1;
-    const int idx = choose_candidate(p, which, oa, ob);
+    const int idx = without_tensormap(p, which, choose_candidate(p, which, oa, ob), oa, ob);
     if (idx == -1) return TTC_ERR_UNSUPPORTED;
     if (idx < 0) return TTC_ERR_MISALIGNED;
     const Candidate& c = p->cands[which][idx];
@@ -822,7 +846,7 @@ int64_t ttc_launch_count(void) { return g_launches.load(); }
 
 uint32_t ttc_debug_fastdiv(uint32_t n, uint32_t d) { return fd_div(n, make_fastdiv(d)); }
 
-const char* ttc_version(void) { return "ttc-b200 0.3 (sm_100a)"; }
+const char* ttc_version(void) { return "ttc-b200 0.4 (sm_100a)"; }
 
 ttc_status ttc_release_host_staging(void) {
     std::lock_guard<std::mutex> lk(g_stage_mu);

@@ -11,6 +11,9 @@
 //                  in the candidate's loop order through WorkSched.
 //   ring_kernel    K2/K3, warp-specialised: a producer warp loads the tile rows with TMA bulk copies
 //                  into a ring of tile buffers, consumer warps run tile_kernel's store phase.
+//   tmap_kernel    K1/K2/K3 for tensors whose strides a CUtensorMap can express (ttc_tmap.cuh): tensor-map
+//                  box loads, in-register micro-tile transposition between swizzled shared-memory boxes,
+//                  tensor-map box stores.
 //
 // Arithmetic (Eq. 1): every product and sum is rounded separately
 // (__fmul_rn/__fadd_rn, never contracted into FMA) so the result is bit-identical to the
@@ -26,6 +29,7 @@
 #include "ttc_internal.h"
 
 #include "ttc_device.cuh"
+#include "ttc_tmap.cuh"
 
 namespace ttc {
 
@@ -166,6 +170,57 @@ static KernelFn get_direct_fn(int dt, const Candidate& c, bool batched) {
     return nullptr;
 }
 
+template <int DT>
+static KernelFn tmap_fn_dt(bool beta, int flavour) {
+    if (flavour == 0) return beta ? (KernelFn)tmap_kernel<DT, true, 0> : (KernelFn)tmap_kernel<DT, false, 0>;
+    return beta ? (KernelFn)tmap_kernel<DT, true, 1> : (KernelFn)tmap_kernel<DT, false, 1>;
+}
+
+static KernelFn get_tmap_fn(int dt, const Candidate& c) {
+    switch (dt) {
+        case TTC_F32: return tmap_fn_dt<TTC_F32>(c.beta_nz, c.mp.flavour);
+        case TTC_F64: return tmap_fn_dt<TTC_F64>(c.beta_nz, c.mp.flavour);
+        case TTC_C64: return tmap_fn_dt<TTC_C64>(c.beta_nz, c.mp.flavour);
+        case TTC_C128: return tmap_fn_dt<TTC_C128>(c.beta_nz, c.mp.flavour);
+    }
+    return nullptr;     // same-type tensors only
+}
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point query (the library does not link libcuda).
+using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn encode_tiled_fn() {
+    static EncodeTiledFn fn = [] {
+        void* f = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess)
+            f = nullptr;
+        return (EncodeTiledFn)f;
+    }();
+    return fn;
+}
+
+static bool encode_maps(const TmapEncode& me, const void* A, void* B, CUtensorMap* mapA, CUtensorMap* mapB) {
+    EncodeTiledFn enc = encode_tiled_fn();
+    if (!enc) return false;
+    const CUtensorMapDataType dt = me.unit_bytes == 4 ? CU_TENSOR_MAP_DATA_TYPE_UINT32 : CU_TENSOR_MAP_DATA_TYPE_UINT64;
+    const CUtensorMapSwizzle sw = me.swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE;
+    static const cuuint32_t ones[kTmapRank] = {1, 1, 1, 1, 1};
+    cuuint64_t dA[kTmapRank], dB[kTmapRank], sA[kTmapRank - 1], sB[kTmapRank - 1];
+    cuuint32_t bA[kTmapRank], bB[kTmapRank];
+    for (int i = 0; i < kTmapRank; ++i) { dA[i] = me.dimA[i]; dB[i] = me.dimB[i]; bA[i] = me.boxA[i]; bB[i] = me.boxB[i]; }
+    for (int i = 0; i < kTmapRank - 1; ++i) { sA[i] = me.strideA[i]; sB[i] = me.strideB[i]; }
+    if (enc(mapA, dt, kTmapRank, const_cast<void*>(A), dA, sA, bA, ones, CU_TENSOR_MAP_INTERLEAVE_NONE, sw,
+            CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) return false;
+    return enc(mapB, dt, kTmapRank, B, dB, sB, bB, ones, CU_TENSOR_MAP_INTERLEAVE_NONE, sw,
+               CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+static uint32_t tmap_smem_bytes(const TmapParams& mp) {
+    return (uint32_t)mp.stages * 2u * mp.buf_bytes + 1024u;     // + alignment slack
+}
+
 // Opt the instance in to the device's maximum of dynamic shared memory (the attribute belongs to the kernel
 // function, which many candidates share); returns that maximum less the kernel's static shared memory.
 static int raise_smem_limit(KernelFn fn, int* optin_out) {
@@ -197,6 +252,25 @@ int prepare_candidate(Candidate* cand, ttc_dtype dtype, ttc_dtype dtype_a, int s
         cand->info.threads = kDirectThreads;
         cand->info.smem_bytes = 0;
         cand->info.grid = (int)(cand->dp.dyn == 1 || need < cap ? need : cap);
+        cand->grid_cap = (int)cap;
+        return 0;
+    }
+    if (cand->info.kernel == TTC_KERNEL_TENSORMAP) {
+        KernelFn fn = dtype == dtype_a ? get_tmap_fn((int)dtype, *cand) : nullptr;
+        if (!fn || !encode_tiled_fn()) return (int)cudaErrorInvalidValue;
+        const int smem = (int)tmap_smem_bytes(cand->mp);
+        int optin = 0;
+        int rc = raise_smem_limit(fn, &optin);
+        if (rc != 0) return rc;
+        if (smem > optin) return (int)cudaErrorInvalidConfiguration;
+        int occ = 0;
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, cand->mp.threads, smem);
+        if (e != cudaSuccess) return (int)e;
+        if (occ < 1) return (int)cudaErrorInvalidConfiguration;
+        const uint64_t cap = (uint64_t)sm_count * (uint64_t)occ;
+        cand->info.threads = cand->mp.threads;
+        cand->info.smem_bytes = smem;
+        cand->info.grid = (int)(cand->mp.dyn == 1 || cand->mp.n_tiles < cap ? cand->mp.n_tiles : cap);
         cand->grid_cap = (int)cap;
         return 0;
     }
@@ -235,6 +309,7 @@ int launch_candidate(const Candidate& cand, ttc_dtype dtype, ttc_dtype dtype_a, 
     uint64_t grid = (uint64_t)cand.info.grid;
     if (batched) {     // one CTA per work item (launch control) or as many as the device holds
         const uint64_t work = (uint64_t)batch->per * (uint64_t)batch->n;
+        if (cand.info.kernel == TTC_KERNEL_TENSORMAP) return (int)cudaErrorNotSupported;   // the maps hold ONE base address each
         const int dyn_b = cand.info.kernel == TTC_KERNEL_COPY ? cand.dp.dyn : cand.tp.dyn;
         grid = (dyn_b == 1 || work < (uint64_t)cand.grid_cap) ? work : (uint64_t)cand.grid_cap;
         if (grid >= (1ull << 31)) return (int)cudaErrorInvalidConfiguration;
@@ -247,7 +322,7 @@ int launch_candidate(const Candidate& cand, ttc_dtype dtype, ttc_dtype dtype_a, 
     // (198 MB): -0.3 .. -1.3 us per launch; neutral for stream launches.  A predecessor that is not one
     // of these kernels never triggers early, which degenerates to ordinary stream order.  TTC_PDL=0: off.
     cudaLaunchAttribute attr[1];
-    const int dyn = cand.info.kernel == TTC_KERNEL_COPY ? cand.dp.dyn : cand.tp.dyn;
+    const int dyn = cand.info.kernel == TTC_KERNEL_COPY ? cand.dp.dyn : cand.info.kernel == TTC_KERNEL_TENSORMAP ? cand.mp.dyn : cand.tp.dyn;
     static const int pdl_env = std::getenv("TTC_PDL") ? std::atoi(std::getenv("TTC_PDL")) : -1;
     if (dyn == 2 && !sched_ctr) return (int)cudaErrorInvalidValue;
     if (pdl_env != 0) {
@@ -258,6 +333,18 @@ int launch_candidate(const Candidate& cand, ttc_dtype dtype, ttc_dtype dtype_a, 
     }
     NoBatch none;
     Scalar al = alpha, be = beta;
+    if (cand.info.kernel == TTC_KERNEL_TENSORMAP) {
+        KernelFn fn = dtype == dtype_a ? get_tmap_fn((int)dtype, cand) : nullptr;
+        if (!fn) return (int)cudaErrorInvalidValue;
+        alignas(64) CUtensorMap mapA, mapB;       // the descriptors carry the base addresses: encoded per call (host only)
+        if (!encode_maps(cand.me, A, B, &mapA, &mapB)) return (int)cudaErrorInvalidValue;
+        cfg.blockDim = dim3((unsigned)cand.mp.threads, 1, 1);
+        cfg.dynamicSmemBytes = (size_t)cand.info.smem_bytes;
+        TmapParams mp = cand.mp;
+        mp.ctr = sched_ctr;
+        void* targs[5] = {&mp, &mapA, &mapB, &al, &be};
+        return (int)cudaLaunchKernelExC(&cfg, fn, targs);
+    }
     void* args[6] = {nullptr, (void*)&A, (void*)&B, (void*)&al, (void*)&be, batched ? (void*)batch : (void*)&none};
     if (cand.info.kernel == TTC_KERNEL_COPY) {
         KernelFn fn = get_direct_fn(pair, cand, batched);

@@ -781,6 +781,219 @@ void add_direct(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz
     out->push_back(cand);
 }
 
+
+// ------------------------------------------------------------------------------------------
+// Tensor-map candidates (TTC_KERNEL_TENSORMAP, ttc_tmap.cuh): same element type on both sides, canonical rank
+// 2..5, every stride but the unit one a multiple of 16 bytes (SURVEY.md 8(d) "TMA feasibility"; the base
+// addresses must be 16-byte aligned too, which align_a / align_b tell ttc_execute).
+// ------------------------------------------------------------------------------------------
+// Largest t in [max(1, want / 2), want] that wastes least of extent e when it is cut into pieces of t.
+int32_t fit_extent(int64_t e, int32_t want) {
+    if (e <= want) return (int32_t)e;
+    int32_t best = want;
+    double best_eff = 0.0;
+    for (int32_t t = want; t >= std::max(1, want / 2); --t) {
+        const double eff = (double)e / (double)(((e + t - 1) / t) * t);
+        if (eff > best_eff + 1e-9) { best_eff = eff; best = t; }
+    }
+    return best;
+}
+
+void add_tmap(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, int sched, int max_smem, std::vector<Candidate>* out) {
+    if (dtype != dtype_a || c.rank < 2 || c.rank > kTmapRank) return;
+    const int es = elem_size(dtype);
+    const int unit = es >= 8 ? 8 : 4, upe = es / unit;
+    const int q = c.orderB[0];
+    if (c.d[0].sA != 1 || c.d[q].sB != 1) return;
+    const int64_t lim = (int64_t)1 << 40;
+    for (int i = 0; i < c.rank; ++i) {
+        if (c.d[i].e >= kInt31 / 2) return;
+        if (i != 0 && ((c.d[i].sA * es) % 16 != 0 || c.d[i].sA * es >= lim)) return;
+        if (i != q && ((c.d[i].sB * es) % 16 != 0 || c.d[i].sB * es >= lim)) return;
+    }
+    const int flavour = q == 0 ? 1 : 0;
+    // the other indices, by ascending stride in A and in B
+    std::vector<int> othA, othB;
+    for (int i = 0; i < c.rank; ++i) if (i != 0 && i != q) othA.push_back(i);
+    for (int k = 0; k < c.rank; ++k) if (c.orderB[k] != 0 && c.orderB[k] != q) othB.push_back(c.orderB[k]);
+    const int T = 128 / es;                              // flavour 0: elements per 128-byte box row
+
+    std::set<std::string> seen;
+    int n_added = 0;
+    auto emit = [&](const int32_t* pe, int32_t box0_units, int nbA, int nbB) {
+        // pe[i]: box extent of canonical index i (flavour 0: the two leading ones are fixed by the swizzle)
+        std::string key((const char*)pe, sizeof(int32_t) * c.rank);
+        key.push_back((char)nbA);
+        key.push_back((char)nbB);
+        key.append((const char*)&box0_units, sizeof(box0_units));
+        if (!seen.insert(key).second) return;
+        Candidate cand;
+        cand.beta_nz = beta_nz;
+        TmapParams& M = cand.mp;
+        TmapEncode& E = cand.me;
+        std::memset(&M, 0, sizeof(M));
+        std::memset(&E, 0, sizeof(E));
+        int idx[kTmapRank];                                  // canonical index of A-map dimension k (-1: padding)
+        int n = 0;
+        if (flavour == 0) {
+            idx[n++] = 0;
+            idx[n++] = q;
+            for (int i : othA) idx[n++] = i;
+        } else {
+            for (int k = 0; k < c.rank; ++k) idx[n++] = c.orderB[k];
+        }
+        for (; n < kTmapRank; ++n) idx[n] = -1;
+        int64_t planes = 1, box_elems = 1;
+        for (int k = 0; k < kTmapRank; ++k) {
+            const int i = idx[k];
+            const int64_t e = i < 0 ? 1 : c.d[i].e;
+            int32_t bx;                                          // box extent (elements) along A-map dimension k
+            if (flavour == 0) bx = k < 2 ? T : (i < 0 ? 1 : pe[i]);
+            else bx = k == 0 ? box0_units / upe : (i < 0 ? 1 : pe[i]);
+            if (bx < 1 || bx > 256) return;
+            if (flavour == 0 && k >= 2) planes *= bx;
+            box_elems *= bx;
+            E.dimA[k] = (uint64_t)e * (k == 0 ? upe : 1);
+            E.boxA[k] = (uint32_t)bx * (k == 0 ? upe : 1);
+            if (k > 0) E.strideA[k - 1] = i < 0 ? 16 : (uint64_t)(c.d[i].sA * es);
+            const int nb = flavour == 0 ? (k == 0 ? nbA : k == 1 ? nbB : 1) : 1;
+            M.step[k] = bx * nb;
+            const int64_t nt = (e + M.step[k] - 1) / M.step[k];
+            M.gdiv[k] = make_fastdiv((uint32_t)nt);
+        }
+        // B's map: flavour 0 swaps the two leading dimensions, flavour 1 keeps A's order
+        for (int k = 0; k < kTmapRank; ++k) {
+            const int ka = flavour == 0 && k < 2 ? 1 - k : k;    // A-map dimension that is B-map dimension k
+            const int i = idx[ka];
+            const int64_t e = i < 0 ? 1 : c.d[i].e;
+            const uint32_t bx = E.boxA[ka] / (ka == 0 ? upe : 1);
+            E.dimB[k] = (uint64_t)e * (k == 0 ? upe : 1);
+            E.boxB[k] = bx * (k == 0 ? upe : 1);
+            if (k > 0) E.strideB[k - 1] = i < 0 ? 16 : (uint64_t)(c.d[i].sB * es);
+        }
+        if (E.boxA[0] > 256 || E.boxB[0] > 256 || (E.boxA[0] * unit) % 16 != 0) return;
+        E.unit_bytes = unit;
+        E.swizzle128 = flavour == 0 ? 1 : 0;
+        const int64_t box_bytes = box_elems * es;
+        const int64_t tile_bytes = (box_bytes * nbA * nbB + 127) / 128 * 128;
+        if (box_bytes < 1024 || tile_bytes > 64 * 1024 || nbA * nbB > kTmapMaxBoxes) return;
+        int stages = 0;
+        for (int st = 4; st >= 2; --st)
+            if (st * 2 * tile_bytes + 1024 <= std::min<int64_t>(max_smem, st == 2 ? 160 * 1024 : 100 * 1024)) { stages = st; break; }
+        if (!stages) return;
+        uint64_t n_tiles = 1;
+        double padded = 1.0, real = 1.0;
+        for (int k = 0; k < kTmapRank; ++k) {
+            n_tiles *= M.gdiv[k].d;
+            if (n_tiles >= (uint64_t)kInt31) return;
+            padded *= (double)M.gdiv[k].d * M.step[k];
+            real *= idx[k] < 0 ? 1.0 : (double)c.d[idx[k]].e;
+        }
+        M.flavour = flavour;
+        M.dyn = sched;
+        M.n_tiles = (uint32_t)n_tiles;
+        M.stages = stages;
+        M.threads = 192;                                         // producer warp, store warp, 4 consumer warps
+        M.nbA = nbA;
+        M.nbB = nbB;
+        M.planes = (int)planes;
+        M.box_bytes = (uint32_t)box_bytes;
+        M.buf_bytes = (uint32_t)tile_bytes;
+        M.upe = upe;
+        M.box0[0] = (int32_t)(E.boxA[0] / upe);
+        M.box0[1] = (int32_t)E.boxA[1];
+        cand.align_a = cand.align_b = 16;
+        ttc_candidate_info& I = cand.info;
+        I.kernel = TTC_KERNEL_TENSORMAP;
+        I.flags = TTC_CAND_TENSORMAP;
+        I.vec_a = I.vec_b = 16 / es;
+        I.threads = M.threads;
+        I.loop_order = 0;
+        I.sched = sched;
+        I.n_tiles = (int64_t)n_tiles;
+        I.tile_u = M.step[0];
+        I.tile_w = flavour == 0 ? M.step[1] : 1;
+        I.n_u = 1;
+        I.n_w = 1;
+        for (int i = 0; i < kMaxRank; ++i) I.tile_ext[i] = i < c.rank ? 1 : 0;
+        for (int k = 0; k < kTmapRank; ++k) if (idx[k] >= 0) I.tile_ext[idx[k]] = M.step[k];
+        // ranked just behind the best fitted ring candidates (fitted costs are time / ideal time), tiles that stick
+        // out of the tensor cost their share of wasted shared-memory work; the tuner decides
+        const double waste = padded / real;
+        I.est_cost = (float)((1.10 + 0.01 * n_added) * waste * (tile_bytes < 8192 ? 1.15 : 1.0));
+        cand.feat[2] = (float)waste;
+        cand.feat[4] = (float)tile_bytes;
+        cand.feat[5] = (float)n_tiles;
+        cand.feat[12] = beta_nz ? 1.f : 0.f;
+        cand.feat[13] = (float)TTC_KERNEL_TENSORMAP;
+        out->push_back(cand);
+        ++n_added;
+    };
+
+    // Box extents over the other indices: `want` planes (flavour 0) or rows (flavour 1), handed out along `order`.
+    auto fill = [&](const std::vector<int>& order, int64_t want, int32_t* pe) {
+        for (int i = 0; i < c.rank; ++i) pe[i] = 1;
+        int64_t left = want;
+        for (int i : order) {
+            if (left < 2) break;
+            const int32_t t = fit_extent(c.d[i].e, (int32_t)std::min<int64_t>(left, 256));
+            pe[i] = t;
+            left /= t;
+        }
+    };
+    int32_t pe[kMaxRank];
+    if (flavour == 0) {
+        const int64_t plane_bytes = 128 * (int64_t)T;
+        struct Var { int dist, kb, nbA, nbB; };
+        static const Var vars[] = {{0, 16, 1, 1}, {1, 16, 1, 1}, {2, 16, 1, 1}, {0, 8, 2, 1}, {1, 8, 1, 2}, {2, 8, 2, 2},
+                                   {0, 8, 1, 1}, {1, 8, 1, 1}, {0, 32, 1, 1}, {1, 32, 1, 1}};
+        for (const Var& v : vars) {
+            if (c.d[0].e < (int64_t)v.nbA * T && v.nbA > 1) continue;
+            if (c.d[q].e < (int64_t)v.nbB * T && v.nbB > 1) continue;
+            const int64_t want = std::max<int64_t>(1, (int64_t)v.kb * 1024 / plane_bytes);
+            if (v.dist == 0) fill(othA, want, pe);
+            else if (v.dist == 1) fill(othB, want, pe);
+            else {
+                // balanced: half of the planes along A's next index, the rest along B's
+                for (int i = 0; i < c.rank; ++i) pe[i] = 1;
+                if (othA.empty()) continue;
+                int64_t h = 1;
+                while (h * h < want) h *= 2;
+                const int ia = othA[0];
+                pe[ia] = fit_extent(c.d[ia].e, (int32_t)h);
+                int64_t left = want / pe[ia];
+                for (int i : othB) {
+                    if (i == ia || left < 2) continue;
+                    pe[i] = fit_extent(c.d[i].e, (int32_t)std::min<int64_t>(left, 256));
+                    left /= pe[i];
+                }
+            }
+            emit(pe, 0, v.nbA, v.nbB);
+        }
+        if (othA.empty()) {      // 2-D: a tile is a few planes side by side
+            for (int i = 0; i < c.rank; ++i) pe[i] = 1;
+            static const int nb[][2] = {{2, 2}, {4, 1}, {1, 4}, {2, 1}, {1, 2}};
+            for (auto& b : nb)
+                if (c.d[0].e >= (int64_t)b[0] * T && c.d[q].e >= (int64_t)b[1] * T) emit(pe, 0, b[0], b[1]);
+        }
+    } else {
+        // copy class: rows of up to 256 map units along the shared leading index, then rows until the box has 8-32 KB
+        const int gran = 16 / unit;
+        const int64_t e0u = c.d[0].e * upe;
+        int32_t b0 = (int32_t)std::min<int64_t>(256, (e0u + gran - 1) / gran * gran);
+        if (e0u > 256) {         // cut long rows evenly
+            const int64_t pieces = (e0u + 255) / 256;
+            b0 = (int32_t)(((e0u + pieces - 1) / pieces + gran - 1) / gran * gran);
+        }
+        for (int kb : {16, 8, 32})
+            for (int dist = 0; dist < 2; ++dist) {
+                const int64_t want = std::max<int64_t>(1, (int64_t)kb * 1024 / ((int64_t)b0 * unit));
+                fill(dist == 0 ? othB : othA, want, pe);
+                emit(pe, b0, 1, 1);
+            }
+    }
+}
+
 }  // namespace
 
 void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, int sm_count,
@@ -802,8 +1015,9 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, boo
         else if (!std::strcmp(e, "all")) scheds = {1, 2, 0};
     }
 
-    // TTC_VARIANTS: bit 0 = staggered-gather ring candidates, bit 1 = shifted-row ring candidates (default: both)
-    const int variants = std::getenv("TTC_VARIANTS") ? std::atoi(std::getenv("TTC_VARIANTS")) : 3;
+    // TTC_VARIANTS: bit 0 = staggered-gather ring candidates, bit 1 = shifted-row ring candidates, bit 2 = tensor-map
+    // candidates (default: all)
+    const int variants = std::getenv("TTC_VARIANTS") ? std::atoi(std::getenv("TTC_VARIANTS")) : 7;
     const int xp_max = (variants & 1) ? 1 : 0;
     const int n_loop_orders = std::getenv("TTC_LOOP_ORDERS") ? std::max(2, std::min(4, std::atoi(std::getenv("TTC_LOOP_ORDERS")))) : 2;
     const int ring_max = std::getenv("TTC_RING") ? std::atoi(std::getenv("TTC_RING")) : 4;
@@ -814,6 +1028,10 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, boo
             add_direct(c, dtype, dtype_a, beta_nz, lo, true, sched, out);
             add_direct(c, dtype, dtype_a, beta_nz, lo, false, sched, out);
         }
+
+    // Tensor-map candidates (TTC_VARIANTS bit 2).
+    if (variants & 4)
+        for (int sched : scheds) add_tmap(c, dtype, dtype_a, beta_nz, sched, max_smem, out);
 
     // K2 / K3: tiles.  A side = leading indices of A, B side = leading indices of B.
     std::vector<int> orderA, orderB;
@@ -884,7 +1102,7 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, boo
     const int n_full = std::min<int>((int)out->size(), std::getenv("TTC_FULL_SEARCH") ? std::atoi(std::getenv("TTC_FULL_SEARCH")) : kFullSearch);
     for (int i = 0; i < n_full; ++i) {
         Candidate& cd = (*out)[i];
-        if (cd.info.kernel == TTC_KERNEL_COPY) continue;
+        if (cd.info.kernel == TTC_KERNEL_COPY || cd.info.kernel == TTC_KERNEL_TENSORMAP) continue;
         const Recipe r = cd.recipe;
         Candidate full;
         if (build_tile_candidate(c, dtype, dtype_a, beta_nz, r.spec, r.loop_order, r.va, r.vb, max_smem, r.sched, r.ring, r.xp,

@@ -7,6 +7,7 @@
 
 #include "ttc.h"
 #include "ttc_params.h"
+#include "ttc_tmap.h"
 
 namespace ttc {
 
@@ -54,6 +55,8 @@ struct Candidate {
     int  align_a = 1, align_b = 1;  // required pointer alignment in bytes
     DirectParams dp{};
     TileParams tp{};
+    TmapParams mp{};             // TTC_KERNEL_TENSORMAP: kernel parameters and what the two tensor maps are encoded from
+    TmapEncode me{};
     float feat[16] = {0};        // raw inputs of the cost heuristic (plan.cpp), exported for re-fitting
     Recipe recipe{};
     int grid_cap = 0;            // resident CTAs the device holds of this kernel (set by prepare_candidate)

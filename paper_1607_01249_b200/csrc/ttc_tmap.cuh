@@ -1,0 +1,256 @@
+// ttc_tmap.cuh -- tmap_kernel: Eq. 1 with tiles that travel as tensor-map boxes in both directions
+// (north_star K2, SURVEY.md 8(d) "TMA feasibility").  One CTA = one producer warp, one store warp, the rest consumers:
+//
+//   producer (lane 0)   waits for a free stage, takes the next tile from the work scheduler, arms the stage's `full`
+//                       mbarrier with the box bytes and issues cp.async.bulk.tensor.5d loads (UTMALDG) of A's boxes
+//                       into the stage's in-buffer and, for beta != 0, of B's boxes into its out-buffer
+//   consumers           wait for `full`; flavour 0: transpose every 2-D plane of the in-boxes into the out-boxes, V x V
+//                       elements per thread held in registers (V = 16 / element size: the paper's in-register micro
+//                       tile), 16-byte LDS/STS only, both sides in the 128-byte swizzle so that every
+//                       quarter-warp access touches all 32 banks once; flavour 1: alpha/beta chunk by chunk; then
+//                       fence.proxy.async and one arrival per warp on `done`
+//   store warp (lane 0) waits for `done`, issues cp.async.bulk.tensor.5d stores (UTMASTG) of the out-boxes, commits
+//                       them as one bulk group and hands the PREVIOUS stage back (`empty`) once its group has
+//                       finished reading shared memory
+//
+// Boxes that stick out of the tensor need no code: loads fill with zeros, stores clip.  No thread issues a global
+// load or store.  Arithmetic: products and sums rounded separately, exactly as the other kernels (readings A7/A10).
+#pragma once
+#include <cuda.h>
+
+#include "ttc_device.cuh"
+#include "ttc_tmap.h"
+
+namespace ttc {
+
+__device__ __forceinline__ void tmap_load(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1, int c2, int c3, int c4) {
+    asm volatile("cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6, %7}], [%2];"
+                 ::"r"(dst), "l"(reinterpret_cast<uint64_t>(map)), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4) : "memory");
+}
+__device__ __forceinline__ void tmap_store(const CUtensorMap* map, uint32_t src, int c0, int c1, int c2, int c3, int c4) {
+    asm volatile("cp.async.bulk.tensor.5d.global.shared::cta.tile.bulk_group [%0, {%2, %3, %4, %5, %6}], [%1];"
+                 ::"l"(reinterpret_cast<uint64_t>(map)), "r"(src), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4) : "memory");
+}
+__device__ __forceinline__ uint4 lds128(uint32_t a) {
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sts128(uint32_t a, const uint4& v) {
+    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
+// Which V x V micro-tile (A2 = 16-byte column of the in-plane, B2 = 16-byte column of the out-plane, both 0..7) lane
+// `lane` takes in pass j (0, 1) of a plane.  In-plane: element (a, b) sits in row b, chunk (a / V) ^ (b & 7);
+// out-plane: row a, chunk (b / V) ^ (a & 7).  The 8 lanes of a quarter-warp read rows V*B2 + d, chunk A2 and write
+// rows V*A2 + d, chunk B2 (d fixed per instruction); the maps below make both chunk positions a bijection of the
+// lane's low three bits for every d, i.e. conflict-free 16-byte accesses on both sides.
+template <int V>
+__device__ __forceinline__ void tmap_lane_map(int lane, int j, int& A2, int& B2) {
+    const int i = lane & 7, q = lane >> 3;
+    if constexpr (V == 1) {
+        A2 = i;
+        B2 = (j << 2) | q;
+    } else if constexpr (V == 2) {
+        A2 = i;
+        B2 = ((j << 2) | q) ^ (i >> 2);
+    } else {
+        A2 = (j << 2) | (i & 3);
+        B2 = ((q >> 1) << 2) | (((((i >> 1) ^ q) & 1)) << 1) | (i >> 2);
+    }
+}
+
+template <typename T> struct tmap_is_real { static constexpr bool value = false; };
+template <> struct tmap_is_real<float> { static constexpr bool value = true; };
+template <> struct tmap_is_real<double> { static constexpr bool value = true; };
+
+template <int DT, bool BETA, int FLAVOUR>
+__global__ void __launch_bounds__(256)
+tmap_kernel(const __grid_constant__ TmapParams P, const __grid_constant__ CUtensorMap mapA,
+            const __grid_constant__ CUtensorMap mapB, const Scalar alpha_in, const Scalar beta_in) {
+    using T = typename ElemT<DT>::T;
+    constexpr int ES = (int)sizeof(T);
+    constexpr int V = 16 / ES;
+    union Chunk { uint4 u; T e[V]; };
+    TScal<T> alpha, beta;
+    typed(alpha_in, alpha);
+    typed(beta_in, beta);
+
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const uint32_t raw = (uint32_t)__cvta_generic_to_shared(smem_raw);
+    const uint32_t base = (raw + 1023u) & ~1023u;              // the 128-byte swizzle repeats every 1024 bytes
+    const int nbox = P.nbA * P.nbB;
+    const uint32_t tile_bytes = P.box_bytes * (uint32_t)nbox;
+
+    __shared__ __align__(16) uint4 sched_resp;
+    __shared__ __align__(8) uint64_t sched_bar;
+    __shared__ __align__(8) uint64_t full_bar[kTmapMaxStages], done_bar[kTmapMaxStages], empty_bar[kTmapMaxStages];
+    __shared__ int32_t coord[kTmapMaxStages][kTmapRank];
+    __shared__ uint32_t tile_of[kTmapMaxStages];
+
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int S = P.stages;
+    const int n_cons_warps = ((int)blockDim.x >> 5) - 2;
+    WorkSched sched;
+    sched.init(P.dyn, &sched_bar, &sched_resp, P.ctr);
+    pdl_launch_dependents();
+    if (tid == 0) {
+        for (int s = 0; s < S; ++s) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"((uint32_t)__cvta_generic_to_shared(&full_bar[s])));
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(&done_bar[s])), "r"(n_cons_warps));
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"((uint32_t)__cvta_generic_to_shared(&empty_bar[s])));
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    pdl_wait();
+
+    // A real alpha == 1 with beta == 0 in the copy class leaves nothing to compute: the box is stored from the buffer it
+    // was loaded into.  (Not for complex types: (1 + 0i) * (inf + i) has 0 * inf = NaN in the oracle's formula too.)
+    bool passthrough = false;
+    if constexpr (FLAVOUR == 1 && !BETA && tmap_is_real<T>::value) passthrough = alpha.re == T(1);
+
+    if (tid < 32) {
+        // ------------------------------------------------------------------ producer warp
+        uint32_t tile_id = blockIdx.x;
+        bool more = true;
+        for (uint32_t it = 0;; ++it) {
+            const int s = (int)(it % (uint32_t)S);
+            const uint32_t full_a = (uint32_t)__cvta_generic_to_shared(&full_bar[s]);
+            if (it >= (uint32_t)S) mbar_wait((uint32_t)__cvta_generic_to_shared(&empty_bar[s]), ((it / (uint32_t)S) - 1u) & 1u);
+            if (!more) {
+                if (lane == 0) {
+                    tile_of[s] = 0xFFFFFFFFu;
+                    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(full_a) : "memory");
+                }
+                break;
+            }
+            sched.prefetch();
+            if (lane == 0) {
+                int32_t c[kTmapRank];
+                uint32_t r = tile_id;
+#pragma unroll
+                for (int d = 0; d < kTmapRank; ++d) {
+                    const uint32_t qq = fd_div(r, P.gdiv[d]);
+                    c[d] = (int32_t)(r - qq * P.gdiv[d].d) * P.step[d];
+                    r = qq;
+                    coord[s][d] = c[d];
+                }
+                tile_of[s] = tile_id;
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(full_a), "r"(tile_bytes * (BETA ? 2u : 1u)) : "memory");
+                const uint32_t in_s = base + (uint32_t)s * 2u * P.buf_bytes, out_s = in_s + P.buf_bytes;
+                int box = 0;
+                for (int bj = 0; bj < P.nbB; ++bj)
+                    for (int bi = 0; bi < P.nbA; ++bi, ++box) {
+                        const int ca = c[0] + bi * P.box0[0];
+                        if constexpr (FLAVOUR == 0) {
+                            const int cb = c[1] + bj * P.box0[1];
+                            tmap_load(in_s + (uint32_t)box * P.box_bytes, &mapA, full_a, ca * P.upe, cb, c[2], c[3], c[4]);
+                            if constexpr (BETA) tmap_load(out_s + (uint32_t)box * P.box_bytes, &mapB, full_a, cb * P.upe, ca, c[2], c[3], c[4]);
+                        } else {
+                            tmap_load(in_s + (uint32_t)box * P.box_bytes, &mapA, full_a, ca * P.upe, c[1], c[2], c[3], c[4]);
+                            if constexpr (BETA) tmap_load(out_s + (uint32_t)box * P.box_bytes, &mapB, full_a, ca * P.upe, c[1], c[2], c[3], c[4]);
+                        }
+                    }
+            }
+            more = sched.next<true>(tile_id, P.n_tiles);
+            __syncwarp();
+        }
+    } else if (tid < 64) {
+        // ------------------------------------------------------------------ store warp (one thread: bulk groups are per thread)
+        if (tid == 32) {
+            for (uint32_t it = 0;; ++it) {
+                const int s = (int)(it % (uint32_t)S);
+                mbar_wait((uint32_t)__cvta_generic_to_shared(&done_bar[s]), (it / (uint32_t)S) & 1u);
+                if (tile_of[s] == 0xFFFFFFFFu) break;
+                int32_t c[kTmapRank];
+#pragma unroll
+                for (int d = 0; d < kTmapRank; ++d) c[d] = coord[s][d];
+                const uint32_t in_s = base + (uint32_t)s * 2u * P.buf_bytes;
+                const uint32_t src_s = passthrough ? in_s : in_s + P.buf_bytes;
+                int box = 0;
+                for (int bj = 0; bj < P.nbB; ++bj)
+                    for (int bi = 0; bi < P.nbA; ++bi, ++box) {
+                        const int ca = c[0] + bi * P.box0[0];
+                        if constexpr (FLAVOUR == 0)
+                            tmap_store(&mapB, src_s + (uint32_t)box * P.box_bytes, (c[1] + bj * P.box0[1]) * P.upe, ca, c[2], c[3], c[4]);
+                        else
+                            tmap_store(&mapB, src_s + (uint32_t)box * P.box_bytes, ca * P.upe, c[1], c[2], c[3], c[4]);
+                    }
+                asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+                if (it >= 1u) {     // the group of the stage before this one has read its buffers: hand that stage back
+                    asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
+                    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];"
+                                 ::"r"((uint32_t)__cvta_generic_to_shared(&empty_bar[(it - 1u) % (uint32_t)S])) : "memory");
+                }
+            }
+            asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+        }
+    } else {
+        // ------------------------------------------------------------------ consumer warps
+        const int cw = (tid >> 5) - 2;
+        for (uint32_t it = 0;; ++it) {
+            const int s = (int)(it % (uint32_t)S);
+            mbar_wait((uint32_t)__cvta_generic_to_shared(&full_bar[s]), (it / (uint32_t)S) & 1u);
+            const bool end = tile_of[s] == 0xFFFFFFFFu;
+            if (!end && !passthrough) {
+                const uint32_t in_s = base + (uint32_t)s * 2u * P.buf_bytes, out_s = in_s + P.buf_bytes;
+                if constexpr (FLAVOUR == 0) {
+                    constexpr uint32_t PB = 1024u * V;          // bytes of one plane: 8 V rows of 128 bytes
+                    const int n_planes = nbox * P.planes;
+                    for (int pl = cw; pl < n_planes; pl += n_cons_warps) {
+                        const uint32_t ip = in_s + (uint32_t)pl * PB, op = out_s + (uint32_t)pl * PB;
+#pragma unroll
+                        for (int j = 0; j < 2; ++j) {
+                            int A2, B2;
+                            tmap_lane_map<V>(lane, j, A2, B2);
+                            Chunk r[V];
+#pragma unroll
+                            for (int d = 0; d < V; ++d) {
+                                const int row = V * B2 + d;
+                                r[d].u = lds128(ip + (uint32_t)(row * 128 + ((A2 ^ (row & 7)) << 4)));
+                            }
+#pragma unroll
+                            for (int d = 0; d < V; ++d) {
+                                const int row = V * A2 + d;
+                                const uint32_t oa = op + (uint32_t)(row * 128 + ((B2 ^ (row & 7)) << 4));
+                                Chunk o, b;
+                                if constexpr (BETA) b.u = lds128(oa);
+#pragma unroll
+                                for (int e = 0; e < V; ++e) {
+                                    T x = scale(alpha, r[e].e[d]);
+                                    if constexpr (BETA) x = add(x, scale(beta, b.e[e]));
+                                    o.e[e] = x;
+                                }
+                                sts128(oa, o.u);
+                            }
+                        }
+                    }
+                } else {
+                    const int n_chunks = (int)(tile_bytes >> 4);
+                    const int n_cons = n_cons_warps * 32;
+                    for (int ch = cw * 32 + lane; ch < n_chunks; ch += n_cons) {
+                        Chunk a, b, o;
+                        a.u = lds128(in_s + ((uint32_t)ch << 4));
+                        if constexpr (BETA) b.u = lds128(out_s + ((uint32_t)ch << 4));
+#pragma unroll
+                        for (int e = 0; e < V; ++e) {
+                            T x = scale(alpha, a.e[e]);
+                            if constexpr (BETA) x = add(x, scale(beta, b.e[e]));
+                            o.e[e] = x;
+                        }
+                        sts128(out_s + ((uint32_t)ch << 4), o.u);
+                    }
+                }
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // the stores read what was just written
+            }
+            __syncwarp();
+            if (lane == 0)
+                asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"((uint32_t)__cvta_generic_to_shared(&done_bar[s])) : "memory");
+            if (end) break;
+        }
+    }
+}
+
+}  // namespace ttc

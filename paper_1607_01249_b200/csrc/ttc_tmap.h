@@ -1,0 +1,49 @@
+// ttc_tmap.h -- parameter blocks of the tensor-map kernel (tmap_kernel, ttc_tmap.cuh): tiles move between global and
+// shared memory as <= 5-D boxes of a CUtensorMap (cp.async.bulk.tensor, SASS UTMALDG / UTMASTG) in BOTH directions;
+// the threads never touch global memory.  north_star K2 "TMA tensor-map loads and stores of <= 5-D boxes where the
+// strides allow"; SURVEY.md section 7 step 7 and the TMA feasibility paragraph of 8(d).  Plain data, host and device.
+#pragma once
+#include <cstdint>
+
+#include "ttc_params.h"
+
+namespace ttc {
+
+constexpr int kTmapRank = 5;         // every map is encoded with 5 dimensions (missing ones have extent 1)
+constexpr int kTmapMaxStages = 4;
+constexpr int kTmapMaxBoxes = 4;     // boxes per tile (nbA * nbB)
+
+// flavour 0 (transposing: the stride-1 index of A is not the stride-1 index of B)
+//   A's map lists the canonical indices as (a0, b0, o1, o2, o3), B's map as (b0, a0, o1, o2, o3); a box has 128 bytes
+//   along a0 resp. b0 (SWIZZLE_128B) and 128 / es elements along the other of the two, so it is a stack of
+//   `planes` square 2-D planes (one per (o1, o2, o3) of the box) that the consumer warps transpose from the in-box
+//   to the out-box with 16-byte shared-memory accesses only.
+// flavour 1 (copy class: a0 == b0): both maps list the indices in B's order, in-box and out-box have the same
+//   layout (no swizzle), the threads only apply alpha and beta chunk by chunk -- or nothing at all for a real
+//   alpha == 1, beta == 0, when the box is stored straight from the buffer it was loaded into.
+struct TmapParams {
+    int flavour;
+    int dyn;                  // work distribution (WorkSched mode)
+    uint32_t* ctr;            // atomic work counter (mode 2), filled in at launch
+    uint32_t n_tiles;
+    int stages, threads;
+    int nbA, nbB;             // boxes per tile along map dimension 0 of A / of B (flavour 1: nbB == 1)
+    int planes;               // flavour 0: planes per box
+    uint32_t box_bytes;       // bytes of one box (the same for A's and B's map)
+    uint32_t buf_bytes;       // nbA * nbB * box_bytes rounded up to 128 (a box's shared-memory address must be 128-byte aligned)
+    int upe;                  // map units per element along a map's dimension 0 (2 for 16-byte elements: 8-byte units)
+    FastDiv gdiv[kTmapRank];  // number of tiles along A-map dimension d
+    int32_t step[kTmapRank];  // tile extent (elements) along A-map dimension d
+    int32_t box0[2];          // box extent (elements) along A-map dimension 0 and 1 (the step between the boxes of a tile)
+};
+
+// What cuTensorMapEncodeTiled needs beside the base address (filled by the planner; encoded at launch).
+struct TmapEncode {
+    int unit_bytes;                       // 4 or 8: CU_TENSOR_MAP_DATA_TYPE_UINT32 / UINT64
+    int swizzle128;                       // 1: CU_TENSOR_MAP_SWIZZLE_128B, 0: none
+    uint64_t dimA[kTmapRank], dimB[kTmapRank];
+    uint64_t strideA[kTmapRank - 1], strideB[kTmapRank - 1];   // bytes, dimensions 1..4
+    uint32_t boxA[kTmapRank], boxB[kTmapRank];
+};
+
+}  // namespace ttc
