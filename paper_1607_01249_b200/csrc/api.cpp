@@ -12,6 +12,7 @@
 #include <cstring>
 #include <map>
 #include <mutex>
+#include <set>
 #include <string>
 #include <vector>
 
@@ -226,6 +227,10 @@ ttc_status tune(ttc_plan_s* p, int top_k, int reps, int budget_ms) {
         float best_us = 0.f;
         const auto t_start = std::chrono::steady_clock::now();
         bool over_budget = false;
+        // the best-ranked tensor-map candidates are timed wherever the (ring-kernel-fitted) cost model puts them
+        std::set<int> also;
+        for (int i = 0; i < (int)cs.size() && (int)also.size() < 4; ++i)
+            if (cs[i].info.kernel == TTC_KERNEL_TENSORMAP) also.insert(i);
         for (int i = 0; i < (int)cs.size(); ++i) {
             // rank order; after the first 16 the list's time budget can end the search
             if (i >= 16 && !over_budget) {
@@ -233,7 +238,7 @@ ttc_status tune(ttc_plan_s* p, int top_k, int reps, int budget_ms) {
                 over_budget = budget_ms > 0 && ms > budget_ms;
             }
             // the scalar fallback is always timed so that it is known to work
-            if ((i >= n || over_budget) && i != p->scalar[which]) continue;
+            if ((i >= n || over_budget) && i != p->scalar[which] && !also.count(i)) continue;
             if (!ensure_prepared(p, which, i)) { ++p->tune_errors; continue; }
             if (launch_candidate(cs[i], p->dtype, p->dtype_a, alpha, beta, next_a(), next_b(), st, p->sched_ctr) != 0) {
                 cudaGetLastError();   // a failed launch of OUR scratch run: cleared, and counted in ttc_info.tune_errors
@@ -767,9 +772,20 @@ ttc_status ttc_plan_specialize(ttc_plan_t p) {
     cudaEventCreate(&e1);
     ttc_status rc = TTC_ERR_UNSUPPORTED;      // stays so if neither list's winner is a ring-kernel candidate
     for (int which = 0; which < 2; ++which) {
-        const int idx = p->winner[which];
-        if (idx < 0) continue;
+        const int win = p->winner[which];
+        if (win < 0) continue;
+        int idx = win;
+        if (p->cands[which][win].info.kernel == TTC_KERNEL_TENSORMAP) {
+            // a tensor-map winner has no twin: the fastest timed ring / direct candidate gets one and has to beat the winner
+            idx = -1;
+            const std::vector<Candidate>& cs = p->cands[which];
+            for (int i = 0; i < (int)cs.size(); ++i)
+                if ((cs[i].info.kernel == TTC_KERNEL_TMA || cs[i].info.kernel == TTC_KERNEL_COPY) && cs[i].info.tuned_us > 0.f &&
+                    (idx < 0 || cs[i].info.tuned_us < cs[idx].info.tuned_us)) idx = i;
+            if (idx < 0 || !ensure_prepared(p, which, win)) continue;
+        }
         Candidate& c = p->cands[which][idx];
+        const Candidate& gen = p->cands[which][win];
         if ((c.info.kernel != TTC_KERNEL_TMA && c.info.kernel != TTC_KERNEL_COPY) || !ensure_prepared(p, which, idx)) continue;
         if (p->spec[which]) { release_specialized(p->spec[which]); p->spec[which] = nullptr; p->spec_active[which] = false; }
         std::string err;
@@ -787,7 +803,7 @@ ttc_status ttc_plan_specialize(ttc_plan_t p) {
                 cudaEventRecord(e0, nullptr);
                 for (int i = 0; i < 4 && ok; ++i)
                     ok = (v ? launch_specialized(k, c, alpha, beta, a, b, nullptr)
-                            : launch_candidate(c, p->dtype, p->dtype_a, alpha, beta, a, b, nullptr, p->sched_ctr)) == 0;
+                            : launch_candidate(gen, p->dtype, p->dtype_a, alpha, beta, a, b, nullptr, p->sched_ctr)) == 0;
                 cudaEventRecord(e1, nullptr);
                 if (cudaEventSynchronize(e1) != cudaSuccess) ok = false;
                 float ms = 0.f;
@@ -803,6 +819,11 @@ ttc_status ttc_plan_specialize(ttc_plan_t p) {
         p->generic_us[which] = t[0][2];
         p->spec_us[which] = t[1][2];
         p->spec_active[which] = t[1][2] < t[0][2] || env_int("TTC_SPECIALIZE", 0) == 2;   // 2: use the twin whatever its time (tests)
+        if (p->spec_active[which] && idx != win) {       // the twin of the runner-up beats the tensor-map winner
+            p->winner[which] = idx;
+            for (int& x : p->fallback[which]) x = -2;
+            for (int& x : p->nomap[which]) x = -2;
+        }
         rc = TTC_OK;
     }
     cudaEventDestroy(e0);

@@ -879,7 +879,7 @@ void add_tmap(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, 
         if (box_bytes < 1024 || tile_bytes > 64 * 1024 || nbA * nbB > kTmapMaxBoxes) return;
         int stages = 0;
         for (int st = 4; st >= 2; --st)
-            if (st * 2 * tile_bytes + 1024 <= std::min<int64_t>(max_smem, st == 2 ? 160 * 1024 : 100 * 1024)) { stages = st; break; }
+            if (st * 2 * tile_bytes + 1024 <= std::min<int64_t>(max_smem, 100 * 1024)) { stages = st; break; }   // >= 2 CTAs per SM
         if (!stages) return;
         uint64_t n_tiles = 1;
         double padded = 1.0, real = 1.0;
@@ -920,7 +920,7 @@ void add_tmap(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, 
         // ranked just behind the best fitted ring candidates (fitted costs are time / ideal time), tiles that stick
         // out of the tensor cost their share of wasted shared-memory work; the tuner decides
         const double waste = padded / real;
-        I.est_cost = (float)((1.10 + 0.01 * n_added) * waste * (tile_bytes < 8192 ? 1.15 : 1.0));
+        I.est_cost = (float)((1.04 + 0.01 * n_added) * waste * (tile_bytes < 8192 ? 1.15 : 1.0));
         cand.feat[2] = (float)waste;
         cand.feat[4] = (float)tile_bytes;
         cand.feat[5] = (float)n_tiles;
@@ -945,11 +945,10 @@ void add_tmap(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, 
     if (flavour == 0) {
         const int64_t plane_bytes = 128 * (int64_t)T;
         struct Var { int dist, kb, nbA, nbB; };
-        static const Var vars[] = {{0, 16, 1, 1}, {1, 16, 1, 1}, {2, 16, 1, 1}, {0, 8, 2, 1}, {1, 8, 1, 2}, {2, 8, 2, 2},
-                                   {0, 8, 1, 1}, {1, 8, 1, 1}, {0, 32, 1, 1}, {1, 32, 1, 1}};
+        static const Var vars[] = {{0, 16, 1, 1}, {1, 16, 1, 1}, {0, 8, 2, 1}, {1, 8, 1, 2}, {2, 16, 1, 1}, {0, 8, 1, 1}, {1, 8, 1, 1},
+                                   {2, 4, 2, 2}};
         for (const Var& v : vars) {
-            if (c.d[0].e < (int64_t)v.nbA * T && v.nbA > 1) continue;
-            if (c.d[q].e < (int64_t)v.nbB * T && v.nbB > 1) continue;
+            if (c.d[0].e <= (int64_t)(v.nbA - 1) * T || c.d[q].e <= (int64_t)(v.nbB - 1) * T) continue;
             const int64_t want = std::max<int64_t>(1, (int64_t)v.kb * 1024 / plane_bytes);
             if (v.dist == 0) fill(othA, want, pe);
             else if (v.dist == 1) fill(othB, want, pe);
@@ -972,9 +971,9 @@ void add_tmap(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, 
         }
         if (othA.empty()) {      // 2-D: a tile is a few planes side by side
             for (int i = 0; i < c.rank; ++i) pe[i] = 1;
-            static const int nb[][2] = {{2, 2}, {4, 1}, {1, 4}, {2, 1}, {1, 2}};
+            static const int nb[][2] = {{2, 2}, {4, 1}, {1, 4}, {4, 2}, {2, 4}, {2, 1}, {1, 2}};
             for (auto& b : nb)
-                if (c.d[0].e >= (int64_t)b[0] * T && c.d[q].e >= (int64_t)b[1] * T) emit(pe, 0, b[0], b[1]);
+                if (c.d[0].e > (int64_t)(b[0] - 1) * T && c.d[q].e > (int64_t)(b[1] - 1) * T) emit(pe, 0, b[0], b[1]);
         }
     } else {
         // copy class: rows of up to 256 map units along the shared leading index, then rows until the box has 8-32 KB
@@ -985,7 +984,7 @@ void add_tmap(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, 
             const int64_t pieces = (e0u + 255) / 256;
             b0 = (int32_t)(((e0u + pieces - 1) / pieces + gran - 1) / gran * gran);
         }
-        for (int kb : {16, 8, 32})
+        for (int kb : {16, 8})
             for (int dist = 0; dist < 2; ++dist) {
                 const int64_t want = std::max<int64_t>(1, (int64_t)kb * 1024 / ((int64_t)b0 * unit));
                 fill(dist == 0 ? othB : othA, want, pe);

@@ -10,8 +10,9 @@
 //                       quarter-warp access touches all 32 banks once; flavour 1: alpha/beta chunk by chunk; then
 //                       fence.proxy.async and one arrival per warp on `done`
 //   store warp (lane 0) waits for `done`, issues cp.async.bulk.tensor.5d stores (UTMASTG) of the out-boxes, commits
-//                       them as one bulk group and hands the PREVIOUS stage back (`empty`) once its group has
-//                       finished reading shared memory
+//                       them as one bulk group and hands the PREVIOUS stage's out-buffer back (`outfree`) once its
+//                       group has finished reading shared memory.  The in-buffer of a stage is free for the next load
+//                       as soon as its consumers are `done`, so loads run stages - 1 tiles ahead of the consumers
 //
 // Boxes that stick out of the tensor need no code: loads fill with zeros, stores clip.  No thread issues a global
 // load or store.  Arithmetic: products and sums rounded separately, exactly as the other kernels (readings A7/A10).
@@ -84,9 +85,11 @@ tmap_kernel(const __grid_constant__ TmapParams P, const __grid_constant__ CUtens
 
     __shared__ __align__(16) uint4 sched_resp;
     __shared__ __align__(8) uint64_t sched_bar;
-    __shared__ __align__(8) uint64_t full_bar[kTmapMaxStages], done_bar[kTmapMaxStages], empty_bar[kTmapMaxStages];
-    __shared__ int32_t coord[kTmapMaxStages][kTmapRank];
-    __shared__ uint32_t tile_of[kTmapMaxStages];
+    __shared__ __align__(8) uint64_t full_bar[kTmapMaxStages], done_bar[kTmapMaxStages], outfree_bar[kTmapMaxStages];
+    // tile origin and id per stage, two deep: the producer may fill a stage again (its consumers are done) before the
+    // store thread has read where the stage's previous tile goes; it cannot get two uses ahead of it
+    __shared__ int32_t coord[kTmapMaxStages][2][kTmapRank];
+    __shared__ uint32_t tile_of[kTmapMaxStages][2];
 
     const int tid = threadIdx.x, lane = tid & 31;
     const int S = P.stages;
@@ -98,7 +101,7 @@ tmap_kernel(const __grid_constant__ TmapParams P, const __grid_constant__ CUtens
         for (int s = 0; s < S; ++s) {
             asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"((uint32_t)__cvta_generic_to_shared(&full_bar[s])));
             asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(&done_bar[s])), "r"(n_cons_warps));
-            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"((uint32_t)__cvta_generic_to_shared(&empty_bar[s])));
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"((uint32_t)__cvta_generic_to_shared(&outfree_bar[s])));
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -116,11 +119,17 @@ tmap_kernel(const __grid_constant__ TmapParams P, const __grid_constant__ CUtens
         bool more = true;
         for (uint32_t it = 0;; ++it) {
             const int s = (int)(it % (uint32_t)S);
+            const int u = (int)((it / (uint32_t)S) & 1u);
             const uint32_t full_a = (uint32_t)__cvta_generic_to_shared(&full_bar[s]);
-            if (it >= (uint32_t)S) mbar_wait((uint32_t)__cvta_generic_to_shared(&empty_bar[s]), ((it / (uint32_t)S) - 1u) & 1u);
+            if (it >= (uint32_t)S) {
+                // the in-buffer is free once the consumers are done with it; the out-buffer (which only beta != 0 loads
+                // into) once the store of its last tile has read it (passthrough: that store read the in-buffer)
+                mbar_wait((uint32_t)__cvta_generic_to_shared(&done_bar[s]), ((it / (uint32_t)S) - 1u) & 1u);
+                if (BETA || passthrough) mbar_wait((uint32_t)__cvta_generic_to_shared(&outfree_bar[s]), ((it / (uint32_t)S) - 1u) & 1u);
+            }
             if (!more) {
                 if (lane == 0) {
-                    tile_of[s] = 0xFFFFFFFFu;
+                    tile_of[s][u] = 0xFFFFFFFFu;
                     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(full_a) : "memory");
                 }
                 break;
@@ -134,9 +143,9 @@ tmap_kernel(const __grid_constant__ TmapParams P, const __grid_constant__ CUtens
                     const uint32_t qq = fd_div(r, P.gdiv[d]);
                     c[d] = (int32_t)(r - qq * P.gdiv[d].d) * P.step[d];
                     r = qq;
-                    coord[s][d] = c[d];
+                    coord[s][u][d] = c[d];
                 }
-                tile_of[s] = tile_id;
+                tile_of[s][u] = tile_id;
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                 asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(full_a), "r"(tile_bytes * (BETA ? 2u : 1u)) : "memory");
                 const uint32_t in_s = base + (uint32_t)s * 2u * P.buf_bytes, out_s = in_s + P.buf_bytes;
@@ -162,11 +171,12 @@ tmap_kernel(const __grid_constant__ TmapParams P, const __grid_constant__ CUtens
         if (tid == 32) {
             for (uint32_t it = 0;; ++it) {
                 const int s = (int)(it % (uint32_t)S);
-                mbar_wait((uint32_t)__cvta_generic_to_shared(&done_bar[s]), (it / (uint32_t)S) & 1u);
-                if (tile_of[s] == 0xFFFFFFFFu) break;
+                const int u = (int)((it / (uint32_t)S) & 1u);
+                mbar_wait((uint32_t)__cvta_generic_to_shared(&done_bar[s]), (uint32_t)u);
+                if (tile_of[s][u] == 0xFFFFFFFFu) break;
                 int32_t c[kTmapRank];
 #pragma unroll
-                for (int d = 0; d < kTmapRank; ++d) c[d] = coord[s][d];
+                for (int d = 0; d < kTmapRank; ++d) c[d] = coord[s][u][d];
                 const uint32_t in_s = base + (uint32_t)s * 2u * P.buf_bytes;
                 const uint32_t src_s = passthrough ? in_s : in_s + P.buf_bytes;
                 int box = 0;
@@ -179,10 +189,10 @@ tmap_kernel(const __grid_constant__ TmapParams P, const __grid_constant__ CUtens
                             tmap_store(&mapB, src_s + (uint32_t)box * P.box_bytes, ca * P.upe, c[1], c[2], c[3], c[4]);
                     }
                 asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-                if (it >= 1u) {     // the group of the stage before this one has read its buffers: hand that stage back
+                if (it >= 1u) {     // the group of the stage before this one has read its out-buffer: hand that buffer back
                     asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
                     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];"
-                                 ::"r"((uint32_t)__cvta_generic_to_shared(&empty_bar[(it - 1u) % (uint32_t)S])) : "memory");
+                                 ::"r"((uint32_t)__cvta_generic_to_shared(&outfree_bar[(it - 1u) % (uint32_t)S])) : "memory");
                 }
             }
             asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
@@ -193,8 +203,11 @@ tmap_kernel(const __grid_constant__ TmapParams P, const __grid_constant__ CUtens
         for (uint32_t it = 0;; ++it) {
             const int s = (int)(it % (uint32_t)S);
             mbar_wait((uint32_t)__cvta_generic_to_shared(&full_bar[s]), (it / (uint32_t)S) & 1u);
-            const bool end = tile_of[s] == 0xFFFFFFFFu;
+            const bool end = tile_of[s][(it / (uint32_t)S) & 1u] == 0xFFFFFFFFu;
             if (!end && !passthrough) {
+                // beta == 0: nobody has waited for the store that last read this out-buffer yet
+                if constexpr (!BETA)
+                    if (it >= (uint32_t)S) mbar_wait((uint32_t)__cvta_generic_to_shared(&outfree_bar[s]), ((it / (uint32_t)S) - 1u) & 1u);
                 const uint32_t in_s = base + (uint32_t)s * 2u * P.buf_bytes, out_s = in_s + P.buf_bytes;
                 if constexpr (FLAVOUR == 0) {
                     constexpr uint32_t PB = 1024u * V;          // bytes of one plane: 8 V rows of 128 bytes

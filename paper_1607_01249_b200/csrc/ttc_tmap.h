@@ -11,7 +11,7 @@ namespace ttc {
 
 constexpr int kTmapRank = 5;         // every map is encoded with 5 dimensions (missing ones have extent 1)
 constexpr int kTmapMaxStages = 4;
-constexpr int kTmapMaxBoxes = 4;     // boxes per tile (nbA * nbB)
+constexpr int kTmapMaxBoxes = 8;     // boxes per tile (nbA * nbB)
 
 // flavour 0 (transposing: the stride-1 index of A is not the stride-1 index of B)
 //   A's map lists the canonical indices as (a0, b0, o1, o2, o3), B's map as (b0, a0, o1, o2, o3); a box has 128 bytes
