@@ -577,9 +577,10 @@ def run_ours(args) -> None:
         dom_us = sum(r["us"] for r in dom)
         achieved = works[0].algorithmic_bytes * len(dom) / dom_us / 1e3
         n_ring = sum(1 for r in dom if r["kernel"] == "tma")
+        n_tmap = sum(1 for r in dom if r["kernel"] == "tensormap")
         roofline = {"bound": "hbm",
-                    "kernel": "K2/K3 transposing kernels (ring_kernel: %d, tile_kernel: %d) of %d launches per step" % (
-                        n_ring, len(dom) - n_ring, len(per_perm)),
+                    "kernel": "K2/K3 transposing kernels (ring_kernel: %d, tmap_kernel: %d, tile_kernel: %d) of %d launches per step" % (
+                        n_ring, n_tmap, len(dom) - n_ring - n_tmap, len(per_perm)),
                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                     "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
                     "avg_launch_us": dom_us / len(dom), "algorithmic_bytes_per_launch": works[0].algorithmic_bytes,

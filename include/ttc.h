@@ -42,6 +42,8 @@
  *   TTC_SPECIALIZE=1      ttc_plan also runs ttc_plan_specialize (NVRTC size-specialised winners)
  *   TTC_PDL=0             launch without programmatic dependent launch (default: with)
  *   TTC_RING=0|2|4        largest ring of tile buffers of the warp-specialised kernel (0: none; default 4)
+ *   TTC_VARIANTS=bits     candidate flavours to generate: 1 staggered-gather ring, 2 shifted-row ring, 4 tensor-map
+ *                         kernels (default 7: all)
  */
 #ifndef TTC_H_
 #define TTC_H_
