@@ -22,6 +22,8 @@
 
 #include <cstdio>
 #include <cstdlib>
+#include <cstring>
+#include <map>
 #include <mutex>
 #include <set>
 #include <type_traits>
@@ -217,6 +219,71 @@ static bool encode_maps(const TmapEncode& me, const void* A, void* B, CUtensorMa
                CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+template <int DT>
+static KernelFn tmapu_fn_dt(bool beta) { return beta ? (KernelFn)tmapu_kernel<DT, true> : (KernelFn)tmapu_kernel<DT, false>; }
+
+static KernelFn get_tmapu_fn(int dt, const Candidate& c) {
+    switch (dt) {
+        case TTC_F32: return tmapu_fn_dt<TTC_F32>(c.beta_nz);
+        case TTC_F64: return tmapu_fn_dt<TTC_F64>(c.beta_nz);
+        case TTC_C64: return tmapu_fn_dt<TTC_C64>(c.beta_nz);
+    }
+    return nullptr;     // 16-byte elements are always 16-byte aligned: flavours 0 and 1
+}
+
+// The 2 V maps per tensor of the residue-class flavour: [skew * 2 + lo] has extents (e + skew, rows of the classes with
+// (lo = 0) or without (lo = 1) one row more, every aligned offset), see ttc_tmap.h.  `A` and `B` are the base addresses rounded DOWN to 16 bytes.
+static bool encode_class_maps(const TmapUEncode& ue, const void* A, void* B, TmapUSet* set) {
+    EncodeTiledFn enc = encode_tiled_fn();
+    if (!enc) return false;
+    const int V = 16 / ue.es, T = 128 / ue.es;
+    const CUtensorMapDataType dt = ue.es == 4 ? CU_TENSOR_MAP_DATA_TYPE_UINT32 : CU_TENSOR_MAP_DATA_TYPE_UINT64;
+    static const cuuint32_t ones[kTmapRank] = {1, 1, 1, 1, 1};
+    const cuuint32_t box[kTmapRank] = {(cuuint32_t)T, (cuuint32_t)(T / V), 1, 1, 1};
+    for (int side = 0; side < 2; ++side) {
+        const int64_t e_in = side == 0 ? ue.e0 : ue.eq, e_row = side == 0 ? ue.eq : ue.e0;
+        const int64_t s_row = side == 0 ? ue.sqA : ue.s0B, span = side == 0 ? ue.spanA : ue.spanB;
+        void* base = side == 0 ? const_cast<void*>(A) : B;
+        CUtensorMap* out = side == 0 ? set->a : set->b;
+        for (int sk = 0; sk < V; ++sk)
+            for (int lo = 0; lo < 2; ++lo) {       // 0: the classes below e_row % V (one row more), 1: the others
+                const int64_t rows = e_row / V + (lo == 0 ? 1 : 0);
+                const cuuint64_t dims[kTmapRank] = {(cuuint64_t)(e_in + sk), (cuuint64_t)(rows < 1 ? 1 : rows), (cuuint64_t)(span / V + 2), 1, 1};
+                const cuuint64_t strides[kTmapRank - 1] = {(cuuint64_t)(V * s_row * ue.es), 16, 16, 16};
+                if (enc(&out[sk * 2 + lo], dt, kTmapRank, base, dims, strides, box, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                        CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+                    return false;
+            }
+    }
+    return true;
+}
+
+// Encoding 4 V maps costs several microseconds of host time: the sets of the last few (shape, A, B) are kept.
+static bool class_maps_cached(const TmapUEncode& ue, const void* A, void* B, TmapUSet* set) {
+    struct Key {
+        TmapUEncode ue; const void* a; void* b;
+        bool operator<(const Key& o) const { return std::memcmp(this, &o, sizeof(Key)) < 0; }
+    };
+    static std::mutex mu;
+    static std::map<Key, TmapUSet> cache;
+    Key k;
+    std::memset(&k, 0, sizeof(k));
+    k.ue = ue;
+    k.a = A;
+    k.b = B;
+    std::lock_guard<std::mutex> lk(mu);
+    auto it = cache.find(k);
+    if (it != cache.end()) { *set = it->second; return true; }
+    if (!encode_class_maps(ue, A, B, set)) return false;
+    if (cache.size() >= 64) cache.clear();
+    cache.emplace(k, *set);
+    return true;
+}
+
+static uint32_t tmapu_smem_bytes(const TmapUParams& up) {
+    return (uint32_t)up.stages * 2u * (uint32_t)up.nP * (uint32_t)up.V * 1024u + 1024u;
+}
+
 static uint32_t tmap_smem_bytes(const TmapParams& mp) {
     return (uint32_t)mp.stages * 2u * mp.buf_bytes + 1024u;     // + alignment slack
 }
@@ -256,9 +323,10 @@ int prepare_candidate(Candidate* cand, ttc_dtype dtype, ttc_dtype dtype_a, int s
         return 0;
     }
     if (cand->info.kernel == TTC_KERNEL_TENSORMAP) {
-        KernelFn fn = dtype == dtype_a ? get_tmap_fn((int)dtype, *cand) : nullptr;
+        const bool classes = cand->mp.flavour == 2;
+        KernelFn fn = dtype != dtype_a ? nullptr : classes ? get_tmapu_fn((int)dtype, *cand) : get_tmap_fn((int)dtype, *cand);
         if (!fn || !encode_tiled_fn()) return (int)cudaErrorInvalidValue;
-        const int smem = (int)tmap_smem_bytes(cand->mp);
+        const int smem = (int)(classes ? tmapu_smem_bytes(cand->up) : tmap_smem_bytes(cand->mp));
         int optin = 0;
         int rc = raise_smem_limit(fn, &optin);
         if (rc != 0) return rc;
@@ -333,6 +401,22 @@ int launch_candidate(const Candidate& cand, ttc_dtype dtype, ttc_dtype dtype_a, 
     }
     NoBatch none;
     Scalar al = alpha, be = beta;
+    if (cand.info.kernel == TTC_KERNEL_TENSORMAP && cand.mp.flavour == 2) {
+        KernelFn fn = dtype == dtype_a ? get_tmapu_fn((int)dtype, cand) : nullptr;
+        if (!fn) return (int)cudaErrorInvalidValue;
+        const int es = cand.ue.es;
+        const uintptr_t a16 = (uintptr_t)A & ~(uintptr_t)15, b16 = (uintptr_t)B & ~(uintptr_t)15;
+        alignas(64) TmapUSet set;
+        if (!class_maps_cached(cand.ue, (const void*)a16, (void*)b16, &set)) return (int)cudaErrorInvalidValue;
+        cfg.blockDim = dim3((unsigned)cand.up.threads, 1, 1);
+        cfg.dynamicSmemBytes = (size_t)cand.info.smem_bytes;
+        TmapUParams up = cand.up;
+        up.ctr = sched_ctr;
+        up.skewA0 = (int)(((uintptr_t)A - a16) / (uintptr_t)es);
+        up.skewB0 = (int)(((uintptr_t)B - b16) / (uintptr_t)es);
+        void* uargs[4] = {&up, &set, &al, &be};
+        return (int)cudaLaunchKernelExC(&cfg, fn, uargs);
+    }
     if (cand.info.kernel == TTC_KERNEL_TENSORMAP) {
         KernelFn fn = dtype == dtype_a ? get_tmap_fn((int)dtype, cand) : nullptr;
         if (!fn) return (int)cudaErrorInvalidValue;

@@ -993,6 +993,138 @@ void add_tmap(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, 
     }
 }
 
+
+// Tensor-map candidates for more than 5 canonical indices (flavour 2, ttc_tmap.h): every index beyond the T x T plane is
+// folded into one map dimension.  Strides must still be multiples of 16 bytes and the bases 16-byte aligned: the hardware
+// refuses a box whose first byte is not 16-byte aligned ("illegal instruction"), so the skew the residue classes were
+// designed to absorb cannot be expressed as a coordinate (round 2).
+void add_tmapu(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, int sched, int max_smem, std::vector<Candidate>* out) {
+    if (dtype != dtype_a || c.rank <= kTmapRank) return;
+    const int es = elem_size(dtype);
+    if (es > 8) return;
+    const int V = 16 / es, T = 128 / es;
+    const int q = c.orderB[0];
+    if (q == 0 || c.d[0].sA != 1 || c.d[q].sB != 1) return;
+    for (int i = 0; i < c.rank; ++i) {
+        if (c.d[i].e >= kInt31 / 2) return;
+        if (i != 0 && (c.d[i].sA * es) % 16 != 0) return;
+        if (i != q && (c.d[i].sB * es) % 16 != 0) return;
+    }
+    if (c.d[0].e < T / 2 || c.d[q].e < T / 2) return;     // more than half of every plane would be padding
+    const int64_t lim = (int64_t)1 << 40;
+    if (c.d[q].sA * es * V >= lim || c.d[0].sB * es * V >= lim) return;
+    if (c.spanA / V >= kInt31 - 4 || c.spanB / V >= kInt31 - 4) return;        // the aligned offset is an int32 coordinate
+    std::vector<int> othA, othB;
+    for (int i = 0; i < c.rank; ++i) if (i != 0 && i != q) othA.push_back(i);
+    for (int k = 0; k < c.rank; ++k) if (c.orderB[k] != 0 && c.orderB[k] != q) othB.push_back(c.orderB[k]);
+    std::set<std::string> seen;
+    int n_added = 0;
+    for (int kb : {16, 8, 4})
+        for (int dist = 0; dist < 2; ++dist) {
+            const int want = std::max(1, std::min(kTmapUMaxPlanes, kb / V));
+            int32_t pe[kMaxRank];
+            for (int i = 0; i < c.rank; ++i) pe[i] = 1;
+            int left = want;
+            for (int i : (dist == 0 ? othA : othB)) {      // planes must divide the extents: no ragged plane stacks
+                if (left < 2) break;
+                int t = 1;
+                for (int d = std::min<int64_t>(left, c.d[i].e); d >= 1; --d)
+                    if (c.d[i].e % d == 0) { t = d; break; }
+                pe[i] = t;
+                left /= t;
+            }
+            std::string key((const char*)pe, sizeof(int32_t) * c.rank);
+            if (!seen.insert(key).second) continue;
+            Candidate cand;
+            cand.beta_nz = beta_nz;
+            TmapUParams& U = cand.up;
+            std::memset(&U, 0, sizeof(U));
+            std::memset(&cand.mp, 0, sizeof(cand.mp));
+            U.V = V;
+            U.T = T;
+            U.nG = c.rank;
+            U.sqA = c.d[q].sA;
+            U.s0B = c.d[0].sB;
+            U.remA = (int)(c.d[q].e % V);
+            U.remB = (int)(c.d[0].e % V);
+            // tile grid: a0, b0, then the others in canonical order
+            int gd[kMaxRank];
+            int n = 0;
+            gd[n++] = 0;
+            gd[n++] = q;
+            for (int i : othA) gd[n++] = i;
+            uint64_t n_tiles = 1;
+            double padded = 1.0, real = 1.0;
+            bool ok = true;
+            for (int k = 0; k < n; ++k) {
+                const int i = gd[k];
+                const int64_t step = k < 2 ? T : pe[i];
+                const int64_t nt = (c.d[i].e + step - 1) / step;
+                U.gdiv[k] = make_fastdiv((uint32_t)nt);
+                U.stepA[k] = k < 2 ? 0 : step * c.d[i].sA;
+                U.stepB[k] = k < 2 ? 0 : step * c.d[i].sB;
+                n_tiles *= (uint64_t)nt;
+                if (n_tiles >= (uint64_t)kInt31) { ok = false; break; }
+                padded *= (double)nt * step;
+                real *= (double)c.d[i].e;
+            }
+            if (!ok) continue;
+            // the planes of a tile: every index combination of the box over the other indices
+            int nP = 1;
+            U.pA[0] = U.pB[0] = 0;
+            for (int i : othA) {
+                const int have = nP;
+                for (int v = 1; v < pe[i]; ++v)
+                    for (int h = 0; h < have; ++h) {
+                        U.pA[nP] = U.pA[h] + (int64_t)v * c.d[i].sA;
+                        U.pB[nP] = U.pB[h] + (int64_t)v * c.d[i].sB;
+                        ++nP;
+                    }
+            }
+            U.nP = nP;
+            const int64_t buf = (int64_t)nP * V * 1024;
+            int stages = 0;
+            for (int st = 4; st >= 2; --st)
+                if (st * 2 * buf + 1024 <= std::min<int64_t>(max_smem, 100 * 1024)) { stages = st; break; }
+            if (!stages) continue;
+            U.dyn = sched;
+            U.n_tiles = (uint32_t)n_tiles;
+            U.stages = stages;
+            U.threads = 192;
+            cand.mp.flavour = 2;                            // what the launcher and prepare_candidate look at
+            cand.mp.dyn = sched;
+            cand.mp.n_tiles = U.n_tiles;
+            cand.mp.stages = stages;
+            cand.mp.threads = U.threads;
+            cand.ue = TmapUEncode{es, c.d[0].e, c.d[q].e, c.d[q].sA, c.d[0].sB, c.spanA, c.spanB};
+            cand.align_a = cand.align_b = 16;
+            ttc_candidate_info& I = cand.info;
+            I.kernel = TTC_KERNEL_TENSORMAP;
+            I.flags = TTC_CAND_TENSORMAP;
+            I.vec_a = I.vec_b = V;
+            I.threads = U.threads;
+            I.loop_order = 0;
+            I.sched = sched;
+            I.n_tiles = (int64_t)n_tiles;
+            I.tile_u = T;
+            I.tile_w = T;
+            I.n_u = 1;
+            I.n_w = 1;
+            for (int i = 0; i < kMaxRank; ++i) I.tile_ext[i] = i < c.rank ? pe[i] : 0;
+            I.tile_ext[0] = T;
+            I.tile_ext[q] = T;
+            const double waste = padded / real;
+            I.est_cost = (float)((1.06 + 0.01 * n_added) * waste * (buf < 8192 ? 1.15 : 1.0));
+            cand.feat[2] = (float)waste;
+            cand.feat[4] = (float)buf;
+            cand.feat[5] = (float)n_tiles;
+            cand.feat[12] = beta_nz ? 1.f : 0.f;
+            cand.feat[13] = (float)TTC_KERNEL_TENSORMAP;
+            out->push_back(cand);
+            ++n_added;
+        }
+}
+
 }  // namespace
 
 void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, int sm_count,
@@ -1030,7 +1162,10 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, boo
 
     // Tensor-map candidates (TTC_VARIANTS bit 2).
     if (variants & 4)
-        for (int sched : scheds) add_tmap(c, dtype, dtype_a, beta_nz, sched, max_smem, out);
+        for (int sched : scheds) {
+            add_tmap(c, dtype, dtype_a, beta_nz, sched, max_smem, out);
+            add_tmapu(c, dtype, dtype_a, beta_nz, sched, max_smem, out);
+        }
 
     // K2 / K3: tiles.  A side = leading indices of A, B side = leading indices of B.
     std::vector<int> orderA, orderB;

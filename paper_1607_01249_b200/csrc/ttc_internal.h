@@ -57,6 +57,8 @@ struct Candidate {
     TileParams tp{};
     TmapParams mp{};             // TTC_KERNEL_TENSORMAP: kernel parameters and what the two tensor maps are encoded from
     TmapEncode me{};
+    TmapUParams up{};            // TTC_KERNEL_TENSORMAP with mp.flavour == 2 (residue classes)
+    TmapUEncode ue{};
     float feat[16] = {0};        // raw inputs of the cost heuristic (plan.cpp), exported for re-fitting
     Recipe recipe{};
     int grid_cap = 0;            // resident CTAs the device holds of this kernel (set by prepare_candidate)

@@ -266,4 +266,180 @@ tmap_kernel(const __grid_constant__ TmapParams P, const __grid_constant__ CUtens
     }
 }
 
+// ------------------------------------------------------------------------------------------
+// tmapu_kernel: the residue-class flavour (ttc_tmap.h) -- strides that are not multiples of 16 bytes, any rank, any
+// element-aligned base.  Same pipeline as tmap_kernel; a plane is V in- and V out-sub-boxes of 1 KB.
+// ------------------------------------------------------------------------------------------
+struct TmapUSet { CUtensorMap a[kTmapUMaxClasses * 2], b[kTmapUMaxClasses * 2]; };   // [skew * 2 + (0: classes with one row more, 1: the others)]
+
+template <int DT, bool BETA>
+__global__ void __launch_bounds__(256)
+tmapu_kernel(const __grid_constant__ TmapUParams P, const __grid_constant__ TmapUSet M, const Scalar alpha_in, const Scalar beta_in) {
+    using T = typename ElemT<DT>::T;
+    constexpr int ES = (int)sizeof(T);
+    constexpr int V = 16 / ES;                 // 4 or 2
+    constexpr int LGV = V == 4 ? 2 : 1;
+    constexpr int TE = 128 / ES;               // plane edge in elements
+    static_assert(V == 4 || V == 2, "residue classes exist for 4- and 8-byte elements only");
+    union Chunk { uint4 u; T e[V]; };
+    TScal<T> alpha, beta;
+    typed(alpha_in, alpha);
+    typed(beta_in, beta);
+
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const uint32_t raw = (uint32_t)__cvta_generic_to_shared(smem_raw);
+    const uint32_t base = (raw + 1023u) & ~1023u;
+    const uint32_t buf_bytes = (uint32_t)P.nP * V * 1024u;
+
+    __shared__ __align__(16) uint4 sched_resp;
+    __shared__ __align__(8) uint64_t sched_bar;
+    __shared__ __align__(8) uint64_t full_bar[kTmapMaxStages], done_bar[kTmapMaxStages], outfree_bar[kTmapMaxStages];
+    __shared__ int64_t off_of[kTmapMaxStages][2][2];      // [stage][use parity][A, B]: offset of the tile's outer indices + base skew
+    __shared__ int32_t org_of[kTmapMaxStages][2][2];      // a_tile, b_tile
+    __shared__ uint32_t tile_of[kTmapMaxStages][2];
+
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int S = P.stages;
+    const int n_cons_warps = ((int)blockDim.x >> 5) - 2;
+    WorkSched sched;
+    sched.init(P.dyn, &sched_bar, &sched_resp, P.ctr);
+    pdl_launch_dependents();
+    if (tid == 0) {
+        for (int s = 0; s < S; ++s) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"((uint32_t)__cvta_generic_to_shared(&full_bar[s])));
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(&done_bar[s])), "r"(n_cons_warps));
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"((uint32_t)__cvta_generic_to_shared(&outfree_bar[s])));
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    pdl_wait();
+
+    if (tid < 32) {
+        // ------------------------------------------------------------------ producer warp
+        uint32_t tile_id = blockIdx.x;
+        bool more = true;
+        for (uint32_t it = 0;; ++it) {
+            const int s = (int)(it % (uint32_t)S);
+            const int u = (int)((it / (uint32_t)S) & 1u);
+            const uint32_t full_a = (uint32_t)__cvta_generic_to_shared(&full_bar[s]);
+            if (it >= (uint32_t)S) {
+                mbar_wait((uint32_t)__cvta_generic_to_shared(&done_bar[s]), ((it / (uint32_t)S) - 1u) & 1u);
+                if constexpr (BETA) mbar_wait((uint32_t)__cvta_generic_to_shared(&outfree_bar[s]), ((it / (uint32_t)S) - 1u) & 1u);
+            }
+            if (!more) {
+                if (lane == 0) {
+                    tile_of[s][u] = 0xFFFFFFFFu;
+                    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(full_a) : "memory");
+                }
+                break;
+            }
+            sched.prefetch();
+            if (lane == 0) {
+                uint32_t r = tile_id;
+                int32_t org[2];
+                int64_t ca = P.skewA0, cb = P.skewB0;
+                for (int d = 0; d < P.nG; ++d) {
+                    const uint32_t qq = fd_div(r, P.gdiv[d]);
+                    const uint32_t c = r - qq * P.gdiv[d].d;
+                    r = qq;
+                    if (d < 2) org[d] = (int32_t)c * TE;
+                    else { ca += (int64_t)c * P.stepA[d]; cb += (int64_t)c * P.stepB[d]; }
+                }
+                org_of[s][u][0] = org[0];
+                org_of[s][u][1] = org[1];
+                off_of[s][u][0] = ca;
+                off_of[s][u][1] = cb;
+                tile_of[s][u] = tile_id;
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(full_a), "r"(buf_bytes * (BETA ? 2u : 1u)) : "memory");
+                const uint32_t in_s = base + (uint32_t)s * 2u * buf_bytes, out_s = in_s + buf_bytes;
+                for (int p = 0; p < P.nP; ++p)
+#pragma unroll
+                    for (int cl = 0; cl < V; ++cl) {
+                        const int64_t ra = (int64_t)cl * P.sqA + ca + P.pA[p];
+                        const int sk = (int)(ra & (V - 1));
+                        tmap_load(in_s + (uint32_t)(p * V + cl) * 1024u, &M.a[sk * 2 + (cl >= P.remA ? 1 : 0)], full_a, org[0] + sk, org[1] >> LGV, (int)(ra >> LGV), 0, 0);
+                        if constexpr (BETA) {
+                            const int64_t rb = (int64_t)cl * P.s0B + cb + P.pB[p];
+                            const int skb = (int)(rb & (V - 1));
+                            tmap_load(out_s + (uint32_t)(p * V + cl) * 1024u, &M.b[skb * 2 + (cl >= P.remB ? 1 : 0)], full_a, org[1] + skb, org[0] >> LGV, (int)(rb >> LGV), 0, 0);
+                        }
+                    }
+            }
+            more = sched.next<true>(tile_id, P.n_tiles);
+            __syncwarp();
+        }
+    } else if (tid < 64) {
+        // ------------------------------------------------------------------ store thread
+        if (tid == 32) {
+            for (uint32_t it = 0;; ++it) {
+                const int s = (int)(it % (uint32_t)S);
+                const int u = (int)((it / (uint32_t)S) & 1u);
+                mbar_wait((uint32_t)__cvta_generic_to_shared(&done_bar[s]), (uint32_t)u);
+                if (tile_of[s][u] == 0xFFFFFFFFu) break;
+                const int32_t org0 = org_of[s][u][0], org1 = org_of[s][u][1];
+                const int64_t cb = off_of[s][u][1];
+                const uint32_t out_s = base + (uint32_t)s * 2u * buf_bytes + buf_bytes;
+                for (int p = 0; p < P.nP; ++p)
+#pragma unroll
+                    for (int cl = 0; cl < V; ++cl) {
+                        const int64_t rb = (int64_t)cl * P.s0B + cb + P.pB[p];
+                        const int skb = (int)(rb & (V - 1));
+                        tmap_store(&M.b[skb * 2 + (cl >= P.remB ? 1 : 0)], out_s + (uint32_t)(p * V + cl) * 1024u, org1 + skb, org0 >> LGV, (int)(rb >> LGV), 0, 0);
+                    }
+                asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+                if (it >= 1u) {
+                    asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
+                    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];"
+                                 ::"r"((uint32_t)__cvta_generic_to_shared(&outfree_bar[(it - 1u) % (uint32_t)S])) : "memory");
+                }
+            }
+            asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+        }
+    } else {
+        // ------------------------------------------------------------------ consumer warps
+        const int cw = (tid >> 5) - 2;
+        const int A2 = lane & 7;
+        for (uint32_t it = 0;; ++it) {
+            const int s = (int)(it % (uint32_t)S);
+            mbar_wait((uint32_t)__cvta_generic_to_shared(&full_bar[s]), (it / (uint32_t)S) & 1u);
+            const bool end = tile_of[s][(it / (uint32_t)S) & 1u] == 0xFFFFFFFFu;
+            if (!end) {
+                if constexpr (!BETA)
+                    if (it >= (uint32_t)S) mbar_wait((uint32_t)__cvta_generic_to_shared(&outfree_bar[s]), ((it / (uint32_t)S) - 1u) & 1u);
+                const uint32_t in_s = base + (uint32_t)s * 2u * buf_bytes, out_s = in_s + buf_bytes;
+                for (int p = cw; p < P.nP; p += n_cons_warps) {
+                    const uint32_t ip = in_s + (uint32_t)p * (V * 1024u), op = out_s + (uint32_t)p * (V * 1024u);
+#pragma unroll
+                    for (int j = 0; j < 2; ++j) {
+                        const int B2 = (j << 2) | (lane >> 3);
+                        Chunk r[V];
+#pragma unroll
+                        for (int d = 0; d < V; ++d) r[d].u = lds128(ip + (uint32_t)(d * 1024 + B2 * 128 + ((A2 ^ B2) << 4)));
+#pragma unroll
+                        for (int d = 0; d < V; ++d) {
+                            const uint32_t oa = op + (uint32_t)(d * 1024 + A2 * 128 + ((B2 ^ A2) << 4));
+                            Chunk o, b;
+                            if constexpr (BETA) b.u = lds128(oa);
+#pragma unroll
+                            for (int e = 0; e < V; ++e) {
+                                T x = scale(alpha, r[e].e[d]);
+                                if constexpr (BETA) x = add(x, scale(beta, b.e[e]));
+                                o.e[e] = x;
+                            }
+                            sts128(oa, o.u);
+                        }
+                    }
+                }
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            }
+            __syncwarp();
+            if (lane == 0)
+                asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"((uint32_t)__cvta_generic_to_shared(&done_bar[s])) : "memory");
+            if (end) break;
+        }
+    }
+}
+
 }  // namespace ttc

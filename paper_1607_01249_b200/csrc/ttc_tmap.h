@@ -46,4 +46,43 @@ struct TmapEncode {
     uint32_t boxA[kTmapRank], boxB[kTmapRank];
 };
 
+// ------------------------------------------------------------------------------------------
+// flavour 2: more than 5 canonical indices (4- and 8-byte elements).  The rows of a T x T plane (T = 128 / es) are split
+// into V = 16 / es classes by row index mod V; a row's offset R = class * stride + (offset of the tile's outer indices) is
+// expressed as the coordinate R / V of a map dimension with a 16-byte stride, which can address ANY 16-byte aligned offset
+// and so absorbs every index beyond the plane: no rank limit.  The design also carries a skew R % V as a shift of the
+// coordinate along the row (for strides that are not multiples of 16 bytes, with 2 V maps per tensor, indexed
+// [skew * 2 + (0: classes with one row more, 1: the others)], for exact clipping) -- but the hardware raises "illegal
+// instruction" for a box whose first byte is not 16-byte aligned (measured: coordinate 17 of an fp64 map fails, 18
+// works), so only skew 0 is ever used and the planner offers this flavour for aligned strides only.  A plane is 2 V
+// sub-boxes of 1 KB (8 rows of 128 bytes, 128-byte swizzle); the thread that owns micro-tile (A2, B2) reads row B2,
+// chunk A2 of the V in-sub-boxes and writes row A2, chunk B2 of the V out-sub-boxes: the sub-box index IS the position
+// inside the micro-tile.
+// ------------------------------------------------------------------------------------------
+constexpr int kTmapUMaxPlanes = 8;
+constexpr int kTmapUMaxClasses = 4;
+
+struct TmapUParams {
+    int dyn;
+    uint32_t* ctr;
+    uint32_t n_tiles;
+    int stages, threads;
+    int V, T;                      // classes (= elements per 16 bytes) and plane edge (elements)
+    int nP;                        // planes per tile
+    int nG;                        // tile-grid dimensions: 0 = a0, 1 = b0, then the other canonical indices
+    int skewA0, skewB0;            // misalignment of the base addresses in elements, filled in at launch
+    int remA, remB;                // rows of A's planes (b0 extent) mod V, rows of B's planes (a0 extent) mod V: classes below have one row more
+    FastDiv gdiv[kMaxRank];
+    int64_t stepA[kMaxRank], stepB[kMaxRank];   // element offset per tile index of grid dimension >= 2
+    int64_t pA[kTmapUMaxPlanes], pB[kTmapUMaxPlanes];   // element offsets of the tile's planes
+    int64_t sqA, s0B;              // stride of b0 in A, of a0 in B (elements)
+};
+
+struct TmapUEncode {
+    int es;
+    int64_t e0, eq;                // extents of a0 and b0
+    int64_t sqA, s0B;
+    int64_t spanA, spanB;          // elements
+};
+
 }  // namespace ttc

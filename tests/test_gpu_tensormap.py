@@ -2,7 +2,7 @@
 swizzled shared-memory boxes, in-register micro-tiles; north_star K2, SURVEY.md 8(d) "TMA feasibility") against
 the oracle, bit for bit: every tensor-map candidate of every shape below, every element type, beta on and off.
 The shapes cover: boxes that stick out of the tensor on every side (loads fill zeros, stores clip), padded A
-and B, 2-D .. 5-D, the copy class (shared leading index: flavour 1, incl. the store-what-was-loaded path for
+and B, 2-D .. 7-D, the copy class (shared leading index: flavour 1, incl. the store-what-was-loaded path for
 real alpha == 1, beta == 0), several boxes per tile, and tensors a map cannot express (no such candidate)."""
 import numpy as np
 import pytest
@@ -102,9 +102,10 @@ def test_no_tensormap_candidate_where_a_map_cannot_express_the_tensor(monkeypatc
     monkeypatch.setenv("TTC_TUNE", "0")
     cases = [
         (wl.F32, wl.F32, (1023, 2301), (1, 0)),              # strides of 4092 / 9204 bytes: not multiples of 16
-        (wl.F64, wl.F64, (7, 96, 40), (2, 1, 0)),            # stride of 56 bytes (configs[4]'s A side)
+        (wl.F64, wl.F64, (33, 9, 21), (2, 0, 1)),            # odd fp64 extents: 8-byte-aligned strides only
+        (wl.F64, wl.F64, (7, 96, 40), (2, 1, 0)),            # rows of 7 fp64 (configs[4]'s A side)
         (wl.F32, wl.F64, (64, 64), (1, 0)),                  # mixed precision
-        (wl.F64, wl.F64, (8, 4, 4, 4, 4, 4, 4), (6, 5, 4, 3, 2, 1, 0)),     # 7-D after canonicalisation
+        (wl.F64, wl.F64, (8, 4, 4, 4, 4, 4, 4), (6, 5, 4, 3, 2, 1, 0)),     # 7-D, 4 elements along B's leading index
     ]
     for da, db, sizes, perm in cases:
         plan = ttc.ttc_plan_mixed(da, db, len(sizes), sizes, perm)
@@ -113,6 +114,33 @@ def test_no_tensormap_candidate_where_a_map_cannot_express_the_tensor(monkeypatc
                 assert not tensormap_candidates(plan, which), (sizes, perm)
         finally:
             ttc.ttc_destroy(plan)
+
+
+# More than 5 canonical indices: flavour 2 (ttc_tmap.h) folds every index beyond the plane into one map dimension.
+HIGH_RANK = [
+    ("r6", (20, 4, 6, 8, 6, 20), (5, 2, 0, 4, 1, 3)),
+    ("r6_ragged", (36, 4, 3, 8, 5, 44), (5, 2, 0, 4, 1, 3)),
+    ("r7", (16, 4, 2, 4, 3, 2, 24), (6, 2, 0, 4, 1, 5, 3)),
+]
+
+
+@pytest.mark.parametrize("dtype", [wl.F32, wl.F64, wl.C64])
+@pytest.mark.parametrize("beta_nz", [False, True])
+@pytest.mark.parametrize("shape", HIGH_RANK, ids=[s[0] for s in HIGH_RANK])
+def test_every_high_rank_tensormap_candidate(dtype, beta_nz, shape):
+    name, sizes, perm = shape
+    alpha, beta = scalars(dtype, beta_nz)
+    w = wl.Workload(name, dtype, sizes, perm, alpha, beta)
+    plan = ttc.ttc_plan(w.dtype, w.n, w.sizes, w.perm)
+    try:
+        assert ttc.ttc_plan_info(plan).canon_rank == len(sizes)
+        which = 1 if beta_nz else 0
+        cands = tensormap_candidates(plan, which)
+        assert cands, "no tensor-map candidate for %s dtype %d" % (name, dtype)
+        for i in cands:
+            check_bit_exact(w, plan=plan, candidate=i)
+    finally:
+        ttc.ttc_destroy(plan)
 
 
 def test_tensormap_candidate_with_misaligned_pointers_falls_back():
