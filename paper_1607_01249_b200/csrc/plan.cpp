@@ -811,6 +811,9 @@ void add_tmap(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, 
         if (i != 0 && ((c.d[i].sA * es) % 16 != 0 || c.d[i].sA * es >= lim)) return;
         if (i != q && ((c.d[i].sB * es) % 16 != 0 || c.d[i].sB * es >= lim)) return;
     }
+    // A store clips at the tensor's edge only in whole 16-byte granules along dimension 0 (measured: a row of 3 fp32 inside a
+    // leading dimension of 4 gets its padding element overwritten): B's rows must be a multiple of 16 bytes long.
+    if ((c.d[q].e * es) % 16 != 0) return;
     const int flavour = q == 0 ? 1 : 0;
     // the other indices, by ascending stride in A and in B
     std::vector<int> othA, othB;
@@ -1010,6 +1013,7 @@ void add_tmapu(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz,
         if (i != 0 && (c.d[i].sA * es) % 16 != 0) return;
         if (i != q && (c.d[i].sB * es) % 16 != 0) return;
     }
+    if ((c.d[q].e * es) % 16 != 0) return;               // stores clip in whole 16-byte granules (see add_tmap)
     if (c.d[0].e < T / 2 || c.d[q].e < T / 2) return;     // more than half of every plane would be padding
     const int64_t lim = (int64_t)1 << 40;
     if (c.d[q].sA * es * V >= lim || c.d[0].sB * es * V >= lim) return;

@@ -40,7 +40,37 @@ SHAPES = [
     ("copy3d", (48, 12, 20), (0, 2, 1), None, None),                     # flavour 1
     ("copy3d_padded", (44, 9, 10), (0, 2, 1), (48, 9, 10), (52, 12, 9)),
     ("copy_long_rows", (1200, 6, 10), (0, 2, 1), None, None),            # rows longer than one box
+    # A's rows are not a multiple of 16 bytes long inside a padded leading dimension that is (B's are: see ODD_B_ROWS)
+    ("t3d_odd_a_rows_padded", (33, 9, 20), (2, 0, 1), (36, 12, 20), (20, 36, 9)),
 ]
+
+# B's rows are not a multiple of 16 bytes long, inside leading dimensions that are: a tensor-map STORE clips at the edge of
+# the tensor in whole 16-byte granules only and would overwrite the padding -- no tensor-map candidate (16-byte elements: fine)
+ODD_B_ROWS = [
+    ("t3d_odd_rows_padded", (33, 9, 21), (2, 0, 1), (36, 12, 21), (24, 36, 9)),
+    ("copy_odd_rows_padded", (3, 5, 7), (0, 2, 1), (4, 8, 7), (8, 8, 5)),
+    ("t2d_tiny_padded", (5, 3), (1, 0), (8, 3), (4, 5)),
+]
+
+
+@pytest.mark.parametrize("dtype", ALL_DTYPES)
+@pytest.mark.parametrize("shape", ODD_B_ROWS, ids=[s[0] for s in ODD_B_ROWS])
+def test_no_tensormap_store_into_rows_that_end_inside_a_granule(dtype, shape):
+    name, sizes, perm, lda, ldb = shape
+    for beta_nz in (False, True):
+        alpha, beta = scalars(dtype, beta_nz)
+        w = wl.Workload(name, dtype, sizes, perm, alpha, beta, lda=lda, ldb=ldb)
+        plan = ttc.ttc_plan(w.dtype, w.n, w.sizes, w.perm, w.lda, w.ldb)
+        try:
+            cands = tensormap_candidates(plan, 1 if beta_nz else 0)
+            if dtype == wl.C128:
+                for i in cands:
+                    check_bit_exact(w, plan=plan, candidate=i)
+            else:
+                assert not cands
+            check_bit_exact(w, plan=plan)            # whatever the plan chose: padding (NaN guards) intact
+        finally:
+            ttc.ttc_destroy(plan)
 
 
 @pytest.mark.parametrize("dtype", ALL_DTYPES)
@@ -141,6 +171,39 @@ def test_every_high_rank_tensormap_candidate(dtype, beta_nz, shape):
             check_bit_exact(w, plan=plan, candidate=i)
     finally:
         ttc.ttc_destroy(plan)
+
+
+@pytest.mark.parametrize("dtype", ALL_DTYPES)
+def test_random_small_padded_shapes_every_tensormap_candidate(dtype):
+    """Seeded random small tensors (rank 2..5, extents 1..20, leading dimensions padded to 16-byte multiples along the
+    first index and arbitrarily along the others, extent-1 indices, tiles far larger than the tensor): every tensor-map
+    candidate a plan offers, and the plan's own choice, against the oracle with NaN guards in every padding element."""
+    rng = np.random.default_rng(1607 + dtype)
+    g = 16 // wl.ELEM_SIZE[dtype]
+    checked = 0
+    for case in range(36):
+        n = int(rng.integers(2, 6))
+        sizes = tuple(int(x) for x in rng.choice([1, 2, 3, 4, 5, 7, 8, 12, 16, 20], size=n))
+        perm = tuple(int(x) for x in rng.permutation(n))
+        szb = tuple(sizes[p] for p in perm)
+
+        def padded(sz):
+            ld = [int(x + rng.integers(0, 3)) for x in sz]
+            ld[0] = -(-int(sz[0] + rng.integers(0, 2 * g)) // g) * g          # rows start on 16-byte boundaries
+            return tuple(ld)
+        lda, ldb = padded(sizes), padded(szb)
+        for beta_nz in (False, True):
+            alpha, beta = scalars(dtype, beta_nz)
+            w = wl.Workload("rnd%d" % case, dtype, sizes, perm, alpha, beta, lda=lda, ldb=ldb)
+            plan = ttc.ttc_plan(w.dtype, w.n, w.sizes, w.perm, w.lda, w.ldb)
+            try:
+                for i in tensormap_candidates(plan, 1 if beta_nz else 0):
+                    check_bit_exact(w, plan=plan, candidate=i)
+                    checked += 1
+                check_bit_exact(w, plan=plan)
+            finally:
+                ttc.ttc_destroy(plan)
+    assert checked >= 20, checked
 
 
 def test_tensormap_candidate_with_misaligned_pointers_falls_back():
