@@ -207,16 +207,17 @@ static bool encode_maps(const TmapEncode& me, const void* A, void* B, CUtensorMa
     EncodeTiledFn enc = encode_tiled_fn();
     if (!enc) return false;
     const CUtensorMapDataType dt = me.unit_bytes == 4 ? CU_TENSOR_MAP_DATA_TYPE_UINT32 : CU_TENSOR_MAP_DATA_TYPE_UINT64;
-    const CUtensorMapSwizzle sw = me.swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE;
+    static const CUtensorMapSwizzle kSwz[4] = {CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_SWIZZLE_32B, CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_SWIZZLE_128B};
+    const CUtensorMapSwizzle swA = kSwz[me.swzA & 3], swB = kSwz[me.swzB & 3];
     static const cuuint32_t ones[kTmapRank] = {1, 1, 1, 1, 1};
     const CUtensorMapL2promotion l2p = CU_TENSOR_MAP_L2_PROMOTION_L2_128B;    // none / 128 B / 256 B measured: no difference
     cuuint64_t dA[kTmapRank], dB[kTmapRank], sA[kTmapRank - 1], sB[kTmapRank - 1];
     cuuint32_t bA[kTmapRank], bB[kTmapRank];
     for (int i = 0; i < kTmapRank; ++i) { dA[i] = me.dimA[i]; dB[i] = me.dimB[i]; bA[i] = me.boxA[i]; bB[i] = me.boxB[i]; }
     for (int i = 0; i < kTmapRank - 1; ++i) { sA[i] = me.strideA[i]; sB[i] = me.strideB[i]; }
-    if (enc(mapA, dt, kTmapRank, const_cast<void*>(A), dA, sA, bA, ones, CU_TENSOR_MAP_INTERLEAVE_NONE, sw,
+    if (enc(mapA, dt, kTmapRank, const_cast<void*>(A), dA, sA, bA, ones, CU_TENSOR_MAP_INTERLEAVE_NONE, swA,
             l2p, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) return false;
-    return enc(mapB, dt, kTmapRank, B, dB, sB, bB, ones, CU_TENSOR_MAP_INTERLEAVE_NONE, sw,
+    return enc(mapB, dt, kTmapRank, B, dB, sB, bB, ones, CU_TENSOR_MAP_INTERLEAVE_NONE, swB,
                l2p, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 

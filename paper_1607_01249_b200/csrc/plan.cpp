@@ -820,6 +820,7 @@ void add_tmap(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, 
     for (int i = 0; i < c.rank; ++i) if (i != 0 && i != q) othA.push_back(i);
     for (int k = 0; k < c.rank; ++k) if (c.orderB[k] != 0 && c.orderB[k] != q) othB.push_back(c.orderB[k]);
     const int T = 128 / es;                              // flavour 0: elements per 128-byte box row
+    int TA = T, TB = T;                                  // plane edges of the variant being emitted (T or T / 2: 64-byte rows)
 
     std::set<std::string> seen;
     int n_added = 0;
@@ -829,6 +830,8 @@ void add_tmap(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, 
         key.push_back((char)nbA);
         key.push_back((char)nbB);
         key.append((const char*)&box0_units, sizeof(box0_units));
+        key.push_back((char)TA);
+        key.push_back((char)TB);
         if (!seen.insert(key).second) return;
         Candidate cand;
         cand.beta_nz = beta_nz;
@@ -851,7 +854,7 @@ void add_tmap(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, 
             const int i = idx[k];
             const int64_t e = i < 0 ? 1 : c.d[i].e;
             int32_t bx;                                          // box extent (elements) along A-map dimension k
-            if (flavour == 0) bx = k < 2 ? T : (i < 0 ? 1 : pe[i]);
+            if (flavour == 0) bx = k == 0 ? TA : k == 1 ? TB : (i < 0 ? 1 : pe[i]);
             else bx = k == 0 ? box0_units / upe : (i < 0 ? 1 : pe[i]);
             if (bx < 1 || bx > 256) return;
             if (flavour == 0 && k >= 2) planes *= bx;
@@ -876,8 +879,13 @@ void add_tmap(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, 
         }
         if (E.boxA[0] > 256 || E.boxB[0] > 256 || (E.boxA[0] * unit) % 16 != 0) return;
         E.unit_bytes = unit;
-        E.swizzle128 = flavour == 0 ? 1 : 0;
+        auto swz = [&](int row_elems) { const int b = row_elems * es; return b >= 128 ? 3 : b == 64 ? 2 : 1; };   // CUtensorMapSwizzle values
+        E.swzA = flavour == 0 ? swz(TA) : 0;
+        E.swzB = flavour == 0 ? swz(TB) : 0;
+        M.ca = TA * es / 16;
+        M.cb = TB * es / 16;
         const int64_t box_bytes = box_elems * es;
+        if (flavour == 0 && box_bytes % 1024 != 0) return;       // every box starts on a swizzle-atom boundary
         const int64_t tile_bytes = (box_bytes * nbA * nbB + 127) / 128 * 128;
         if (box_bytes < 1024 || tile_bytes > 64 * 1024 || nbA * nbB > kTmapMaxBoxes) return;
         int stages = 0;
@@ -946,12 +954,25 @@ void add_tmap(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, 
     };
     int32_t pe[kMaxRank];
     if (flavour == 0) {
-        const int64_t plane_bytes = 128 * (int64_t)T;
         struct Var { int dist, kb, nbA, nbB; };
         static const Var vars[] = {{0, 16, 1, 1}, {1, 16, 1, 1}, {0, 8, 2, 1}, {1, 8, 1, 2}, {2, 16, 1, 1}, {0, 8, 1, 1}, {1, 8, 1, 1},
                                    {2, 4, 2, 2}};
+        // plane edges: 128-byte rows on both sides, and 64-byte rows on a side whose extent they fit with at least 20 % less
+        // padding (24 fp64 = 1.5 rows of 128 bytes but 3 of 64).  Measured on c2: for 72 and 56 fp64 (4.5 and 3.5 rows,
+        // 11-14 % padding) the 64-byte rows are no faster (3210: 82-84 us against 80-82), so small gains are not offered.
+        auto padded_to = [](int64_t e, int t) { return (e + t - 1) / t * t; };
+        std::vector<std::pair<int, int>> edges = {{T, T}};
+        const bool half_a = T >= 2 && padded_to(c.d[0].e, T / 2) * 6 <= padded_to(c.d[0].e, T) * 5;
+        const bool half_b = T >= 2 && ((T / 2) * es) % 16 == 0 && padded_to(c.d[q].e, T / 2) * 6 <= padded_to(c.d[q].e, T) * 5;
+        if (half_b) edges.push_back({T, T / 2});
+        if (half_a && ((T / 2) * es) % 16 == 0) edges.push_back({T / 2, T});
+        if (half_a && half_b && ((T / 2) * es) % 16 == 0) edges.push_back({T / 2, T / 2});
+        for (auto& ed : edges) {
+        TA = ed.first;
+        TB = ed.second;
+        const int64_t plane_bytes = (int64_t)TA * TB * es;
         for (const Var& v : vars) {
-            if (c.d[0].e <= (int64_t)(v.nbA - 1) * T || c.d[q].e <= (int64_t)(v.nbB - 1) * T) continue;
+            if (c.d[0].e <= (int64_t)(v.nbA - 1) * TA || c.d[q].e <= (int64_t)(v.nbB - 1) * TB) continue;
             const int64_t want = std::max<int64_t>(1, (int64_t)v.kb * 1024 / plane_bytes);
             if (v.dist == 0) fill(othA, want, pe);
             else if (v.dist == 1) fill(othB, want, pe);
@@ -976,8 +997,10 @@ void add_tmap(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, 
             for (int i = 0; i < c.rank; ++i) pe[i] = 1;
             static const int nb[][2] = {{2, 2}, {4, 1}, {1, 4}, {4, 2}, {2, 4}, {2, 1}, {1, 2}};
             for (auto& b : nb)
-                if (c.d[0].e > (int64_t)(b[0] - 1) * T && c.d[q].e > (int64_t)(b[1] - 1) * T) emit(pe, 0, b[0], b[1]);
+                if (c.d[0].e > (int64_t)(b[0] - 1) * TA && c.d[q].e > (int64_t)(b[1] - 1) * TB) emit(pe, 0, b[0], b[1]);
         }
+        }
+        TA = TB = T;
     } else {
         // copy class: rows of up to 256 map units along the shared leading index, then rows until the box has 8-32 KB
         const int gran = 16 / unit;

@@ -210,8 +210,9 @@ tmap_kernel(const __grid_constant__ TmapParams P, const __grid_constant__ CUtens
                     if (it >= (uint32_t)S) mbar_wait((uint32_t)__cvta_generic_to_shared(&outfree_bar[s]), ((it / (uint32_t)S) - 1u) & 1u);
                 const uint32_t in_s = base + (uint32_t)s * 2u * P.buf_bytes, out_s = in_s + P.buf_bytes;
                 if constexpr (FLAVOUR == 0) {
-                    constexpr uint32_t PB = 1024u * V;          // bytes of one plane: 8 V rows of 128 bytes
                     const int n_planes = nbox * P.planes;
+                    if (P.ca == 8 && P.cb == 8) {
+                    constexpr uint32_t PB = 1024u * V;          // bytes of one plane: 8 V rows of 128 bytes
                     for (int pl = cw; pl < n_planes; pl += n_cons_warps) {
                         const uint32_t ip = in_s + (uint32_t)pl * PB, op = out_s + (uint32_t)pl * PB;
 #pragma unroll
@@ -239,6 +240,42 @@ tmap_kernel(const __grid_constant__ TmapParams P, const __grid_constant__ CUtens
                                 sts128(oa, o.u);
                             }
                         }
+                    }
+                    } else {
+                    // 64-byte rows on one or both sides (ca, cb in {8, 4}): a plane has ca x cb micro-tiles; the hardware
+                    // swizzle of a row of c chunks is chunk ^= (address >> 7) & (c - 1), computed here on the byte offset
+                    // from the stage buffer (1024-byte aligned).  Up to two-way bank conflicts: the kernel is bound by
+                    // DRAM, not by shared memory.
+                    const uint32_t ca = (uint32_t)P.ca, cb = (uint32_t)P.cb;
+                    const uint32_t pb = ca * cb * (uint32_t)V * 16u;          // bytes of one plane
+                    const uint32_t n_micro = ca * cb;
+                    const uint32_t lg_ca = ca == 8u ? 3u : 2u;
+                    for (int pl = cw; pl < n_planes; pl += n_cons_warps) {
+                        const uint32_t pbase = (uint32_t)pl * pb;
+                        for (uint32_t m = (uint32_t)lane; m < n_micro; m += 32u) {
+                            const uint32_t A2 = m & (ca - 1u), B2 = m >> lg_ca;
+                            Chunk r[V];
+#pragma unroll
+                            for (int d = 0; d < V; ++d) {
+                                const uint32_t L = pbase + ((uint32_t)V * B2 + (uint32_t)d) * (ca << 4) + (A2 << 4);
+                                r[d].u = lds128(in_s + (L ^ (((L >> 7) & (ca - 1u)) << 4)));
+                            }
+#pragma unroll
+                            for (int d = 0; d < V; ++d) {
+                                const uint32_t L = pbase + ((uint32_t)V * A2 + (uint32_t)d) * (cb << 4) + (B2 << 4);
+                                const uint32_t oa = out_s + (L ^ (((L >> 7) & (cb - 1u)) << 4));
+                                Chunk o, b;
+                                if constexpr (BETA) b.u = lds128(oa);
+#pragma unroll
+                                for (int e = 0; e < V; ++e) {
+                                    T x = scale(alpha, r[e].e[d]);
+                                    if constexpr (BETA) x = add(x, scale(beta, b.e[e]));
+                                    o.e[e] = x;
+                                }
+                                sts128(oa, o.u);
+                            }
+                        }
+                    }
                     }
                 } else {
                     const int n_chunks = (int)(tile_bytes >> 4);

@@ -29,6 +29,7 @@ struct TmapParams {
     int stages, threads;
     int nbA, nbB;             // boxes per tile along map dimension 0 of A / of B (flavour 1: nbB == 1)
     int planes;               // flavour 0: planes per box
+    int ca, cb;               // flavour 0: 16-byte chunks per in-row / per out-row (8: 128-byte rows, 4: 64-byte rows)
     uint32_t box_bytes;       // bytes of one box (the same for A's and B's map)
     uint32_t buf_bytes;       // nbA * nbB * box_bytes rounded up to 128 (a box's shared-memory address must be 128-byte aligned)
     int upe;                  // map units per element along a map's dimension 0 (2 for 16-byte elements: 8-byte units)
@@ -40,7 +41,7 @@ struct TmapParams {
 // What cuTensorMapEncodeTiled needs beside the base address (filled by the planner; encoded at launch).
 struct TmapEncode {
     int unit_bytes;                       // 4 or 8: CU_TENSOR_MAP_DATA_TYPE_UINT32 / UINT64
-    int swizzle128;                       // 1: CU_TENSOR_MAP_SWIZZLE_128B, 0: none
+    int swzA, swzB;                       // CUtensorMapSwizzle of A's / B's map: 0 none, 1 32-byte, 2 64-byte, 3 128-byte rows
     uint64_t dimA[kTmapRank], dimB[kTmapRank];
     uint64_t strideA[kTmapRank - 1], strideB[kTmapRank - 1];   // bytes, dimensions 1..4
     uint32_t boxA[kTmapRank], boxB[kTmapRank];

@@ -35,6 +35,7 @@ SHAPES = [
     ("t2d_ragged", (100, 52), (1, 0), None, None),                       # edge boxes on both sides
     ("t3d", (64, 24, 48), (2, 1, 0), None, None),
     ("t3d_ragged_padded", (100, 36, 44), (1, 2, 0), (104, 40, 44), (36, 48, 100)),
+    ("t3d_half_rows", (40, 20, 24), (2, 1, 0), None, None),                # 64-byte rows: 40 and 24 fp64 / c64 without padding
     ("t4d", (36, 8, 12, 20), (3, 1, 0, 2), None, None),
     ("t5d", (20, 4, 12, 8, 16), (4, 2, 0, 3, 1), None, None),
     ("copy3d", (48, 12, 20), (0, 2, 1), None, None),                     # flavour 1
