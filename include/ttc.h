@@ -216,7 +216,10 @@ ttc_status ttc_execute(ttc_plan_t plan, const void* alpha, const void* A,
  * paying a launch and a machine fill-and-drain per block.  A_list and B_list are HOST arrays of DEVICE
  * pointers, read before the call returns; the pairs must not overlap one another.  alpha, beta, alignment
  * rules (the least aligned pointer decides the candidate), errors and asynchrony are those of ttc_execute;
- * batch == 0 is a no-op, batch < 0 is TTC_ERR_INVALID_ARG.
+ * batch == 0 is a no-op, batch < 0 is TTC_ERR_INVALID_ARG.  A tensor-map winner serves the batch through ONE pair of
+ * maps (the pair's distance from the lowest address, in 16-byte units, is the coordinate of the fifth map dimension)
+ * when the canonical rank is <= 4 and the 64 pairs of a launch lie within 32 GB; otherwise the plan's best other
+ * candidate takes the batch.
  */
 ttc_status ttc_execute_batched(ttc_plan_t plan, const void* alpha, const void* const* A_list,
                                const void* beta, void* const* B_list, int batch, void* cuda_stream);

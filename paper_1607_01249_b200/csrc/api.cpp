@@ -341,10 +341,12 @@ int choose_candidate(ttc_plan_s* p, int which, uintptr_t A, uintptr_t B) {
     return slot < 0 ? -2 : slot;
 }
 
-// ttc_execute_batched cannot launch a tensor-map candidate (its two maps hold ONE base address each): the best
-// other candidate whose accesses fit the pointers' alignment, looked up once per alignment class.
+// ttc_execute_batched can launch a tensor-map candidate only when the fifth map dimension is free to carry the batch
+// offset (canonical rank <= 4); otherwise: the best other candidate whose accesses fit the pointers' alignment, looked
+// up once per alignment class.
 int without_tensormap(ttc_plan_s* p, int which, int idx, uintptr_t A, uintptr_t B) {
     if (idx < 0 || p->cands[which][idx].info.kernel != TTC_KERNEL_TENSORMAP) return idx;
+    if (p->cands[which][idx].mp.flavour != 2 && p->cands[which][idx].mp.batchable) return idx;     // one map pair serves the batch
     auto lg = [](uintptr_t x) { int l = 0; while (l < 4 && !((x >> l) & 1)) ++l; return l; };
     const int la = lg(A), lb = lg(B);
     int& slot = p->nomap[which][5 * la + lb];
@@ -514,12 +516,40 @@ ttc_status ttc_execute_batched(ttc_plan_t p, const void* alpha, const void* cons
     }
     if ((oa % esA) != 0 || (ob % es) != 0) return TTC_ERR_MISALIGNED;
     const int which = is_zero(p->dtype, beta) ? 0 : 1;
-    const int idx = without_tensormap(p, which, choose_candidate(p, which, oa, ob), oa, ob);
+    int idx = without_tensormap(p, which, choose_candidate(p, which, oa, ob), oa, ob);
+    if (idx >= 0 && p->cands[which][idx].info.kernel == TTC_KERNEL_TENSORMAP) {
+        // one pair of maps addresses the batch by (address - lowest address) / 16 as an int32 coordinate: problems of one
+        // launch must lie within 32 GB of each other, else the best other candidate takes the batch
+        bool fits = true;
+        for (int first = 0; first < batch && fits; first += kMaxBatch) {
+            const int n = std::min(kMaxBatch, batch - first);
+            uintptr_t lo_a = ~(uintptr_t)0, hi_a = 0, lo_b = ~(uintptr_t)0, hi_b = 0;
+            for (int i = first; i < first + n; ++i) {
+                lo_a = std::min(lo_a, (uintptr_t)A_list[i]);
+                hi_a = std::max(hi_a, (uintptr_t)A_list[i]);
+                lo_b = std::min(lo_b, (uintptr_t)B_list[i]);
+                hi_b = std::max(hi_b, (uintptr_t)B_list[i]);
+            }
+            fits = (hi_a - lo_a) / 16 < (uintptr_t)0x7fffffff && (hi_b - lo_b) / 16 < (uintptr_t)0x7fffffff;
+        }
+        if (!fits) {
+            int alt = -1;
+            float alt_us = 0.f;
+            const std::vector<Candidate>& cs = p->cands[which];
+            for (int i = 0; i < (int)cs.size(); ++i) {
+                if (cs[i].info.kernel == TTC_KERNEL_TENSORMAP || (oa % cs[i].align_a) != 0 || (ob % cs[i].align_b) != 0) continue;
+                const float us = cs[i].info.tuned_us;
+                if (alt < 0) { alt = i; alt_us = us; continue; }
+                if (us > 0.f && (alt_us <= 0.f || us < alt_us)) { alt = i; alt_us = us; }
+            }
+            idx = alt < 0 ? -2 : alt;
+        }
+    }
     if (idx == -1) return TTC_ERR_UNSUPPORTED;
     if (idx < 0) return TTC_ERR_MISALIGNED;
     const Candidate& c = p->cands[which][idx];
     if (!ensure_prepared(p, which, idx)) return TTC_ERR_CUDA;
-    const uint32_t per = c.info.kernel == TTC_KERNEL_COPY ? c.dp.n_chunks : c.tp.n_tiles;
+    const uint32_t per = c.info.kernel == TTC_KERNEL_COPY ? c.dp.n_chunks : c.info.kernel == TTC_KERNEL_TENSORMAP ? c.mp.n_tiles : c.tp.n_tiles;
     // one launch per kMaxBatch problems (the pointers travel as kernel parameters)
     for (int first = 0; first < batch; first += kMaxBatch) {
         BatchPtrs bt{};

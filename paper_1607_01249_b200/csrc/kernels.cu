@@ -20,6 +20,7 @@
 // definition evaluated in the tensor's own precision (reading A7).
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -172,18 +173,23 @@ static KernelFn get_direct_fn(int dt, const Candidate& c, bool batched) {
     return nullptr;
 }
 
-template <int DT>
-static KernelFn tmap_fn_dt(bool beta, int flavour) {
-    if (flavour == 0) return beta ? (KernelFn)tmap_kernel<DT, true, 0> : (KernelFn)tmap_kernel<DT, false, 0>;
-    return beta ? (KernelFn)tmap_kernel<DT, true, 1> : (KernelFn)tmap_kernel<DT, false, 1>;
+template <int DT, typename BT>
+static KernelFn tmap_fn_bt(bool beta, int flavour) {
+    if (flavour == 0) return beta ? (KernelFn)tmap_kernel<DT, true, 0, BT> : (KernelFn)tmap_kernel<DT, false, 0, BT>;
+    return beta ? (KernelFn)tmap_kernel<DT, true, 1, BT> : (KernelFn)tmap_kernel<DT, false, 1, BT>;
 }
 
-static KernelFn get_tmap_fn(int dt, const Candidate& c) {
+template <int DT>
+static KernelFn tmap_fn_dt(bool beta, int flavour, bool batched) {
+    return batched ? tmap_fn_bt<DT, TmapBatch>(beta, flavour) : tmap_fn_bt<DT, NoBatch>(beta, flavour);
+}
+
+static KernelFn get_tmap_fn(int dt, const Candidate& c, bool batched = false) {
     switch (dt) {
-        case TTC_F32: return tmap_fn_dt<TTC_F32>(c.beta_nz, c.mp.flavour);
-        case TTC_F64: return tmap_fn_dt<TTC_F64>(c.beta_nz, c.mp.flavour);
-        case TTC_C64: return tmap_fn_dt<TTC_C64>(c.beta_nz, c.mp.flavour);
-        case TTC_C128: return tmap_fn_dt<TTC_C128>(c.beta_nz, c.mp.flavour);
+        case TTC_F32: return tmap_fn_dt<TTC_F32>(c.beta_nz, c.mp.flavour, batched);
+        case TTC_F64: return tmap_fn_dt<TTC_F64>(c.beta_nz, c.mp.flavour, batched);
+        case TTC_C64: return tmap_fn_dt<TTC_C64>(c.beta_nz, c.mp.flavour, batched);
+        case TTC_C128: return tmap_fn_dt<TTC_C128>(c.beta_nz, c.mp.flavour, batched);
     }
     return nullptr;     // same-type tensors only
 }
@@ -203,7 +209,9 @@ static EncodeTiledFn encode_tiled_fn() {
     return fn;
 }
 
-static bool encode_maps(const TmapEncode& me, const void* A, void* B, CUtensorMap* mapA, CUtensorMap* mapB) {
+// dim4A / dim4B > 0 (batched launch): extent of the fifth dimension, whose stride is 16 bytes: the batch offset.
+static bool encode_maps(const TmapEncode& me, const void* A, void* B, CUtensorMap* mapA, CUtensorMap* mapB, uint64_t dim4A = 0,
+                        uint64_t dim4B = 0) {
     EncodeTiledFn enc = encode_tiled_fn();
     if (!enc) return false;
     const CUtensorMapDataType dt = me.unit_bytes == 4 ? CU_TENSOR_MAP_DATA_TYPE_UINT32 : CU_TENSOR_MAP_DATA_TYPE_UINT64;
@@ -215,6 +223,8 @@ static bool encode_maps(const TmapEncode& me, const void* A, void* B, CUtensorMa
     cuuint32_t bA[kTmapRank], bB[kTmapRank];
     for (int i = 0; i < kTmapRank; ++i) { dA[i] = me.dimA[i]; dB[i] = me.dimB[i]; bA[i] = me.boxA[i]; bB[i] = me.boxB[i]; }
     for (int i = 0; i < kTmapRank - 1; ++i) { sA[i] = me.strideA[i]; sB[i] = me.strideB[i]; }
+    if (dim4A) { dA[4] = dim4A; sA[3] = 16; }
+    if (dim4B) { dB[4] = dim4B; sB[3] = 16; }
     if (enc(mapA, dt, kTmapRank, const_cast<void*>(A), dA, sA, bA, ones, CU_TENSOR_MAP_INTERLEAVE_NONE, swA,
             l2p, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) return false;
     return enc(mapB, dt, kTmapRank, B, dB, sB, bB, ones, CU_TENSOR_MAP_INTERLEAVE_NONE, swB,
@@ -379,8 +389,8 @@ int launch_candidate(const Candidate& cand, ttc_dtype dtype, ttc_dtype dtype_a, 
     uint64_t grid = (uint64_t)cand.info.grid;
     if (batched) {     // one CTA per work item (launch control) or as many as the device holds
         const uint64_t work = (uint64_t)batch->per * (uint64_t)batch->n;
-        if (cand.info.kernel == TTC_KERNEL_TENSORMAP) return (int)cudaErrorNotSupported;   // the maps hold ONE base address each
-        const int dyn_b = cand.info.kernel == TTC_KERNEL_COPY ? cand.dp.dyn : cand.tp.dyn;
+        if (cand.info.kernel == TTC_KERNEL_TENSORMAP && (cand.mp.flavour == 2 || !cand.mp.batchable)) return (int)cudaErrorNotSupported;
+        const int dyn_b = cand.info.kernel == TTC_KERNEL_COPY ? cand.dp.dyn : cand.info.kernel == TTC_KERNEL_TENSORMAP ? cand.mp.dyn : cand.tp.dyn;
         grid = (dyn_b == 1 || work < (uint64_t)cand.grid_cap) ? work : (uint64_t)cand.grid_cap;
         if (grid >= (1ull << 31)) return (int)cudaErrorInvalidConfiguration;
     }
@@ -420,15 +430,48 @@ int launch_candidate(const Candidate& cand, ttc_dtype dtype, ttc_dtype dtype_a, 
         return (int)cudaLaunchKernelExC(&cfg, fn, uargs);
     }
     if (cand.info.kernel == TTC_KERNEL_TENSORMAP) {
-        KernelFn fn = dtype == dtype_a ? get_tmap_fn((int)dtype, cand) : nullptr;
+        KernelFn fn = dtype == dtype_a ? get_tmap_fn((int)dtype, cand, batched) : nullptr;
         if (!fn) return (int)cudaErrorInvalidValue;
         alignas(64) CUtensorMap mapA, mapB;       // the descriptors carry the base addresses: encoded per call (host only)
-        if (!encode_maps(cand.me, A, B, &mapA, &mapB)) return (int)cudaErrorInvalidValue;
+        TmapBatch tb;
+        if (batched) {
+            // one pair of maps for the whole batch: based at the lowest addresses, problem i at coordinate
+            // (A_i - min A) / 16 of the fifth dimension (stride 16 bytes)
+            uintptr_t lo_a = (uintptr_t)batch->a[0], lo_b = (uintptr_t)batch->b[0], hi_a = lo_a, hi_b = lo_b;
+            for (int i = 1; i < batch->n; ++i) {
+                lo_a = std::min(lo_a, (uintptr_t)batch->a[i]);
+                hi_a = std::max(hi_a, (uintptr_t)batch->a[i]);
+                lo_b = std::min(lo_b, (uintptr_t)batch->b[i]);
+                hi_b = std::max(hi_b, (uintptr_t)batch->b[i]);
+            }
+            if ((hi_a - lo_a) / 16 >= (uintptr_t)0x7fffffff || (hi_b - lo_b) / 16 >= (uintptr_t)0x7fffffff) return (int)cudaErrorNotSupported;
+            tb.n = batch->n;
+            tb.per = batch->per;
+            tb.div = batch->div;
+            for (int i = 0; i < batch->n; ++i) {
+                if ((((uintptr_t)batch->a[i] | (uintptr_t)batch->b[i]) & 15) != 0) return (int)cudaErrorMisalignedAddress;
+                tb.offA[i] = (int32_t)(((uintptr_t)batch->a[i] - lo_a) / 16);
+                tb.offB[i] = (int32_t)(((uintptr_t)batch->b[i] - lo_b) / 16);
+            }
+            if (!encode_maps(cand.me, (const void*)lo_a, (void*)lo_b, &mapA, &mapB, (hi_a - lo_a) / 16 + 1, (hi_b - lo_b) / 16 + 1))
+                return (int)cudaErrorInvalidValue;
+            static std::mutex mu;
+            static std::set<KernelFn> raised;
+            std::lock_guard<std::mutex> lk(mu);
+            if (!raised.count(fn)) {
+                int optin = 0;
+                const int rc = raise_smem_limit(fn, &optin);
+                if (rc != 0) return rc;
+                raised.insert(fn);
+            }
+        } else if (!encode_maps(cand.me, A, B, &mapA, &mapB)) {
+            return (int)cudaErrorInvalidValue;
+        }
         cfg.blockDim = dim3((unsigned)cand.mp.threads, 1, 1);
         cfg.dynamicSmemBytes = (size_t)cand.info.smem_bytes;
         TmapParams mp = cand.mp;
         mp.ctr = sched_ctr;
-        void* targs[5] = {&mp, &mapA, &mapB, &al, &be};
+        void* targs[6] = {&mp, &mapA, &mapB, &al, &be, batched ? (void*)&tb : (void*)&none};
         return (int)cudaLaunchKernelExC(&cfg, fn, targs);
     }
     void* args[6] = {nullptr, (void*)&A, (void*)&B, (void*)&al, (void*)&be, batched ? (void*)batch : (void*)&none};

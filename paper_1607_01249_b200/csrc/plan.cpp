@@ -913,6 +913,7 @@ void add_tmap(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, 
         M.upe = upe;
         M.box0[0] = (int32_t)(E.boxA[0] / upe);
         M.box0[1] = (int32_t)E.boxA[1];
+        M.batchable = idx[kTmapRank - 1] < 0 ? 1 : 0;            // the fifth map dimension is free for the batch offset
         cand.align_a = cand.align_b = 16;
         ttc_candidate_info& I = cand.info;
         I.kernel = TTC_KERNEL_TENSORMAP;

@@ -65,10 +65,10 @@ template <typename T> struct tmap_is_real { static constexpr bool value = false;
 template <> struct tmap_is_real<float> { static constexpr bool value = true; };
 template <> struct tmap_is_real<double> { static constexpr bool value = true; };
 
-template <int DT, bool BETA, int FLAVOUR>
+template <int DT, bool BETA, int FLAVOUR, typename BT>
 __global__ void __launch_bounds__(256)
 tmap_kernel(const __grid_constant__ TmapParams P, const __grid_constant__ CUtensorMap mapA,
-            const __grid_constant__ CUtensorMap mapB, const Scalar alpha_in, const Scalar beta_in) {
+            const __grid_constant__ CUtensorMap mapB, const Scalar alpha_in, const Scalar beta_in, const __grid_constant__ BT Bt) {
     using T = typename ElemT<DT>::T;
     constexpr int ES = (int)sizeof(T);
     constexpr int V = 16 / ES;
@@ -89,6 +89,7 @@ tmap_kernel(const __grid_constant__ TmapParams P, const __grid_constant__ CUtens
     // tile origin and id per stage, two deep: the producer may fill a stage again (its consumers are done) before the
     // store thread has read where the stage's previous tile goes; it cannot get two uses ahead of it
     __shared__ int32_t coord[kTmapMaxStages][2][kTmapRank];
+    __shared__ int32_t coord_b4[kTmapMaxStages][2];          // batched: B's coordinate along the fifth dimension (A's is coord[..][4])
     __shared__ uint32_t tile_of[kTmapMaxStages][2];
 
     const int tid = threadIdx.x, lane = tid & 31;
@@ -138,13 +139,24 @@ tmap_kernel(const __grid_constant__ TmapParams P, const __grid_constant__ CUtens
             if (lane == 0) {
                 int32_t c[kTmapRank];
                 uint32_t r = tile_id;
+                int32_t c4a = 0, c4b = 0;
+                if constexpr (!tt_is_same<BT, NoBatch>::value) {
+                    const uint32_t pair = fd_div(r, Bt.div);
+                    r -= pair * Bt.per;
+                    c4a = Bt.offA[pair];
+                    c4b = Bt.offB[pair];
+                }
 #pragma unroll
                 for (int d = 0; d < kTmapRank; ++d) {
                     const uint32_t qq = fd_div(r, P.gdiv[d]);
                     c[d] = (int32_t)(r - qq * P.gdiv[d].d) * P.step[d];
                     r = qq;
-                    coord[s][u][d] = c[d];
                 }
+                if constexpr (!tt_is_same<BT, NoBatch>::value) c[4] = c4a;
+                else c4b = c[4];
+#pragma unroll
+                for (int d = 0; d < kTmapRank; ++d) coord[s][u][d] = c[d];
+                coord_b4[s][u] = c4b;
                 tile_of[s][u] = tile_id;
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                 asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(full_a), "r"(tile_bytes * (BETA ? 2u : 1u)) : "memory");
@@ -156,14 +168,14 @@ tmap_kernel(const __grid_constant__ TmapParams P, const __grid_constant__ CUtens
                         if constexpr (FLAVOUR == 0) {
                             const int cb = c[1] + bj * P.box0[1];
                             tmap_load(in_s + (uint32_t)box * P.box_bytes, &mapA, full_a, ca * P.upe, cb, c[2], c[3], c[4]);
-                            if constexpr (BETA) tmap_load(out_s + (uint32_t)box * P.box_bytes, &mapB, full_a, cb * P.upe, ca, c[2], c[3], c[4]);
+                            if constexpr (BETA) tmap_load(out_s + (uint32_t)box * P.box_bytes, &mapB, full_a, cb * P.upe, ca, c[2], c[3], c4b);
                         } else {
                             tmap_load(in_s + (uint32_t)box * P.box_bytes, &mapA, full_a, ca * P.upe, c[1], c[2], c[3], c[4]);
-                            if constexpr (BETA) tmap_load(out_s + (uint32_t)box * P.box_bytes, &mapB, full_a, ca * P.upe, c[1], c[2], c[3], c[4]);
+                            if constexpr (BETA) tmap_load(out_s + (uint32_t)box * P.box_bytes, &mapB, full_a, ca * P.upe, c[1], c[2], c[3], c4b);
                         }
                     }
             }
-            more = sched.next<true>(tile_id, P.n_tiles);
+            more = sched.next<true>(tile_id, Bt.n ? P.n_tiles * (uint32_t)Bt.n : P.n_tiles);
             __syncwarp();
         }
     } else if (tid < 64) {
@@ -177,6 +189,7 @@ tmap_kernel(const __grid_constant__ TmapParams P, const __grid_constant__ CUtens
                 int32_t c[kTmapRank];
 #pragma unroll
                 for (int d = 0; d < kTmapRank; ++d) c[d] = coord[s][u][d];
+                c[4] = coord_b4[s][u];
                 const uint32_t in_s = base + (uint32_t)s * 2u * P.buf_bytes;
                 const uint32_t src_s = passthrough ? in_s : in_s + P.buf_bytes;
                 int box = 0;

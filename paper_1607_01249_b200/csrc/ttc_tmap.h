@@ -36,6 +36,17 @@ struct TmapParams {
     FastDiv gdiv[kTmapRank];  // number of tiles along A-map dimension d
     int32_t step[kTmapRank];  // tile extent (elements) along A-map dimension d
     int32_t box0[2];          // box extent (elements) along A-map dimension 0 and 1 (the step between the boxes of a tile)
+    int batchable;            // the fifth map dimension is unused (planner): ttc_execute_batched can use the candidate
+};
+
+// ttc_execute_batched through ONE pair of maps: when the fifth map dimension is free (canonical rank <= 4) it gets a stride
+// of 16 bytes, and problem i of the batch is addressed by the coordinate (A_i - min A) / 16 along it (B alike): a dimension
+// with a 16-byte stride reaches any 16-byte aligned address.  Work item w belongs to problem w / per.
+struct TmapBatch {
+    int n;
+    uint32_t per;
+    FastDiv div;
+    int32_t offA[kMaxBatch], offB[kMaxBatch];
 };
 
 // What cuTensorMapEncodeTiled needs beside the base address (filled by the planner; encoded at launch).

@@ -84,6 +84,35 @@ def test_batched_every_kernel_class(dtype, beta):
             ttc.ttc_destroy(plan)
 
 
+@pytest.mark.parametrize("dtype", [wl.F32, wl.F64, wl.C64, wl.C128])
+@pytest.mark.parametrize("beta", [0.0, 0.5])
+def test_batched_tensormap_candidates(dtype, beta):
+    """Tensor-map candidates serve a batch through ONE pair of maps (the batch offset is the fifth map coordinate, stride
+    16 bytes) when the canonical rank is <= 4: transposing and copy-class flavours, blocks of one big buffer and separately
+    allocated tensors, 1 .. 70 pairs; a rank-5 plan's tensor-map candidates are replaced (their fifth dimension is taken)."""
+    for sizes, perm, lda, ldb in (((40, 20, 24), (2, 1, 0), None, None), ((48, 12, 20), (0, 2, 1), (52, 12, 20), None),
+                                  ((36, 8, 12, 20), (3, 1, 0, 2), None, None)):
+        plan = ttc.ttc_plan(dtype, len(sizes), sizes, perm, lda, ldb)
+        try:
+            which = 1 if beta else 0
+            tm = [i for i in range(ttc.ttc_plan_num_candidates(plan, which)) if ttc.ttc_plan_candidate(plan, which, i).kernel == 6]
+            assert tm
+            for idx in tm[:3]:
+                for batch, views in ((5, True), (3, False), (70, True)):
+                    run_batched(dtype, dtype, sizes, perm, lda, ldb, 1.5, beta, batch, plan=plan, candidate=idx, views=views)
+        finally:
+            ttc.ttc_destroy(plan)
+    sizes, perm = (20, 4, 12, 8, 16), (4, 2, 0, 3, 1)          # rank 5: no free map dimension
+    plan = ttc.ttc_plan(dtype, 5, sizes, perm)
+    try:
+        which = 1 if beta else 0
+        tm = [i for i in range(ttc.ttc_plan_num_candidates(plan, which)) if ttc.ttc_plan_candidate(plan, which, i).kernel == 6]
+        assert tm
+        run_batched(dtype, dtype, sizes, perm, None, None, 1.5, beta, 4, plan=plan, candidate=tm[0], views=True)
+    finally:
+        ttc.ttc_destroy(plan)
+
+
 def test_batch_sizes_and_edge_cases():
     sizes, perm = (24, 10, 12), (1, 2, 0)
     for batch in (1, 2, 63, 64, 65, 130):
