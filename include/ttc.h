@@ -43,7 +43,7 @@
  *   TTC_PDL=0             launch without programmatic dependent launch (default: with)
  *   TTC_RING=0|2|4        largest ring of tile buffers of the warp-specialised kernel (0: none; default 4)
  *   TTC_VARIANTS=bits     candidate flavours to generate: 1 staggered-gather ring, 2 shifted-row ring, 4 tensor-map
- *                         kernels (default 7: all)
+ *                         kernels, 8 skew kernels (default 15: all)
  */
 #ifndef TTC_H_
 #define TTC_H_
@@ -80,9 +80,11 @@ typedef enum {
     TTC_KERNEL_WIDE = 4,    /* K2 on "wide elements": a >=16-byte run that leads both A and B         */
     TTC_KERNEL_TMA = 5,     /* K2/K3 warp-specialised: a producer warp fetches the tile rows by TMA
                                bulk copies (cp.async.bulk) into a ring of buffers, consumers store  */
-    TTC_KERNEL_TENSORMAP = 6 /* K1/K2/K3 through tensor maps: cp.async.bulk.tensor box loads AND stores
+    TTC_KERNEL_TENSORMAP = 6, /* K1/K2/K3 through tensor maps: cp.async.bulk.tensor box loads AND stores
                                (<= 5-D, strides multiples of 16 bytes, 16-byte aligned A and B, same
                                element type), swizzled shared-memory boxes, in-register micro-tiles  */
+    TTC_KERNEL_SKEW = 7     /* K2/K3 for rows that are not 16-byte aligned (odd extents): bulk copies of aligned
+                               supersets in, skewed shared-memory rows, bulk stores of aligned bodies out    */
 } ttc_kernel_class;
 
 typedef struct ttc_plan_s* ttc_plan_t;

@@ -17,6 +17,7 @@ LIB_PATH = os.path.join(HERE, "libttc.so")
 SOURCES = ["kernels.cu", "api.cpp", "plan.cpp", "canon.cpp", "specialize.cpp", "static_scratch.cu"]
 HEADERS = [os.path.join(CSRC, "ttc_internal.h"), os.path.join(CSRC, "ttc_params.h"), os.path.join(CSRC, "ttc_device.cuh"),
            os.path.join(CSRC, "ttc_tmap.h"), os.path.join(CSRC, "ttc_tmap.cuh"),
+           os.path.join(CSRC, "ttc_skew.h"), os.path.join(CSRC, "ttc_skew.cuh"),
            os.path.join(INCLUDE, "ttc.h")]
 # Never -use_fast_math: it would flush denormals and contract roundings (reading A10).
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

@@ -229,8 +229,10 @@ ttc_status tune(ttc_plan_s* p, int top_k, int reps, int budget_ms) {
         bool over_budget = false;
         // the best-ranked tensor-map candidates are timed wherever the (ring-kernel-fitted) cost model puts them
         std::set<int> also;
-        for (int i = 0; i < (int)cs.size() && (int)also.size() < 4; ++i)
-            if (cs[i].info.kernel == TTC_KERNEL_TENSORMAP) also.insert(i);
+        for (int i = 0, n_map = 0, n_skew = 0; i < (int)cs.size(); ++i) {
+            if (cs[i].info.kernel == TTC_KERNEL_TENSORMAP && n_map < 4) { also.insert(i); ++n_map; }
+            if (cs[i].info.kernel == TTC_KERNEL_SKEW && n_skew < 4) { also.insert(i); ++n_skew; }
+        }
         for (int i = 0; i < (int)cs.size(); ++i) {
             // rank order; after the first 16 the list's time budget can end the search
             if (i >= 16 && !over_budget) {
@@ -345,8 +347,10 @@ int choose_candidate(ttc_plan_s* p, int which, uintptr_t A, uintptr_t B) {
 // offset (canonical rank <= 4); otherwise: the best other candidate whose accesses fit the pointers' alignment, looked
 // up once per alignment class.
 int without_tensormap(ttc_plan_s* p, int which, int idx, uintptr_t A, uintptr_t B) {
-    if (idx < 0 || p->cands[which][idx].info.kernel != TTC_KERNEL_TENSORMAP) return idx;
-    if (p->cands[which][idx].mp.flavour != 2 && p->cands[which][idx].mp.batchable) return idx;     // one map pair serves the batch
+    if (idx < 0) return idx;
+    const int kern = p->cands[which][idx].info.kernel;
+    if (kern != TTC_KERNEL_TENSORMAP && kern != TTC_KERNEL_SKEW) return idx;
+    if (kern == TTC_KERNEL_TENSORMAP && p->cands[which][idx].mp.flavour != 2 && p->cands[which][idx].mp.batchable) return idx;     // one map pair serves the batch
     auto lg = [](uintptr_t x) { int l = 0; while (l < 4 && !((x >> l) & 1)) ++l; return l; };
     const int la = lg(A), lb = lg(B);
     int& slot = p->nomap[which][5 * la + lb];
@@ -355,7 +359,7 @@ int without_tensormap(ttc_plan_s* p, int which, int idx, uintptr_t A, uintptr_t 
         float best_us = 0.f;
         const std::vector<Candidate>& cs = p->cands[which];
         for (int i = 0; i < (int)cs.size(); ++i) {
-            if (cs[i].info.kernel == TTC_KERNEL_TENSORMAP) continue;
+            if (cs[i].info.kernel == TTC_KERNEL_TENSORMAP || cs[i].info.kernel == TTC_KERNEL_SKEW) continue;
             if ((1 << la) % cs[i].align_a != 0 || (1 << lb) % cs[i].align_b != 0) continue;
             const float us = cs[i].info.tuned_us;
             if (slot < 0) { slot = i; best_us = us; continue; }
@@ -537,7 +541,8 @@ ttc_status ttc_execute_batched(ttc_plan_t p, const void* alpha, const void* cons
             float alt_us = 0.f;
             const std::vector<Candidate>& cs = p->cands[which];
             for (int i = 0; i < (int)cs.size(); ++i) {
-                if (cs[i].info.kernel == TTC_KERNEL_TENSORMAP || (oa % cs[i].align_a) != 0 || (ob % cs[i].align_b) != 0) continue;
+                if (cs[i].info.kernel == TTC_KERNEL_TENSORMAP || cs[i].info.kernel == TTC_KERNEL_SKEW || (oa % cs[i].align_a) != 0 ||
+                    (ob % cs[i].align_b) != 0) continue;
                 const float us = cs[i].info.tuned_us;
                 if (alt < 0) { alt = i; alt_us = us; continue; }
                 if (us > 0.f && (alt_us <= 0.f || us < alt_us)) { alt = i; alt_us = us; }
@@ -805,7 +810,7 @@ ttc_status ttc_plan_specialize(ttc_plan_t p) {
         const int win = p->winner[which];
         if (win < 0) continue;
         int idx = win;
-        if (p->cands[which][win].info.kernel == TTC_KERNEL_TENSORMAP) {
+        if (p->cands[which][win].info.kernel == TTC_KERNEL_TENSORMAP || p->cands[which][win].info.kernel == TTC_KERNEL_SKEW) {
             // a tensor-map winner has no twin: the fastest timed ring / direct candidate gets one and has to beat the winner
             idx = -1;
             const std::vector<Candidate>& cs = p->cands[which];

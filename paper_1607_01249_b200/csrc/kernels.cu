@@ -33,6 +33,7 @@
 
 #include "ttc_device.cuh"
 #include "ttc_tmap.cuh"
+#include "ttc_skew.cuh"
 
 namespace ttc {
 
@@ -292,6 +293,23 @@ static bool class_maps_cached(const TmapUEncode& ue, const void* A, void* B, Tma
     return true;
 }
 
+template <int DT>
+static KernelFn skew_fn_dt(bool beta) { return beta ? (KernelFn)skew_kernel<DT, true> : (KernelFn)skew_kernel<DT, false>; }
+
+static KernelFn get_skew_fn(int dt, const Candidate& c) {
+    switch (dt) {
+        case TTC_F32: return skew_fn_dt<TTC_F32>(c.beta_nz);
+        case TTC_F64: return skew_fn_dt<TTC_F64>(c.beta_nz);
+        case TTC_C64: return skew_fn_dt<TTC_C64>(c.beta_nz);
+    }
+    return nullptr;
+}
+
+static uint32_t skew_smem_bytes(const SkewParams& sp) {
+    const uint32_t rowsA = (uint32_t)sp.nP << sp.lgTB, rowsB = (uint32_t)sp.nP << sp.lgTA;
+    return (uint32_t)sp.stages * (rowsA * (uint32_t)sp.pitchA + rowsB * (uint32_t)sp.pitchB) + 128u;
+}
+
 static uint32_t tmapu_smem_bytes(const TmapUParams& up) {
     return (uint32_t)up.stages * 2u * (uint32_t)up.nP * (uint32_t)up.V * 1024u + 1024u;
 }
@@ -331,6 +349,25 @@ int prepare_candidate(Candidate* cand, ttc_dtype dtype, ttc_dtype dtype_a, int s
         cand->info.threads = kDirectThreads;
         cand->info.smem_bytes = 0;
         cand->info.grid = (int)(cand->dp.dyn == 1 || need < cap ? need : cap);
+        cand->grid_cap = (int)cap;
+        return 0;
+    }
+    if (cand->info.kernel == TTC_KERNEL_SKEW) {
+        KernelFn fn = dtype == dtype_a ? get_skew_fn((int)dtype, *cand) : nullptr;
+        if (!fn) return (int)cudaErrorInvalidValue;
+        const int smem = (int)skew_smem_bytes(cand->sp);
+        int optin = 0;
+        int rc = raise_smem_limit(fn, &optin);
+        if (rc != 0) return rc;
+        if (smem > optin) return (int)cudaErrorInvalidConfiguration;
+        int occ = 0;
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, cand->sp.threads, smem);
+        if (e != cudaSuccess) return (int)e;
+        if (occ < 1) return (int)cudaErrorInvalidConfiguration;
+        const uint64_t cap = (uint64_t)sm_count * (uint64_t)occ;
+        cand->info.threads = cand->sp.threads;
+        cand->info.smem_bytes = smem;
+        cand->info.grid = (int)(cand->sp.dyn == 1 || cand->sp.n_tiles < cap ? cand->sp.n_tiles : cap);
         cand->grid_cap = (int)cap;
         return 0;
     }
@@ -389,6 +426,7 @@ int launch_candidate(const Candidate& cand, ttc_dtype dtype, ttc_dtype dtype_a, 
     uint64_t grid = (uint64_t)cand.info.grid;
     if (batched) {     // one CTA per work item (launch control) or as many as the device holds
         const uint64_t work = (uint64_t)batch->per * (uint64_t)batch->n;
+        if (cand.info.kernel == TTC_KERNEL_SKEW) return (int)cudaErrorNotSupported;
         if (cand.info.kernel == TTC_KERNEL_TENSORMAP && (cand.mp.flavour == 2 || !cand.mp.batchable)) return (int)cudaErrorNotSupported;
         const int dyn_b = cand.info.kernel == TTC_KERNEL_COPY ? cand.dp.dyn : cand.info.kernel == TTC_KERNEL_TENSORMAP ? cand.mp.dyn : cand.tp.dyn;
         grid = (dyn_b == 1 || work < (uint64_t)cand.grid_cap) ? work : (uint64_t)cand.grid_cap;
@@ -402,7 +440,8 @@ int launch_candidate(const Candidate& cand, ttc_dtype dtype, ttc_dtype dtype_a, 
     // (198 MB): -0.3 .. -1.3 us per launch; neutral for stream launches.  A predecessor that is not one
     // of these kernels never triggers early, which degenerates to ordinary stream order.  TTC_PDL=0: off.
     cudaLaunchAttribute attr[1];
-    const int dyn = cand.info.kernel == TTC_KERNEL_COPY ? cand.dp.dyn : cand.info.kernel == TTC_KERNEL_TENSORMAP ? cand.mp.dyn : cand.tp.dyn;
+    const int dyn = cand.info.kernel == TTC_KERNEL_COPY ? cand.dp.dyn : cand.info.kernel == TTC_KERNEL_TENSORMAP ? cand.mp.dyn
+                    : cand.info.kernel == TTC_KERNEL_SKEW ? cand.sp.dyn : cand.tp.dyn;
     static const int pdl_env = std::getenv("TTC_PDL") ? std::atoi(std::getenv("TTC_PDL")) : -1;
     if (dyn == 2 && !sched_ctr) return (int)cudaErrorInvalidValue;
     if (pdl_env != 0) {
@@ -413,6 +452,16 @@ int launch_candidate(const Candidate& cand, ttc_dtype dtype, ttc_dtype dtype_a, 
     }
     NoBatch none;
     Scalar al = alpha, be = beta;
+    if (cand.info.kernel == TTC_KERNEL_SKEW) {
+        KernelFn fn = dtype == dtype_a ? get_skew_fn((int)dtype, cand) : nullptr;
+        if (!fn) return (int)cudaErrorInvalidValue;
+        cfg.blockDim = dim3((unsigned)cand.sp.threads, 1, 1);
+        cfg.dynamicSmemBytes = (size_t)cand.info.smem_bytes;
+        SkewParams sp = cand.sp;
+        sp.ctr = sched_ctr;
+        void* sargs[5] = {&sp, (void*)&A, (void*)&B, &al, &be};
+        return (int)cudaLaunchKernelExC(&cfg, fn, sargs);
+    }
     if (cand.info.kernel == TTC_KERNEL_TENSORMAP && cand.mp.flavour == 2) {
         KernelFn fn = dtype == dtype_a ? get_tmapu_fn((int)dtype, cand) : nullptr;
         if (!fn) return (int)cudaErrorInvalidValue;

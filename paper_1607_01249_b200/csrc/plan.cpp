@@ -1153,6 +1153,135 @@ void add_tmapu(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz,
         }
 }
 
+
+// Skew-kernel candidates (TTC_KERNEL_SKEW, ttc_skew.cuh): 4- and 8-byte elements of one type, transposing class, offered
+// where a tensor map cannot express the tensors (a stride or B's row length is not a multiple of 16 bytes).
+void add_skew(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, int sched, int max_smem, std::vector<Candidate>* out) {
+    if (dtype != dtype_a || c.rank < 2) return;
+    const int es = elem_size(dtype);
+    if (es > 8) return;
+    const int q = c.orderB[0];
+    if (q == 0 || c.d[0].sA != 1 || c.d[q].sB != 1) return;
+    bool mappable = (c.d[q].e * es) % 16 == 0;
+    for (int i = 0; i < c.rank; ++i) {
+        if (c.d[i].e >= kInt31 / 2) return;
+        if (i != 0 && (c.d[i].sA * es) % 16 != 0) mappable = false;
+        if (i != q && (c.d[i].sB * es) % 16 != 0) mappable = false;
+    }
+    if (mappable) return;
+    if (c.d[0].e < 16 || c.d[q].e < 16) return;
+    std::vector<int> othA, othB;
+    for (int i = 0; i < c.rank; ++i) if (i != 0 && i != q) othA.push_back(i);
+    for (int k = 0; k < c.rank; ++k) if (c.orderB[k] != 0 && c.orderB[k] != q) othB.push_back(c.orderB[k]);
+    struct Var { int lgA, lgB, planes, dist; };
+    static const Var vars[] = {{6, 5, 1, 0}, {5, 6, 1, 0}, {6, 6, 1, 0}, {7, 5, 1, 0}, {5, 7, 1, 0}, {5, 5, 2, 0}, {5, 5, 2, 1},
+                               {6, 5, 2, 0}, {5, 6, 2, 1}, {5, 5, 4, 0}, {5, 5, 4, 1}, {7, 6, 1, 0}, {6, 7, 1, 0}};
+    std::set<std::string> seen;
+    int n_added = 0;
+    for (const Var& v : vars) {
+        const int TA = 1 << v.lgA, TB = 1 << v.lgB;
+        if (c.d[0].e * 2 < TA || c.d[q].e * 2 < TB) continue;                 // more than half of the tile would be padding
+        int32_t pe[kMaxRank];
+        for (int i = 0; i < c.rank; ++i) pe[i] = 1;
+        int left = v.planes;
+        for (int i : (v.dist == 0 ? othA : othB)) {                            // planes divide the extents
+            if (left < 2) break;
+            int t = 1;
+            for (int d = (int)std::min<int64_t>(left, c.d[i].e); d >= 1; --d)
+                if (c.d[i].e % d == 0) { t = d; break; }
+            pe[i] = t;
+            left /= t;
+        }
+        std::string key((const char*)pe, sizeof(int32_t) * c.rank);
+        key.push_back((char)v.lgA);
+        key.push_back((char)v.lgB);
+        if (!seen.insert(key).second) continue;
+        Candidate cand;
+        cand.beta_nz = beta_nz;
+        SkewParams& K = cand.sp;
+        std::memset(&K, 0, sizeof(K));
+        K.lgTA = v.lgA;
+        K.lgTB = v.lgB;
+        K.nG = c.rank;
+        K.sqA = c.d[q].sA;
+        K.s0B = c.d[0].sB;
+        K.e0 = c.d[0].e;
+        K.eq = c.d[q].e;
+        K.spanA = c.spanA;
+        K.spanB = c.spanB;
+        K.pitchA = TA * es + 32;         // the aligned superset of a row: up to 12 bytes before and after it
+        K.pitchB = TB * es + 32;
+        int gd[kMaxRank];
+        int n = 0;
+        gd[n++] = 0;
+        gd[n++] = q;
+        for (int i : othA) gd[n++] = i;
+        uint64_t n_tiles = 1;
+        double padded = 1.0, real = 1.0;
+        bool ok = true;
+        for (int k = 0; k < n; ++k) {
+            const int i = gd[k];
+            const int64_t step = k == 0 ? TA : k == 1 ? TB : pe[i];
+            const int64_t nt = (c.d[i].e + step - 1) / step;
+            K.gdiv[k] = make_fastdiv((uint32_t)nt);
+            K.stepA[k] = k < 2 ? 0 : step * c.d[i].sA;
+            K.stepB[k] = k < 2 ? 0 : step * c.d[i].sB;
+            n_tiles *= (uint64_t)nt;
+            if (n_tiles >= (uint64_t)kInt31) { ok = false; break; }
+            padded *= (double)nt * step;
+            real *= (double)c.d[i].e;
+        }
+        if (!ok) continue;
+        int nP = 1;
+        K.pA[0] = K.pB[0] = 0;
+        for (int i : othA) {
+            const int have = nP;
+            for (int t = 1; t < pe[i]; ++t)
+                for (int h = 0; h < have; ++h) {
+                    K.pA[nP] = K.pA[h] + (int64_t)t * c.d[i].sA;
+                    K.pB[nP] = K.pB[h] + (int64_t)t * c.d[i].sB;
+                    ++nP;
+                }
+        }
+        if (nP > kSkewMaxPlanes || nP * TA > kSkewMaxRows || nP * TB > kSkewMaxRows) continue;
+        K.nP = nP;
+        const int64_t stage = (int64_t)nP * ((int64_t)TB * K.pitchA + (int64_t)TA * K.pitchB);
+        int stages = 0;
+        for (int st = 3; st >= 2; --st)
+            if (st * stage + 128 <= std::min<int64_t>(max_smem, 100 * 1024)) { stages = st; break; }
+        if (!stages) continue;
+        K.dyn = sched;
+        K.n_tiles = (uint32_t)n_tiles;
+        K.stages = stages;
+        K.threads = 192;
+        cand.align_a = cand.align_b = es;
+        ttc_candidate_info& I = cand.info;
+        I.kernel = TTC_KERNEL_SKEW;
+        I.flags = 0;
+        I.vec_a = I.vec_b = 16 / es;
+        I.threads = K.threads;
+        I.loop_order = 0;
+        I.sched = sched;
+        I.n_tiles = (int64_t)n_tiles;
+        I.tile_u = TA;
+        I.tile_w = TB;
+        I.n_u = 1;
+        I.n_w = 1;
+        for (int i = 0; i < kMaxRank; ++i) I.tile_ext[i] = i < c.rank ? pe[i] : 0;
+        I.tile_ext[0] = TA;
+        I.tile_ext[q] = TB;
+        const double waste = padded / real;
+        I.est_cost = (float)((1.20 + 0.01 * n_added) * waste);
+        cand.feat[2] = (float)waste;
+        cand.feat[4] = (float)stage;
+        cand.feat[5] = (float)n_tiles;
+        cand.feat[12] = beta_nz ? 1.f : 0.f;
+        cand.feat[13] = (float)TTC_KERNEL_SKEW;
+        out->push_back(cand);
+        ++n_added;
+    }
+}
+
 }  // namespace
 
 void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, int sm_count,
@@ -1176,7 +1305,7 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, boo
 
     // TTC_VARIANTS: bit 0 = staggered-gather ring candidates, bit 1 = shifted-row ring candidates, bit 2 = tensor-map
     // candidates (default: all)
-    const int variants = std::getenv("TTC_VARIANTS") ? std::atoi(std::getenv("TTC_VARIANTS")) : 7;
+    const int variants = std::getenv("TTC_VARIANTS") ? std::atoi(std::getenv("TTC_VARIANTS")) : 15;
     const int xp_max = (variants & 1) ? 1 : 0;
     const int n_loop_orders = std::getenv("TTC_LOOP_ORDERS") ? std::max(2, std::min(4, std::atoi(std::getenv("TTC_LOOP_ORDERS")))) : 2;
     const int ring_max = std::getenv("TTC_RING") ? std::atoi(std::getenv("TTC_RING")) : 4;
@@ -1194,6 +1323,9 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, boo
             add_tmap(c, dtype, dtype_a, beta_nz, sched, max_smem, out);
             add_tmapu(c, dtype, dtype_a, beta_nz, sched, max_smem, out);
         }
+    // Skew-kernel candidates (TTC_VARIANTS bit 3).
+    if (variants & 8)
+        for (int sched : scheds) add_skew(c, dtype, dtype_a, beta_nz, sched, max_smem, out);
 
     // K2 / K3: tiles.  A side = leading indices of A, B side = leading indices of B.
     std::vector<int> orderA, orderB;
@@ -1264,7 +1396,7 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, boo
     const int n_full = std::min<int>((int)out->size(), std::getenv("TTC_FULL_SEARCH") ? std::atoi(std::getenv("TTC_FULL_SEARCH")) : kFullSearch);
     for (int i = 0; i < n_full; ++i) {
         Candidate& cd = (*out)[i];
-        if (cd.info.kernel == TTC_KERNEL_COPY || cd.info.kernel == TTC_KERNEL_TENSORMAP) continue;
+        if (cd.info.kernel == TTC_KERNEL_COPY || cd.info.kernel == TTC_KERNEL_TENSORMAP || cd.info.kernel == TTC_KERNEL_SKEW) continue;
         const Recipe r = cd.recipe;
         Candidate full;
         if (build_tile_candidate(c, dtype, dtype_a, beta_nz, r.spec, r.loop_order, r.va, r.vb, max_smem, r.sched, r.ring, r.xp,

@@ -8,6 +8,7 @@
 #include "ttc.h"
 #include "ttc_params.h"
 #include "ttc_tmap.h"
+#include "ttc_skew.h"
 
 namespace ttc {
 
@@ -57,6 +58,7 @@ struct Candidate {
     TileParams tp{};
     TmapParams mp{};             // TTC_KERNEL_TENSORMAP: kernel parameters and what the two tensor maps are encoded from
     TmapEncode me{};
+    SkewParams sp{};             // TTC_KERNEL_SKEW
     TmapUParams up{};            // TTC_KERNEL_TENSORMAP with mp.flavour == 2 (residue classes)
     TmapUEncode ue{};
     float feat[16] = {0};        // raw inputs of the cost heuristic (plan.cpp), exported for re-fitting

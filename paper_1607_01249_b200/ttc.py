@@ -23,7 +23,7 @@ STATUS_NAMES = ["TTC_OK", "TTC_ERR_INVALID_ARG", "TTC_ERR_NOT_PERMUTATION", "TTC
                 "TTC_ERR_UNSUPPORTED", "TTC_ERR_ALLOC", "TTC_ERR_CUDA", "TTC_ERR_MISALIGNED", "TTC_ERR_SCRATCH_LIMIT"]
 TTC_ERR_SCRATCH_LIMIT = 8
 TTC_STATIC_SCRATCH_BYTES = 8 << 20
-KERNEL_NAMES = {0: "none", 1: "copy", 2: "tile", 3: "gather", 4: "wide", 5: "tma", 6: "tensormap"}
+KERNEL_NAMES = {0: "none", 1: "copy", 2: "tile", 3: "gather", 4: "wide", 5: "tma", 6: "tensormap", 7: "skew"}
 NP_DTYPE = {TTC_F32: np.float32, TTC_F64: np.float64, TTC_C64: np.complex64, TTC_C128: np.complex128}
 
 EXPORTS = ["ttc_plan", "ttc_plan_mixed", "ttc_plan_strided", "ttc_plan_dtype_a", "ttc_execute", "ttc_execute_batched", "ttc_execute_host", "ttc_execute_host_static", "ttc_destroy", "ttc_last_error",
