@@ -43,7 +43,8 @@
  *   TTC_PDL=0             launch without programmatic dependent launch (default: with)
  *   TTC_RING=0|2|4        largest ring of tile buffers of the warp-specialised kernel (0: none; default 4)
  *   TTC_VARIANTS=bits     candidate flavours to generate: 1 staggered-gather ring, 2 shifted-row ring, 4 tensor-map
- *                         kernels, 8 skew kernels (default 15: all)
+ *                         kernels, 8 skew kernels (default 7: the skew kernels are slower than the ring kernel's
+ *                         shifted rows on B200 and are offered only on request)
  */
 #ifndef TTC_H_
 #define TTC_H_

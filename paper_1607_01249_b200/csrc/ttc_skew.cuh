@@ -17,7 +17,7 @@
 namespace ttc {
 
 template <int DT, bool BETA>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(384)
 skew_kernel(const __grid_constant__ SkewParams P, const void* __restrict__ Ain, void* __restrict__ Bout,
             const Scalar alpha_in, const Scalar beta_in) {
     using T = typename ElemT<DT>::T;
@@ -42,12 +42,15 @@ skew_kernel(const __grid_constant__ SkewParams P, const void* __restrict__ Ain, 
     __shared__ int64_t off_of[kSkewMaxStages][2][2];         // [stage][use parity][A, B]: element offset of the tile's outer indices
     __shared__ int32_t org_of[kSkewMaxStages][2][2];         // first a0, first b0 of the tile
     __shared__ uint32_t tile_of[kSkewMaxStages][2];
+    __shared__ uint32_t tile_pub[2];                         // the tile the producer warps load in iteration it (slot it & 1)
     __shared__ uint8_t skA[kSkewMaxStages][kSkewMaxRows];    // skew of every in-row (read by the consumers only)
     __shared__ uint8_t skB[kSkewMaxStages][2][kSkewMaxRows]; // skew of every out-row (consumers and, later, the store warp)
 
     const int tid = threadIdx.x, lane = tid & 31;
     const int S = P.stages;
-    const int n_cons_warps = ((int)blockDim.x >> 5) - 2;
+    const int NP = P.np, NS = P.ns;
+    const int n_cons_warps = ((int)blockDim.x >> 5) - NP - NS;
+    const int warp = tid >> 5;
     const char* const A = static_cast<const char*>(Ain);
     char* const B = static_cast<char*>(Bout);
     WorkSched sched;
@@ -55,34 +58,44 @@ skew_kernel(const __grid_constant__ SkewParams P, const void* __restrict__ Ain, 
     pdl_launch_dependents();
     if (tid == 0) {
         for (int s = 0; s < S; ++s) {
-            asm volatile("mbarrier.init.shared::cta.b64 [%0], 32;" ::"r"((uint32_t)__cvta_generic_to_shared(&full_bar[s])));
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(&full_bar[s])), "r"(32 * NP));
             asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(&done_bar[s])), "r"(n_cons_warps));
-            asm volatile("mbarrier.init.shared::cta.b64 [%0], 32;" ::"r"((uint32_t)__cvta_generic_to_shared(&outfree_bar[s])));
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(&outfree_bar[s])), "r"(32 * NS));
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
     pdl_wait();
 
-    if (tid < 32) {
-        // ------------------------------------------------------------------ producer warp
+    if (warp < NP) {
+        // ------------------------------------------------------------------ producer warps (warp 0 draws the tiles)
         uint32_t tile_id = blockIdx.x;
         bool more = true;
         for (uint32_t it = 0;; ++it) {
+            if (NP > 1) {        // warp 0 publishes the tile of this iteration (0xFFFFFFFF: none left), the others pick it up
+                if (tid == 0) tile_pub[it & 1u] = more ? tile_id : 0xFFFFFFFFu;
+                asm volatile("bar.sync 1, %0;" ::"r"(32 * NP) : "memory");
+                if (warp != 0) {
+                    tile_id = tile_pub[it & 1u];
+                    more = tile_id != 0xFFFFFFFFu;
+                }
+            }
             const int s = (int)(it % (uint32_t)S);
             const int u = (int)((it / (uint32_t)S) & 1u);
             const uint32_t full_a = (uint32_t)__cvta_generic_to_shared(&full_bar[s]);
             if (it >= (uint32_t)S) {
+                // the in-tile is free once its consumers are done; the out-tile, which only beta != 0 loads into, once the
+                // store warp's copies of its last use have read it (beta == 0: the consumers wait for that instead)
                 mbar_wait((uint32_t)__cvta_generic_to_shared(&done_bar[s]), ((it / (uint32_t)S) - 1u) & 1u);
-                mbar_wait((uint32_t)__cvta_generic_to_shared(&outfree_bar[s]), ((it / (uint32_t)S) - 1u) & 1u);
+                if constexpr (BETA) mbar_wait((uint32_t)__cvta_generic_to_shared(&outfree_bar[s]), ((it / (uint32_t)S) - 1u) & 1u);
             }
             if (!more) {
-                if (lane == 0) tile_of[s][u] = 0xFFFFFFFFu;
+                if (tid == 0) tile_of[s][u] = 0xFFFFFFFFu;
                 __syncwarp();
                 asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(full_a) : "memory");
                 break;
             }
-            sched.prefetch();
+            if (warp == 0) sched.prefetch();
             // every lane decodes the tile (cheap) and takes rows lane, lane + 32, ...
             int32_t org0 = 0, org1 = 0;
             int64_t ca = 0, cb = 0;
@@ -97,7 +110,7 @@ skew_kernel(const __grid_constant__ SkewParams P, const void* __restrict__ Ain, 
                     else { ca += (int64_t)c * P.stepA[d]; cb += (int64_t)c * P.stepB[d]; }
                 }
             }
-            if (lane == 0) {
+            if (tid == 0) {
                 org_of[s][u][0] = org0;
                 org_of[s][u][1] = org1;
                 off_of[s][u][0] = ca;
@@ -112,7 +125,7 @@ skew_kernel(const __grid_constant__ SkewParams P, const void* __restrict__ Ain, 
                 const int64_t left = P.e0 - org0;
                 const int len = (int)(left < TA ? left : TA);
                 const uintptr_t lo = (uintptr_t)A, hi = lo + (uintptr_t)P.spanA * ES;
-                for (int r = lane; r < rowsA; r += 32) {
+                for (int r = warp * 32 + lane; r < rowsA; r += 32 * NP) {      // one row per lane and pass
                     const int p = r >> P.lgTB, b = r & (TB - 1);
                     const int64_t bg = (int64_t)org1 + b;
                     if (bg >= P.eq) { skA[s][r] = 0; continue; }
@@ -138,7 +151,7 @@ skew_kernel(const __grid_constant__ SkewParams P, const void* __restrict__ Ain, 
                 const int64_t left = P.eq - org1;
                 const int len = (int)(left < TB ? left : TB);
                 const uintptr_t lo = (uintptr_t)B, hi = lo + (uintptr_t)P.spanB * ES;
-                for (int r = lane; r < rowsB; r += 32) {
+                for (int r = warp * 32 + lane; r < rowsB; r += 32 * NP) {
                     const int p = r >> P.lgTA, a = r & (TA - 1);
                     const int64_t ag = (int64_t)org0 + a;
                     if (ag >= P.e0) { skB[s][u][r] = 0; continue; }
@@ -162,11 +175,11 @@ skew_kernel(const __grid_constant__ SkewParams P, const void* __restrict__ Ain, 
                 }
             }
             asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(full_a) : "memory");
-            more = sched.next<true>(tile_id, P.n_tiles);
+            if (warp == 0) more = sched.next<true>(tile_id, P.n_tiles);
             __syncwarp();
         }
-    } else if (tid < 64) {
-        // ------------------------------------------------------------------ store warp
+    } else if (warp < NP + NS) {
+        // ------------------------------------------------------------------ store warps
         for (uint32_t it = 0;; ++it) {
             const int s = (int)(it % (uint32_t)S);
             const int u = (int)((it / (uint32_t)S) & 1u);
@@ -177,7 +190,7 @@ skew_kernel(const __grid_constant__ SkewParams P, const void* __restrict__ Ain, 
             unsigned char* const out_s = smem + (uint32_t)s * stage_bytes + in_bytes;
             const int64_t left = P.eq - org1;
             const int len = (int)(left < TB ? left : TB);
-            for (int r = lane; r < rowsB; r += 32) {
+            for (int r = (warp - NP) * 32 + lane; r < rowsB; r += 32 * NS) {      // one out-row per lane and pass
                 const int p = r >> P.lgTA, a = r & (TA - 1);
                 const int64_t ag = (int64_t)org0 + a;
                 if (ag >= P.e0) continue;
@@ -203,26 +216,40 @@ skew_kernel(const __grid_constant__ SkewParams P, const void* __restrict__ Ain, 
         asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
     } else {
         // ------------------------------------------------------------------ consumer warps
-        const int cw = (tid >> 5) - 2;
+        const int cw = warp - NP - NS;
         for (uint32_t it = 0;; ++it) {
             const int s = (int)(it % (uint32_t)S);
             const int u = (int)((it / (uint32_t)S) & 1u);
             mbar_wait((uint32_t)__cvta_generic_to_shared(&full_bar[s]), (uint32_t)u);
             const bool end = tile_of[s][u] == 0xFFFFFFFFu;
             if (!end) {
+                if constexpr (!BETA)
+                    if (it >= (uint32_t)S) mbar_wait((uint32_t)__cvta_generic_to_shared(&outfree_bar[s]), ((it / (uint32_t)S) - 1u) & 1u);
                 unsigned char* const in_s = smem + (uint32_t)s * stage_bytes;
                 unsigned char* const out_s = in_s + in_bytes;
+                // 32 x 32 blocks, walked along diagonals: in step j lane l moves element (a0 + l, b0 + (l + j) % 32).  With row
+                // pitches of an odd number of 16-byte units (4 mod 32 words) the 32 lanes hit banks 5 l + 4 j + skew on the
+                // in-side and 5 l + j + skew on the out-side: both conflict-free up to the skews' perturbation.  The warps
+                // share every block (warp w takes the steps j = w, w + warps, ...).
+                const int dq = (int)(P.sqA & (V - 1)), d0 = (int)(P.s0B & (V - 1));
                 for (int p = 0; p < P.nP; ++p) {
+                    const int sA0 = skA[s][p << P.lgTB], sB0 = skB[s][u][p << P.lgTA];      // skews of the plane's first rows
                     for (int a0 = 0; a0 < TA; a0 += 32) {
                         const int a = a0 + lane;
-                        const int rb = (p << P.lgTA) + a;
-                        T* const orow = reinterpret_cast<T*>(out_s + (uint32_t)rb * (uint32_t)P.pitchB) + skB[s][u][rb];
-                        for (int b = cw; b < TB; b += n_cons_warps) {
-                            const int ra = (p << P.lgTB) + b;
-                            const T* const irow = reinterpret_cast<const T*>(in_s + (uint32_t)ra * (uint32_t)P.pitchA) + skA[s][ra];
-                            T x = scale(alpha, irow[a]);
-                            if constexpr (BETA) x = add(x, scale(beta, orow[b]));
-                            orow[b] = x;
+                        const int skb = (sB0 + a * d0) & (V - 1);
+                        unsigned char* const orow = out_s + (uint32_t)((p << P.lgTA) + a) * (uint32_t)P.pitchB + skb * ES;
+                        const unsigned char* const icol = in_s + (uint32_t)(p << P.lgTB) * (uint32_t)P.pitchA + a * ES;
+                        for (int b0 = 0; b0 < TB; b0 += 32) {
+#pragma unroll 4
+                            for (int j = cw; j < 32; j += n_cons_warps) {
+                                const int b = b0 + ((lane + j) & 31);
+                                const int ska = (sA0 + b * dq) & (V - 1);
+                                const T* const src = reinterpret_cast<const T*>(icol + (uint32_t)b * (uint32_t)P.pitchA + ska * ES);
+                                T* const dst = reinterpret_cast<T*>(orow + b * ES);
+                                T x = scale(alpha, *src);
+                                if constexpr (BETA) x = add(x, scale(beta, *dst));
+                                *dst = x;
+                            }
                         }
                     }
                 }

@@ -13,7 +13,7 @@
 
 namespace ttc {
 
-constexpr int kSkewMaxStages = 3;
+constexpr int kSkewMaxStages = 4;
 constexpr int kSkewMaxPlanes = 8;
 constexpr int kSkewMaxRows = 512;      // rows of one side of a tile (planes x tile extent)
 
@@ -22,6 +22,7 @@ struct SkewParams {
     uint32_t* ctr;
     uint32_t n_tiles;
     int stages, threads;
+    int np, ns;                    // producer warps, store warps (the rest of the CTA's warps are consumers)
     int lgTA, lgTB;                // tile extents along a0 and b0 are powers of two
     int nP;                        // planes (index combinations of the other indices) per tile
     int nG;                        // tile-grid dimensions: 0 = a0, 1 = b0, then the other canonical indices
