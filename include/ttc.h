@@ -43,8 +43,8 @@
  *   TTC_PDL=0             launch without programmatic dependent launch (default: with)
  *   TTC_RING=0|2|4        largest ring of tile buffers of the warp-specialised kernel (0: none; default 4)
  *   TTC_VARIANTS=bits     candidate flavours to generate: 1 staggered-gather ring, 2 shifted-row ring, 4 tensor-map
- *                         kernels, 8 skew kernels (default 7: the skew kernels are slower than the ring kernel's
- *                         shifted rows on B200 and are offered only on request)
+ *                         kernels, 8 skew kernels that store to B directly, 16 skew kernels with an out-tile and bulk
+ *                         stores (default 15; the out-tile variants are 2x slower on B200: only on request)
  */
 #ifndef TTC_H_
 #define TTC_H_
@@ -115,6 +115,7 @@ typedef struct {
 
 #define TTC_CAND_STAGGERED 1   /* ring kernel: bank-conflict-free "staggered" gather from the tile      */
 #define TTC_CAND_SHIFTED_ROWS 4 /* ring kernel, rows not 16-byte aligned: aligned bodies by bulk copy, skewed tile */
+#define TTC_CAND_DIRECT_OUT 8  /* skew kernel without out-tile: the consumers store to B themselves            */
 #define TTC_CAND_TENSORMAP 2   /* tiles moved by TMA tensor-map loads / stores (cp.async.bulk.tensor)  */
 
 /* One candidate implementation (loop order x blocking; here also kernel class). */

@@ -3,4 +3,4 @@
 ``csrc/``; :mod:`paper_1607_01249_b200.ttc` is its thin ctypes binding (argument
 marshalling only).  Nothing is loaded at package import; the binding fails loudly on
 first use if the CUDA library has not been built."""
-__version__ = "0.4.0"   # == the number in ttc_version() (tests/test_host_abi.py)
+__version__ = "0.5.0"   # == the number in ttc_version() (tests/test_host_abi.py)

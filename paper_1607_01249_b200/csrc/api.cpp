@@ -902,7 +902,7 @@ int64_t ttc_launch_count(void) { return g_launches.load(); }
 
 uint32_t ttc_debug_fastdiv(uint32_t n, uint32_t d) { return fd_div(n, make_fastdiv(d)); }
 
-const char* ttc_version(void) { return "ttc-b200 0.4 (sm_100a)"; }
+const char* ttc_version(void) { return "ttc-b200 0.5 (sm_100a)"; }
 
 ttc_status ttc_release_host_staging(void) {
     std::lock_guard<std::mutex> lk(g_stage_mu);

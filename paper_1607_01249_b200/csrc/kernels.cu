@@ -294,13 +294,17 @@ static bool class_maps_cached(const TmapUEncode& ue, const void* A, void* B, Tma
 }
 
 template <int DT>
-static KernelFn skew_fn_dt(bool beta) { return beta ? (KernelFn)skew_kernel<DT, true> : (KernelFn)skew_kernel<DT, false>; }
+static KernelFn skew_fn_dt(bool beta, bool direct) {
+    if (direct) return beta ? (KernelFn)skew_kernel<DT, true, true> : (KernelFn)skew_kernel<DT, false, true>;
+    return beta ? (KernelFn)skew_kernel<DT, true, false> : (KernelFn)skew_kernel<DT, false, false>;
+}
 
 static KernelFn get_skew_fn(int dt, const Candidate& c) {
+    const bool direct = c.sp.ns == 0;          // no store warps: the consumers write B
     switch (dt) {
-        case TTC_F32: return skew_fn_dt<TTC_F32>(c.beta_nz);
-        case TTC_F64: return skew_fn_dt<TTC_F64>(c.beta_nz);
-        case TTC_C64: return skew_fn_dt<TTC_C64>(c.beta_nz);
+        case TTC_F32: return skew_fn_dt<TTC_F32>(c.beta_nz, direct);
+        case TTC_F64: return skew_fn_dt<TTC_F64>(c.beta_nz, direct);
+        case TTC_C64: return skew_fn_dt<TTC_C64>(c.beta_nz, direct);
     }
     return nullptr;
 }

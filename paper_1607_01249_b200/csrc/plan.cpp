@@ -1173,12 +1173,18 @@ void add_skew(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, 
     std::vector<int> othA, othB;
     for (int i = 0; i < c.rank; ++i) if (i != 0 && i != q) othA.push_back(i);
     for (int k = 0; k < c.rank; ++k) if (c.orderB[k] != 0 && c.orderB[k] != q) othB.push_back(c.orderB[k]);
-    struct Var { int lgA, lgB, planes, dist; };
-    static const Var vars[] = {{6, 5, 1, 0}, {5, 6, 1, 0}, {6, 6, 1, 0}, {7, 5, 1, 0}, {5, 7, 1, 0}, {5, 5, 2, 0}, {5, 5, 2, 1},
-                               {6, 5, 2, 0}, {5, 6, 2, 1}, {5, 5, 4, 0}, {5, 5, 4, 1}, {7, 6, 1, 0}, {6, 7, 1, 0}};
+    // direct = 1: no out-tile, the consumers store to B themselves (coalesced element stores)
+    struct Var { int lgA, lgB, planes, dist, direct; };
+    static const Var vars[] = {{7, 6, 1, 0, 1}, {6, 7, 1, 0, 1}, {7, 5, 1, 0, 1}, {6, 5, 1, 0, 1}, {8, 5, 1, 0, 1}, {6, 6, 1, 0, 1},
+                               {5, 6, 1, 0, 1}, {5, 7, 1, 0, 1}, {5, 5, 1, 0, 1}, {5, 5, 2, 0, 1}, {6, 5, 2, 0, 1}, {6, 5, 2, 1, 1}, {5, 6, 2, 0, 1}, {5, 6, 2, 1, 1},
+                               {6, 5, 1, 0, 0}, {5, 6, 1, 0, 0}, {6, 6, 1, 0, 0}, {7, 5, 1, 0, 0}, {5, 7, 1, 0, 0}, {5, 5, 2, 0, 0}, {5, 5, 2, 1, 0},
+                               {6, 5, 2, 0, 0}, {5, 6, 2, 1, 0}, {5, 5, 4, 0, 0}, {5, 5, 4, 1, 0}, {7, 6, 1, 0, 0}, {6, 7, 1, 0, 0}};
+    // TTC_VARIANTS bit 3 offers the direct-out variants (default), bit 4 the out-tile variants as well (measured 2x slower)
+    const int variants = std::getenv("TTC_VARIANTS") ? std::atoi(std::getenv("TTC_VARIANTS")) : 15;
     std::set<std::string> seen;
     int n_added = 0;
     for (const Var& v : vars) {
+        if (!v.direct && !(variants & 16)) continue;
         const int TA = 1 << v.lgA, TB = 1 << v.lgB;
         if (c.d[0].e * 2 < TA || c.d[q].e * 2 < TB) continue;                 // more than half of the tile would be padding
         int32_t pe[kMaxRank];
@@ -1195,6 +1201,7 @@ void add_skew(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, 
         std::string key((const char*)pe, sizeof(int32_t) * c.rank);
         key.push_back((char)v.lgA);
         key.push_back((char)v.lgB);
+        key.push_back((char)v.direct);
         if (!seen.insert(key).second) continue;
         Candidate cand;
         cand.beta_nz = beta_nz;
@@ -1210,7 +1217,7 @@ void add_skew(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, 
         K.spanA = c.spanA;
         K.spanB = c.spanB;
         K.pitchA = TA * es + 48;         // the aligned superset of a row (up to 12 bytes before and after it); an odd number
-        K.pitchB = TB * es + 48;         // of 16-byte units, so that the consumers' diagonal walk spreads over all banks
+        K.pitchB = v.direct ? 0 : TB * es + 48;   // of 16-byte units, so that the consumers' diagonal walk spreads over all banks
         int gd[kMaxRank];
         int n = 0;
         gd[n++] = 0;
@@ -1254,13 +1261,13 @@ void add_skew(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, 
         K.n_tiles = (uint32_t)n_tiles;
         K.stages = stages;
         K.np = 4;
-        K.ns = 4;
+        K.ns = v.direct ? 0 : 4;
         K.threads = 384;                 // 4 producer warps, 4 store warps, 4 consumer warps: a bulk copy costs its issuing
                                          // warp ~150 cycles, so the row copies are spread over several warps
         cand.align_a = cand.align_b = es;
         ttc_candidate_info& I = cand.info;
         I.kernel = TTC_KERNEL_SKEW;
-        I.flags = 0;
+        I.flags = v.direct ? TTC_CAND_DIRECT_OUT : 0;
         I.vec_a = I.vec_b = 16 / es;
         I.threads = K.threads;
         I.loop_order = 0;
@@ -1307,9 +1314,9 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, boo
     }
 
     // TTC_VARIANTS: bit 0 = staggered-gather ring candidates, bit 1 = shifted-row ring candidates, bit 2 = tensor-map
-    // candidates, bit 3 = skew-kernel candidates (default 7: the skew kernel is correct but measured 2x slower than the ring
-    // kernel's shifted rows, so it is not offered unless asked for)
-    const int variants = std::getenv("TTC_VARIANTS") ? std::atoi(std::getenv("TTC_VARIANTS")) : 7;
+    // candidates, bit 3 = skew-kernel candidates that store to B directly (default 15: all of these), bit 4 = the skew
+    // kernel's out-tile variants (correct but measured 2x slower: only on request)
+    const int variants = std::getenv("TTC_VARIANTS") ? std::atoi(std::getenv("TTC_VARIANTS")) : 15;
     const int xp_max = (variants & 1) ? 1 : 0;
     const int n_loop_orders = std::getenv("TTC_LOOP_ORDERS") ? std::max(2, std::min(4, std::atoi(std::getenv("TTC_LOOP_ORDERS")))) : 2;
     const int ring_max = std::getenv("TTC_RING") ? std::atoi(std::getenv("TTC_RING")) : 4;
@@ -1327,7 +1334,7 @@ void generate_candidates(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, boo
             add_tmap(c, dtype, dtype_a, beta_nz, sched, max_smem, out);
             add_tmapu(c, dtype, dtype_a, beta_nz, sched, max_smem, out);
         }
-    // Skew-kernel candidates (TTC_VARIANTS bit 3, off by default).
+    // Skew-kernel candidates (TTC_VARIANTS bits 3 and 4).
     if (variants & 8)
         for (int sched : scheds) add_skew(c, dtype, dtype_a, beta_nz, sched, max_smem, out);
 

@@ -10,13 +10,16 @@
 //   consumers  out[a][skewB(a) + b] = alpha * in[b][skewA(b) + a] (+ beta * what is there): lanes along a (conflict-free
 //              loads), a warp per b
 //   store warp out-row = head (< 16 bytes, element stores) + aligned body (one cp.async.bulk shared -> global) + tail
+//
+// DIRECT = true: no out-tile and no store warps; the consumers write B themselves, a warp per row of B with its lanes
+// along b0 (coalesced element stores, and element loads of B for beta != 0).
 #pragma once
 #include "ttc_device.cuh"
 #include "ttc_skew.h"
 
 namespace ttc {
 
-template <int DT, bool BETA>
+template <int DT, bool BETA, bool DIRECT>
 __global__ void __launch_bounds__(384)
 skew_kernel(const __grid_constant__ SkewParams P, const void* __restrict__ Ain, void* __restrict__ Bout,
             const Scalar alpha_in, const Scalar beta_in) {
@@ -33,7 +36,7 @@ skew_kernel(const __grid_constant__ SkewParams P, const void* __restrict__ Ain, 
     unsigned char* const smem = smem_raw + ((128u - (raw & 127u)) & 127u);
     const int TA = 1 << P.lgTA, TB = 1 << P.lgTB;
     const int rowsA = P.nP << P.lgTB, rowsB = P.nP << P.lgTA;
-    const uint32_t in_bytes = (uint32_t)(rowsA * P.pitchA), out_bytes = (uint32_t)(rowsB * P.pitchB);
+    const uint32_t in_bytes = (uint32_t)(rowsA * P.pitchA), out_bytes = DIRECT ? 0u : (uint32_t)(rowsB * P.pitchB);
     const uint32_t stage_bytes = in_bytes + out_bytes;
 
     __shared__ __align__(16) uint4 sched_resp;
@@ -48,7 +51,7 @@ skew_kernel(const __grid_constant__ SkewParams P, const void* __restrict__ Ain, 
 
     const int tid = threadIdx.x, lane = tid & 31;
     const int S = P.stages;
-    const int NP = P.np, NS = P.ns;
+    const int NP = P.np, NS = DIRECT ? 0 : P.ns;
     const int n_cons_warps = ((int)blockDim.x >> 5) - NP - NS;
     const int warp = tid >> 5;
     const char* const A = static_cast<const char*>(Ain);
@@ -60,7 +63,7 @@ skew_kernel(const __grid_constant__ SkewParams P, const void* __restrict__ Ain, 
         for (int s = 0; s < S; ++s) {
             asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(&full_bar[s])), "r"(32 * NP));
             asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(&done_bar[s])), "r"(n_cons_warps));
-            asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(&outfree_bar[s])), "r"(32 * NS));
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(&outfree_bar[s])), "r"(NS > 0 ? 32 * NS : 1));
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -87,7 +90,7 @@ skew_kernel(const __grid_constant__ SkewParams P, const void* __restrict__ Ain, 
                 // the in-tile is free once its consumers are done; the out-tile, which only beta != 0 loads into, once the
                 // store warp's copies of its last use have read it (beta == 0: the consumers wait for that instead)
                 mbar_wait((uint32_t)__cvta_generic_to_shared(&done_bar[s]), ((it / (uint32_t)S) - 1u) & 1u);
-                if constexpr (BETA) mbar_wait((uint32_t)__cvta_generic_to_shared(&outfree_bar[s]), ((it / (uint32_t)S) - 1u) & 1u);
+                if constexpr (BETA && !DIRECT) mbar_wait((uint32_t)__cvta_generic_to_shared(&outfree_bar[s]), ((it / (uint32_t)S) - 1u) & 1u);
             }
             if (!more) {
                 if (tid == 0) tile_of[s][u] = 0xFFFFFFFFu;
@@ -147,7 +150,7 @@ skew_kernel(const __grid_constant__ SkewParams P, const void* __restrict__ Ain, 
                 }
             }
             // rows of B: TB elements from (org1, org0 + a) of plane p -- loaded for beta != 0, their skews always
-            {
+            if constexpr (!DIRECT) {
                 const int64_t left = P.eq - org1;
                 const int len = (int)(left < TB ? left : TB);
                 const uintptr_t lo = (uintptr_t)B, hi = lo + (uintptr_t)P.spanB * ES;
@@ -178,7 +181,7 @@ skew_kernel(const __grid_constant__ SkewParams P, const void* __restrict__ Ain, 
             if (warp == 0) more = sched.next<true>(tile_id, P.n_tiles);
             __syncwarp();
         }
-    } else if (warp < NP + NS) {
+    } else if (!DIRECT && warp < NP + NS) {
         // ------------------------------------------------------------------ store warps
         for (uint32_t it = 0;; ++it) {
             const int s = (int)(it % (uint32_t)S);
@@ -222,7 +225,46 @@ skew_kernel(const __grid_constant__ SkewParams P, const void* __restrict__ Ain, 
             const int u = (int)((it / (uint32_t)S) & 1u);
             mbar_wait((uint32_t)__cvta_generic_to_shared(&full_bar[s]), (uint32_t)u);
             const bool end = tile_of[s][u] == 0xFFFFFFFFu;
-            if (!end) {
+            if constexpr (DIRECT) {
+                // no out-tile, no store warps: a warp takes one row of B (fixed a) at a time, its lanes run along b0, so the
+                // global accesses are coalesced (element-aligned); the column reads of the in-tile cost up to four wavefronts
+                if (!end) {
+                    const unsigned char* const in_s = smem + (uint32_t)s * stage_bytes;
+                    const int32_t org0 = org_of[s][u][0], org1 = org_of[s][u][1];
+                    const int64_t cb = off_of[s][u][1];
+                    const int64_t la = P.e0 - org0, lb = P.eq - org1;
+                    const int lenA = (int)(la < TA ? la : TA), lenB = (int)(lb < TB ? lb : TB);
+                    const int dq = (int)(P.sqA & (V - 1));
+                    for (int p = 0; p < P.nP; ++p) {
+                        const int sA0 = skA[s][p << P.lgTB];
+                        const unsigned char* const plane = in_s + (uint32_t)(p << P.lgTB) * (uint32_t)P.pitchA;
+                        // beta != 0: eight rows of B per warp and pass, so that their loads of B are in flight together
+                        constexpr int RA = BETA ? 8 : 1;
+                        for (int a = cw * RA; a < lenA; a += n_cons_warps * RA) {
+                            T* const drow = reinterpret_cast<T*>(B) + (cb + P.pB[p] + ((int64_t)org0 + a) * P.s0B + org1);
+                            const int na = lenA - a < RA ? lenA - a : RA;
+                            for (int b = lane; b < lenB; b += 32) {
+                                const int ska = (sA0 + b * dq) & (V - 1);
+                                const T* const src = reinterpret_cast<const T*>(plane + (uint32_t)b * (uint32_t)P.pitchA + (ska + a) * ES);
+                                T bv[RA];
+                                if constexpr (BETA) {
+#pragma unroll
+                                    for (int k = 0; k < RA; ++k)
+                                        if (k < na) bv[k] = drow[(int64_t)k * P.s0B + b];
+                                }
+#pragma unroll
+                                for (int k = 0; k < RA; ++k) {
+                                    if (k < na) {
+                                        T x = scale(alpha, src[k]);
+                                        if constexpr (BETA) x = add(x, scale(beta, bv[k]));
+                                        drow[(int64_t)k * P.s0B + b] = x;
+                                    }
+                                }
+                            }
+                        }
+                    }
+                }
+            } else if (!end) {
                 if constexpr (!BETA)
                     if (it >= (uint32_t)S) mbar_wait((uint32_t)__cvta_generic_to_shared(&outfree_bar[s]), ((it / (uint32_t)S) - 1u) & 1u);
                 unsigned char* const in_s = smem + (uint32_t)s * stage_bytes;

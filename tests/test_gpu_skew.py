@@ -3,8 +3,8 @@ whose rows are NOT 16-byte aligned (odd extents of 4- and 8-byte elements) move 
 directions -- the aligned superset of every row in, the aligned body of every row out, heads and tails element-wise.
 Guards (NaN) around and inside every padded tensor catch a store that reaches past its row; pointers that are only
 element-aligned add one more skew; tiny tensors put every row at the end of the tensor (element-wise fallback).
-The class is correct but slower than the ring kernel's shifted rows on B200, so plans offer it
-only with TTC_VARIANTS bit 3, which these tests set."""
+Two variants: consumers that store to B themselves (coalesced element stores; offered by default) and an out-tile with bulk
+stores (correct but 2x slower on B200: offered only with TTC_VARIANTS bit 4, which these tests set)."""
 import numpy as np
 import pytest
 import torch
@@ -19,7 +19,7 @@ pytestmark = pytest.mark.gpu
 
 @pytest.fixture(autouse=True)
 def offer_skew_candidates(monkeypatch):
-    monkeypatch.setenv("TTC_VARIANTS", "15")          # bit 3: the class is not offered by default
+    monkeypatch.setenv("TTC_VARIANTS", "31")          # bit 4: the out-tile variants too (not offered by default)
 
 
 def scalars(dtype, beta_nz):
@@ -58,12 +58,16 @@ def test_every_skew_candidate(dtype, beta_nz, shape):
         which = 1 if beta_nz else 0
         cands = skew_candidates(plan, which)
         assert cands, "no skew candidate for %s dtype %d" % (name, dtype)
+        flavours = {ttc.ttc_plan_candidate(plan, which, i).flags & 8 for i in cands}
+        assert flavours == {0, 8}, flavours                              # out-tile and direct-out variants
         for i in cands:
             check_bit_exact(w, plan=plan, candidate=i)
-        for ma, mb in ((1, 0), (0, 1), (3, 2)):                          # element-aligned pointers: one more skew
-            if dtype != wl.F32:
-                ma, mb = ma % 2, mb % 2
-            check_bit_exact(w, plan=plan, candidate=cands[0], misalign_a=ma, misalign_b=mb)
+        for flag in (0, 8):
+            first = [i for i in cands if ttc.ttc_plan_candidate(plan, which, i).flags & 8 == flag][0]
+            for ma, mb in ((1, 0), (0, 1), (3, 2)):                      # element-aligned pointers: one more skew
+                if dtype != wl.F32:
+                    ma, mb = ma % 2, mb % 2
+                check_bit_exact(w, plan=plan, candidate=first, misalign_a=ma, misalign_b=mb)
     finally:
         ttc.ttc_destroy(plan)
 
