@@ -105,3 +105,41 @@ def test_padded_a_rows_are_fine_and_copy_class_gets_its_flavour():
         assert cs and all(c.tile_ext[0] == 8 for c in cs)
     finally:
         ttc.ttc_destroy(plan)
+
+
+def skew(plan, which=0):
+    return [ttc.ttc_plan_candidate(plan, which, i) for i in range(ttc.ttc_plan_num_candidates(plan, which))
+            if ttc.ttc_plan_candidate(plan, which, i).kernel == 7]
+
+
+def test_skew_candidates_only_where_no_tensor_map_fits(monkeypatch):
+    """The skew kernel (csrc/ttc_skew.cuh) is for what tensor maps cannot take: rows that are not 16-byte aligned.  By
+    default only its direct-out variants (flag 8) are offered, the out-tile variants with TTC_VARIANTS bit 4."""
+    plan = ttc.ttc_plan(wl.F32, 2, (1023, 2301), (1, 0))
+    try:
+        for which in (0, 1):
+            cs = skew(plan, which)
+            assert cs and all(c.flags & 8 for c in cs) and not tmap(plan, which)
+            for c in cs:
+                assert c.tile_ext[0] in (32, 64, 128, 256) and c.tile_ext[1] in (32, 64, 128)
+    finally:
+        ttc.ttc_destroy(plan)
+    for dtype, sizes, perm in ((wl.F64, (96, 72, 64, 56), (3, 2, 1, 0)), (wl.C128, (37, 45), (1, 0)), (wl.F32, (48, 13, 21), (0, 2, 1)),
+                               (wl.F32, (1023, 7), (1, 0))):
+        plan = ttc.ttc_plan(dtype, len(sizes), sizes, perm)
+        try:
+            assert not skew(plan, 0) and not skew(plan, 1), (sizes, perm)
+        finally:
+            ttc.ttc_destroy(plan)
+    monkeypatch.setenv("TTC_VARIANTS", "31")
+    plan = ttc.ttc_plan(wl.F64, 3, (37, 21, 45), (2, 1, 0))
+    try:
+        assert {c.flags & 8 for c in skew(plan, 1)} == {0, 8}
+    finally:
+        ttc.ttc_destroy(plan)
+    monkeypatch.setenv("TTC_VARIANTS", "7")
+    plan = ttc.ttc_plan(wl.F32, 2, (1023, 2301), (1, 0))
+    try:
+        assert not skew(plan, 0)
+    finally:
+        ttc.ttc_destroy(plan)
