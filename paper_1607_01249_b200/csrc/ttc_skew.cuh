@@ -238,26 +238,33 @@ skew_kernel(const __grid_constant__ SkewParams P, const void* __restrict__ Ain, 
                     for (int p = 0; p < P.nP; ++p) {
                         const int sA0 = skA[s][p << P.lgTB];
                         const unsigned char* const plane = in_s + (uint32_t)(p << P.lgTB) * (uint32_t)P.pitchA;
-                        // beta != 0: eight rows of B per warp and pass, so that their loads of B are in flight together
-                        constexpr int RA = BETA ? 8 : 1;
-                        for (int a = cw * RA; a < lenA; a += n_cons_warps * RA) {
-                            T* const drow = reinterpret_cast<T*>(B) + (cb + P.pB[p] + ((int64_t)org0 + a) * P.s0B + org1);
-                            const int na = lenA - a < RA ? lenA - a : RA;
-                            for (int b = lane; b < lenB; b += 32) {
-                                const int ska = (sA0 + b * dq) & (V - 1);
-                                const T* const src = reinterpret_cast<const T*>(plane + (uint32_t)b * (uint32_t)P.pitchA + (ska + a) * ES);
-                                T bv[RA];
-                                if constexpr (BETA) {
+                        // a lane owns the columns b = lane + 32 j of B's rows (its skew and its addresses are then fixed: the inner
+                        // loop is a load from the in-tile, the arithmetic, a store and two pointer increments); a warp takes
+                        // RA rows of B per pass, whose loads of B (beta != 0) are in flight together
+                        constexpr int RA = BETA ? 8 : 4;
+                        for (int b = lane; b < lenB; b += 32) {
+                            const int ska = (sA0 + b * dq) & (V - 1);
+                            const T* const srow = reinterpret_cast<const T*>(plane + (uint32_t)b * (uint32_t)P.pitchA) + ska;
+                            T* const dcol = reinterpret_cast<T*>(B) + (cb + P.pB[p] + (int64_t)org0 * P.s0B + org1 + b);
+                            for (int a = cw * RA; a < lenA; a += n_cons_warps * RA) {
+                                T* const d = dcol + (int64_t)a * P.s0B;
+                                if (a + RA <= lenA) {
+                                    T bv[RA];
+                                    if constexpr (BETA) {
 #pragma unroll
-                                    for (int k = 0; k < RA; ++k)
-                                        if (k < na) bv[k] = drow[(int64_t)k * P.s0B + b];
-                                }
+                                        for (int k = 0; k < RA; ++k) bv[k] = d[(int64_t)k * P.s0B];
+                                    }
 #pragma unroll
-                                for (int k = 0; k < RA; ++k) {
-                                    if (k < na) {
-                                        T x = scale(alpha, src[k]);
+                                    for (int k = 0; k < RA; ++k) {
+                                        T x = scale(alpha, srow[a + k]);
                                         if constexpr (BETA) x = add(x, scale(beta, bv[k]));
-                                        drow[(int64_t)k * P.s0B + b] = x;
+                                        d[(int64_t)k * P.s0B] = x;
+                                    }
+                                } else {
+                                    for (int k = 0; a + k < lenA; ++k) {
+                                        T x = scale(alpha, srow[a + k]);
+                                        if constexpr (BETA) x = add(x, scale(beta, d[(int64_t)k * P.s0B]));
+                                        d[(int64_t)k * P.s0B] = x;
                                     }
                                 }
                             }
