@@ -1169,10 +1169,27 @@ void add_skew(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, 
         if (i != q && (c.d[i].sB * es) % 16 != 0) mappable = false;
     }
     if (mappable) return;
-    if (c.d[0].e < 16 || c.d[q].e < 16) return;
+    // Runs (ttc_skew.h): B's leading indices while they are contiguous in B, until the run has 64 positions; then A's
+    // leading indices (none of them in the B-run) while they are contiguous in A, until 128 positions; at most 3 each.
+    std::vector<int> runA = {0}, runB = {q};
+    int64_t LA = c.d[0].e, LB = c.d[q].e;
+    for (int k = 1; k < c.rank && (int)runB.size() < 3 && LB < 64; ++k) {
+        const int i = c.orderB[k];
+        if (i == 0 || c.d[i].sB != LB) break;                  // LB == stride the next index needs to continue the run
+        runB.push_back(i);
+        LB *= c.d[i].e;
+    }
+    auto in_run = [](const std::vector<int>& r, int i) { return std::find(r.begin(), r.end(), i) != r.end(); };
+    for (int i = 1; i < c.rank && (int)runA.size() < 3 && LA < 128; ++i) {
+        if (in_run(runB, i) || c.d[i].sA != LA) break;
+        runA.push_back(i);
+        LA *= c.d[i].e;
+    }
+    if (LA < 16 || LB < 16 || LA >= kInt31 / 2 || LB >= kInt31 / 2) return;
+    const bool plain_runs = runA.size() == 1 && runB.size() == 1;
     std::vector<int> othA, othB;
-    for (int i = 0; i < c.rank; ++i) if (i != 0 && i != q) othA.push_back(i);
-    for (int k = 0; k < c.rank; ++k) if (c.orderB[k] != 0 && c.orderB[k] != q) othB.push_back(c.orderB[k]);
+    for (int i = 0; i < c.rank; ++i) if (!in_run(runA, i) && !in_run(runB, i)) othA.push_back(i);
+    for (int k = 0; k < c.rank; ++k) if (!in_run(runA, c.orderB[k]) && !in_run(runB, c.orderB[k])) othB.push_back(c.orderB[k]);
     // direct = 1: no out-tile, the consumers store to B themselves (coalesced element stores)
     struct Var { int lgA, lgB, planes, dist, direct; };
     static const Var vars[] = {{7, 6, 1, 0, 1}, {6, 7, 1, 0, 1}, {7, 5, 1, 0, 1}, {6, 5, 1, 0, 1}, {8, 5, 1, 0, 1}, {6, 6, 1, 0, 1},
@@ -1184,9 +1201,9 @@ void add_skew(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, 
     std::set<std::string> seen;
     int n_added = 0;
     for (const Var& v : vars) {
-        if (!v.direct && !(variants & 16)) continue;
+        if (!v.direct && (!(variants & 16) || !plain_runs)) continue;        // the out-tile variants know single-index runs only
         const int TA = 1 << v.lgA, TB = 1 << v.lgB;
-        if (c.d[0].e * 2 < TA || c.d[q].e * 2 < TB) continue;                 // more than half of the tile would be padding
+        if (LA * 2 < TA || LB * 2 < TB) continue;                             // more than half of the tile would be padding
         int32_t pe[kMaxRank];
         for (int i = 0; i < c.rank; ++i) pe[i] = 1;
         int left = v.planes;
@@ -1209,11 +1226,12 @@ void add_skew(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, 
         std::memset(&K, 0, sizeof(K));
         K.lgTA = v.lgA;
         K.lgTB = v.lgB;
-        K.nG = c.rank;
-        K.sqA = c.d[q].sA;
-        K.s0B = c.d[0].sB;
-        K.e0 = c.d[0].e;
-        K.eq = c.d[q].e;
+        K.nA = (int)runA.size();
+        K.nB = (int)runB.size();
+        for (int k = 0; k < K.nA; ++k) { K.divA[k] = make_fastdiv((uint32_t)c.d[runA[k]].e); K.sBA[k] = c.d[runA[k]].sB; }
+        for (int k = 0; k < K.nB; ++k) { K.divB[k] = make_fastdiv((uint32_t)c.d[runB[k]].e); K.sAB[k] = c.d[runB[k]].sA; }
+        K.e0 = LA;
+        K.eq = LB;
         K.spanA = c.spanA;
         K.spanB = c.spanB;
         K.pitchA = TA * es + 48;         // the aligned superset of a row (up to 12 bytes before and after it); an odd number
@@ -1229,16 +1247,18 @@ void add_skew(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, 
         for (int k = 0; k < n; ++k) {
             const int i = gd[k];
             const int64_t step = k == 0 ? TA : k == 1 ? TB : pe[i];
-            const int64_t nt = (c.d[i].e + step - 1) / step;
+            const int64_t ext = k == 0 ? LA : k == 1 ? LB : c.d[i].e;
+            const int64_t nt = (ext + step - 1) / step;
             K.gdiv[k] = make_fastdiv((uint32_t)nt);
             K.stepA[k] = k < 2 ? 0 : step * c.d[i].sA;
             K.stepB[k] = k < 2 ? 0 : step * c.d[i].sB;
             n_tiles *= (uint64_t)nt;
             if (n_tiles >= (uint64_t)kInt31) { ok = false; break; }
             padded *= (double)nt * step;
-            real *= (double)c.d[i].e;
+            real *= (double)ext;
         }
         if (!ok) continue;
+        K.nG = n;
         int nP = 1;
         K.pA[0] = K.pB[0] = 0;
         for (int i : othA) {
@@ -1283,7 +1303,7 @@ void add_skew(const Canon& c, ttc_dtype dtype, ttc_dtype dtype_a, bool beta_nz, 
         const double waste = padded / real;
         // measured: rows of A shorter than 256 bytes make the bulk copies too many (448 against 152 us on 27 x 179 x 115 x 94);
         // such variants rank behind the ring kernel's candidates (whose fitted costs are about 2 for unaligned rows)
-        I.est_cost = (float)((1.20 + 0.01 * n_added) * waste * (TA * es < 256 ? 2.0 : 1.0) * (TB * es < 256 ? 1.15 : 1.0) *
+        I.est_cost = (float)((1.20 + 0.01 * n_added) * waste * (std::min<int64_t>(TA, LA) * es < 256 ? 2.0 : 1.0) * (TB * es < 256 ? 1.15 : 1.0) *
                              (v.direct ? 1.0 : 1.5));
         cand.feat[2] = (float)waste;
         cand.feat[4] = (float)stage;

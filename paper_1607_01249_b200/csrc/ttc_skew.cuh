@@ -12,12 +12,27 @@
 //   store warp out-row = head (< 16 bytes, element stores) + aligned body (one cp.async.bulk shared -> global) + tail
 //
 // DIRECT = true: no out-tile and no store warps; the consumers write B themselves, a warp per row of B with its lanes
-// along b0 (coalesced element stores, and element loads of B for beta != 0).
+// along b0 (coalesced element stores, and element loads of B for beta != 0).  In this variant "a0" and "b0" are RUNS of
+// merged leading indices (ttc_skew.h): a row of the in-tile is TA consecutive positions of the A-run (contiguous in A),
+// a lane's column is one position of the B-run (contiguous in B); the offset in B of an a-position comes from a per-tile
+// table (boff), the offset in A of a b-position from decoding it index by index.
 #pragma once
 #include "ttc_device.cuh"
 #include "ttc_skew.h"
 
 namespace ttc {
+
+// Offset in the other tensor of position `idx` of a run (ttc_skew.h).
+__device__ __forceinline__ int64_t skew_run_offset(uint32_t idx, int n, const FastDiv* div, const int64_t* stride) {
+    int64_t off = 0;
+    uint32_t r = idx;
+    for (int k = 0; k < n; ++k) {
+        const uint32_t q = fd_div(r, div[k]);
+        off += (int64_t)(r - q * div[k].d) * stride[k];
+        r = q;
+    }
+    return off;
+}
 
 template <int DT, bool BETA, bool DIRECT>
 __global__ void __launch_bounds__(384)
@@ -46,6 +61,7 @@ skew_kernel(const __grid_constant__ SkewParams P, const void* __restrict__ Ain, 
     __shared__ int32_t org_of[kSkewMaxStages][2][2];         // first a0, first b0 of the tile
     __shared__ uint32_t tile_of[kSkewMaxStages][2];
     __shared__ uint32_t tile_pub[2];                         // the tile the producer warps load in iteration it (slot it & 1)
+    __shared__ int64_t boff[kSkewMaxStages][256];            // direct-out: offset in B of every a-position of the tile
     __shared__ uint8_t skA[kSkewMaxStages][kSkewMaxRows];    // skew of every in-row (read by the consumers only)
     __shared__ uint8_t skB[kSkewMaxStages][2][kSkewMaxRows]; // skew of every out-row (consumers and, later, the store warp)
 
@@ -132,7 +148,7 @@ skew_kernel(const __grid_constant__ SkewParams P, const void* __restrict__ Ain, 
                     const int p = r >> P.lgTB, b = r & (TB - 1);
                     const int64_t bg = (int64_t)org1 + b;
                     if (bg >= P.eq) { skA[s][r] = 0; continue; }
-                    const uintptr_t addr = lo + (uintptr_t)(ca + P.pA[p] + bg * P.sqA + org0) * ES;
+                    const uintptr_t addr = lo + (uintptr_t)(ca + P.pA[p] + skew_run_offset((uint32_t)bg, P.nB, P.divB, P.sAB) + org0) * ES;
                     const int sk = (int)((addr & 15u) / ES);
                     skA[s][r] = (uint8_t)sk;
                     unsigned char* const slot = in_s + (uint32_t)r * (uint32_t)P.pitchA;
@@ -149,6 +165,10 @@ skew_kernel(const __grid_constant__ SkewParams P, const void* __restrict__ Ain, 
                     }
                 }
             }
+            if constexpr (DIRECT) {
+                for (int a = warp * 32 + lane; a < TA; a += 32 * NP)
+                    boff[s][a] = (int64_t)org0 + a < P.e0 ? skew_run_offset((uint32_t)(org0 + a), P.nA, P.divA, P.sBA) : 0;
+            }
             // rows of B: TB elements from (org1, org0 + a) of plane p -- loaded for beta != 0, their skews always
             if constexpr (!DIRECT) {
                 const int64_t left = P.eq - org1;
@@ -158,7 +178,7 @@ skew_kernel(const __grid_constant__ SkewParams P, const void* __restrict__ Ain, 
                     const int p = r >> P.lgTA, a = r & (TA - 1);
                     const int64_t ag = (int64_t)org0 + a;
                     if (ag >= P.e0) { skB[s][u][r] = 0; continue; }
-                    const uintptr_t addr = lo + (uintptr_t)(cb + P.pB[p] + ag * P.s0B + org1) * ES;
+                    const uintptr_t addr = lo + (uintptr_t)(cb + P.pB[p] + skew_run_offset((uint32_t)ag, P.nA, P.divA, P.sBA) + org1) * ES;
                     const int sk = (int)((addr & 15u) / ES);
                     skB[s][u][r] = (uint8_t)sk;
                     if constexpr (BETA) {
@@ -197,7 +217,7 @@ skew_kernel(const __grid_constant__ SkewParams P, const void* __restrict__ Ain, 
                 const int p = r >> P.lgTA, a = r & (TA - 1);
                 const int64_t ag = (int64_t)org0 + a;
                 if (ag >= P.e0) continue;
-                T* const dst = reinterpret_cast<T*>(B) + (cb + P.pB[p] + ag * P.s0B + org1);
+                T* const dst = reinterpret_cast<T*>(B) + (cb + P.pB[p] + skew_run_offset((uint32_t)ag, P.nA, P.divA, P.sBA) + org1);
                 const int sk = (int)skB[s][u][r];
                 const T* const row = reinterpret_cast<const T*>(out_s + (uint32_t)r * (uint32_t)P.pitchB) + sk;
                 int head = (V - sk) & (V - 1);
@@ -234,37 +254,35 @@ skew_kernel(const __grid_constant__ SkewParams P, const void* __restrict__ Ain, 
                     const int64_t cb = off_of[s][u][1];
                     const int64_t la = P.e0 - org0, lb = P.eq - org1;
                     const int lenA = (int)(la < TA ? la : TA), lenB = (int)(lb < TB ? lb : TB);
-                    const int dq = (int)(P.sqA & (V - 1));
                     for (int p = 0; p < P.nP; ++p) {
-                        const int sA0 = skA[s][p << P.lgTB];
+                        const uint8_t* const skp = &skA[s][p << P.lgTB];
                         const unsigned char* const plane = in_s + (uint32_t)(p << P.lgTB) * (uint32_t)P.pitchA;
                         // a lane owns the columns b = lane + 32 j of B's rows (its skew and its addresses are then fixed: the inner
                         // loop is a load from the in-tile, the arithmetic, a store and two pointer increments); a warp takes
                         // RA rows of B per pass, whose loads of B (beta != 0) are in flight together
                         constexpr int RA = BETA ? 8 : 4;
                         for (int b = lane; b < lenB; b += 32) {
-                            const int ska = (sA0 + b * dq) & (V - 1);
-                            const T* const srow = reinterpret_cast<const T*>(plane + (uint32_t)b * (uint32_t)P.pitchA) + ska;
-                            T* const dcol = reinterpret_cast<T*>(B) + (cb + P.pB[p] + (int64_t)org0 * P.s0B + org1 + b);
+                            const T* const srow = reinterpret_cast<const T*>(plane + (uint32_t)b * (uint32_t)P.pitchA) + skp[b];
+                            T* const dcol = reinterpret_cast<T*>(B) + (cb + P.pB[p] + org1 + b);
+                            const int64_t* const bo = boff[s];
                             for (int a = cw * RA; a < lenA; a += n_cons_warps * RA) {
-                                T* const d = dcol + (int64_t)a * P.s0B;
                                 if (a + RA <= lenA) {
                                     T bv[RA];
                                     if constexpr (BETA) {
 #pragma unroll
-                                        for (int k = 0; k < RA; ++k) bv[k] = d[(int64_t)k * P.s0B];
+                                        for (int k = 0; k < RA; ++k) bv[k] = dcol[bo[a + k]];
                                     }
 #pragma unroll
                                     for (int k = 0; k < RA; ++k) {
                                         T x = scale(alpha, srow[a + k]);
                                         if constexpr (BETA) x = add(x, scale(beta, bv[k]));
-                                        d[(int64_t)k * P.s0B] = x;
+                                        dcol[bo[a + k]] = x;
                                     }
                                 } else {
                                     for (int k = 0; a + k < lenA; ++k) {
                                         T x = scale(alpha, srow[a + k]);
-                                        if constexpr (BETA) x = add(x, scale(beta, d[(int64_t)k * P.s0B]));
-                                        d[(int64_t)k * P.s0B] = x;
+                                        if constexpr (BETA) x = add(x, scale(beta, dcol[bo[a + k]]));
+                                        dcol[bo[a + k]] = x;
                                     }
                                 }
                             }
@@ -280,7 +298,7 @@ skew_kernel(const __grid_constant__ SkewParams P, const void* __restrict__ Ain, 
                 // pitches of an odd number of 16-byte units (4 mod 32 words) the 32 lanes hit banks 5 l + 4 j + skew on the
                 // in-side and 5 l + j + skew on the out-side: both conflict-free up to the skews' perturbation.  The warps
                 // share every block (warp w takes the steps j = w, w + warps, ...).
-                const int dq = (int)(P.sqA & (V - 1)), d0 = (int)(P.s0B & (V - 1));
+                const int dq = (int)(P.sAB[0] & (V - 1)), d0 = (int)(P.sBA[0] & (V - 1));      // out-tile variants: nA == nB == 1
                 for (int p = 0; p < P.nP; ++p) {
                     const int sA0 = skA[s][p << P.lgTB], sB0 = skB[s][u][p << P.lgTA];      // skews of the plane's first rows
                     for (int a0 = 0; a0 < TA; a0 += 32) {

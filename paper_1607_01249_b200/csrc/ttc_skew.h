@@ -27,12 +27,18 @@ struct SkewParams {
     int nP;                        // planes (index combinations of the other indices) per tile
     int nG;                        // tile-grid dimensions: 0 = a0, 1 = b0, then the other canonical indices
     int pitchA, pitchB;            // bytes per shared-memory row of the in-tile / out-tile (multiples of 16)
-    int64_t e0, eq;                // extents of a0 and b0
+    int64_t e0, eq;                // lengths of the A-run and of the B-run
     int64_t spanA, spanB;          // elements from the first to one past the last element of A / B
     FastDiv gdiv[kMaxRank];
     int64_t stepA[kMaxRank], stepB[kMaxRank];   // element offset per tile index of grid dimension >= 2
     int64_t pA[kSkewMaxPlanes], pB[kSkewMaxPlanes];
-    int64_t sqA, s0B;              // stride of b0 in A, of a0 in B (elements)
+    // Runs: the tile's a-range is a range of positions in the A-run = the first nA indices of A merged (they are
+    // contiguous in A: lda == extent), its b-range a range of positions in the B-run = the first nB indices of B merged.
+    // Position -> element offset in the OTHER tensor goes index by index (divX by the extents, innermost first).
+    int nA, nB;
+    FastDiv divA[3], divB[3];
+    int64_t sBA[3];                // strides in B of the A-run's indices
+    int64_t sAB[3];                // strides in A of the B-run's indices
 };
 
 }  // namespace ttc

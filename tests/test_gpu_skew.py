@@ -43,6 +43,12 @@ SHAPES = [
     ("s4d", (19, 6, 10, 35), (3, 1, 0, 2), None, None),
     ("s5d", (21, 3, 5, 4, 17), (4, 2, 0, 3, 1), None, None),
     ("s2d_wide", (300, 257), (1, 0), None, None),                       # several tiles in both directions, ragged tails
+    # short leading extents: the tile's b-range runs over B's two leading indices (15 x 27 contiguous in B), ...
+    ("s5d_b_run", (63, 27, 10, 15, 4), (3, 1, 0, 4, 2), None, None),
+    # ... its a-range over A's two leading indices (11 x 37 contiguous in A), b-range over 14 x 8
+    ("s5d_ab_runs", (11, 37, 8, 9, 14), (4, 2, 1, 3, 0), None, None),
+    ("s4d_runs_of_three", (5, 7, 3, 9, 5, 3), (5, 4, 3, 2, 1, 0), None, None),
+    ("s4d_padded_no_runs", (21, 19, 5, 17), (3, 1, 0, 2), (22, 19, 5, 17), (18, 19, 21, 5)),
 ]
 
 
@@ -59,10 +65,10 @@ def test_every_skew_candidate(dtype, beta_nz, shape):
         cands = skew_candidates(plan, which)
         assert cands, "no skew candidate for %s dtype %d" % (name, dtype)
         flavours = {ttc.ttc_plan_candidate(plan, which, i).flags & 8 for i in cands}
-        assert flavours == {0, 8}, flavours                              # out-tile and direct-out variants
+        assert 8 in flavours, flavours                                   # direct-out always; out-tile variants for single-index runs
         for i in cands:
             check_bit_exact(w, plan=plan, candidate=i)
-        for flag in (0, 8):
+        for flag in sorted(flavours):
             first = [i for i in cands if ttc.ttc_plan_candidate(plan, which, i).flags & 8 == flag][0]
             for ma, mb in ((1, 0), (0, 1), (3, 2)):                      # element-aligned pointers: one more skew
                 if dtype != wl.F32:
