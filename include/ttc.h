@@ -293,8 +293,9 @@ ttc_status ttc_plan_candidate_features(ttc_plan_t plan, int which, int index, fl
  * shape, table shapes -- as a compile-time constant, so that they become immediates and the loops over them
  * unroll.  The twin is timed against the generic instance (interleaved, median of 5 x 4 launches on scratch
  * buffers) and used by ttc_execute only if it is faster; ttc_info.specialized / spec_us / generic_us report the
- * outcome.  Warp-specialised (TTC_KERNEL_TMA) and copy-class (TTC_KERNEL_COPY) winners have a twin; ttc_execute_batched and misaligned
- * pointers keep the generic kernels.  Costs about a second of compile time per winner (cubins are kept under
+ * outcome.  Warp-specialised (TTC_KERNEL_TMA) and copy-class (TTC_KERNEL_COPY) winners have a twin; a tensor-map or
+ * skew-kernel winner (not issue-bound: nothing to gain) is challenged by the twin of the fastest timed ring / copy candidate,
+ * which becomes the plan's winner if it is faster; ttc_execute_batched and misaligned pointers keep the generic kernels.  Costs about a second of compile time per winner (cubins are kept under
  * <TTC_CACHE_FILE>.cubins/ when that variable is set); TTC_SPECIALIZE=1 makes ttc_plan call it.
  * Returns TTC_ERR_UNSUPPORTED when libnvrtc cannot be loaded or no winner is specialisable -- the plan then
  * simply keeps its generic kernels -- and TTC_ERR_CUDA / TTC_ERR_ALLOC on device trouble.
