@@ -85,7 +85,8 @@ typedef enum {
                                (<= 5-D, strides multiples of 16 bytes, 16-byte aligned A and B, same
                                element type), swizzled shared-memory boxes, in-register micro-tiles  */
     TTC_KERNEL_SKEW = 7     /* K2/K3 for rows that are not 16-byte aligned (odd extents): bulk copies of aligned
-                               supersets in, skewed shared-memory rows, bulk stores of aligned bodies out    */
+                               supersets in, skewed shared-memory rows, coalesced element stores out (flag
+                               TTC_CAND_DIRECT_OUT) or, on request, an out-tile and bulk stores of aligned bodies */
 } ttc_kernel_class;
 
 typedef struct ttc_plan_s* ttc_plan_t;
